@@ -1,0 +1,123 @@
+/* mfdn_b200.h -- C ABI of libmfdn_b200.so
+ *
+ * Coupled-JT -> M-scheme transformation of 2- and 3-body interaction matrix elements
+ * (the hot path arXiv:1412.5989 moved to the GPU inside MFDn's matrix construction),
+ * B200 / sm_100a only.  No torch types, plain pointers and sizes.  Every function returns
+ * MFDN_OK or a negative mfdn_status and never throws.  "PAPER.md:n" = line n of the paper
+ * text; "DESIGN.md Qn" = the reading taken where the paper is silent.
+ *
+ * Call order:  mfdn_orbitals_init -> mfdn_cg_build -> mfdn_coupled_upload_2b / _3b ->
+ *              mfdn_mscheme_2b / _3b (any number of times, any stream) -> mfdn_destroy.
+ * Out-of-order calls return MFDN_ERR_STATE.
+ *
+ * Conventions: all indices 0-based.  Orbital o = (n, l, 2j), e = 2n+l.
+ * SPS s = (orbital, 2m, 2tz), table-driven.  A request is the SPS indices of the bra then of the
+ * ket ("a 3-body element request takes the form of a set of six SPS indices").
+ * Canonical particle order inside a bra/ket = ascending (orbital, SPS); a request in any other
+ * order is answered with the permutation sign applied.
+ */
+#ifndef MFDN_B200_H
+#define MFDN_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mfdn_ctx mfdn_ctx; /* opaque; owns every device table */
+
+typedef enum {
+    MFDN_OK = 0,
+    MFDN_ERR_ARG = -1,   /* null pointer, negative size, quantum number out of supported range */
+    MFDN_ERR_STATE = -2, /* call order violated */
+    MFDN_ERR_CUDA = -3,  /* a CUDA runtime call failed; see mfdn_last_error */
+    MFDN_ERR_OOM = -4,   /* host or device allocation failed, or caller scratch too small */
+    MFDN_ERR_TABLE = -5  /* coupled table violates its structural rules */
+} mfdn_status;
+
+/* flags of mfdn_mscheme_2b/3b */
+enum {
+    MFDN_PRESORTED = 1,   /* requests are already ordered by orbital-tuple group (bra tuple, ket tuple):
+                             skip the internal group sort (step H2) */
+    MFDN_FORCE_NAIVE = 2, /* one thread per request in request order, no sort, no staging: the paper's own
+                             kernel design; kept as on-device reference */
+    MFDN_FORCE_DENSE = 4  /* reserved for the dense-block path; currently ignored */
+};
+
+/* A0. Single-particle basis (quantum numbers flattened into one linear SPS index).
+ * HOST arrays, borrowed for the duration of the call.  n,l,twoj: [n_orb]; sps_*: [n_sps];
+ * sps_twom odd with |2m| <= 2j, sps_twotz = +1 or -1.  Limits: n_orb <= 1023, 2j <= 21.
+ * Creates the context on CUDA device `device`. */
+int mfdn_orbitals_init(mfdn_ctx** out, int device, int32_t n_orb, const int32_t* n, const int32_t* l,
+                       const int32_t* twoj, int32_t n_sps, const int32_t* sps_orb, const int32_t* sps_twom,
+                       const int32_t* sps_twotz);
+
+/* A1. Device-resident fp64 Clebsch-Gordan tables ("D is developed from a series of angular momentum and
+ * isospin coupling coefficients"; Q1/Q2/Q10), built by one kernel from Racah's
+ * formula with a double-double log-factorial table.  Asynchronous on `stream` (cudaStream_t). */
+int mfdn_cg_build(mfdn_ctx*, void* stream);
+
+/* Test hook: copy a CG table to HOST memory (synchronises).  stage 1 = <j1 m1 j2 m2|J M> for half-integer
+ * j1,j2 <= jmax; stage 2 = <J12 M12 j m|J M> for integer J12 <= 2*jmax and half-integer j <= jmax.
+ * Layout: blocks in ascending (first, second) angular momentum order; stage-1 block (2j1,2j2) holds
+ * [i1][i2][iJ] (iJ fastest), i = (2m+2j)/2, iJ = (2J - |2j1-2j2|)/2, value <j1 m1 j2 m2|J m1+m2>
+ * (0 where |m1+m2| > J); stage-2 block (J12, 2j) likewise with j1 = J12.
+ * *n receives the entry count; if host_out is NULL or cap < *n nothing is copied. */
+int mfdn_cg_download(mfdn_ctx*, int stage, double* host_out, int64_t cap, int64_t* n);
+
+/* A2. Coupled-JT tables, channel-major (only potentially-nonzero elements, one block per
+ * orbital combination).  chan_* have length n_chan; state_* have length sum(chan_dim), listed channel by
+ * channel; channel c is a row-major chan_dim[c] x chan_dim[c] fp64 square at values + chan_off[c].
+ * Index arrays are HOST; `values` is HOST or DEVICE (values_on_device != 0).  The library copies and
+ * re-tiles (group-major, in the order the kernel's nested loops read them); the caller keeps
+ * ownership.  Structural rules (else MFDN_ERR_TABLE): orbitals in range and a <= b (<= c); triangle rules;
+ * channel parity = parity of the state's orbitals; a == b only with J+T (2-body) resp. J12+T12 (3-body) odd;
+ * 3-body: e_a+e_b+e_c <= e3max, 2T in {1,3}, T12 in {0,1}; no duplicate channel or state.
+ * 2-body: chan_J, chan_T are J and T; 3-body: chan_twoJ, chan_twoT are 2J and 2T.  chan_par: 0 even, 1 odd.
+ * Synchronises `stream` before returning. */
+int mfdn_coupled_upload_2b(mfdn_ctx*, int32_t n_chan, const int32_t* chan_J, const int32_t* chan_T,
+                           const int32_t* chan_par, const int32_t* chan_dim, const int64_t* chan_off,
+                           const int32_t* state_a, const int32_t* state_b, const double* values,
+                           int values_on_device, void* stream);
+int mfdn_coupled_upload_3b(mfdn_ctx*, int32_t e3max, int32_t n_chan, const int32_t* chan_twoJ,
+                           const int32_t* chan_twoT, const int32_t* chan_par, const int32_t* chan_dim,
+                           const int64_t* chan_off, const int32_t* state_a, const int32_t* state_b,
+                           const int32_t* state_c, const int32_t* state_J12, const int32_t* state_T12,
+                           const double* values, int values_on_device, void* stream);
+
+/* H1-H6. The transformation (formulas in DESIGN.md "What is computed").
+ * d_req : DEVICE int32 [n][4] = (bra0,bra1,ket0,ket1)  /  [n][6] = (bra0..2, ket0..2); 16-byte aligned.
+ * d_out : DEVICE double [n]; d_mask: DEVICE uint8 [n] or NULL.  Caller-owned, results in REQUEST order.
+ *         mask[i] = 1 iff the request passes the integer selection rules S1-S7; where
+ *         mask[i] = 0 the value is exactly +0.0.
+ * d_work/work_bytes: caller-provided DEVICE scratch, 256-byte aligned.  Call with d_work == NULL to get
+ *         the size needed for n requests in *work_bytes (nothing is launched).  The call itself never
+ *         allocates and never synchronises: it is asynchronous on `stream`.
+ * Per-request problems never fail the call: an out-of-range SPS index gives value 0, mask 0 and is
+ * counted (mfdn_bad_request_count).  Concurrent calls on different streams are allowed provided
+ * each uses its own scratch (one stream per host thread). */
+int mfdn_mscheme_2b(mfdn_ctx*, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_mask, void* d_work,
+                    size_t* work_bytes, uint32_t flags, void* stream);
+int mfdn_mscheme_3b(mfdn_ctx*, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_mask, void* d_work,
+                    size_t* work_bytes, uint32_t flags, void* stream);
+
+/* Number of requests with an out-of-range SPS index seen so far (synchronises `stream`). */
+int64_t mfdn_bad_request_count(mfdn_ctx*, void* stream);
+
+/* Sizes of what was uploaded, for reports: which = 0 tuples (2b), 1 tuples (3b), 2 slab bytes (2b),
+ * 3 slab bytes (3b), 4 CG entries stage 1, 5 CG entries stage 2, 6 kernels launched so far by mscheme_*. */
+int64_t mfdn_info(mfdn_ctx*, int which);
+
+/* Group key of every request, for producing MFDN_PRESORTED input: d_key[i] = bra_tuple * n_tuples +
+ * ket_tuple, or 0xFFFFFFFF for requests that fail S1-S6.  body = 2 or 3.  Asynchronous on `stream`. */
+int mfdn_group_keys(mfdn_ctx*, int body, int64_t n, const int32_t* d_req, uint32_t* d_key, void* stream);
+
+const char* mfdn_last_error(mfdn_ctx*);
+void mfdn_destroy(mfdn_ctx*);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MFDN_B200_H */

@@ -41,9 +41,13 @@ def cg_allowed(tj1: int, tm1: int, tj2: int, tm2: int, tJ: int, tM: int) -> bool
     return True
 
 
-@lru_cache(maxsize=None)
 def cg_exact_square(tj1: int, tm1: int, tj2: int, tm2: int, tJ: int, tM: int):
     """(sign, P*S^2) with sign in {-1, 0, +1} and P*S^2 an exact Fraction."""
+    return _cg_exact_square(int(tj1), int(tm1), int(tj2), int(tm2), int(tJ), int(tM))   # no numpy ints
+
+
+@lru_cache(maxsize=None)
+def _cg_exact_square(tj1: int, tm1: int, tj2: int, tm2: int, tJ: int, tM: int):
     if not cg_allowed(tj1, tm1, tj2, tm2, tJ, tM):
         return 0, Fraction(0)
     f = factorial

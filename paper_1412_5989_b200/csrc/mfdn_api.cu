@@ -1,0 +1,742 @@
+// Host side of libmfdn_b200.so: context, A0 orbital tables, A1 CG-table build kernel,
+// A2 coupled-table upload + re-tiling kernels.  See include/mfdn_b200.h for the ABI.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <new>
+
+#include "mfdn_internal.cuh"
+
+using namespace mfdn;
+
+namespace mfdn {
+int fail(mfdn_ctx* c, int code, const std::string& msg)
+{
+    if (c) c->err = msg;
+    return code;
+}
+int cuda_fail(mfdn_ctx* c, cudaError_t e, const char* what)
+{
+    if (c) c->err = std::string(what) + ": " + cudaGetErrorString(e);
+    return e == cudaErrorMemoryAllocation ? MFDN_ERR_OOM : MFDN_ERR_CUDA;
+}
+}  // namespace mfdn
+
+// One contiguous host arena -> one cudaMalloc + one cudaMemcpy (the paper's fix for its index
+// array: "a single GPU allocate and GPU copy").  Offsets instead of pointers.
+struct Arena {
+    std::vector<char> buf;
+    size_t add(const void* src, size_t bytes)
+    {
+        size_t off = (buf.size() + 255) & ~size_t(255);
+        buf.resize(off + bytes);
+        if (bytes) memcpy(buf.data() + off, src, bytes);
+        return off;
+    }
+    template <class T>
+    size_t add(const std::vector<T>& v) { return add(v.data(), v.size() * sizeof(T)); }
+};
+
+static int arena_upload(mfdn_ctx* c, Arena& a, char** dbase, cudaStream_t st)
+{
+    void* d = nullptr;
+    MFDN_CUDA(c, cudaMalloc(&d, std::max<size_t>(a.buf.size(), 256)));
+    c->owned.push_back(d);
+    MFDN_CUDA(c, cudaMemcpyAsync(d, a.buf.data(), a.buf.size(), cudaMemcpyHostToDevice, st));
+    MFDN_CUDA(c, cudaStreamSynchronize(st));
+    *dbase = (char*)d;
+    return MFDN_OK;
+}
+
+// ------------------------------------------------------------------------------------------ A0
+extern "C" int mfdn_orbitals_init(mfdn_ctx** out, int device, int32_t n_orb, const int32_t* n, const int32_t* l,
+                                  const int32_t* twoj, int32_t n_sps, const int32_t* sps_orb,
+                                  const int32_t* sps_twom, const int32_t* sps_twotz)
+{
+    if (!out) return MFDN_ERR_ARG;
+    *out = nullptr;
+    if (!n || !l || !twoj || !sps_orb || !sps_twom || !sps_twotz) return MFDN_ERR_ARG;
+    if (n_orb <= 0 || n_orb > 1023 || n_sps <= 0 || n_sps > 65535) return MFDN_ERR_ARG;
+    mfdn_ctx* c = new (std::nothrow) mfdn_ctx();
+    if (!c) return MFDN_ERR_OOM;
+    c->device = device;
+    cudaError_t e = cudaSetDevice(device);
+    if (e != cudaSuccess) { delete c; return MFDN_ERR_CUDA; }
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) == cudaSuccess) c->num_sms = prop.multiProcessorCount;
+    int tjmax = 0;
+    for (int o = 0; o < n_orb; o++) {
+        int e_o = 2 * n[o] + l[o];
+        if (n[o] < 0 || l[o] < 0 || twoj[o] < 1 || !(twoj[o] & 1) || twoj[o] > MAX_TWOJ || e_o > 63 ||
+            (twoj[o] != 2 * l[o] + 1 && twoj[o] != 2 * l[o] - 1)) { delete c; return MFDN_ERR_ARG; }
+        tjmax = std::max(tjmax, (int)twoj[o]);
+    }
+    c->orb_n.assign(n, n + n_orb);
+    c->orb_l.assign(l, l + n_orb);
+    c->orb_twoj.assign(twoj, twoj + n_orb);
+    c->tjmax = tjmax;
+    c->h_sps_rec.resize(n_sps);
+    for (int s = 0; s < n_sps; s++) {
+        int o = sps_orb[s];
+        if (o < 0 || o >= n_orb) { delete c; return MFDN_ERR_ARG; }
+        int tm = sps_twom[s], tz = sps_twotz[s];
+        if (std::abs(tm) > twoj[o] || !(tm & 1) || (tz != 1 && tz != -1)) { delete c; return MFDN_ERR_ARG; }
+        c->h_sps_rec[s] = sps_pack(o, (tm + twoj[o]) / 2, tz == 1, twoj[o], 2 * n[o] + l[o], l[o] & 1);
+    }
+    void* d = nullptr;
+    if (cudaMalloc(&d, n_sps * sizeof(uint32_t) + 256) != cudaSuccess) { delete c; return MFDN_ERR_OOM; }
+    c->owned.push_back(d);
+    if (cudaMemcpy(d, c->h_sps_rec.data(), n_sps * sizeof(uint32_t), cudaMemcpyHostToDevice) != cudaSuccess) {
+        mfdn_destroy(c);
+        return MFDN_ERR_CUDA;
+    }
+    c->t.sps_rec = (const uint32_t*)d;
+    c->t.n_sps = n_sps;
+    c->t.n_orb = n_orb;
+    c->t.nj = (tjmax + 1) / 2;
+    void* bad = nullptr;
+    if (cudaMalloc(&bad, 256) != cudaSuccess) { mfdn_destroy(c); return MFDN_ERR_OOM; }
+    c->owned.push_back(bad);
+    cudaMemset(bad, 0, 256);
+    c->t.bad_count = (unsigned long long*)bad;
+
+    // isospin weights, "precalculated with several conditionals"; closed forms of the
+    // j = 1/2 Clebsch-Gordan coefficients.
+    const double r12 = std::sqrt(0.5), r13 = std::sqrt(1.0 / 3.0), r23 = std::sqrt(2.0 / 3.0);
+    for (int ta = 0; ta < 2; ta++)
+        for (int tb = 0; tb < 2; tb++) {
+            int m12 = (ta ? 1 : -1) + (tb ? 1 : -1);  // 2*MT12
+            double c0 = (m12 != 0) ? 0.0 : (ta ? r12 : -r12);  // <1/2 ta 1/2 tb|0 0>
+            double c1 = (m12 != 0) ? 1.0 : r12;                // <1/2 ta 1/2 tb|1 MT12>
+            c->t.iso2[ta * 2 + tb][0] = c0;
+            c->t.iso2[ta * 2 + tb][1] = c1;
+            for (int tc = 0; tc < 2; tc++) {
+                // <1 MT12 1/2 tc|1/2 MT> and <1 MT12 1/2 tc|3/2 MT>
+                double h, q;
+                if (m12 == 2) { h = tc ? 0.0 : r23; q = tc ? 1.0 : r13; }
+                else if (m12 == 0) { h = tc ? -r13 : r13; q = r23; }
+                else { h = tc ? -r23 : 0.0; q = tc ? r13 : 1.0; }
+                double* w = c->t.iso3[ta * 4 + tb * 2 + tc];
+                w[0] = c0;       // (T12,T) = (0,1/2):  <0 0 1/2 tc|1/2 tc> = 1
+                w[1] = c1 * h;   // (1,1/2)
+                w[2] = c1 * q;   // (1,3/2)
+            }
+        }
+    c->stage = 1;
+    *out = c;
+    return MFDN_OK;
+}
+
+// ------------------------------------------------------------------------------------------ A1
+// Racah's closed form.  Two measures keep every entry within a few 1e-16 of the exact value
+// (DESIGN.md "CG accuracy"):
+//  * the alternating k-sum is rewritten over binomials,
+//      sum_k (-1)^k / [k!(a-k)!(b-k)!(c-k)!(d+k)!(e+k)!]
+//        = [a!(b+d)!(c+e)!]^-1 * sum_k (-1)^k C(a,k) C(b+d,b-k) C(c+e,c-k),
+//    an INTEGER sum (< 2^70 for 2j <= 21) accumulated exactly in double-double, so the
+//    cancellation between terms costs nothing;
+//  * the prefactor sqrt(P)/[a!(b+d)!(c+e)!] is exp of a log-factorial sum carried as double-double
+//    (hi+lo): the log sums reach ~150, so plain fp64 sums would lose ~3e-14.
+struct dd { double hi, lo; };
+__device__ __forceinline__ dd dd_add(dd a, dd b)
+{
+    double s = a.hi + b.hi, bb = s - a.hi;
+    double e = (a.hi - (s - bb)) + (b.hi - bb);
+    double t = a.lo + b.lo, tb = t - a.lo;
+    double f = (a.lo - (t - tb)) + (b.lo - tb);
+    e += t;
+    double s2 = s + e;
+    e = e - (s2 - s);
+    e += f;
+    dd r;
+    r.hi = s2 + e;
+    r.lo = e - (r.hi - s2);
+    return r;
+}
+__device__ __forceinline__ dd dd_neg(dd a) { return dd{-a.hi, -a.lo}; }
+__device__ __forceinline__ dd dd_mul_d(dd x, double y)
+{
+    double p = x.hi * y;
+    double e = fma(x.hi, y, -p);
+    e = fma(x.lo, y, e);
+    dd r;
+    r.hi = p + e;
+    r.lo = e - (r.hi - p);
+    return r;
+}
+
+struct CgBlock { int tj1, tj2, off, count; };
+constexpr int BINOM_N = 64;   // Pascal triangle rows 0..63 as doubles (exact below 2^53: rows <= 56)
+
+__global__ void k_cg_build(const CgBlock* __restrict__ blocks, const double2* __restrict__ lfact,
+                           const double* __restrict__ binom, double* __restrict__ out)
+{
+    CgBlock b = blocks[blockIdx.y];
+    auto LF = [&](int n) { double2 v = lfact[n]; return dd{v.x, v.y}; };
+    auto BIN = [&](int n, int k) { return binom[n * BINOM_N + k]; };
+    const int nJ = min(b.tj1, b.tj2) + 1;
+    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < b.count; idx += gridDim.x * blockDim.x) {
+        int iJ = idx % nJ;
+        int i2 = (idx / nJ) % (b.tj2 + 1);
+        int i1 = idx / (nJ * (b.tj2 + 1));
+        int tJ = abs(b.tj1 - b.tj2) + 2 * iJ, tm1 = 2 * i1 - b.tj1, tm2 = 2 * i2 - b.tj2, tM = tm1 + tm2;
+        double val = 0.0;
+        if (abs(tM) <= tJ) {
+            // all halves below are integers by construction
+            int a = (b.tj1 + b.tj2 - tJ) / 2, bq = (b.tj1 - tm1) / 2, cq = (b.tj2 + tm2) / 2;
+            int d = (tJ - b.tj2 + tm1) / 2, e = (tJ - b.tj1 - tm2) / 2;
+            dd sum{0.0, 0.0};
+            int k0 = max(0, max(-d, -e)), k1 = min(a, min(bq, cq));
+            for (int k = k0; k <= k1; k++) {
+                dd t{BIN(a, k), 0.0};
+                t = dd_mul_d(t, BIN(bq + d, bq - k));
+                t = dd_mul_d(t, BIN(cq + e, cq - k));
+                sum = dd_add(sum, (k & 1) ? dd_neg(t) : t);
+            }
+            dd lp = LF(a);
+            lp = dd_add(lp, LF((b.tj1 - b.tj2 + tJ) / 2));
+            lp = dd_add(lp, LF((-b.tj1 + b.tj2 + tJ) / 2));
+            lp = dd_add(lp, dd_neg(LF((b.tj1 + b.tj2 + tJ) / 2 + 1)));
+            lp = dd_add(lp, LF((tJ + tM) / 2));
+            lp = dd_add(lp, LF((tJ - tM) / 2));
+            lp = dd_add(lp, LF(bq));
+            lp = dd_add(lp, LF((b.tj1 + tm1) / 2));
+            lp = dd_add(lp, LF((b.tj2 - tm2) / 2));
+            lp = dd_add(lp, LF(cq));
+            lp.hi *= 0.5;  // sqrt of the prefactor
+            lp.lo *= 0.5;
+            lp = dd_add(lp, dd_neg(LF(a)));
+            lp = dd_add(lp, dd_neg(LF(bq + d)));
+            lp = dd_add(lp, dd_neg(LF(cq + e)));
+            val = (sum.hi + sum.lo) * (exp(lp.hi) * (1.0 + lp.lo)) * sqrt((double)(tJ + 1));
+        }
+        out[b.off + idx] = val;
+    }
+}
+
+extern "C" int mfdn_cg_build(mfdn_ctx* c, void* stream)
+{
+    if (!c) return MFDN_ERR_ARG;
+    if (c->stage < 1) return fail(c, MFDN_ERR_STATE, "mfdn_cg_build before mfdn_orbitals_init");
+    if (c->stage >= 2) return MFDN_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    MFDN_CUDA(c, cudaSetDevice(c->device));
+    const int nj = c->t.nj;
+    std::vector<CgBlock> blocks;
+    std::vector<int32_t> off1(nj * nj), off2(2 * nj * nj);
+    int64_t pos = 0;
+    for (int a = 0; a < nj; a++)
+        for (int b = 0; b < nj; b++) {
+            int tj1 = 2 * a + 1, tj2 = 2 * b + 1;
+            int cnt = (tj1 + 1) * (tj2 + 1) * (std::min(tj1, tj2) + 1);
+            off1[a * nj + b] = (int32_t)pos;
+            blocks.push_back({tj1, tj2, (int)pos, cnt});
+            pos += cnt;
+        }
+    c->n_cg1 = pos;
+    for (int J12 = 0; J12 < 2 * nj; J12++)
+        for (int b = 0; b < nj; b++) {
+            int tj1 = 2 * J12, tj2 = 2 * b + 1;
+            int cnt = (tj1 + 1) * (tj2 + 1) * (std::min(tj1, tj2) + 1);
+            off2[J12 * nj + b] = (int32_t)(pos - c->n_cg1);
+            blocks.push_back({tj1, tj2, (int)pos, cnt});
+            pos += cnt;
+        }
+    c->n_cg2 = pos - c->n_cg1;
+    // log-factorial table as double-double, from long double accumulation of log(k)
+    const int NF = 4 * (2 * nj) + 8;
+    std::vector<double> lf(2 * NF);
+    long double acc = 0.0L;
+    for (int k = 0; k < NF; k++) {
+        if (k > 1) acc += logl((long double)k);
+        double hi = (double)acc;
+        lf[2 * k] = hi;
+        lf[2 * k + 1] = (double)(acc - (long double)hi);
+    }
+    std::vector<double> binom(BINOM_N * BINOM_N, 0.0);
+    {
+        std::vector<unsigned long long> row(BINOM_N, 0), prev(BINOM_N, 0);
+        for (int nn = 0; nn < BINOM_N; nn++) {
+            for (int k = 0; k <= nn; k++) row[k] = (k == 0 || k == nn) ? 1ull : prev[k - 1] + prev[k];
+            for (int k = 0; k <= nn; k++) binom[nn * BINOM_N + k] = (double)row[k];
+            prev = row;
+        }
+    }
+    Arena a;
+    size_t o_blocks = a.add(blocks), o_lf = a.add(lf), o_off1 = a.add(off1), o_off2 = a.add(off2), o_bin = a.add(binom);
+    char* base = nullptr;
+    int rc = arena_upload(c, a, &base, st);
+    if (rc) return rc;
+    void* dcg = nullptr;
+    MFDN_CUDA(c, cudaMalloc(&dcg, pos * sizeof(double)));
+    c->owned.push_back(dcg);
+    dim3 grid(8, (unsigned)blocks.size());
+    k_cg_build<<<grid, 128, 0, st>>>((const CgBlock*)(base + o_blocks), (const double2*)(base + o_lf),
+                                     (const double*)(base + o_bin), (double*)dcg);
+    MFDN_CUDA(c, cudaGetLastError());
+    c->t.cg1 = (const double*)dcg;
+    c->t.cg2 = (const double*)dcg + c->n_cg1;
+    c->t.cg1_off = (const int32_t*)(base + o_off1);
+    c->t.cg2_off = (const int32_t*)(base + o_off2);
+    c->stage = 2;
+    return MFDN_OK;
+}
+
+extern "C" int mfdn_cg_download(mfdn_ctx* c, int stage, double* host_out, int64_t cap, int64_t* n)
+{
+    if (!c || !n || (stage != 1 && stage != 2)) return MFDN_ERR_ARG;
+    if (c->stage < 2) return fail(c, MFDN_ERR_STATE, "mfdn_cg_download before mfdn_cg_build");
+    *n = stage == 1 ? c->n_cg1 : c->n_cg2;
+    MFDN_CUDA(c, cudaSetDevice(c->device));
+    MFDN_CUDA(c, cudaDeviceSynchronize());
+    if (host_out && cap >= *n)
+        MFDN_CUDA(c, cudaMemcpy(host_out, stage == 1 ? c->t.cg1 : c->t.cg2, *n * sizeof(double), cudaMemcpyDeviceToHost));
+    return MFDN_OK;
+}
+
+// ------------------------------------------------------------------------------------------ A2
+// Re-tiling kernels: channel-major squares -> group-major slabs in kernel loop order (PAPER.md:61
+// "arranged in the order that the nested loops will reference them").
+struct Retile3 {
+    int n_tup;
+    const int4* tdesc;
+    const uint32_t* slab_off;
+    const int32_t* rowmap;
+    const int32_t* chan_of;   // [(twoJ>>1)*4 + (twoT>>1)*2 + par]
+    const int64_t* chan_off;
+    const int32_t* chan_dim;
+    const double* values;
+    double* slab;
+};
+
+__device__ __forceinline__ void j12_range(int4 d, int twoJ, int& lo, int& hi)
+{
+    int jc = (d.x >> 16) & 255;
+    lo = max(d.y & 255, abs(twoJ - jc) >> 1);
+    hi = min((d.y >> 8) & 255, (twoJ + jc) >> 1);
+}
+
+__global__ void k_retile3(Retile3 p)
+{
+    for (long long g = blockIdx.x; g < (long long)p.n_tup * p.n_tup; g += gridDim.x) {
+        uint32_t so = p.slab_off[g];
+        if (so == NO_SLAB) continue;
+        int tb = (int)(g / p.n_tup), tk = (int)(g % p.n_tup);
+        int4 db = p.tdesc[tb], dk = p.tdesc[tk];
+        int par = (db.x >> 25) & 1;
+        int Jlo = max((db.y >> 16) & 255, (dk.y >> 16) & 255), Jhi = min((db.y >> 24) & 255, (dk.y >> 24) & 255);
+        int nJb = (((db.y >> 24) & 255) - ((db.y >> 16) & 255)) / 2 + 1, nJk = (((dk.y >> 24) & 255) - ((dk.y >> 16) & 255)) / 2 + 1;
+        double* dst = p.slab + (size_t)so * CELL3;
+        for (int twoJ = Jlo; twoJ <= Jhi; twoJ += 2) {
+            int lb, hb, lk, hk;
+            j12_range(db, twoJ, lb, hb);
+            j12_range(dk, twoJ, lk, hk);
+            int nb = hb - lb + 1, nk = hk - lk + 1;
+            if (nb <= 0 || nk <= 0) continue;
+            int iJb = (twoJ - ((db.y >> 16) & 255)) / 2, iJk = (twoJ - ((dk.y >> 16) & 255)) / 2;
+            for (int idx = threadIdx.x; idx < nb * nk * CELL3; idx += blockDim.x) {
+                int slot = idx % CELL3, cell = idx / CELL3;
+                int i = cell / nk, k = cell % nk;
+                double v = 0.0;
+                if (slot < 5) {
+                    int T12 = slot >> 1 & 1, T12p = slot & 1, Ti = 0;
+                    if (slot == 4) { T12 = 1; T12p = 1; Ti = 1; }
+                    int ch = p.chan_of[(twoJ >> 1) * 4 + Ti * 2 + par];
+                    if (ch >= 0) {
+                        int r = p.rowmap[db.w + ((((lb + i) - (db.y & 255)) * 2 + T12) * nJb + iJb) * 2 + Ti];
+                        int q = p.rowmap[dk.w + ((((lk + k) - (dk.y & 255)) * 2 + T12p) * nJk + iJk) * 2 + Ti];
+                        if (r >= 0 && q >= 0) v = p.values[p.chan_off[ch] + (long long)r * p.chan_dim[ch] + q];
+                    }
+                }
+                dst[idx] = v;
+            }
+            dst += (size_t)nb * nk * CELL3;
+        }
+    }
+}
+
+struct Retile2 {
+    int n_tup;
+    const int4* tdesc;
+    const uint32_t* slab_off;
+    const int32_t* rowmap;
+    const int32_t* rowmap_off;
+    const int32_t* chan_of;   // [J*4 + T*2 + par]
+    const int64_t* chan_off;
+    const int32_t* chan_dim;
+    const double* values;
+    double* slab;
+};
+
+__global__ void k_retile2(Retile2 p)
+{
+    long long total = (long long)p.n_tup * p.n_tup;
+    for (long long g = blockIdx.x * (long long)blockDim.x + threadIdx.x; g < total; g += (long long)gridDim.x * blockDim.x) {
+        uint32_t so = p.slab_off[g];
+        if (so == NO_SLAB) continue;
+        int tb = (int)(g / p.n_tup), tk = (int)(g % p.n_tup);
+        int4 db = p.tdesc[tb], dk = p.tdesc[tk];
+        int par = (db.x >> 25) & 1;
+        int Jlo = max(db.y & 255, dk.y & 255), Jhi = min((db.y >> 8) & 255, (dk.y >> 8) & 255);
+        double* dst = p.slab + (size_t)so * CELL2;
+        for (int J = Jlo; J <= Jhi; J++)
+            for (int T = 0; T < 2; T++) {
+                double v = 0.0;
+                int ch = p.chan_of[J * 4 + T * 2 + par];
+                if (ch >= 0) {
+                    int r = p.rowmap[p.rowmap_off[tb] + (J - (db.y & 255)) * 2 + T];
+                    int q = p.rowmap[p.rowmap_off[tk] + (J - (dk.y & 255)) * 2 + T];
+                    if (r >= 0 && q >= 0) v = p.values[p.chan_off[ch] + (long long)r * p.chan_dim[ch] + q];
+                }
+                *dst++ = v;
+            }
+    }
+}
+
+static int stage_values(mfdn_ctx* c, const double* values, int on_device, int64_t count, cudaStream_t st,
+                        const double** dvals, void** tmp)
+{
+    *tmp = nullptr;
+    if (on_device) { *dvals = values; return MFDN_OK; }
+    MFDN_CUDA(c, cudaMalloc(tmp, std::max<int64_t>(count, 1) * sizeof(double)));
+    MFDN_CUDA(c, cudaMemcpyAsync(*tmp, values, count * sizeof(double), cudaMemcpyHostToDevice, st));
+    *dvals = (const double*)*tmp;
+    return MFDN_OK;
+}
+
+extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan, const int32_t* chan_twoJ,
+                                      const int32_t* chan_twoT, const int32_t* chan_par, const int32_t* chan_dim,
+                                      const int64_t* chan_off, const int32_t* state_a, const int32_t* state_b,
+                                      const int32_t* state_c, const int32_t* state_J12, const int32_t* state_T12,
+                                      const double* values, int values_on_device, void* stream)
+{
+    if (!c) return MFDN_ERR_ARG;
+    if (c->stage < 2) return fail(c, MFDN_ERR_STATE, "mfdn_coupled_upload_3b before mfdn_cg_build");
+    if (c->has3) return fail(c, MFDN_ERR_STATE, "3-body table already uploaded");
+    if (n_chan <= 0 || !chan_twoJ || !chan_twoT || !chan_par || !chan_dim || !chan_off || !state_a || !state_b ||
+        !state_c || !state_J12 || !state_T12 || !values || e3max < 0)
+        return fail(c, MFDN_ERR_ARG, "null or empty argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    MFDN_CUDA(c, cudaSetDevice(c->device));
+    const int No = c->t.n_orb;
+    const auto& tj = c->orb_twoj;
+    // ---- validate channels, collect tuples
+    std::vector<int32_t> chan_of(32 * 4, -1);
+    int64_t n_states = 0, n_values = 0;
+    for (int ch = 0; ch < n_chan; ch++) {
+        int J = chan_twoJ[ch], T = chan_twoT[ch], P = chan_par[ch];
+        if (J < 1 || !(J & 1) || J > 3 * MAX_TWOJ || (T != 1 && T != 3) || (P != 0 && P != 1) || chan_dim[ch] < 0 || chan_off[ch] < 0)
+            return fail(c, MFDN_ERR_TABLE, "bad channel quantum numbers");
+        int32_t& slot = chan_of[(J >> 1) * 4 + (T >> 1) * 2 + P];
+        if (slot >= 0) return fail(c, MFDN_ERR_TABLE, "duplicate channel");
+        slot = ch;
+        n_states += chan_dim[ch];
+        n_values = std::max<int64_t>(n_values, chan_off[ch] + (int64_t)chan_dim[ch] * chan_dim[ch]);
+    }
+    std::vector<int64_t> tkeys;
+    tkeys.reserve(n_states);
+    {
+        int64_t s = 0;
+        for (int ch = 0; ch < n_chan; ch++)
+            for (int r = 0; r < chan_dim[ch]; r++, s++) {
+                int a = state_a[s], b = state_b[s], cc = state_c[s], J12 = state_J12[s], T12 = state_T12[s];
+                if (a < 0 || a > b || b > cc || cc >= No) return fail(c, MFDN_ERR_TABLE, "state orbitals not a<=b<=c in range");
+                int e = 2 * (c->orb_n[a] + c->orb_n[b] + c->orb_n[cc]) + c->orb_l[a] + c->orb_l[b] + c->orb_l[cc];
+                if (e > e3max) return fail(c, MFDN_ERR_TABLE, "state above E3max");
+                if (((c->orb_l[a] + c->orb_l[b] + c->orb_l[cc]) & 1) != chan_par[ch]) return fail(c, MFDN_ERR_TABLE, "state parity != channel parity");
+                if (T12 < 0 || T12 > 1 || 2 * J12 < std::abs(tj[a] - tj[b]) || 2 * J12 > tj[a] + tj[b])
+                    return fail(c, MFDN_ERR_TABLE, "J12/T12 triangle");
+                if (a == b && !((J12 + T12) & 1)) return fail(c, MFDN_ERR_TABLE, "a==b needs J12+T12 odd");
+                if (chan_twoJ[ch] < std::abs(2 * J12 - tj[cc]) || chan_twoJ[ch] > 2 * J12 + tj[cc]) return fail(c, MFDN_ERR_TABLE, "J triangle");
+                if (chan_twoT[ch] < std::abs(2 * T12 - 1) || chan_twoT[ch] > 2 * T12 + 1) return fail(c, MFDN_ERR_TABLE, "T triangle");
+                tkeys.push_back(((int64_t)a * No + b) * No + cc);
+            }
+    }
+    std::vector<int64_t> tuples = tkeys;
+    std::sort(tuples.begin(), tuples.end());
+    tuples.erase(std::unique(tuples.begin(), tuples.end()), tuples.end());
+    const int nt = (int)tuples.size();
+    if (nt == 0) return fail(c, MFDN_ERR_TABLE, "empty table");
+    std::vector<int32_t> tuple_id((size_t)No * No * No, -1);
+    std::vector<int4> tdesc(nt);
+    std::vector<int32_t> nJ12v(nt), nJv(nt);
+    size_t rm_size = 0, sm_size = 0;
+    for (int t = 0; t < nt; t++) {
+        int64_t k = tuples[t];
+        int a = (int)(k / ((int64_t)No * No)), b = (int)((k / No) % No), cc = (int)(k % No);
+        tuple_id[k] = t;
+        int ja = tj[a], jb = tj[b], jc = tj[cc];
+        int J12min = std::abs(ja - jb) / 2, J12max = (ja + jb) / 2;
+        int twoJmin = 1 << 30;
+        for (int J12 = J12min; J12 <= J12max; J12++) twoJmin = std::min(twoJmin, std::abs(2 * J12 - jc));
+        int twoJmax = ja + jb + jc;
+        int par = (c->orb_l[a] + c->orb_l[b] + c->orb_l[cc]) & 1;
+        nJ12v[t] = J12max - J12min + 1;
+        nJv[t] = (twoJmax - twoJmin) / 2 + 1;
+        tdesc[t].x = ja | (jb << 8) | (jc << 16) | ((a == b) << 24) | (par << 25);
+        tdesc[t].y = J12min | (J12max << 8) | (twoJmin << 16) | (twoJmax << 24);
+        tdesc[t].z = (int)sm_size;
+        tdesc[t].w = (int)rm_size;
+        sm_size += (size_t)nJ12v[t] * 2;
+        rm_size += (size_t)nJ12v[t] * 2 * nJv[t] * 2;
+    }
+    std::vector<int32_t> rowmap(rm_size, -1);
+    std::vector<unsigned long long> stmask(sm_size, 0ull);
+    {
+        int64_t s = 0;
+        for (int ch = 0; ch < n_chan; ch++)
+            for (int r = 0; r < chan_dim[ch]; r++, s++) {
+                int t = tuple_id[tkeys[s]];
+                int4 d = tdesc[t];
+                int i12 = state_J12[s] - (d.y & 255), T12 = state_T12[s];
+                int iJ = (chan_twoJ[ch] - ((d.y >> 16) & 255)) / 2, Ti = chan_twoT[ch] >> 1;
+                int32_t& slot = rowmap[d.w + ((size_t)(i12 * 2 + T12) * nJv[t] + iJ) * 2 + Ti];
+                if (slot >= 0) return fail(c, MFDN_ERR_TABLE, "duplicate state in channel");
+                slot = r;
+                stmask[d.z + i12 * 2 + T12] |= 1ull << ((chan_twoJ[ch] >> 1) * 2 + Ti);
+            }
+    }
+    // ---- slab offsets: cells per (bra tuple, ket tuple) group in loop order J, J12, J12'
+    std::vector<uint32_t> slab_off((size_t)nt * nt, NO_SLAB);
+    uint64_t cells = 0;
+    auto range = [&](int4 d, int twoJ, int& lo, int& hi) {
+        int jc = (d.x >> 16) & 255;
+        lo = std::max(d.y & 255, std::abs(twoJ - jc) >> 1);
+        hi = std::min((d.y >> 8) & 255, (twoJ + jc) >> 1);
+    };
+    for (int tb = 0; tb < nt; tb++)
+        for (int tk = 0; tk < nt; tk++) {
+            int4 db = tdesc[tb], dk = tdesc[tk];
+            if (((db.x ^ dk.x) >> 25) & 1) continue;
+            int Jlo = std::max((db.y >> 16) & 255, (dk.y >> 16) & 255), Jhi = std::min((db.y >> 24) & 255, (dk.y >> 24) & 255);
+            uint64_t n = 0;
+            for (int twoJ = Jlo; twoJ <= Jhi; twoJ += 2) {
+                int lb, hb, lk, hk;
+                range(db, twoJ, lb, hb);
+                range(dk, twoJ, lk, hk);
+                if (hb >= lb && hk >= lk) n += (uint64_t)(hb - lb + 1) * (hk - lk + 1);
+            }
+            if (n == 0) continue;
+            if (cells + n >= 0xFFFFFFF0ull) return fail(c, MFDN_ERR_OOM, "table too large for 32-bit cell offsets");
+            slab_off[(size_t)tb * nt + tk] = (uint32_t)cells;
+            cells += n;
+        }
+    // ---- one arena for the resident index tables, one for the upload-only ones
+    Arena res, tmp;
+    size_t o_tid = res.add(tuple_id), o_desc = res.add(tdesc), o_soff = res.add(slab_off), o_sm = res.add(stmask);
+    std::vector<int64_t> coff(chan_off, chan_off + n_chan);
+    std::vector<int32_t> cdim(chan_dim, chan_dim + n_chan);
+    size_t o_rm = tmp.add(rowmap), o_cof = tmp.add(chan_of), o_coff = tmp.add(coff), o_cdim = tmp.add(cdim);
+    char* dres = nullptr;
+    int rc = arena_upload(c, res, &dres, st);
+    if (rc) return rc;
+    void* dtmp = nullptr;
+    MFDN_CUDA(c, cudaMalloc(&dtmp, tmp.buf.size()));
+    MFDN_CUDA(c, cudaMemcpyAsync(dtmp, tmp.buf.data(), tmp.buf.size(), cudaMemcpyHostToDevice, st));
+    const double* dvals = nullptr;
+    void* vtmp = nullptr;
+    rc = stage_values(c, values, values_on_device, n_values, st, &dvals, &vtmp);
+    if (rc) { cudaFree(dtmp); return rc; }
+    void* dslab = nullptr;
+    cudaError_t e = cudaMalloc(&dslab, std::max<uint64_t>(cells, 1) * CELL3 * sizeof(double));
+    if (e != cudaSuccess) { cudaFree(dtmp); if (vtmp) cudaFree(vtmp); return cuda_fail(c, e, "cudaMalloc(slab3)"); }
+    c->owned.push_back(dslab);
+    Retile3 p;
+    p.n_tup = nt;
+    p.tdesc = (const int4*)(dres + o_desc);
+    p.slab_off = (const uint32_t*)(dres + o_soff);
+    p.rowmap = (const int32_t*)((char*)dtmp + o_rm);
+    p.chan_of = (const int32_t*)((char*)dtmp + o_cof);
+    p.chan_off = (const int64_t*)((char*)dtmp + o_coff);
+    p.chan_dim = (const int32_t*)((char*)dtmp + o_cdim);
+    p.values = dvals;
+    p.slab = (double*)dslab;
+    long long groups = (long long)nt * nt;
+    k_retile3<<<(unsigned)std::min<long long>(groups, 1 << 20), 64, 0, st>>>(p);
+    e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(dtmp);
+    if (vtmp) cudaFree(vtmp);
+    if (e != cudaSuccess) return cuda_fail(c, e, "k_retile3");
+    c->t.n_tup3 = nt;
+    c->t.e3max = e3max;
+    c->t.tuple_id3 = (const int32_t*)(dres + o_tid);
+    c->t.tdesc3 = p.tdesc;
+    c->t.slab_off3 = p.slab_off;
+    c->t.slab3 = (const double*)dslab;
+    c->t.stmask3 = (const unsigned long long*)(dres + o_sm);
+    c->slab_bytes3 = (int64_t)(cells * CELL3 * sizeof(double));
+    c->has3 = true;
+    return MFDN_OK;
+}
+
+extern "C" int mfdn_coupled_upload_2b(mfdn_ctx* c, int32_t n_chan, const int32_t* chan_J, const int32_t* chan_T,
+                                      const int32_t* chan_par, const int32_t* chan_dim, const int64_t* chan_off,
+                                      const int32_t* state_a, const int32_t* state_b, const double* values,
+                                      int values_on_device, void* stream)
+{
+    if (!c) return MFDN_ERR_ARG;
+    if (c->stage < 2) return fail(c, MFDN_ERR_STATE, "mfdn_coupled_upload_2b before mfdn_cg_build");
+    if (c->has2) return fail(c, MFDN_ERR_STATE, "2-body table already uploaded");
+    if (n_chan <= 0 || !chan_J || !chan_T || !chan_par || !chan_dim || !chan_off || !state_a || !state_b || !values)
+        return fail(c, MFDN_ERR_ARG, "null or empty argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    MFDN_CUDA(c, cudaSetDevice(c->device));
+    const int No = c->t.n_orb;
+    const auto& tj = c->orb_twoj;
+    std::vector<int32_t> chan_of(32 * 4, -1);
+    int64_t n_states = 0, n_values = 0;
+    for (int ch = 0; ch < n_chan; ch++) {
+        int J = chan_J[ch], T = chan_T[ch], P = chan_par[ch];
+        if (J < 0 || J > MAX_TWOJ || (T != 0 && T != 1) || (P != 0 && P != 1) || chan_dim[ch] < 0 || chan_off[ch] < 0)
+            return fail(c, MFDN_ERR_TABLE, "bad channel quantum numbers");
+        int32_t& slot = chan_of[J * 4 + T * 2 + P];
+        if (slot >= 0) return fail(c, MFDN_ERR_TABLE, "duplicate channel");
+        slot = ch;
+        n_states += chan_dim[ch];
+        n_values = std::max<int64_t>(n_values, chan_off[ch] + (int64_t)chan_dim[ch] * chan_dim[ch]);
+    }
+    std::vector<int64_t> tkeys;
+    tkeys.reserve(n_states);
+    {
+        int64_t s = 0;
+        for (int ch = 0; ch < n_chan; ch++)
+            for (int r = 0; r < chan_dim[ch]; r++, s++) {
+                int a = state_a[s], b = state_b[s];
+                if (a < 0 || a > b || b >= No) return fail(c, MFDN_ERR_TABLE, "state orbitals not a<=b in range");
+                if (((c->orb_l[a] + c->orb_l[b]) & 1) != chan_par[ch]) return fail(c, MFDN_ERR_TABLE, "state parity != channel parity");
+                if (2 * chan_J[ch] < std::abs(tj[a] - tj[b]) || 2 * chan_J[ch] > tj[a] + tj[b]) return fail(c, MFDN_ERR_TABLE, "J triangle");
+                if (a == b && !((chan_J[ch] + chan_T[ch]) & 1)) return fail(c, MFDN_ERR_TABLE, "a==b needs J+T odd");
+                tkeys.push_back((int64_t)a * No + b);
+            }
+    }
+    std::vector<int64_t> tuples = tkeys;
+    std::sort(tuples.begin(), tuples.end());
+    tuples.erase(std::unique(tuples.begin(), tuples.end()), tuples.end());
+    const int nt = (int)tuples.size();
+    if (nt == 0) return fail(c, MFDN_ERR_TABLE, "empty table");
+    std::vector<int32_t> tuple_id((size_t)No * No, -1), rowmap_off(nt);
+    std::vector<int4> tdesc(nt);
+    size_t rm_size = 0;
+    for (int t = 0; t < nt; t++) {
+        int a = (int)(tuples[t] / No), b = (int)(tuples[t] % No);
+        tuple_id[tuples[t]] = t;
+        int Jmin = std::abs(tj[a] - tj[b]) / 2, Jmax = (tj[a] + tj[b]) / 2;
+        int par = (c->orb_l[a] + c->orb_l[b]) & 1;
+        tdesc[t].x = tj[a] | (tj[b] << 8) | ((a == b) << 24) | (par << 25);
+        tdesc[t].y = Jmin | (Jmax << 8);
+        tdesc[t].z = tdesc[t].w = 0;
+        rowmap_off[t] = (int32_t)rm_size;
+        rm_size += (size_t)(Jmax - Jmin + 1) * 2;
+    }
+    std::vector<int32_t> rowmap(rm_size, -1);
+    {
+        int64_t s = 0;
+        for (int ch = 0; ch < n_chan; ch++)
+            for (int r = 0; r < chan_dim[ch]; r++, s++) {
+                int t = tuple_id[tkeys[s]];
+                int32_t& slot = rowmap[rowmap_off[t] + (chan_J[ch] - (tdesc[t].y & 255)) * 2 + chan_T[ch]];
+                if (slot >= 0) return fail(c, MFDN_ERR_TABLE, "duplicate state in channel");
+                slot = r;
+                unsigned long long m = ((unsigned long long)(uint32_t)tdesc[t].z) | ((unsigned long long)(uint32_t)tdesc[t].w << 32);
+                m |= 1ull << (chan_J[ch] * 2 + chan_T[ch]);
+                tdesc[t].z = (int)(uint32_t)(m & 0xFFFFFFFFu);
+                tdesc[t].w = (int)(uint32_t)(m >> 32);
+            }
+    }
+    std::vector<uint32_t> slab_off((size_t)nt * nt, NO_SLAB);
+    uint64_t cells = 0;
+    for (int tb = 0; tb < nt; tb++)
+        for (int tk = 0; tk < nt; tk++) {
+            int4 db = tdesc[tb], dk = tdesc[tk];
+            if (((db.x ^ dk.x) >> 25) & 1) continue;
+            int Jlo = std::max(db.y & 255, dk.y & 255), Jhi = std::min((db.y >> 8) & 255, (dk.y >> 8) & 255);
+            if (Jhi < Jlo) continue;
+            if (cells + (Jhi - Jlo + 1) >= 0xFFFFFFF0ull) return fail(c, MFDN_ERR_OOM, "table too large for 32-bit cell offsets");
+            slab_off[(size_t)tb * nt + tk] = (uint32_t)cells;
+            cells += Jhi - Jlo + 1;
+        }
+    Arena res, tmp;
+    size_t o_tid = res.add(tuple_id), o_desc = res.add(tdesc), o_soff = res.add(slab_off);
+    std::vector<int64_t> coff(chan_off, chan_off + n_chan);
+    std::vector<int32_t> cdim(chan_dim, chan_dim + n_chan);
+    size_t o_rm = tmp.add(rowmap), o_rmo = tmp.add(rowmap_off), o_cof = tmp.add(chan_of), o_coff = tmp.add(coff), o_cdim = tmp.add(cdim);
+    char* dres = nullptr;
+    int rc = arena_upload(c, res, &dres, st);
+    if (rc) return rc;
+    void* dtmp = nullptr;
+    MFDN_CUDA(c, cudaMalloc(&dtmp, tmp.buf.size()));
+    MFDN_CUDA(c, cudaMemcpyAsync(dtmp, tmp.buf.data(), tmp.buf.size(), cudaMemcpyHostToDevice, st));
+    const double* dvals = nullptr;
+    void* vtmp = nullptr;
+    rc = stage_values(c, values, values_on_device, n_values, st, &dvals, &vtmp);
+    if (rc) { cudaFree(dtmp); return rc; }
+    void* dslab = nullptr;
+    cudaError_t e = cudaMalloc(&dslab, std::max<uint64_t>(cells, 1) * CELL2 * sizeof(double));
+    if (e != cudaSuccess) { cudaFree(dtmp); if (vtmp) cudaFree(vtmp); return cuda_fail(c, e, "cudaMalloc(slab2)"); }
+    c->owned.push_back(dslab);
+    Retile2 p;
+    p.n_tup = nt;
+    p.tdesc = (const int4*)(dres + o_desc);
+    p.slab_off = (const uint32_t*)(dres + o_soff);
+    p.rowmap = (const int32_t*)((char*)dtmp + o_rm);
+    p.rowmap_off = (const int32_t*)((char*)dtmp + o_rmo);
+    p.chan_of = (const int32_t*)((char*)dtmp + o_cof);
+    p.chan_off = (const int64_t*)((char*)dtmp + o_coff);
+    p.chan_dim = (const int32_t*)((char*)dtmp + o_cdim);
+    p.values = dvals;
+    p.slab = (double*)dslab;
+    long long groups = (long long)nt * nt;
+    k_retile2<<<(unsigned)std::min<long long>((groups + 127) / 128, 1 << 16), 128, 0, st>>>(p);
+    e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(dtmp);
+    if (vtmp) cudaFree(vtmp);
+    if (e != cudaSuccess) return cuda_fail(c, e, "k_retile2");
+    c->t.n_tup2 = nt;
+    c->t.tuple_id2 = (const int32_t*)(dres + o_tid);
+    c->t.tdesc2 = p.tdesc;
+    c->t.slab_off2 = p.slab_off;
+    c->t.slab2 = (const double*)dslab;
+    c->slab_bytes2 = (int64_t)(cells * CELL2 * sizeof(double));
+    c->has2 = true;
+    return MFDN_OK;
+}
+
+// ------------------------------------------------------------------------------------------ misc
+extern "C" int64_t mfdn_bad_request_count(mfdn_ctx* c, void* stream)
+{
+    if (!c || c->stage < 1) return -1;
+    unsigned long long v = 0;
+    cudaSetDevice(c->device);
+    if (cudaStreamSynchronize((cudaStream_t)stream) != cudaSuccess) return -1;
+    if (cudaMemcpy(&v, c->t.bad_count, sizeof(v), cudaMemcpyDeviceToHost) != cudaSuccess) return -1;
+    return (int64_t)v;
+}
+
+extern "C" int64_t mfdn_info(mfdn_ctx* c, int which)
+{
+    if (!c) return -1;
+    switch (which) {
+        case 0: return c->t.n_tup2;
+        case 1: return c->t.n_tup3;
+        case 2: return c->slab_bytes2;
+        case 3: return c->slab_bytes3;
+        case 4: return c->n_cg1;
+        case 5: return c->n_cg2;
+        case 6: return c->launches;
+        default: return -1;
+    }
+}
+
+extern "C" const char* mfdn_last_error(mfdn_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+extern "C" void mfdn_destroy(mfdn_ctx* c)
+{
+    if (!c) return;
+    cudaSetDevice(c->device);
+    for (void* p : c->owned) cudaFree(p);
+    delete c;
+}

@@ -1,0 +1,95 @@
+// Internal layout of the device tables (N0) shared by the host API and the kernels.
+// Not part of the ABI.  Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#include "../../include/mfdn_b200.h"
+
+namespace mfdn {
+
+// ---- SPS record (A0): one 32-bit word per single-particle state -------------------------------
+//  [0,10) orbital   [10,15) im = (2m+2j)/2   [15] tz bit (1 <=> 2tz = +1)
+//  [16,21) 2j       [21,27) e = 2n+l         [27] l & 1
+__host__ __device__ inline uint32_t sps_pack(int orb, int im, int tzbit, int twoj, int e, int lpar)
+{
+    return (uint32_t)orb | ((uint32_t)im << 10) | ((uint32_t)tzbit << 15) | ((uint32_t)twoj << 16) |
+           ((uint32_t)e << 21) | ((uint32_t)lpar << 27);
+}
+__host__ __device__ inline int rec_orb(uint32_t r) { return r & 1023; }
+__host__ __device__ inline int rec_im(uint32_t r) { return (r >> 10) & 31; }
+__host__ __device__ inline int rec_tz(uint32_t r) { return (r >> 15) & 1; }
+__host__ __device__ inline int rec_twoj(uint32_t r) { return (r >> 16) & 31; }
+__host__ __device__ inline int rec_e(uint32_t r) { return (r >> 21) & 63; }
+__host__ __device__ inline int rec_lpar(uint32_t r) { return (r >> 27) & 1; }
+
+constexpr int MAX_TWOJ = 21;       // 3*MAX_TWOJ <= 63 so that (2J,2T) fits a 64-bit channel mask
+constexpr int CELL3 = 6;           // doubles per 3-body slab cell: 5 isospin slots + 1 pad (48 B)
+constexpr int CELL2 = 2;           // doubles per 2-body slab cell: T = 0, 1 (16 B)
+constexpr uint32_t NO_SLAB = 0xFFFFFFFFu;
+
+// ---- per-tuple descriptor (A2), 16 bytes ---------------------------------------------------------
+// 3-body: x = ja | jb<<8 | jc<<16 | (a==b)<<24 | par<<25      (ja.. are 2j)
+//         y = J12min | J12max<<8 | twoJmin<<16 | twoJmax<<24
+//         z = offset of the tuple's state masks in stmask3 (entries: [J12-J12min][T12])
+//         w = offset of the tuple's row map (upload only)
+// 2-body: x = ja | jb<<8 | (a==b)<<24 | par<<25,  y = Jmin | Jmax<<8,  z = state mask (low), w = (high)
+struct Tables {
+    // A0
+    const uint32_t* sps_rec;
+    int n_sps, n_orb;
+    // A1: CG tables.  nj = number of half-integer j values (2j = 1,3,..,2*nj-1)
+    int nj;
+    const double* cg1;       // stage 1 blocks [(2j1-1)/2 * nj + (2j2-1)/2]
+    const int32_t* cg1_off;
+    const double* cg2;       // stage 2 blocks [J12 * nj + (2j-1)/2],  J12 = 0..2*nj-1
+    const int32_t* cg2_off;
+    double iso3[8][3];       // [ta<<2|tb<<1|tc][(T12,T) = (0,1/2),(1,1/2),(1,3/2)]
+    double iso2[4][2];       // [ta<<1|tb][T]
+    // A2, 3-body
+    int n_tup3, e3max;
+    const int32_t* tuple_id3;      // [n_orb^3] -> tuple or -1
+    const int4* tdesc3;
+    const uint32_t* slab_off3;     // [n_tup3^2] first cell of the group's slab or NO_SLAB
+    const double* slab3;           // cells of CELL3 doubles
+    const unsigned long long* stmask3;
+    // A2, 2-body
+    int n_tup2;
+    const int32_t* tuple_id2;      // [n_orb^2]
+    const int4* tdesc2;
+    const uint32_t* slab_off2;
+    const double* slab2;
+    unsigned long long* bad_count;
+};
+
+}  // namespace mfdn
+
+struct mfdn_ctx {
+    int device = 0;
+    int stage = 0;  // 1 orbitals, 2 cg built
+    bool has2 = false, has3 = false;
+    std::string err;
+    mfdn::Tables t{};
+    int tjmax = 0;
+    // host copies
+    std::vector<int32_t> orb_n, orb_l, orb_twoj;
+    std::vector<uint32_t> h_sps_rec;
+    std::vector<void*> owned;  // device allocations
+    int64_t n_cg1 = 0, n_cg2 = 0;
+    int64_t slab_bytes2 = 0, slab_bytes3 = 0;
+    int64_t launches = 0;
+    int num_sms = 148;
+};
+
+namespace mfdn {
+int fail(mfdn_ctx* c, int code, const std::string& msg);
+int cuda_fail(mfdn_ctx* c, cudaError_t e, const char* what);
+}  // namespace mfdn
+
+#define MFDN_CUDA(ctx, call)                                                  \
+    do {                                                                      \
+        cudaError_t e__ = (call);                                             \
+        if (e__ != cudaSuccess) return mfdn::cuda_fail((ctx), e__, #call);    \
+    } while (0)

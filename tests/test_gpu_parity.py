@@ -1,0 +1,270 @@
+"""GPU parity tests proper: the CUDA path (through the C ABI) against the CPU oracle, element by element,
+on the same seeded inputs.  Bars (BASELINE.json north_star): max|delta| <= 1e-12 * max|V| in fp64;
+selection mask bit-exact."""
+import numpy as np
+import pytest
+
+from paper_1412_5989_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-12
+MODES = {"sorted_internally": 0, "naive": 2}
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    return torch
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_1412_5989_b200 import binding
+    return binding
+
+
+@pytest.fixture(scope="module")
+def oracle():
+    from oracle import mscheme_c
+    return mscheme_c
+
+
+_cfg_cache = {}
+
+
+def get_cfg(i):
+    if i not in _cfg_cache:
+        _cfg_cache[i] = W.make_config(i)
+    return _cfg_cache[i]
+
+
+_ctx_cache = {}
+
+
+def get_ctx(B, i):
+    if i not in _ctx_cache:
+        cfg = get_cfg(i)
+        _ctx_cache[i] = B.Context(cfg.basis, 0).upload(cfg.table)
+    return _ctx_cache[i]
+
+
+def run_gpu(torch, ctx, req, flags=0):
+    d_req = torch.from_numpy(np.ascontiguousarray(req, np.int32)).cuda()
+    out, mask = ctx.mscheme(d_req, flags=flags)
+    torch.cuda.synchronize()
+    return out.cpu().numpy(), mask.cpu().numpy()
+
+
+def presort(torch, ctx, req):
+    d_req = torch.from_numpy(np.ascontiguousarray(req, np.int32)).cuda()
+    keys = ctx.group_keys(d_req).cpu().numpy().view(np.uint32)
+    order = np.argsort(keys, kind="stable")
+    return req[order], order
+
+
+def check(cfg, got, gmask, want, wmask):
+    vmax = float(np.max(np.abs(cfg.table.values)))
+    assert np.array_equal(gmask, wmask), f"mask differs at {np.nonzero(gmask != wmask)[0][:10]}"
+    err = float(np.max(np.abs(got - want))) if len(got) else 0.0
+    assert err <= TOL * vmax, f"max|delta| {err:.3e} > {TOL * vmax:.3e}"
+    assert np.all(got[gmask == 0] == 0.0)
+    assert not np.any(np.signbit(got[gmask == 0]))
+
+
+# --------------------------------------------------------------------------------- CG tables
+@pytest.mark.parametrize("emax", [2, 8])
+def test_cg_tables_match_exact(torch, B, emax):
+    """A1: every entry of the device tables against exact-rational values (gate 1e-15)."""
+    from oracle.cg_exact import cg_exact
+    basis = W.ho_basis(emax)
+    ctx = B.Context(basis, 0)
+    nj = (int(basis.twoj.max()) + 1) // 2
+    rng = np.random.default_rng(0)
+    for stage in (1, 2):
+        tab = B.mfdn_cg_download(ctx.ctx, stage)
+        pos = 0
+        worst = 0.0
+        firsts = [2 * a + 1 for a in range(nj)] if stage == 1 else [2 * J for J in range(2 * nj)]
+        for tj1 in firsts:
+            for tj2 in [2 * b + 1 for b in range(nj)]:
+                nJ = min(tj1, tj2) + 1
+                cnt = (tj1 + 1) * (tj2 + 1) * nJ
+                blk = tab[pos:pos + cnt].reshape(tj1 + 1, tj2 + 1, nJ)
+                pos += cnt
+                # all entries for small blocks, a random sample for big ones (exact arithmetic is slow)
+                idx = np.ndindex(blk.shape) if cnt <= 400 else \
+                    [np.unravel_index(k, blk.shape) for k in rng.choice(cnt, 150, replace=False)]
+                for (i1, i2, iJ) in idx:
+                    tm1, tm2, tJ = 2 * i1 - tj1, 2 * i2 - tj2, abs(tj1 - tj2) + 2 * iJ
+                    worst = max(worst, abs(blk[i1, i2, iJ] - cg_exact(tj1, tm1, tj2, tm2, tJ, tm1 + tm2)))
+        assert pos == len(tab)
+        assert worst <= 1e-15, f"stage {stage}: max CG error {worst:.2e}"
+    ctx.close()
+
+
+# --------------------------------------------------------------------------------- whole small configs
+@pytest.mark.parametrize("mode", list(MODES) + ["presorted"])
+@pytest.mark.parametrize("idx", [0, 2])
+def test_all_pairs_configs(torch, B, oracle, idx, mode):
+    cfg = get_cfg(idx)
+    ctx = get_ctx(B, idx)
+    req = cfg.requests()
+    want, wmask, _, _ = oracle.mscheme(cfg.basis, cfg.table, req)
+    if mode == "presorted":
+        sreq, order = presort(torch, ctx, req)
+        got, gmask = run_gpu(torch, ctx, sreq, B.MFDN_PRESORTED)
+        check(cfg, got, gmask, want[order], wmask[order])
+    else:
+        got, gmask = run_gpu(torch, ctx, req, MODES[mode])
+        check(cfg, got, gmask, want, wmask)
+    assert ctx.bad_request_count() == 0
+
+
+# --------------------------------------------------------------------------------- sampled large configs
+@pytest.mark.parametrize("idx,n", [(1, 1 << 20), (3, (1 << 19) + 77), (4, 1 << 18)])
+def test_sampled_configs_prefix(torch, B, oracle, idx, n):
+    """First n requests of the stream (with 1% randomly permuted particle lists: sign path), all modes."""
+    cfg = get_cfg(idx)
+    ctx = get_ctx(B, idx)
+    req = cfg.requests(n, permute_frac=0.01)
+    want, wmask, nt, _ = oracle.mscheme(cfg.basis, cfg.table, req)
+    assert 0.85 < wmask.mean() < 1.0
+    for mode, flags in MODES.items():
+        got, gmask = run_gpu(torch, ctx, req, flags)
+        check(cfg, got, gmask, want, wmask)
+    sreq, order = presort(torch, ctx, req)
+    got, gmask = run_gpu(torch, ctx, sreq, B.MFDN_PRESORTED)
+    check(cfg, got, gmask, want[order], wmask[order])
+
+
+# --------------------------------------------------------------------------------- edge cases
+@pytest.mark.parametrize("idx", [0, 2])
+def test_edge_sizes_and_bad_indices(torch, B, oracle, idx):
+    cfg = get_cfg(idx)
+    ctx = get_ctx(B, idx)
+    allreq = cfg.requests()
+    rng = np.random.default_rng(9)
+    for n in (0, 1, 31, 32, 33, 127, 128, 129, 4097):
+        req = allreq[rng.choice(len(allreq), n, replace=False)] if n else allreq[:0]
+        want, wmask, _, _ = oracle.mscheme(cfg.basis, cfg.table, req)
+        for flags in (0, 2):
+            got, gmask = run_gpu(torch, ctx, req, flags)
+            check(cfg, got, gmask, want, wmask)
+    # random (mostly forbidden) requests, duplicates inside bra/ket, and out-of-range SPS indices
+    width = allreq.shape[1]
+    req = rng.integers(0, cfg.basis.n_sps, size=(20000, width)).astype(np.int32)
+    req[:200, 0] = cfg.basis.n_sps
+    req[200:300, width - 1] = -1
+    req[300:400, 1] = 2 ** 31 - 1
+    before = ctx.bad_request_count()
+    want, wmask, _, nbad = oracle.mscheme(cfg.basis, cfg.table, req)
+    got, gmask = run_gpu(torch, ctx, req, 2)
+    check(cfg, got, gmask, want, wmask)
+    assert ctx.bad_request_count() - before == nbad == 400
+    got, gmask = run_gpu(torch, ctx, req, 0)
+    check(cfg, got, gmask, want, wmask)
+    # mask pointer may be NULL
+    d_req = torch.from_numpy(allreq[:1000].copy()).cuda()
+    out = torch.empty(1000, dtype=torch.float64, device="cuda")
+    body = width // 2
+    fn = B.mfdn_mscheme_3b if body == 3 else B.mfdn_mscheme_2b
+    need = fn(ctx.ctx, 1000, 0, 0, 0, 0, 0, 0)
+    work = torch.empty(need, dtype=torch.uint8, device="cuda")
+    fn(ctx.ctx, 1000, d_req.data_ptr(), out.data_ptr(), 0, work.data_ptr(), need, 0)
+    torch.cuda.synchronize()
+    want, *_ = oracle.mscheme(cfg.basis, cfg.table, allreq[:1000])
+    assert np.max(np.abs(out.cpu().numpy() - want)) <= TOL * np.max(np.abs(cfg.table.values))
+
+
+def test_order_chunk_and_stream_invariance(torch, B):
+    """Element values are independent of one another and of request order: any
+    permutation or chunking gives bitwise identical per-request results."""
+    cfg = get_cfg(2)
+    ctx = get_ctx(B, 2)
+    req = cfg.requests()
+    rng = np.random.default_rng(4)
+    req = req[rng.choice(len(req), 200000, replace=False)]
+    base, bmask = run_gpu(torch, ctx, req, 0)
+    perm = rng.permutation(len(req))
+    got, gmask = run_gpu(torch, ctx, req[perm], 0)
+    assert np.array_equal(got, base[perm]) and np.array_equal(gmask, bmask[perm])
+    naive, nmask = run_gpu(torch, ctx, req, 2)
+    assert np.array_equal(naive, base) and np.array_equal(nmask, bmask)
+    # chunks of ~20 000 (the paper's buffer size) on two streams
+    d_req = torch.from_numpy(req).cuda()
+    out = torch.empty(len(req), dtype=torch.float64, device="cuda")
+    mask = torch.empty(len(req), dtype=torch.uint8, device="cuda")
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    need = ctx.work_bytes(3, 20000)
+    works = [torch.empty(need, dtype=torch.uint8, device="cuda") for _ in streams]
+    torch.cuda.synchronize()
+    for k, lo in enumerate(range(0, len(req), 20000)):
+        hi = min(lo + 20000, len(req))
+        s = streams[k % 2]
+        with torch.cuda.stream(s):
+            ctx.mscheme(d_req[lo:hi], out[lo:hi], mask[lo:hi], 0, works[k % 2], s.cuda_stream)
+    torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy(), base) and np.array_equal(mask.cpu().numpy(), bmask)
+
+
+def test_call_order_and_table_validation(torch, B):
+    cfg = get_cfg(0)
+    b = cfg.basis
+    ctx = B.mfdn_orbitals_init(0, b.n, b.l, b.twoj, b.sps_orb, b.sps_twom, b.sps_twotz)
+    t = cfg.table
+    args = (t.chan_J, t.chan_T, t.chan_par, t.chan_dim, t.chan_off, t.state_a, t.state_b, t.values)
+    with pytest.raises(B.MfdnError) as e:
+        B.mfdn_coupled_upload_2b(ctx, *args)
+    assert e.value.code == B.MFDN_ERR_STATE
+    B.mfdn_cg_build(ctx)
+    with pytest.raises(B.MfdnError) as e:
+        B.mfdn_mscheme_2b(ctx, 10, 0, 0, 0, 0, 0)
+    assert e.value.code == B.MFDN_ERR_STATE
+    bad_T = t.chan_T.copy()
+    bad_T[0] = 1 - bad_T[0]                      # breaks "a == b only with J+T odd" or duplicates a channel
+    with pytest.raises(B.MfdnError) as e:
+        B.mfdn_coupled_upload_2b(ctx, t.chan_J, bad_T, *args[2:])
+    assert e.value.code == B.MFDN_ERR_TABLE
+    bad_a = t.state_a.copy()
+    bad_a[3] = b.n_orb
+    with pytest.raises(B.MfdnError) as e:
+        B.mfdn_coupled_upload_2b(ctx, *args[:5], bad_a, *args[6:])
+    assert e.value.code == B.MFDN_ERR_TABLE
+    B.mfdn_coupled_upload_2b(ctx, *args)        # a failed upload leaves the context usable
+    B.mfdn_destroy(ctx)
+
+
+# --------------------------------------------------------------------------------- full size, bench launch config
+def test_full_size_config3_sampled(torch, B, oracle):
+    """2^26 requests of config 3 in the configuration bench.py times (one call, internal sort and PRESORTED),
+    checked on 2^16 sampled outputs the oracle computes one by one + properties that hold at any size."""
+    cfg = get_cfg(3)
+    ctx = get_ctx(B, 3)
+    n = 1 << 26
+    req = cfg.requests(n)
+    d_req = torch.from_numpy(req).cuda()
+    out, mask = ctx.mscheme(d_req, flags=0)
+    torch.cuda.synchronize()
+    sample = np.random.default_rng(77).choice(n, 1 << 16, replace=False)
+    sample.sort()
+    want, wmask, _, _ = oracle.mscheme(cfg.basis, cfg.table, req[sample])
+    ds = torch.from_numpy(sample).cuda()
+    check(cfg, out[ds].cpu().numpy(), mask[ds].cpu().numpy(), want, wmask)
+    frac = float(mask.float().mean())
+    assert 0.975 < frac < 0.985                       # ~98.1% of sampled pairs have mask 1
+    assert bool((out[mask == 0] == 0).all())
+    # hermiticity at full size: swap bra and ket
+    d_swapped = torch.cat([d_req[:, 3:], d_req[:, :3]], dim=1).contiguous()
+    out2, mask2 = ctx.mscheme(d_swapped, flags=0)
+    torch.cuda.synchronize()
+    assert bool((mask2 == mask).all())
+    assert float((out2 - out).abs().max()) <= TOL * float(np.max(np.abs(cfg.table.values)))
+    del d_swapped, out2, mask2
+    # PRESORTED on the key-ordered multiset gives bitwise the same values
+    keys = ctx.group_keys(d_req)
+    order = torch.argsort(keys.view(torch.int32).to(torch.int64) & 0xFFFFFFFF)
+    d_sorted = d_req[order].contiguous()
+    out3, mask3 = ctx.mscheme(d_sorted, flags=B.MFDN_PRESORTED)
+    torch.cuda.synchronize()
+    assert bool((out3 == out[order]).all()) and bool((mask3 == mask[order]).all())
