@@ -103,6 +103,24 @@ int mfdn_mscheme_2b(mfdn_ctx*, int64_t n, const int32_t* d_req, double* d_out, u
 int mfdn_mscheme_3b(mfdn_ctx*, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_mask, void* d_work,
                     size_t* work_bytes, uint32_t flags, void* stream);
 
+/* The paper's wrapper ("transfer a chunk of 3-body element requests to the GPU, invoke the kernel,
+ * and transfer the results back"), for HOST request/result buffers (pinned memory recommended).  The n requests
+ * are cut into chunks of `chunk` (0 = library default) and H2D copy / transform / D2H copy of successive chunks
+ * overlap on two internal streams.  body = 2 or 3; h_mask may be NULL; flags as above (MFDN_PRESORTED then means
+ * the whole host array is group-ordered).  d_work/work_bytes: DEVICE scratch, queried with d_work == NULL.
+ * BLOCKING: returns after the last result byte has landed in h_out. */
+int mfdn_mscheme_host(mfdn_ctx*, int body, int64_t n, const int32_t* h_req, double* h_out, uint8_t* h_mask,
+                      void* d_work, size_t* work_bytes, uint32_t flags, int64_t chunk);
+
+/* Measurement hooks.  mfdn_profile(ctx, 1) makes every later mfdn_mscheme_2b/3b call bracket its group-sort
+ * kernels (H1-H2) and its transform kernel (H3-H6) with CUDA events on the call's stream; mfdn_profile_read
+ * synchronises those events, returns the accumulated milliseconds and call count since the last read and resets
+ * them.  mfdn_fp64_peak runs a register-resident DFMA micro-benchmark on all SMs (the fp64 roofline
+ * denominator; MEASURED_PEAKS.json has no fp64 entry) and returns TFLOP/s (2 flops per FMA); synchronises. */
+int mfdn_profile(mfdn_ctx*, int enable);
+int mfdn_profile_read(mfdn_ctx*, double* ms_sort, double* ms_transform, int64_t* calls);
+int mfdn_fp64_peak(mfdn_ctx*, double* tflops);
+
 /* Number of requests with an out-of-range SPS index seen so far (synchronises `stream`). */
 int64_t mfdn_bad_request_count(mfdn_ctx*, void* stream);
 

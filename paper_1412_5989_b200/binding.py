@@ -21,7 +21,8 @@ MFDN_PRESORTED, MFDN_FORCE_NAIVE, MFDN_FORCE_DENSE = 1, 2, 4
 # every symbol include/mfdn_b200.h declares
 SYMBOLS = ["mfdn_orbitals_init", "mfdn_cg_build", "mfdn_cg_download", "mfdn_coupled_upload_2b",
            "mfdn_coupled_upload_3b", "mfdn_mscheme_2b", "mfdn_mscheme_3b", "mfdn_bad_request_count",
-           "mfdn_info", "mfdn_group_keys", "mfdn_last_error", "mfdn_destroy"]
+           "mfdn_info", "mfdn_group_keys", "mfdn_last_error", "mfdn_destroy", "mfdn_mscheme_host", "mfdn_profile",
+           "mfdn_profile_read", "mfdn_fp64_peak"]
 
 _lib = None
 
@@ -48,6 +49,10 @@ def lib():
         L.mfdn_coupled_upload_3b.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, C.c_int, vp]
         for f in (L.mfdn_mscheme_2b, L.mfdn_mscheme_3b):
             f.argtypes = [vp, i64, vp, vp, vp, vp, C.POINTER(C.c_size_t), u32, vp]
+        L.mfdn_mscheme_host.argtypes = [vp, C.c_int, i64, vp, vp, vp, vp, C.POINTER(C.c_size_t), u32, i64]
+        L.mfdn_profile.argtypes = [vp, C.c_int]
+        L.mfdn_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(i64)]
+        L.mfdn_fp64_peak.argtypes = [vp, C.POINTER(C.c_double)]
         L.mfdn_bad_request_count.argtypes = [vp, vp]
         L.mfdn_bad_request_count.restype = i64
         L.mfdn_info.argtypes = [vp, C.c_int]
@@ -149,6 +154,30 @@ def mfdn_mscheme_3b(ctx, n, d_req, d_out, d_mask, d_work, work_bytes, flags=0, s
     return _mscheme(lib().mfdn_mscheme_3b, ctx, n, d_req, d_out, d_mask, d_work, work_bytes, flags, stream)
 
 
+def mfdn_mscheme_host(ctx, body, n, h_req, h_out, h_mask, d_work, work_bytes, flags=0, chunk=0):
+    """Host-buffer wrapper: h_* are host addresses (ints, 0 = NULL).  Returns work_bytes."""
+    wb = C.c_size_t(int(work_bytes))
+    _check(ctx, lib().mfdn_mscheme_host(ctx, int(body), int(n), C.c_void_p(h_req), C.c_void_p(h_out), C.c_void_p(h_mask),
+                                        C.c_void_p(d_work), C.byref(wb), int(flags), int(chunk)))
+    return wb.value
+
+
+def mfdn_profile(ctx, enable):
+    _check(ctx, lib().mfdn_profile(ctx, int(bool(enable))))
+
+
+def mfdn_profile_read(ctx):
+    a, b, n = C.c_double(0), C.c_double(0), C.c_int64(0)
+    _check(ctx, lib().mfdn_profile_read(ctx, C.byref(a), C.byref(b), C.byref(n)))
+    return a.value, b.value, n.value
+
+
+def mfdn_fp64_peak(ctx):
+    t = C.c_double(0)
+    _check(ctx, lib().mfdn_fp64_peak(ctx, C.byref(t)))
+    return t.value
+
+
 def mfdn_group_keys(ctx, body, n, d_req, d_key, stream=None):
     _check(ctx, lib().mfdn_group_keys(ctx, int(body), int(n), C.c_void_p(d_req), C.c_void_p(d_key), _stream(stream)))
 
@@ -214,6 +243,22 @@ class Context:
         fn(self.ctx, n, d_req.data_ptr(), d_out.data_ptr(), d_mask.data_ptr(), work.data_ptr(), work.numel(), flags,
            stream)
         return d_out, d_mask
+
+    def mscheme_host(self, h_req, h_out=None, h_mask=None, flags=0, chunk=0):
+        """h_req: CPU int32 tensor [n][4|6] (pinned recommended).  Returns (h_out, h_mask) CPU tensors."""
+        torch = self.torch
+        assert (not h_req.is_cuda) and h_req.dtype == torch.int32 and h_req.is_contiguous()
+        n, width = h_req.shape
+        if h_out is None:
+            h_out = torch.empty(n, dtype=torch.float64).pin_memory()
+        if h_mask is None:
+            h_mask = torch.empty(n, dtype=torch.uint8).pin_memory()
+        need = mfdn_mscheme_host(self.ctx, width // 2, n, 0, 0, 0, 0, 0, flags, chunk)
+        if getattr(self, "_hwork", None) is None or self._hwork.numel() < need:
+            self._hwork = torch.empty(max(need, 256), dtype=torch.uint8, device=f"cuda:{self.device}")
+        mfdn_mscheme_host(self.ctx, width // 2, n, h_req.data_ptr(), h_out.data_ptr(), h_mask.data_ptr(),
+                          self._hwork.data_ptr(), self._hwork.numel(), flags, chunk)
+        return h_out, h_mask
 
     def group_keys(self, d_req):
         torch = self.torch

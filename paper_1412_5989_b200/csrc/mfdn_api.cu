@@ -261,7 +261,7 @@ extern "C" int mfdn_cg_build(mfdn_ctx* c, void* stream)
         for (int nn = 0; nn < BINOM_N; nn++) {
             for (int k = 0; k <= nn; k++) row[k] = (k == 0 || k == nn) ? 1ull : prev[k - 1] + prev[k];
             for (int k = 0; k <= nn; k++) binom[nn * BINOM_N + k] = (double)row[k];
-            prev = row;
+            prev.swap(row);
         }
     }
     Arena a;
@@ -738,5 +738,8 @@ extern "C" void mfdn_destroy(mfdn_ctx* c)
     if (!c) return;
     cudaSetDevice(c->device);
     for (void* p : c->owned) cudaFree(p);
+    for (auto& ev : c->ev_pending) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); cudaEventDestroy(ev.c); }
+    for (auto e : c->ev_pool) cudaEventDestroy(e);
+    for (auto s : c->hs) if (s) cudaStreamDestroy(s);
     delete c;
 }

@@ -81,6 +81,13 @@ struct mfdn_ctx {
     int64_t slab_bytes2 = 0, slab_bytes3 = 0;
     int64_t launches = 0;
     int num_sms = 148;
+    // measurement hooks
+    bool profile = false;
+    struct EvTriple { cudaEvent_t a, b, c; bool has_sort; };
+    std::vector<EvTriple> ev_pending;
+    std::vector<cudaEvent_t> ev_pool;
+    // host-buffer wrapper
+    cudaStream_t hs[2] = {nullptr, nullptr};
 };
 
 namespace mfdn {

@@ -9,6 +9,7 @@
 //           angular momentum values").
 //   2-body  v = sign * sqrt((1+d_ab)(1+d_cd)) * sum_J cg_b(J) cg_k(J) * (w0*cell[J][0] + w1*cell[J][1])
 // The slab cells of a (bra tuple, ket tuple) group are stored in exactly this loop order (A2).
+#include <algorithm>
 #include <cstdio>
 
 #include "mfdn_internal.cuh"
@@ -382,6 +383,15 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
     if (nt * nt >= 0xFFFFFFF0ll) return fail(c, MFDN_ERR_ARG, "too many tuples for 32-bit group keys");
     cudaStream_t st = (cudaStream_t)stream;
     const uint32_t* order = nullptr;
+    mfdn_ctx::EvTriple ev{nullptr, nullptr, nullptr, sorted_path};
+    if (c->profile) {
+        cudaEvent_t* e3[3] = {&ev.a, &ev.b, &ev.c};
+        for (auto pe : e3) {
+            if (!c->ev_pool.empty()) { *pe = c->ev_pool.back(); c->ev_pool.pop_back(); }
+            else MFDN_CUDA(c, cudaEventCreate(pe));
+        }
+        MFDN_CUDA(c, cudaEventRecord(ev.a, st));
+    }
     if (sorted_path) {
         char* w = (char*)d_work;
         uint32_t* keys = (uint32_t*)(w + o_keys);
@@ -397,10 +407,27 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
         c->launches += 5;
         order = ord;
     }
+    if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.b, st));
     k_mscheme<BODY><<<(unsigned)((n + 127) / 128), 128, 0, st>>>(c->t, n, d_req, order, d_out, d_mask);
     c->launches += 1;
     MFDN_CUDA(c, cudaGetLastError());
+    if (c->profile) {
+        MFDN_CUDA(c, cudaEventRecord(ev.c, st));
+        c->ev_pending.push_back(ev);
+    }
     return MFDN_OK;
+}
+
+// register-resident DFMA chains: 8 independent accumulators per thread, no memory traffic
+__global__ void __launch_bounds__(256) k_fp64_peak(double* out, int iters, double a, double b)
+{
+    double x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+    for (int i = 0; i < iters; i++) {
+        x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+        x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+    }
+    double s = x0 + x1 + x2 + x3 + x4 + x5 + x6 + x7;
+    if (s == 12345.678) out[0] = s;   // never true; keeps the chains alive
 }
 
 }  // namespace
@@ -428,5 +455,98 @@ extern "C" int mfdn_group_keys(mfdn_ctx* c, int body, int64_t n, const int32_t* 
     else
         k_keys<2><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(c->t, n, d_req, d_key, nullptr, 0xFFFFFFFFu, 0u);
     MFDN_CUDA(c, cudaGetLastError());
+    return MFDN_OK;
+}
+
+extern "C" int mfdn_profile(mfdn_ctx* c, int enable)
+{
+    if (!c) return MFDN_ERR_ARG;
+    c->profile = enable != 0;
+    return MFDN_OK;
+}
+
+extern "C" int mfdn_profile_read(mfdn_ctx* c, double* ms_sort, double* ms_transform, int64_t* calls)
+{
+    if (!c || !ms_sort || !ms_transform || !calls) return MFDN_ERR_ARG;
+    *ms_sort = *ms_transform = 0.0;
+    *calls = 0;
+    for (auto& ev : c->ev_pending) {
+        MFDN_CUDA(c, cudaEventSynchronize(ev.c));
+        float t1 = 0.f, t2 = 0.f;
+        MFDN_CUDA(c, cudaEventElapsedTime(&t1, ev.a, ev.b));
+        MFDN_CUDA(c, cudaEventElapsedTime(&t2, ev.b, ev.c));
+        *ms_sort += t1;
+        *ms_transform += t2;
+        *calls += 1;
+        c->ev_pool.push_back(ev.a); c->ev_pool.push_back(ev.b); c->ev_pool.push_back(ev.c);
+    }
+    c->ev_pending.clear();
+    return MFDN_OK;
+}
+
+extern "C" int mfdn_fp64_peak(mfdn_ctx* c, double* tflops)
+{
+    if (!c || !tflops) return MFDN_ERR_ARG;
+    MFDN_CUDA(c, cudaSetDevice(c->device));
+    cudaEvent_t a, b;
+    MFDN_CUDA(c, cudaEventCreate(&a));
+    MFDN_CUDA(c, cudaEventCreate(&b));
+    const int iters = 1 << 14, blocks = c->num_sms * 8, threads = 256;
+    double best = 0.0;
+    for (int rep = 0; rep < 5; rep++) {
+        MFDN_CUDA(c, cudaEventRecord(a, 0));
+        k_fp64_peak<<<blocks, threads>>>((double*)c->t.bad_count + 8, iters, 0.999999, 1e-9);
+        MFDN_CUDA(c, cudaEventRecord(b, 0));
+        MFDN_CUDA(c, cudaEventSynchronize(b));
+        float ms = 0.f;
+        MFDN_CUDA(c, cudaEventElapsedTime(&ms, a, b));
+        double tf = 2.0 * 8.0 * iters * (double)blocks * threads / (ms * 1e-3) * 1e-12;
+        if (rep > 0 && tf > best) best = tf;
+    }
+    cudaEventDestroy(a);
+    cudaEventDestroy(b);
+    *tflops = best;
+    return MFDN_OK;
+}
+
+// The paper's wrapper, double-buffered: chunk k uses stream k % 2.
+extern "C" int mfdn_mscheme_host(mfdn_ctx* c, int body, int64_t n, const int32_t* h_req, double* h_out, uint8_t* h_mask,
+                                 void* d_work, size_t* work_bytes, uint32_t flags, int64_t chunk)
+{
+    if (!c || !work_bytes || (body != 2 && body != 3) || n < 0 || chunk < 0) return c ? fail(c, MFDN_ERR_ARG, "bad argument") : MFDN_ERR_ARG;
+    if (chunk == 0) chunk = 1 << 22;
+    if (chunk > n && n > 0) chunk = n;
+    const int width = 2 * body;
+    size_t inner = 0;
+    int rc = body == 3 ? run<3>(c, chunk, nullptr, nullptr, nullptr, nullptr, &inner, flags, nullptr)
+                       : run<2>(c, chunk, nullptr, nullptr, nullptr, nullptr, &inner, flags, nullptr);
+    if (rc) return rc;
+    const size_t b_req = align256((size_t)chunk * width * 4), b_out = align256((size_t)chunk * 8), b_mask = align256((size_t)chunk);
+    const size_t per = b_req + b_out + b_mask + align256(inner);
+    if (!d_work) { *work_bytes = 2 * per; return MFDN_OK; }
+    if (*work_bytes < 2 * per) return fail(c, MFDN_ERR_OOM, "scratch too small");
+    if (n == 0) return MFDN_OK;
+    if (!h_req || !h_out) return fail(c, MFDN_ERR_ARG, "null host pointer");
+    MFDN_CUDA(c, cudaSetDevice(c->device));
+    for (int k = 0; k < 2; k++)
+        if (!c->hs[k]) MFDN_CUDA(c, cudaStreamCreateWithFlags(&c->hs[k], cudaStreamNonBlocking));
+    int64_t k = 0;
+    for (int64_t lo = 0; lo < n; lo += chunk, k++) {
+        int64_t m = std::min<int64_t>(chunk, n - lo);
+        cudaStream_t st = c->hs[k & 1];
+        char* base = (char*)d_work + (k & 1) * per;
+        int32_t* dreq = (int32_t*)base;
+        double* dout = (double*)(base + b_req);
+        uint8_t* dmask = (uint8_t*)(base + b_req + b_out);
+        void* dw = base + b_req + b_out + b_mask;
+        size_t wb = align256(inner);
+        MFDN_CUDA(c, cudaMemcpyAsync(dreq, h_req + lo * width, (size_t)m * width * 4, cudaMemcpyHostToDevice, st));
+        rc = body == 3 ? run<3>(c, m, dreq, dout, dmask, dw, &wb, flags, st) : run<2>(c, m, dreq, dout, dmask, dw, &wb, flags, st);
+        if (rc) return rc;
+        MFDN_CUDA(c, cudaMemcpyAsync(h_out + lo, dout, (size_t)m * 8, cudaMemcpyDeviceToHost, st));
+        if (h_mask) MFDN_CUDA(c, cudaMemcpyAsync(h_mask + lo, dmask, (size_t)m, cudaMemcpyDeviceToHost, st));
+    }
+    MFDN_CUDA(c, cudaStreamSynchronize(c->hs[0]));
+    MFDN_CUDA(c, cudaStreamSynchronize(c->hs[1]));
     return MFDN_OK;
 }
