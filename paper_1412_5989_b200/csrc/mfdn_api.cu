@@ -124,6 +124,27 @@ extern "C" int mfdn_orbitals_init(mfdn_ctx** out, int device, int32_t n_orb, con
                 w[2] = c1 * q;   // (1,3/2)
             }
         }
+    // the five 3-body weights (and two 2-body weights) per tz-bit pattern of a packed record
+    std::vector<double> w3(64 * 6, 0.0), w2(16 * 2, 0.0);
+    for (int tb = 0; tb < 8; tb++)
+        for (int tk = 0; tk < 8; tk++) {
+            const double* ib = c->t.iso3[tb];
+            const double* ik = c->t.iso3[tk];
+            double* w = &w3[(tb * 8 + tk) * 6];
+            w[0] = ib[0] * ik[0]; w[1] = ib[0] * ik[1]; w[2] = ib[1] * ik[0]; w[3] = ib[1] * ik[1]; w[4] = ib[2] * ik[2];
+        }
+    for (int tb = 0; tb < 4; tb++)
+        for (int tk = 0; tk < 4; tk++) {
+            w2[(tb * 4 + tk) * 2 + 0] = c->t.iso2[tb][0] * c->t.iso2[tk][0];
+            w2[(tb * 4 + tk) * 2 + 1] = c->t.iso2[tb][1] * c->t.iso2[tk][1];
+        }
+    void* dw = nullptr;
+    if (cudaMalloc(&dw, (w3.size() + w2.size()) * sizeof(double)) != cudaSuccess) { mfdn_destroy(c); return MFDN_ERR_OOM; }
+    c->owned.push_back(dw);
+    cudaMemcpy(dw, w3.data(), w3.size() * sizeof(double), cudaMemcpyHostToDevice);
+    cudaMemcpy((double*)dw + w3.size(), w2.data(), w2.size() * sizeof(double), cudaMemcpyHostToDevice);
+    c->t.wtab3 = (const double*)dw;
+    c->t.wtab2 = (const double*)dw + w3.size();
     c->stage = 1;
     *out = c;
     return MFDN_OK;
@@ -264,20 +285,25 @@ extern "C" int mfdn_cg_build(mfdn_ctx* c, void* stream)
             prev.swap(row);
         }
     }
+    // device layout: [stage 1 | CG_GUARD zeros | stage 2 | CG_GUARD zeros]
+    void* dcg = nullptr;
+    MFDN_CUDA(c, cudaMalloc(&dcg, (pos + 2 * CG_GUARD) * sizeof(double)));
+    c->owned.push_back(dcg);
+    MFDN_CUDA(c, cudaMemsetAsync(dcg, 0, (pos + 2 * CG_GUARD) * sizeof(double), st));
+    for (size_t k = (size_t)nj * nj; k < blocks.size(); k++) blocks[k].off += CG_GUARD;
     Arena a;
     size_t o_blocks = a.add(blocks), o_lf = a.add(lf), o_off1 = a.add(off1), o_off2 = a.add(off2), o_bin = a.add(binom);
+    c->h_cg2_off = off2;
     char* base = nullptr;
     int rc = arena_upload(c, a, &base, st);
     if (rc) return rc;
-    void* dcg = nullptr;
-    MFDN_CUDA(c, cudaMalloc(&dcg, pos * sizeof(double)));
-    c->owned.push_back(dcg);
     dim3 grid(8, (unsigned)blocks.size());
     k_cg_build<<<grid, 128, 0, st>>>((const CgBlock*)(base + o_blocks), (const double2*)(base + o_lf),
                                      (const double*)(base + o_bin), (double*)dcg);
     MFDN_CUDA(c, cudaGetLastError());
     c->t.cg1 = (const double*)dcg;
-    c->t.cg2 = (const double*)dcg + c->n_cg1;
+    c->t.cg2 = (const double*)dcg + c->n_cg1 + CG_GUARD;
+    c->t.cg2g = (const double*)dcg + c->n_cg1;
     c->t.cg1_off = (const int32_t*)(base + o_off1);
     c->t.cg2_off = (const int32_t*)(base + o_off2);
     c->stage = 2;
@@ -328,7 +354,7 @@ __global__ void k_retile3(Retile3 p)
         int par = (db.x >> 25) & 1;
         int Jlo = max((db.y >> 16) & 255, (dk.y >> 16) & 255), Jhi = min((db.y >> 24) & 255, (dk.y >> 24) & 255);
         int nJb = (((db.y >> 24) & 255) - ((db.y >> 16) & 255)) / 2 + 1, nJk = (((dk.y >> 24) & 255) - ((dk.y >> 16) & 255)) / 2 + 1;
-        double* dst = p.slab + (size_t)so * CELL3;
+        double* dst = p.slab + (size_t)so * 2;
         for (int twoJ = Jlo; twoJ <= Jhi; twoJ += 2) {
             int lb, hb, lk, hk;
             j12_range(db, twoJ, lb, hb);
@@ -336,11 +362,12 @@ __global__ void k_retile3(Retile3 p)
             int nb = hb - lb + 1, nk = hk - lk + 1;
             if (nb <= 0 || nk <= 0) continue;
             int iJb = (twoJ - ((db.y >> 16) & 255)) / 2, iJk = (twoJ - ((dk.y >> 16) & 255)) / 2;
-            for (int idx = threadIdx.x; idx < nb * nk * CELL3; idx += blockDim.x) {
-                int slot = idx % CELL3, cell = idx / CELL3;
-                int i = cell / nk, k = cell % nk;
+            const int pitch = row_pitch3(nk);
+            for (int idx = threadIdx.x; idx < nb * pitch; idx += blockDim.x) {
+                int i = idx / pitch, o = idx % pitch;
                 double v = 0.0;
-                if (slot < 5) {
+                if (o < NISO3 * nk) {
+                    int k = o / NISO3, slot = o % NISO3;
                     int T12 = slot >> 1 & 1, T12p = slot & 1, Ti = 0;
                     if (slot == 4) { T12 = 1; T12p = 1; Ti = 1; }
                     int ch = p.chan_of[(twoJ >> 1) * 4 + Ti * 2 + par];
@@ -352,7 +379,7 @@ __global__ void k_retile3(Retile3 p)
                 }
                 dst[idx] = v;
             }
-            dst += (size_t)nb * nk * CELL3;
+            dst += (size_t)nb * pitch;
         }
     }
 }
@@ -498,14 +525,41 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
                 stmask[d.z + i12 * 2 + T12] |= 1ull << ((chan_twoJ[ch] >> 1) * 2 + Ti);
             }
     }
-    // ---- slab offsets: cells per (bra tuple, ket tuple) group in loop order J, J12, J12'
-    std::vector<uint32_t> slab_off((size_t)nt * nt, NO_SLAB);
-    uint64_t cells = 0;
     auto range = [&](int4 d, int twoJ, int& lo, int& hi) {
         int jc = (d.x >> 16) & 255;
         lo = std::max(d.y & 255, std::abs(twoJ - jc) >> 1);
         hi = std::min((d.y >> 8) & 255, (twoJ + jc) >> 1);
     };
+    // ---- row tables: per (tuple, J, J12) the address part of <J12 M12 jc mc|J M> that does not depend on the
+    //      request: offset = cg2_off[J12][jc] + J12*(jc+1)*nJ + iJ (+ CG_GUARD); the kernel adds A*nJ with
+    //      A = M12*(jc+1) + imc  (A2 "tile index": flat offsets, no pointers -- PAPER.md:109-121)
+    std::vector<int2> trow(nt), rowtab;
+    std::vector<uint32_t> jinfo;
+    for (int t = 0; t < nt; t++) {
+        int4 d = tdesc[t];
+        int jc = (d.x >> 16) & 255;
+        trow[t].x = (int)rowtab.size();
+        trow[t].y = (int)jinfo.size();
+        uint32_t rows = 0;
+        for (int twoJ = (d.y >> 16) & 255; twoJ <= ((d.y >> 24) & 255); twoJ += 2) {
+            int lo, hi;
+            range(d, twoJ, lo, hi);
+            int nrow = std::max(0, hi - lo + 1);
+            if (rows > 0xFFFF || nrow > 255) return fail(c, MFDN_ERR_ARG, "tuple has too many rows");
+            jinfo.push_back(rows | ((uint32_t)(lo - (d.y & 255)) << 16) | ((uint32_t)nrow << 24));
+            for (int J12 = lo; J12 <= hi; J12++) {
+                int nJ = std::min(2 * J12, jc) + 1;
+                int2 e;
+                e.x = CG_GUARD + c->h_cg2_off[J12 * c->t.nj + (jc >> 1)] + J12 * (jc + 1) * nJ + (twoJ - std::abs(2 * J12 - jc)) / 2;
+                e.y = nJ;
+                rowtab.push_back(e);
+            }
+            rows += nrow;
+        }
+    }
+    // ---- slab offsets (16-byte units) per (bra tuple, ket tuple) group, rows in loop order J, J12
+    std::vector<uint32_t> slab_off((size_t)nt * nt, NO_SLAB);
+    uint64_t cells = 0;   // in 16-byte units
     for (int tb = 0; tb < nt; tb++)
         for (int tk = 0; tk < nt; tk++) {
             int4 db = tdesc[tb], dk = tdesc[tk];
@@ -516,16 +570,17 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
                 int lb, hb, lk, hk;
                 range(db, twoJ, lb, hb);
                 range(dk, twoJ, lk, hk);
-                if (hb >= lb && hk >= lk) n += (uint64_t)(hb - lb + 1) * (hk - lk + 1);
+                if (hb >= lb && hk >= lk) n += (uint64_t)(hb - lb + 1) * (row_pitch3(hk - lk + 1) / 2);
             }
             if (n == 0) continue;
-            if (cells + n >= 0xFFFFFFF0ull) return fail(c, MFDN_ERR_OOM, "table too large for 32-bit cell offsets");
+            if (cells + n >= 0xFFFFFFF0ull) return fail(c, MFDN_ERR_OOM, "table too large for 32-bit slab offsets");
             slab_off[(size_t)tb * nt + tk] = (uint32_t)cells;
             cells += n;
         }
     // ---- one arena for the resident index tables, one for the upload-only ones
     Arena res, tmp;
     size_t o_tid = res.add(tuple_id), o_desc = res.add(tdesc), o_soff = res.add(slab_off), o_sm = res.add(stmask);
+    size_t o_trow = res.add(trow), o_rowtab = res.add(rowtab), o_jinfo = res.add(jinfo);
     std::vector<int64_t> coff(chan_off, chan_off + n_chan);
     std::vector<int32_t> cdim(chan_dim, chan_dim + n_chan);
     size_t o_rm = tmp.add(rowmap), o_cof = tmp.add(chan_of), o_coff = tmp.add(coff), o_cdim = tmp.add(cdim);
@@ -540,7 +595,7 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     rc = stage_values(c, values, values_on_device, n_values, st, &dvals, &vtmp);
     if (rc) { cudaFree(dtmp); return rc; }
     void* dslab = nullptr;
-    cudaError_t e = cudaMalloc(&dslab, std::max<uint64_t>(cells, 1) * CELL3 * sizeof(double));
+    cudaError_t e = cudaMalloc(&dslab, std::max<uint64_t>(cells, 1) * 16 + 256);
     if (e != cudaSuccess) { cudaFree(dtmp); if (vtmp) cudaFree(vtmp); return cuda_fail(c, e, "cudaMalloc(slab3)"); }
     c->owned.push_back(dslab);
     Retile3 p;
@@ -567,7 +622,10 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     c->t.slab_off3 = p.slab_off;
     c->t.slab3 = (const double*)dslab;
     c->t.stmask3 = (const unsigned long long*)(dres + o_sm);
-    c->slab_bytes3 = (int64_t)(cells * CELL3 * sizeof(double));
+    c->t.trow3 = (const int2*)(dres + o_trow);
+    c->t.rowtab3 = (const int2*)(dres + o_rowtab);
+    c->t.jinfo3 = (const uint32_t*)(dres + o_jinfo);
+    c->slab_bytes3 = (int64_t)(cells * 16);
     c->has3 = true;
     return MFDN_OK;
 }

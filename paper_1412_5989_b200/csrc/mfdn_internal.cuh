@@ -26,9 +26,21 @@ __host__ __device__ inline int rec_e(uint32_t r) { return (r >> 21) & 63; }
 __host__ __device__ inline int rec_lpar(uint32_t r) { return (r >> 27) & 1; }
 
 constexpr int MAX_TWOJ = 21;       // 3*MAX_TWOJ <= 63 so that (2J,2T) fits a 64-bit channel mask
-constexpr int CELL3 = 6;           // doubles per 3-body slab cell: 5 isospin slots + 1 pad (48 B)
+constexpr int NISO3 = 5;           // isospin slots per 3-body cell: (T12,T12',T) = (0,0,1/2) (0,1,1/2) (1,0,1/2) (1,1,1/2) (1,1,3/2)
 constexpr int CELL2 = 2;           // doubles per 2-body slab cell: T = 0, 1 (16 B)
 constexpr uint32_t NO_SLAB = 0xFFFFFFFFu;
+constexpr int CG_GUARD = 8192;     // zero doubles before and after the stage-2 table (see Tables::cg2g)
+
+// 3-body slab of a (bra tuple, ket tuple) group, in the order the kernel's loops read it:
+//   for J (common range, ascending) / for bra J12 in range(J) / [ for ket J12' in range(J) / 5 isospin slots ]
+// one "row" = the NISO3*nk(J) doubles of a fixed (J, J12), padded to an even count (16-byte units).
+__host__ __device__ inline int row_pitch3(int nk) { return (NISO3 * nk + 1) & ~1; }
+
+// ---- packed canonical request record (H1 output), 64 bit --------------------------------------------
+//  [0,30) im of the canonical particles (5 bits each: bra then ket)   [30,36) tz bits (bra then ket)
+//  [36] 1 = odd permutation (sign -1)                                  [37,64) group key, REC_INVALID if S1-S6 fail
+constexpr unsigned REC_KEY_SHIFT = 37;
+constexpr uint32_t REC_INVALID = 0x7FFFFFFu;
 
 // ---- per-tuple descriptor (A2), 16 bytes ---------------------------------------------------------
 // 3-body: x = ja | jb<<8 | jc<<16 | (a==b)<<24 | par<<25      (ja.. are 2j)
@@ -46,15 +58,22 @@ struct Tables {
     const int32_t* cg1_off;
     const double* cg2;       // stage 2 blocks [J12 * nj + (2j-1)/2],  J12 = 0..2*nj-1
     const int32_t* cg2_off;
+    const double* cg2g;      // = cg2 - CG_GUARD: row-table offsets are relative to this, so that a lane whose
+                             // |M12| > J12 (stage-1 factor = 0) still reads valid, finite memory
+    const double* wtab3;     // [64][6] isospin weights w[5] (+pad) indexed by the 6 tz bits of a record
+    const double* wtab2;     // [16][2]
     double iso3[8][3];       // [ta<<2|tb<<1|tc][(T12,T) = (0,1/2),(1,1/2),(1,3/2)]
     double iso2[4][2];       // [ta<<1|tb][T]
     // A2, 3-body
     int n_tup3, e3max;
     const int32_t* tuple_id3;      // [n_orb^3] -> tuple or -1
     const int4* tdesc3;
-    const uint32_t* slab_off3;     // [n_tup3^2] first cell of the group's slab or NO_SLAB
-    const double* slab3;           // cells of CELL3 doubles
+    const uint32_t* slab_off3;     // [n_tup3^2] start of the group's slab in 16-byte units, or NO_SLAB
+    const double* slab3;
     const unsigned long long* stmask3;
+    const int2* trow3;             // [n_tup3] {first row of the tuple in rowtab3, first entry in jinfo3}
+    const int2* rowtab3;           // per (tuple, J, J12) row: {offset into cg2g of <J12 . jc .|J .> at A = 0, nJ}
+    const uint32_t* jinfo3;        // per (tuple, J): row start (16 b) | (first J12 - J12min) << 16 | n rows << 24
     // A2, 2-body
     int n_tup2;
     const int32_t* tuple_id2;      // [n_orb^2]
@@ -74,7 +93,7 @@ struct mfdn_ctx {
     mfdn::Tables t{};
     int tjmax = 0;
     // host copies
-    std::vector<int32_t> orb_n, orb_l, orb_twoj;
+    std::vector<int32_t> orb_n, orb_l, orb_twoj, h_cg2_off;
     std::vector<uint32_t> h_sps_rec;
     std::vector<void*> owned;  // device allocations
     int64_t n_cg1 = 0, n_cg2 = 0;

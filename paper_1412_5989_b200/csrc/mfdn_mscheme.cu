@@ -1,14 +1,20 @@
 // H1-H6: the coupled-JT -> M-scheme transformation kernels and their launchers.
 //
 // What one request computes:
-//   3-body  v = sign * sum_J sum_{J12} sum_{J12'} cb(J12,J) ck(J12',J) * sum_{s<5} w[s] * cell[J,J12,J12'][s]
+//   3-body  v = sign * sum_J sum_{J12} cb(J12,J) * sum_{J12'} ck(J12',J) * sum_{s<5} w[s] * slab[J,J12,J12'][s]
 //           cb(J12,J) = <ja ma jb mb|J12 M12> <J12 M12 jc mc|J M>,  ck likewise for the ket,
 //           w[s] = isospin weights of the five (T12,T12',T) combinations ("the isospin
 //           coupling coefficients are precalculated with several conditionals, and the isospin loops are
 //           unrolled into a single weighted summation. The core ... three nested loops over coupled
 //           angular momentum values").
 //   2-body  v = sign * sqrt((1+d_ab)(1+d_cd)) * sum_J cg_b(J) cg_k(J) * (w0*cell[J][0] + w1*cell[J][1])
-// The slab cells of a (bra tuple, ket tuple) group are stored in exactly this loop order (A2).
+// The slab of a (bra tuple, ket tuple) group is stored in exactly this loop order (A2).
+//
+// Pipeline of one call:
+//   k_keys      H1  decode, selection S1-S7 -> mask, canonicalise -> 64-bit record (group key | sign | tz | m)
+//   k_scan_*    H2  exclusive scan of the group histogram            (skipped if MFDN_PRESORTED)
+//   k_scatter   H2  records -> group order (+ original index)        (skipped if MFDN_PRESORTED)
+//   k_transform H3-H6  one warp per 32 consecutive records of the group-ordered stream
 #include <algorithm>
 #include <cstdio>
 
@@ -116,35 +122,63 @@ __device__ __forceinline__ unsigned long long chanmask3(const Tables& T, int4 d,
     return m;
 }
 
-// ------------------------------------------------------------------------------- H3-H5, 3-body
-__device__ __forceinline__ double eval3(const Tables& T, const Side3& B, const Side3& K, int& mask)
+// S7 for a decoded 3-body request that passed S1-S6: at least one admissible channel term
+__device__ __forceinline__ bool mask3(const Tables& T, const Side3& B, const Side3& K, int4 db, int4 dk)
+{
+    const int ja = db.x & 255, jb = (db.x >> 8) & 255, jd = dk.x & 255, je = (dk.x >> 8) & 255;
+    const int twoM12b = 2 * (B.ima + B.imb) - ja - jb, twoM12k = 2 * (K.ima + K.imb) - jd - je;
+    const int tzb12 = (B.tz >> 2) + ((B.tz >> 1) & 1) - 1, tzk12 = (K.tz >> 2) + ((K.tz >> 1) & 1) - 1;  // MT12
+    unsigned long long mm = chanmask3(T, db, twoM12b, 2 * tzb12) & chanmask3(T, dk, twoM12k, 2 * tzk12);
+    mm &= ~0ull << (2 * (abs(B.twoM) >> 1));                   // J >= |M|
+    if (abs(B.twoMT) == 3) mm &= 0xAAAAAAAAAAAAAAAAull;        // T = 3/2 only
+    return mm != 0;
+}
+__device__ __forceinline__ bool mask2(const Side2& B, int4 db, int4 dk)
+{
+    unsigned long long mb = (unsigned long long)(uint32_t)db.z | ((unsigned long long)(uint32_t)db.w << 32);
+    unsigned long long mk = (unsigned long long)(uint32_t)dk.z | ((unsigned long long)(uint32_t)dk.w << 32);
+    unsigned long long mm = mb & mk & (~0ull << (2 * ((abs(B.twoM) + 1) >> 1)));   // J >= |M|
+    if (B.twoMT != 0) mm &= 0xAAAAAAAAAAAAAAAAull;                                 // T = 1 only
+    return mm != 0;
+}
+
+// ------------------------------------------------------------------------------- request loads
+__device__ __forceinline__ void load_req3(const int32_t* req, long long r, int s[6])
+{
+    const int2* p = (const int2*)(req + 6 * r);
+    int2 a = __ldg(p), b = __ldg(p + 1), c = __ldg(p + 2);
+    s[0] = a.x; s[1] = a.y; s[2] = b.x; s[3] = b.y; s[4] = c.x; s[5] = c.y;
+}
+__device__ __forceinline__ void load_req2(const int32_t* req, long long r, int s[6])
+{
+    int4 a = __ldg((const int4*)(req + 4 * r));
+    s[0] = a.x; s[1] = a.y; s[2] = a.z; s[3] = a.w; s[4] = 0; s[5] = 0;
+}
+
+// =============================================================================== naive kernel
+// MFDN_FORCE_NAIVE: the paper's design -- one thread per request, in request order, the
+// loop nest inside the kernel, every index recomputed per thread.  Kept as the on-device reference.
+__device__ __forceinline__ double eval3_naive(const Tables& T, const Side3& B, const Side3& K, int& mask)
 {
     mask = 0;
     if (!select3(T, B, K)) return 0.0;
     const uint32_t so = __ldg(T.slab_off3 + (size_t)B.tup * T.n_tup3 + K.tup);
     if (so == NO_SLAB) return 0.0;
     const int4 db = __ldg(T.tdesc3 + B.tup), dk = __ldg(T.tdesc3 + K.tup);
+    if (!mask3(T, B, K, db, dk)) return 0.0;
+    mask = 1;
     const int ja = db.x & 255, jb = (db.x >> 8) & 255, jc = (db.x >> 16) & 255;
     const int jd = dk.x & 255, je = (dk.x >> 8) & 255, jf = (dk.x >> 16) & 255;
     const int twoM12b = 2 * (B.ima + B.imb) - ja - jb, twoM12k = 2 * (K.ima + K.imb) - jd - je;
-    const int tzb12 = (B.tz >> 2) + ((B.tz >> 1) & 1) - 1, tzk12 = (K.tz >> 2) + ((K.tz >> 1) & 1) - 1;  // MT12
-    // S7
     const int aM = abs(B.twoM);
-    unsigned long long mm = chanmask3(T, db, twoM12b, 2 * tzb12) & chanmask3(T, dk, twoM12k, 2 * tzk12);
-    mm &= ~0ull << (2 * (aM >> 1));
-    if (abs(B.twoMT) == 3) mm &= 0xAAAAAAAAAAAAAAAAull;
-    if (mm == 0) return 0.0;
-    mask = 1;
-    // isospin weights
     const double* ib = T.iso3[B.tz];
     const double* ik = T.iso3[K.tz];
     const double w0 = ib[0] * ik[0], w1 = ib[0] * ik[1], w2 = ib[1] * ik[0], w3 = ib[1] * ik[1], w4 = ib[2] * ik[2];
-    // stage-1 rows
     const int nj = T.nj;
     const int J12minb = db.y & 255, J12mink = dk.y & 255;
     const double* c1b = T.cg1 + __ldg(T.cg1_off + (ja >> 1) * nj + (jb >> 1)) + (B.ima * (jb + 1) + B.imb) * (min(ja, jb) + 1);
     const double* c1k = T.cg1 + __ldg(T.cg1_off + (jd >> 1) * nj + (je >> 1)) + (K.ima * (je + 1) + K.imb) * (min(jd, je) + 1);
-    const double* cell = T.slab3 + (size_t)so * CELL3;
+    const double* row = T.slab3 + (size_t)so * 2;
     const int Jlo = max((db.y >> 16) & 255, (dk.y >> 16) & 255), Jhi = min((db.y >> 24) & 255, (dk.y >> 24) & 255);
     double total = 0.0;
     for (int twoJ = Jlo; twoJ <= Jhi; twoJ += 2) {
@@ -152,7 +186,8 @@ __device__ __forceinline__ double eval3(const Tables& T, const Side3& B, const S
         int lk = max(J12mink, abs(twoJ - jf) >> 1), hk = min((dk.y >> 8) & 255, (twoJ + jf) >> 1);
         int nb = hb - lb + 1, nk = hk - lk + 1;
         if (nb <= 0 || nk <= 0) continue;
-        if (twoJ < aM) { cell += (size_t)nb * nk * CELL3; continue; }
+        const int pitch = row_pitch3(nk);
+        if (twoJ < aM) { row += (size_t)nb * pitch; continue; }
         for (int J12 = lb; J12 <= hb; J12++) {
             double cb = 0.0;
             if (abs(twoM12b) <= 2 * J12) {
@@ -170,36 +205,29 @@ __device__ __forceinline__ double eval3(const Tables& T, const Side3& B, const S
                     ck = __ldg(c1k + (J12p - J12mink)) *
                          __ldg(c2 + (((twoM12k + 2 * J12p) >> 1) * (jf + 1) + K.imc) * nJ + ((twoJ - abs(2 * J12p - jf)) >> 1));
                 }
-                const double2 v01 = __ldg((const double2*)cell), v23 = __ldg((const double2*)cell + 1),
-                              v45 = __ldg((const double2*)cell + 2);
-                double inner = w0 * v01.x;
-                inner = fma(w1, v01.y, inner);
-                inner = fma(w2, v23.x, inner);
-                inner = fma(w3, v23.y, inner);
-                inner = fma(w4, v45.x, inner);
+                const double* cell = row + NISO3 * (J12p - lk);
+                double inner = w0 * __ldg(cell);
+                inner = fma(w1, __ldg(cell + 1), inner);
+                inner = fma(w2, __ldg(cell + 2), inner);
+                inner = fma(w3, __ldg(cell + 3), inner);
+                inner = fma(w4, __ldg(cell + 4), inner);
                 acc = fma(ck, inner, acc);
-                cell += CELL3;
             }
             total = fma(cb, acc, total);
+            row += pitch;
         }
     }
     return (B.sign * K.sign) * total;
 }
 
-// ------------------------------------------------------------------------------- H3-H5, 2-body
-__device__ __forceinline__ double eval2(const Tables& T, const Side2& B, const Side2& K, int& mask)
+__device__ __forceinline__ double eval2_naive(const Tables& T, const Side2& B, const Side2& K, int& mask)
 {
     mask = 0;
     if (!select2(B, K)) return 0.0;
     const uint32_t so = __ldg(T.slab_off2 + (size_t)B.tup * T.n_tup2 + K.tup);
     if (so == NO_SLAB) return 0.0;
     const int4 db = __ldg(T.tdesc2 + B.tup), dk = __ldg(T.tdesc2 + K.tup);
-    const int aM = abs(B.twoM);
-    unsigned long long mb = (unsigned long long)(uint32_t)db.z | ((unsigned long long)(uint32_t)db.w << 32);
-    unsigned long long mk = (unsigned long long)(uint32_t)dk.z | ((unsigned long long)(uint32_t)dk.w << 32);
-    unsigned long long mm = mb & mk & (~0ull << (2 * ((aM + 1) >> 1)));   // J >= |M|  (2J >= |2M|, 2M even)
-    if (B.twoMT != 0) mm &= 0xAAAAAAAAAAAAAAAAull;                       // T = 1 only
-    if (mm == 0) return 0.0;
+    if (!mask2(B, db, dk)) return 0.0;
     mask = 1;
     const int ja = db.x & 255, jb = (db.x >> 8) & 255, jc = dk.x & 255, jd = (dk.x >> 8) & 255;
     const double w0 = T.iso2[B.tz][0] * T.iso2[K.tz][0], w1 = T.iso2[B.tz][1] * T.iso2[K.tz][1];
@@ -220,72 +248,70 @@ __device__ __forceinline__ double eval2(const Tables& T, const Side2& B, const S
     return (B.sign * K.sign) * norm * total;
 }
 
-// ------------------------------------------------------------------------------- request loads
-__device__ __forceinline__ void load_req3(const int32_t* req, long long r, int s[6])
-{
-    const int2* p = (const int2*)(req + 6 * r);
-    int2 a = __ldg(p), b = __ldg(p + 1), c = __ldg(p + 2);
-    s[0] = a.x; s[1] = a.y; s[2] = b.x; s[3] = b.y; s[4] = c.x; s[5] = c.y;
-}
-__device__ __forceinline__ void load_req2(const int32_t* req, long long r, int s[6])
-{
-    int4 a = __ldg((const int4*)(req + 4 * r));
-    s[0] = a.x; s[1] = a.y; s[2] = a.z; s[3] = a.w; s[4] = 0; s[5] = 0;
-}
-
-// ------------------------------------------------------------------------------- kernels
-// Thread per request.  ORDER != nullptr: thread i handles request order[i] (after the group sort),
-// so that the threads of a warp share the (bra tuple, ket tuple) slab and the loop bounds.
 template <int BODY>
-__global__ void __launch_bounds__(128) k_mscheme(Tables T, long long n, const int32_t* __restrict__ req,
-                                                const uint32_t* __restrict__ order, double* __restrict__ out,
-                                                uint8_t* __restrict__ maskout)
+__global__ void __launch_bounds__(128) k_mscheme_naive(Tables T, long long n, const int32_t* __restrict__ req,
+                                                      double* __restrict__ out, uint8_t* __restrict__ maskout)
 {
     long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    long long r = order ? (long long)__ldg(order + i) : i;
     int s[6];
-    if (BODY == 3) load_req3(req, r, s); else load_req2(req, r, s);
+    if (BODY == 3) load_req3(req, i, s); else load_req2(req, i, s);
     double v = 0.0;
     int mask = 0;
     if (!in_range(T, s, 2 * BODY)) {
         atomicAdd(T.bad_count, 1ull);
     } else if (BODY == 3) {
         Side3 B = decode3(T, s[0], s[1], s[2]), K = decode3(T, s[3], s[4], s[5]);
-        v = eval3(T, B, K, mask);
+        v = eval3_naive(T, B, K, mask);
     } else {
         Side2 B = decode2(T, s[0], s[1]), K = decode2(T, s[2], s[3]);
-        v = eval2(T, B, K, mask);
+        v = eval2_naive(T, B, K, mask);
     }
-    out[r] = mask ? v : 0.0;
-    if (maskout) maskout[r] = (uint8_t)mask;
+    out[i] = mask ? v : 0.0;
+    if (maskout) maskout[i] = (uint8_t)mask;
 }
 
-// H1 key generation (+ histogram when hist != nullptr)
+// =============================================================================== H1: records
+// One thread per request: decode, S1-S7 -> mask (request order, coalesced), canonical packed record.
 template <int BODY>
 __global__ void __launch_bounds__(256) k_keys(Tables T, long long n, const int32_t* __restrict__ req,
-                                              uint32_t* __restrict__ keys, uint32_t* __restrict__ hist, uint32_t invalid_key,
-                                              uint32_t invalid_bucket)
+                                              unsigned long long* __restrict__ recs, uint8_t* __restrict__ maskout,
+                                              uint32_t* __restrict__ hist, uint32_t invalid_bucket,
+                                              uint32_t* __restrict__ keys32)
 {
     long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     int s[6];
     if (BODY == 3) load_req3(req, i, s); else load_req2(req, i, s);
-    uint32_t key = invalid_key;
-    if (in_range(T, s, 2 * BODY)) {
-        if (BODY == 3) {
-            Side3 B = decode3(T, s[0], s[1], s[2]), K = decode3(T, s[3], s[4], s[5]);
-            if (select3(T, B, K)) key = (uint32_t)B.tup * T.n_tup3 + K.tup;
-        } else {
-            Side2 B = decode2(T, s[0], s[1]), K = decode2(T, s[2], s[3]);
-            if (select2(B, K)) key = (uint32_t)B.tup * T.n_tup2 + K.tup;
+    uint32_t key = REC_INVALID;
+    unsigned long long low = 0;
+    int mask = 0;
+    if (!in_range(T, s, 2 * BODY)) {
+        if (recs) atomicAdd(T.bad_count, 1ull);
+    } else if (BODY == 3) {
+        Side3 B = decode3(T, s[0], s[1], s[2]), K = decode3(T, s[3], s[4], s[5]);
+        if (select3(T, B, K)) {
+            key = (uint32_t)B.tup * T.n_tup3 + K.tup;
+            if (__ldg(T.slab_off3 + key) != NO_SLAB) mask = mask3(T, B, K, __ldg(T.tdesc3 + B.tup), __ldg(T.tdesc3 + K.tup));
+            low = (unsigned long long)(B.ima | (B.imb << 5) | (B.imc << 10) | (K.ima << 15) | (K.imb << 20) | (K.imc << 25)) |
+                  ((unsigned long long)((B.tz << 3) | K.tz) << 30) | ((unsigned long long)(B.sign * K.sign < 0) << 36);
+        }
+    } else {
+        Side2 B = decode2(T, s[0], s[1]), K = decode2(T, s[2], s[3]);
+        if (select2(B, K)) {
+            key = (uint32_t)B.tup * T.n_tup2 + K.tup;
+            if (__ldg(T.slab_off2 + key) != NO_SLAB) mask = mask2(B, __ldg(T.tdesc2 + B.tup), __ldg(T.tdesc2 + K.tup));
+            low = (unsigned long long)(B.ima | (B.imb << 5) | (K.ima << 15) | (K.imb << 20)) |
+                  ((unsigned long long)((B.tz << 3) | K.tz) << 30) | ((unsigned long long)(B.sign * K.sign < 0) << 36);
         }
     }
-    keys[i] = key;
-    if (hist) atomicAdd(hist + (key == invalid_key ? invalid_bucket : key), 1u);
+    if (recs) recs[i] = ((unsigned long long)key << REC_KEY_SHIFT) | low;
+    if (maskout) maskout[i] = (uint8_t)mask;
+    if (hist) atomicAdd(hist + (key == REC_INVALID ? invalid_bucket : key), 1u);
+    if (keys32) keys32[i] = key == REC_INVALID ? 0xFFFFFFFFu : key;
 }
 
-// H2: exclusive scan of the histogram (three small kernels), then scatter of request indices.
+// =============================================================================== H2: group sort
 constexpr int SCAN_T = 256, SCAN_E = 16, SCAN_TILE = SCAN_T * SCAN_E;
 
 __global__ void __launch_bounds__(SCAN_T) k_scan_tiles(uint32_t* __restrict__ data, long long m, uint32_t* __restrict__ tile_sums)
@@ -345,14 +371,212 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_add(uint32_t* __restrict__ data
         if (base + k < m) data[base + k] += add;
 }
 
-__global__ void __launch_bounds__(256) k_scatter(long long n, const uint32_t* __restrict__ keys, uint32_t* __restrict__ cursor,
-                                                 uint32_t* __restrict__ order, uint32_t invalid_key, uint32_t invalid_bucket)
+__global__ void __launch_bounds__(256) k_scatter(long long n, const unsigned long long* __restrict__ recs,
+                                                 uint32_t* __restrict__ cursor, unsigned long long* __restrict__ sorted,
+                                                 uint32_t* __restrict__ order, uint32_t invalid_bucket)
 {
     long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    uint32_t key = keys[i];
-    uint32_t pos = atomicAdd(cursor + (key == invalid_key ? invalid_bucket : key), 1u);
+    unsigned long long r = recs[i];
+    uint32_t key = (uint32_t)(r >> REC_KEY_SHIFT);
+    uint32_t pos = atomicAdd(cursor + (key == REC_INVALID ? invalid_bucket : key), 1u);
+    sorted[pos] = r;
     order[pos] = (uint32_t)i;
+}
+
+// =============================================================================== H3-H6: transform
+// One J block of the 3-body sum with the ket range size NK known at compile time: the NK ket coefficients live
+// in registers, one bra row (5*NK slab doubles, 128-bit loads at warp-uniform addresses) per iteration.
+template <int NK>
+__device__ __forceinline__ void j_block3(const double* __restrict__ cg2g, const int2* __restrict__ rtb,
+                                         const int2* __restrict__ rtk, int nb, const double* __restrict__ c1b,
+                                         const double* __restrict__ c1k, int Ab, int Ak, const double2*& rowp,
+                                         const double (&w)[5], double& total)
+{
+    double ck[NK];
+#pragma unroll
+    for (int k = 0; k < NK; k++) {
+        int2 rt = __ldg(rtk + k);
+        ck[k] = __ldg(c1k + k) * __ldg(cg2g + (rt.x + Ak * rt.y));
+    }
+    constexpr int NV = (NISO3 * NK + 1) / 2;
+    const double2* rp = rowp;
+    for (int i = 0; i < nb; i++) {
+        int2 rt = __ldg(rtb + i);
+        double cb = __ldg(c1b + i) * __ldg(cg2g + (rt.x + Ab * rt.y));
+        double v[2 * NV];
+#pragma unroll
+        for (int q = 0; q < NV; q++) {
+            double2 t = __ldg(rp + q);
+            v[2 * q] = t.x;
+            v[2 * q + 1] = t.y;
+        }
+        double acc = 0.0;
+#pragma unroll
+        for (int k = 0; k < NK; k++) {
+            double inner = w[0] * v[5 * k];
+            inner = fma(w[1], v[5 * k + 1], inner);
+            inner = fma(w[2], v[5 * k + 2], inner);
+            inner = fma(w[3], v[5 * k + 3], inner);
+            inner = fma(w[4], v[5 * k + 4], inner);
+            acc = fma(ck[k], inner, acc);
+        }
+        total = fma(cb, acc, total);
+        rp += NV;
+    }
+    rowp = rp;
+}
+
+// any ket range size (rare: nk > 8): ket coefficient recomputed per cell
+__device__ __noinline__ double j_block3_generic(const double* __restrict__ cg2g, const int2* __restrict__ rtb,
+                                                const int2* __restrict__ rtk, int nb, int nk, const double* __restrict__ c1b,
+                                                const double* __restrict__ c1k, int Ab, int Ak, const double* row,
+                                                double w0, double w1, double w2, double w3, double w4)
+{
+    const int pitch = row_pitch3(nk);
+    double total = 0.0;
+    for (int i = 0; i < nb; i++) {
+        int2 rt = __ldg(rtb + i);
+        double cb = __ldg(c1b + i) * __ldg(cg2g + (rt.x + Ab * rt.y));
+        double acc = 0.0;
+        for (int k = 0; k < nk; k++) {
+            int2 rk = __ldg(rtk + k);
+            double ck = __ldg(c1k + k) * __ldg(cg2g + (rk.x + Ak * rk.y));
+            const double* cell = row + NISO3 * k;
+            double inner = w0 * __ldg(cell);
+            inner = fma(w1, __ldg(cell + 1), inner);
+            inner = fma(w2, __ldg(cell + 2), inner);
+            inner = fma(w3, __ldg(cell + 3), inner);
+            inner = fma(w4, __ldg(cell + 4), inner);
+            acc = fma(ck, inner, acc);
+        }
+        total = fma(cb, acc, total);
+        row += pitch;
+    }
+    return total;
+}
+
+// One warp = 32 consecutive records of the group-ordered stream.  The warp walks over the (few) distinct groups
+// among its lanes; inside a group every loop bound, table row and slab address is warp-uniform, the lanes differ
+// only in their m/tz projections (the irregular loop structure is per element -- here it is per group).
+__global__ void __launch_bounds__(128) k_transform3(Tables T, long long n, const unsigned long long* __restrict__ recs,
+                                                   const uint32_t* __restrict__ order, double* __restrict__ out)
+{
+    const long long pos = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool valid = pos < n;
+    const unsigned long long rec = valid ? __ldg(recs + pos) : ~0ull;
+    const uint32_t key = (uint32_t)(rec >> REC_KEY_SHIFT);
+    bool done = !valid || key == REC_INVALID;
+    double result = 0.0;
+    const uint32_t nt = (uint32_t)T.n_tup3;
+    for (;;) {
+        unsigned pending = __ballot_sync(0xFFFFFFFFu, !done);
+        if (pending == 0) break;
+        const uint32_t g = __shfl_sync(0xFFFFFFFFu, key, __ffs(pending) - 1);
+        const bool mine = !done && key == g;
+        if (mine) done = true;
+        const uint32_t so = __ldg(T.slab_off3 + g);
+        if (so == NO_SLAB) continue;                        // no common channel: value 0
+        const uint32_t tb = g / nt, tk = g - tb * nt;
+        const int4 db = __ldg(T.tdesc3 + tb), dk = __ldg(T.tdesc3 + tk);
+        const int2 trb = __ldg(T.trow3 + tb), trk = __ldg(T.trow3 + tk);
+        const int ja = db.x & 255, jb = (db.x >> 8) & 255, jc = (db.x >> 16) & 255;
+        const int jd = dk.x & 255, je = (dk.x >> 8) & 255, jf = (dk.x >> 16) & 255;
+        // lane part (a lane of another group runs with m = 0: harmless, result discarded)
+        const uint32_t mrec = mine ? (uint32_t)rec : 0u;
+        const int ima = mrec & 31, imb = (mrec >> 5) & 31, imc = (mrec >> 10) & 31;
+        const int imd = (mrec >> 15) & 31, ime = (mrec >> 20) & 31, imf = (mrec >> 25) & 31;
+        const int Ab = (ima + imb - ((ja + jb) >> 1)) * (jc + 1) + imc;     // M12*(jc+1) + imc
+        const int Ak = (imd + ime - ((jd + je) >> 1)) * (jf + 1) + imf;
+        const int nj = T.nj;
+        const double* c1b = T.cg1 + __ldg(T.cg1_off + (ja >> 1) * nj + (jb >> 1)) + (ima * (jb + 1) + imb) * (min(ja, jb) + 1);
+        const double* c1k = T.cg1 + __ldg(T.cg1_off + (jd >> 1) * nj + (je >> 1)) + (imd * (je + 1) + ime) * (min(jd, je) + 1);
+        const int tz6 = mine ? (int)((rec >> 30) & 63) : 0;
+        double w[5];
+        {
+            const double2* wp = (const double2*)(T.wtab3 + tz6 * 6);
+            double2 a = __ldg(wp), b = __ldg(wp + 1), c = __ldg(wp + 2);
+            w[0] = a.x; w[1] = a.y; w[2] = b.x; w[3] = b.y; w[4] = c.x;
+        }
+        const int Jminb = (db.y >> 16) & 255, Jmink = (dk.y >> 16) & 255;
+        const int Jlo = max(Jminb, Jmink), Jhi = min((db.y >> 24) & 255, (dk.y >> 24) & 255);
+        const uint32_t* jib = T.jinfo3 + trb.y + ((Jlo - Jminb) >> 1);
+        const uint32_t* jik = T.jinfo3 + trk.y + ((Jlo - Jmink) >> 1);
+        const int2* rowb = T.rowtab3 + trb.x;
+        const int2* rowk = T.rowtab3 + trk.x;
+        const double2* rowp = (const double2*)T.slab3 + so;
+        double total = 0.0;
+        const int nJ = ((Jhi - Jlo) >> 1) + 1;
+        for (int q = 0; q < nJ; q++) {
+            const uint32_t ib = __ldg(jib + q), ik = __ldg(jik + q);
+            const int nb = ib >> 24, nk = ik >> 24;
+            const int2* rtb = rowb + (ib & 0xFFFF);
+            const int2* rtk = rowk + (ik & 0xFFFF);
+            const double* pb = c1b + ((ib >> 16) & 255);
+            const double* pk = c1k + ((ik >> 16) & 255);
+            switch (nk) {
+                case 0: break;
+                case 1: j_block3<1>(T.cg2g, rtb, rtk, nb, pb, pk, Ab, Ak, rowp, w, total); break;
+                case 2: j_block3<2>(T.cg2g, rtb, rtk, nb, pb, pk, Ab, Ak, rowp, w, total); break;
+                case 3: j_block3<3>(T.cg2g, rtb, rtk, nb, pb, pk, Ab, Ak, rowp, w, total); break;
+                case 4: j_block3<4>(T.cg2g, rtb, rtk, nb, pb, pk, Ab, Ak, rowp, w, total); break;
+                case 5: j_block3<5>(T.cg2g, rtb, rtk, nb, pb, pk, Ab, Ak, rowp, w, total); break;
+                case 6: j_block3<6>(T.cg2g, rtb, rtk, nb, pb, pk, Ab, Ak, rowp, w, total); break;
+                case 7: j_block3<7>(T.cg2g, rtb, rtk, nb, pb, pk, Ab, Ak, rowp, w, total); break;
+                case 8: j_block3<8>(T.cg2g, rtb, rtk, nb, pb, pk, Ab, Ak, rowp, w, total); break;
+                default:
+                    total += j_block3_generic(T.cg2g, rtb, rtk, nb, nk, pb, pk, Ab, Ak, (const double*)rowp, w[0], w[1], w[2], w[3], w[4]);
+                    rowp += (size_t)nb * (row_pitch3(nk) >> 1);
+                    break;
+            }
+        }
+        if (mine) result = (((rec >> 36) & 1) ? -total : total) + 0.0;   // + 0.0: never store -0
+    }
+    if (valid) out[order ? (long long)__ldg(order + pos) : pos] = result;
+}
+
+__global__ void __launch_bounds__(128) k_transform2(Tables T, long long n, const unsigned long long* __restrict__ recs,
+                                                   const uint32_t* __restrict__ order, double* __restrict__ out)
+{
+    const long long pos = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool valid = pos < n;
+    const unsigned long long rec = valid ? __ldg(recs + pos) : ~0ull;
+    const uint32_t key = (uint32_t)(rec >> REC_KEY_SHIFT);
+    bool done = !valid || key == REC_INVALID;
+    double result = 0.0;
+    const uint32_t nt = (uint32_t)T.n_tup2;
+    for (;;) {
+        unsigned pending = __ballot_sync(0xFFFFFFFFu, !done);
+        if (pending == 0) break;
+        const uint32_t g = __shfl_sync(0xFFFFFFFFu, key, __ffs(pending) - 1);
+        const bool mine = !done && key == g;
+        if (mine) done = true;
+        const uint32_t so = __ldg(T.slab_off2 + g);
+        if (so == NO_SLAB) continue;
+        const uint32_t tb = g / nt, tk = g - tb * nt;
+        const int4 db = __ldg(T.tdesc2 + tb), dk = __ldg(T.tdesc2 + tk);
+        const int ja = db.x & 255, jb = (db.x >> 8) & 255, jc = dk.x & 255, jd = (dk.x >> 8) & 255;
+        const uint32_t mrec = mine ? (uint32_t)rec : 0u;
+        const int ima = mrec & 31, imb = (mrec >> 5) & 31, imc = (mrec >> 15) & 31, imd = (mrec >> 20) & 31;
+        const int tzb = mine ? (int)((rec >> 33) & 3) : 0, tzk = mine ? (int)((rec >> 30) & 3) : 0;
+        const double2 w = __ldg((const double2*)T.wtab2 + (tzb * 4 + tzk));
+        const int nj = T.nj;
+        const int Jminb = db.y & 255, Jmink = dk.y & 255;
+        const int Jlo = max(Jminb, Jmink), Jhi = min((db.y >> 8) & 255, (dk.y >> 8) & 255);
+        const double* cb = T.cg1 + __ldg(T.cg1_off + (ja >> 1) * nj + (jb >> 1)) + (ima * (jb + 1) + imb) * (min(ja, jb) + 1) + (Jlo - Jminb);
+        const double* ck = T.cg1 + __ldg(T.cg1_off + (jc >> 1) * nj + (jd >> 1)) + (imc * (jd + 1) + imd) * (min(jc, jd) + 1) + (Jlo - Jmink);
+        const double2* cell = (const double2*)T.slab2 + so;
+        double total = 0.0;
+        for (int q = 0; q <= Jhi - Jlo; q++) {
+            double2 v = __ldg(cell + q);
+            double c = __ldg(cb + q) * __ldg(ck + q);
+            total = fma(c, fma(w.y, v.y, w.x * v.x), total);
+        }
+        double norm = ((db.x >> 24) & 1) ? (((dk.x >> 24) & 1) ? 2.0 : 1.4142135623730951)
+                                         : (((dk.x >> 24) & 1) ? 1.4142135623730951 : 1.0);
+        if (mine) result = (((rec >> 36) & 1) ? -(norm * total) : norm * total) + 0.0;
+    }
+    if (valid) out[order ? (long long)__ldg(order + pos) : pos] = result;
 }
 
 size_t align256(size_t x) { return (x + 255) & ~size_t(255); }
@@ -364,26 +588,30 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
     if (!c || !work_bytes || n < 0 || n >= (int64_t)0xFFFFFFF0ll) return c ? fail(c, MFDN_ERR_ARG, "bad n / work_bytes") : MFDN_ERR_ARG;
     if (BODY == 3 ? !c->has3 : !c->has2) return fail(c, MFDN_ERR_STATE, "mscheme before coupled upload");
     const long long nt = BODY == 3 ? c->t.n_tup3 : c->t.n_tup2;
+    if (nt * nt >= (long long)REC_INVALID) return fail(c, MFDN_ERR_ARG, "too many tuples for 27-bit group keys");
     const long long n_buckets = nt * nt + 1;   // last bucket: requests failing S1-S6
     const long long n_tiles = (n_buckets + SCAN_TILE - 1) / SCAN_TILE;
-    const bool sorted_path = !(flags & (MFDN_PRESORTED | MFDN_FORCE_NAIVE));
+    const bool naive = flags & MFDN_FORCE_NAIVE;
+    const bool sort = !naive && !(flags & MFDN_PRESORTED);
     size_t need = 256;
-    size_t o_keys = 0, o_order = 0, o_hist = 0, o_sums = 0;
-    if (sorted_path) {
-        o_keys = 0;
-        o_order = o_keys + align256((size_t)n * 4);
-        o_hist = o_order + align256((size_t)n * 4);
-        o_sums = o_hist + align256((size_t)n_buckets * 4);
-        need = o_sums + align256((size_t)n_tiles * 4);
+    size_t o_recs = 0, o_sorted = 0, o_order = 0, o_hist = 0, o_sums = 0;
+    if (!naive) {
+        o_recs = 0;
+        need = o_recs + align256((size_t)n * 8);
+        if (sort) {
+            o_sorted = need;
+            o_order = o_sorted + align256((size_t)n * 8);
+            o_hist = o_order + align256((size_t)n * 4);
+            o_sums = o_hist + align256((size_t)n_buckets * 4);
+            need = o_sums + align256((size_t)n_tiles * 4);
+        }
     }
     if (!d_work) { *work_bytes = need; return MFDN_OK; }
     if (*work_bytes < need) return fail(c, MFDN_ERR_OOM, "scratch too small");
     if (n == 0) return MFDN_OK;
     if (!d_req || !d_out) return fail(c, MFDN_ERR_ARG, "null request/output pointer");
-    if (nt * nt >= 0xFFFFFFF0ll) return fail(c, MFDN_ERR_ARG, "too many tuples for 32-bit group keys");
     cudaStream_t st = (cudaStream_t)stream;
-    const uint32_t* order = nullptr;
-    mfdn_ctx::EvTriple ev{nullptr, nullptr, nullptr, sorted_path};
+    mfdn_ctx::EvTriple ev{nullptr, nullptr, nullptr, sort};
     if (c->profile) {
         cudaEvent_t* e3[3] = {&ev.a, &ev.b, &ev.c};
         for (auto pe : e3) {
@@ -392,24 +620,39 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
         }
         MFDN_CUDA(c, cudaEventRecord(ev.a, st));
     }
-    if (sorted_path) {
+    if (naive) {
+        if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.b, st));
+        k_mscheme_naive<BODY><<<(unsigned)((n + 127) / 128), 128, 0, st>>>(c->t, n, d_req, d_out, d_mask);
+        c->launches += 1;
+    } else {
         char* w = (char*)d_work;
-        uint32_t* keys = (uint32_t*)(w + o_keys);
-        uint32_t* ord = (uint32_t*)(w + o_order);
-        uint32_t* hist = (uint32_t*)(w + o_hist);
-        uint32_t* sums = (uint32_t*)(w + o_sums);
-        MFDN_CUDA(c, cudaMemsetAsync(hist, 0, (size_t)n_buckets * 4, st));
-        k_keys<BODY><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(c->t, n, d_req, keys, hist, 0xFFFFFFFFu, (uint32_t)(nt * nt));
-        k_scan_tiles<<<(unsigned)n_tiles, SCAN_T, 0, st>>>(hist, n_buckets, sums);
-        k_scan_sums<<<1, 1024, 0, st>>>(sums, (int)n_tiles);
-        k_scan_add<<<(unsigned)n_tiles, SCAN_T, 0, st>>>(hist, n_buckets, sums);
-        k_scatter<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, keys, hist, ord, 0xFFFFFFFFu, (uint32_t)(nt * nt));
-        c->launches += 5;
-        order = ord;
+        unsigned long long* recs = (unsigned long long*)(w + o_recs);
+        const unsigned long long* trecs = recs;
+        const uint32_t* order = nullptr;
+        const unsigned gk = (unsigned)((n + 255) / 256);
+        if (sort) {
+            unsigned long long* sorted = (unsigned long long*)(w + o_sorted);
+            uint32_t* ord = (uint32_t*)(w + o_order);
+            uint32_t* hist = (uint32_t*)(w + o_hist);
+            uint32_t* sums = (uint32_t*)(w + o_sums);
+            MFDN_CUDA(c, cudaMemsetAsync(hist, 0, (size_t)n_buckets * 4, st));
+            k_keys<BODY><<<gk, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, (uint32_t)(nt * nt), nullptr);
+            k_scan_tiles<<<(unsigned)n_tiles, SCAN_T, 0, st>>>(hist, n_buckets, sums);
+            k_scan_sums<<<1, 1024, 0, st>>>(sums, (int)n_tiles);
+            k_scan_add<<<(unsigned)n_tiles, SCAN_T, 0, st>>>(hist, n_buckets, sums);
+            k_scatter<<<gk, 256, 0, st>>>(n, recs, hist, sorted, ord, (uint32_t)(nt * nt));
+            c->launches += 5;
+            trecs = sorted;
+            order = ord;
+        } else {
+            k_keys<BODY><<<gk, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, nullptr, 0u, nullptr);
+            c->launches += 1;
+        }
+        if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.b, st));
+        if (BODY == 3) k_transform3<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(c->t, n, trecs, order, d_out);
+        else k_transform2<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(c->t, n, trecs, order, d_out);
+        c->launches += 1;
     }
-    if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.b, st));
-    k_mscheme<BODY><<<(unsigned)((n + 127) / 128), 128, 0, st>>>(c->t, n, d_req, order, d_out, d_mask);
-    c->launches += 1;
     MFDN_CUDA(c, cudaGetLastError());
     if (c->profile) {
         MFDN_CUDA(c, cudaEventRecord(ev.c, st));
@@ -450,10 +693,8 @@ extern "C" int mfdn_group_keys(mfdn_ctx* c, int body, int64_t n, const int32_t* 
     if (body == 3 ? !c->has3 : !c->has2) return fail(c, MFDN_ERR_STATE, "group_keys before coupled upload");
     if (n == 0) return MFDN_OK;
     cudaStream_t st = (cudaStream_t)stream;
-    if (body == 3)
-        k_keys<3><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(c->t, n, d_req, d_key, nullptr, 0xFFFFFFFFu, 0u);
-    else
-        k_keys<2><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(c->t, n, d_req, d_key, nullptr, 0xFFFFFFFFu, 0u);
+    if (body == 3) k_keys<3><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(c->t, n, d_req, nullptr, nullptr, nullptr, 0u, d_key);
+    else k_keys<2><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(c->t, n, d_req, nullptr, nullptr, nullptr, 0u, d_key);
     MFDN_CUDA(c, cudaGetLastError());
     return MFDN_OK;
 }
