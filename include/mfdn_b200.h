@@ -62,7 +62,7 @@ int mfdn_cg_build(mfdn_ctx*, void* stream);
 /* Test hook: copy a CG table to HOST memory (synchronises).  stage 1 = <j1 m1 j2 m2|J M> for half-integer
  * j1,j2 <= jmax; stage 2 = <J12 M12 j m|J M> for integer J12 <= 2*jmax and half-integer j <= jmax.
  * Layout: blocks in ascending (first, second) angular momentum order; stage-1 block (2j1,2j2) holds
- * [i1][i2][iJ] (iJ fastest), i = (2m+2j)/2, iJ = (2J - |2j1-2j2|)/2, value <j1 m1 j2 m2|J m1+m2>
+ * [iJ][i1][i2] (i2 fastest), i = (2m+2j)/2, iJ = (2J - |2j1-2j2|)/2, value <j1 m1 j2 m2|J m1+m2>
  * (0 where |m1+m2| > J); stage-2 block (J12, 2j) likewise with j1 = J12.
  * *n receives the entry count; if host_out is NULL or cap < *n nothing is copied. */
 int mfdn_cg_download(mfdn_ctx*, int stage, double* host_out, int64_t cap, int64_t* n);

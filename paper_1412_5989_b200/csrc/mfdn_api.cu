@@ -197,11 +197,11 @@ __global__ void k_cg_build(const CgBlock* __restrict__ blocks, const double2* __
     CgBlock b = blocks[blockIdx.y];
     auto LF = [&](int n) { double2 v = lfact[n]; return dd{v.x, v.y}; };
     auto BIN = [&](int n, int k) { return binom[n * BINOM_N + k]; };
-    const int nJ = min(b.tj1, b.tj2) + 1;
     for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < b.count; idx += gridDim.x * blockDim.x) {
-        int iJ = idx % nJ;
-        int i2 = (idx / nJ) % (b.tj2 + 1);
-        int i1 = idx / (nJ * (b.tj2 + 1));
+        // layout [iJ][i1][i2] (projections fastest: the lanes of a warp differ only in their projections)
+        int i2 = idx % (b.tj2 + 1);
+        int i1 = (idx / (b.tj2 + 1)) % (b.tj1 + 1);
+        int iJ = idx / ((b.tj1 + 1) * (b.tj2 + 1));
         int tJ = abs(b.tj1 - b.tj2) + 2 * iJ, tm1 = 2 * i1 - b.tj1, tm2 = 2 * i2 - b.tj2, tM = tm1 + tm2;
         double val = 0.0;
         if (abs(tM) <= tJ) {
@@ -530,31 +530,31 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
         lo = std::max(d.y & 255, std::abs(twoJ - jc) >> 1);
         hi = std::min((d.y >> 8) & 255, (twoJ + jc) >> 1);
     };
-    // ---- row tables: per (tuple, J, J12) the address part of <J12 M12 jc mc|J M> that does not depend on the
-    //      request: offset = cg2_off[J12][jc] + J12*(jc+1)*nJ + iJ (+ CG_GUARD); the kernel adds A*nJ with
-    //      A = M12*(jc+1) + imc  (A2 "tile index": flat offsets, no pointers -- PAPER.md:109-121)
-    std::vector<int2> trow(nt), rowtab;
-    std::vector<uint32_t> jinfo;
+    // ---- row tables (A2 "tile index": flat offsets, no pointers -- PAPER.md:109-121).  Per (tuple, J, J12) row the
+    //      request-independent parts of the two coefficient addresses:
+    //        x: <J12 M12 jc mc|J M> lives at cg2g[x + A],  A = M12*(jc+1) + imc  (x includes CG_GUARD and J12*(jc+1))
+    //        y: <ja ma jb mb|J12 M12> lives at cg1[c1_lane + y],  c1_lane = off(ja,jb) + ima*(jb+1) + imb
+    //      and per (tuple, J): {first row (absolute), number of rows}
+    std::vector<int2> trow(nt), rowtab, jinfo;
     for (int t = 0; t < nt; t++) {
         int4 d = tdesc[t];
-        int jc = (d.x >> 16) & 255;
+        int ja = d.x & 255, jb = (d.x >> 8) & 255, jc = (d.x >> 16) & 255;
         trow[t].x = (int)rowtab.size();
         trow[t].y = (int)jinfo.size();
-        uint32_t rows = 0;
         for (int twoJ = (d.y >> 16) & 255; twoJ <= ((d.y >> 24) & 255); twoJ += 2) {
             int lo, hi;
             range(d, twoJ, lo, hi);
-            int nrow = std::max(0, hi - lo + 1);
-            if (rows > 0xFFFF || nrow > 255) return fail(c, MFDN_ERR_ARG, "tuple has too many rows");
-            jinfo.push_back(rows | ((uint32_t)(lo - (d.y & 255)) << 16) | ((uint32_t)nrow << 24));
+            int2 ji;
+            ji.x = (int)rowtab.size();
+            ji.y = std::max(0, hi - lo + 1);
+            jinfo.push_back(ji);
             for (int J12 = lo; J12 <= hi; J12++) {
-                int nJ = std::min(2 * J12, jc) + 1;
+                int iJ = (twoJ - std::abs(2 * J12 - jc)) / 2;
                 int2 e;
-                e.x = CG_GUARD + c->h_cg2_off[J12 * c->t.nj + (jc >> 1)] + J12 * (jc + 1) * nJ + (twoJ - std::abs(2 * J12 - jc)) / 2;
-                e.y = nJ;
+                e.x = CG_GUARD + c->h_cg2_off[J12 * c->t.nj + (jc >> 1)] + (iJ * (2 * J12 + 1) + J12) * (jc + 1);
+                e.y = (J12 - (d.y & 255)) * (ja + 1) * (jb + 1);
                 rowtab.push_back(e);
             }
-            rows += nrow;
         }
     }
     // ---- slab offsets (16-byte units) per (bra tuple, ket tuple) group, rows in loop order J, J12
@@ -624,7 +624,7 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     c->t.stmask3 = (const unsigned long long*)(dres + o_sm);
     c->t.trow3 = (const int2*)(dres + o_trow);
     c->t.rowtab3 = (const int2*)(dres + o_rowtab);
-    c->t.jinfo3 = (const uint32_t*)(dres + o_jinfo);
+    c->t.jinfo3 = (const int2*)(dres + o_jinfo);
     c->slab_bytes3 = (int64_t)(cells * 16);
     c->has3 = true;
     return MFDN_OK;

@@ -72,8 +72,8 @@ struct Tables {
     const double* slab3;
     const unsigned long long* stmask3;
     const int2* trow3;             // [n_tup3] {first row of the tuple in rowtab3, first entry in jinfo3}
-    const int2* rowtab3;           // per (tuple, J, J12) row: {offset into cg2g of <J12 . jc .|J .> at A = 0, nJ}
-    const uint32_t* jinfo3;        // per (tuple, J): row start (16 b) | (first J12 - J12min) << 16 | n rows << 24
+    const int2* rowtab3;           // per (tuple, J, J12) row: {cg2g offset at A = 0, cg1 offset relative to the lane base}
+    const int2* jinfo3;            // per (tuple, J): {first row in rowtab3 (absolute), number of rows}
     // A2, 2-body
     int n_tup2;
     const int32_t* tuple_id2;      // [n_orb^2]

@@ -176,8 +176,10 @@ __device__ __forceinline__ double eval3_naive(const Tables& T, const Side3& B, c
     const double w0 = ib[0] * ik[0], w1 = ib[0] * ik[1], w2 = ib[1] * ik[0], w3 = ib[1] * ik[1], w4 = ib[2] * ik[2];
     const int nj = T.nj;
     const int J12minb = db.y & 255, J12mink = dk.y & 255;
-    const double* c1b = T.cg1 + __ldg(T.cg1_off + (ja >> 1) * nj + (jb >> 1)) + (B.ima * (jb + 1) + B.imb) * (min(ja, jb) + 1);
-    const double* c1k = T.cg1 + __ldg(T.cg1_off + (jd >> 1) * nj + (je >> 1)) + (K.ima * (je + 1) + K.imb) * (min(jd, je) + 1);
+    // CG blocks are [iJ][i1][i2]
+    const double* c1b = T.cg1 + __ldg(T.cg1_off + (ja >> 1) * nj + (jb >> 1)) + B.ima * (jb + 1) + B.imb;
+    const double* c1k = T.cg1 + __ldg(T.cg1_off + (jd >> 1) * nj + (je >> 1)) + K.ima * (je + 1) + K.imb;
+    const int S1b = (ja + 1) * (jb + 1), S1k = (jd + 1) * (je + 1);
     const double* row = T.slab3 + (size_t)so * 2;
     const int Jlo = max((db.y >> 16) & 255, (dk.y >> 16) & 255), Jhi = min((db.y >> 24) & 255, (dk.y >> 24) & 255);
     double total = 0.0;
@@ -192,18 +194,18 @@ __device__ __forceinline__ double eval3_naive(const Tables& T, const Side3& B, c
             double cb = 0.0;
             if (abs(twoM12b) <= 2 * J12) {
                 const double* c2 = T.cg2 + __ldg(T.cg2_off + J12 * nj + (jc >> 1));
-                int nJ = min(2 * J12, jc) + 1;
-                cb = __ldg(c1b + (J12 - J12minb)) *
-                     __ldg(c2 + (((twoM12b + 2 * J12) >> 1) * (jc + 1) + B.imc) * nJ + ((twoJ - abs(2 * J12 - jc)) >> 1));
+                int iJ = (twoJ - abs(2 * J12 - jc)) >> 1;
+                cb = __ldg(c1b + (J12 - J12minb) * S1b) *
+                     __ldg(c2 + (iJ * (2 * J12 + 1) + ((twoM12b + 2 * J12) >> 1)) * (jc + 1) + B.imc);
             }
             double acc = 0.0;
             for (int J12p = lk; J12p <= hk; J12p++) {
                 double ck = 0.0;
                 if (abs(twoM12k) <= 2 * J12p) {
                     const double* c2 = T.cg2 + __ldg(T.cg2_off + J12p * nj + (jf >> 1));
-                    int nJ = min(2 * J12p, jf) + 1;
-                    ck = __ldg(c1k + (J12p - J12mink)) *
-                         __ldg(c2 + (((twoM12k + 2 * J12p) >> 1) * (jf + 1) + K.imc) * nJ + ((twoJ - abs(2 * J12p - jf)) >> 1));
+                    int iJ = (twoJ - abs(2 * J12p - jf)) >> 1;
+                    ck = __ldg(c1k + (J12p - J12mink) * S1k) *
+                         __ldg(c2 + (iJ * (2 * J12p + 1) + ((twoM12k + 2 * J12p) >> 1)) * (jf + 1) + K.imc);
                 }
                 const double* cell = row + NISO3 * (J12p - lk);
                 double inner = w0 * __ldg(cell);
@@ -233,14 +235,15 @@ __device__ __forceinline__ double eval2_naive(const Tables& T, const Side2& B, c
     const double w0 = T.iso2[B.tz][0] * T.iso2[K.tz][0], w1 = T.iso2[B.tz][1] * T.iso2[K.tz][1];
     const int nj = T.nj;
     const int Jminb = db.y & 255, Jmink = dk.y & 255;
-    const double* cb = T.cg1 + __ldg(T.cg1_off + (ja >> 1) * nj + (jb >> 1)) + (B.ima * (jb + 1) + B.imb) * (min(ja, jb) + 1);
-    const double* ck = T.cg1 + __ldg(T.cg1_off + (jc >> 1) * nj + (jd >> 1)) + (K.ima * (jd + 1) + K.imb) * (min(jc, jd) + 1);
+    const double* cb = T.cg1 + __ldg(T.cg1_off + (ja >> 1) * nj + (jb >> 1)) + B.ima * (jb + 1) + B.imb;
+    const double* ck = T.cg1 + __ldg(T.cg1_off + (jc >> 1) * nj + (jd >> 1)) + K.ima * (jd + 1) + K.imb;
+    const int Sb = (ja + 1) * (jb + 1), Sk = (jc + 1) * (jd + 1);
     const int Jlo = max(Jminb, Jmink), Jhi = min((db.y >> 8) & 255, (dk.y >> 8) & 255);
     const double2* cell = (const double2*)(T.slab2 + (size_t)so * CELL2);
     double total = 0.0;
     for (int J = Jlo; J <= Jhi; J++) {
         double2 v = __ldg(cell + (J - Jlo));
-        double c = __ldg(cb + (J - Jminb)) * __ldg(ck + (J - Jmink));
+        double c = __ldg(cb + (J - Jminb) * Sb) * __ldg(ck + (J - Jmink) * Sk);
         total = fma(c, fma(w1, v.y, w0 * v.x), total);
     }
     double norm = ((db.x >> 24) & 1) ? (((dk.x >> 24) & 1) ? 2.0 : 1.4142135623730951)
@@ -385,29 +388,31 @@ __global__ void __launch_bounds__(256) k_scatter(long long n, const unsigned lon
 }
 
 // =============================================================================== H3-H6: transform
+// All table accesses are 32-bit indices off kernel-parameter base pointers (one IMAD.WIDE per load).
 // One J block of the 3-body sum with the ket range size NK known at compile time: the NK ket coefficients live
 // in registers, one bra row (5*NK slab doubles, 128-bit loads at warp-uniform addresses) per iteration.
 template <int NK>
-__device__ __forceinline__ void j_block3(const double* __restrict__ cg2g, const int2* __restrict__ rtb,
-                                         const int2* __restrict__ rtk, int nb, const double* __restrict__ c1b,
-                                         const double* __restrict__ c1k, int Ab, int Ak, const double2*& rowp,
-                                         const double (&w)[5], double& total)
+__device__ __forceinline__ double j_block3(const Tables& T, uint32_t rb0, uint32_t rk0, int nb, uint32_t c1b, uint32_t c1k,
+                                           int Ab, int Ak, uint32_t& so, const double (&w)[5])
 {
     double ck[NK];
 #pragma unroll
     for (int k = 0; k < NK; k++) {
-        int2 rt = __ldg(rtk + k);
-        ck[k] = __ldg(c1k + k) * __ldg(cg2g + (rt.x + Ak * rt.y));
+        int2 rt = __ldg(T.rowtab3 + rk0 + k);
+        ck[k] = __ldg(T.cg1 + (c1k + (uint32_t)rt.y)) * __ldg(T.cg2g + (uint32_t)(rt.x + Ak));
     }
     constexpr int NV = (NISO3 * NK + 1) / 2;
-    const double2* rp = rowp;
+    const double2* slab = (const double2*)T.slab3;
+    uint32_t rp = so;
+    double total = 0.0;
+#pragma unroll 2
     for (int i = 0; i < nb; i++) {
-        int2 rt = __ldg(rtb + i);
-        double cb = __ldg(c1b + i) * __ldg(cg2g + (rt.x + Ab * rt.y));
+        int2 rt = __ldg(T.rowtab3 + rb0 + i);
+        double cb = __ldg(T.cg1 + (c1b + (uint32_t)rt.y)) * __ldg(T.cg2g + (uint32_t)(rt.x + Ab));
         double v[2 * NV];
 #pragma unroll
         for (int q = 0; q < NV; q++) {
-            double2 t = __ldg(rp + q);
+            double2 t = __ldg(slab + rp + q);
             v[2 * q] = t.x;
             v[2 * q + 1] = t.y;
         }
@@ -424,24 +429,26 @@ __device__ __forceinline__ void j_block3(const double* __restrict__ cg2g, const 
         total = fma(cb, acc, total);
         rp += NV;
     }
-    rowp = rp;
+    so = rp;
+    return total;
 }
 
 // any ket range size (rare: nk > 8): ket coefficient recomputed per cell
-__device__ __noinline__ double j_block3_generic(const double* __restrict__ cg2g, const int2* __restrict__ rtb,
-                                                const int2* __restrict__ rtk, int nb, int nk, const double* __restrict__ c1b,
-                                                const double* __restrict__ c1k, int Ab, int Ak, const double* row,
-                                                double w0, double w1, double w2, double w3, double w4)
+struct GenericPtrs { const int2* rowtab3; const double* cg1; const double* cg2g; const double* slab3; };
+__device__ __noinline__ double j_block3_generic(GenericPtrs T, uint32_t rb0, uint32_t rk0, int nb, int nk, uint32_t c1b,
+                                                uint32_t c1k, int Ab, int Ak, uint32_t so, double w0, double w1, double w2,
+                                                double w3, double w4)
 {
     const int pitch = row_pitch3(nk);
+    const double* row = T.slab3 + (size_t)so * 2;
     double total = 0.0;
     for (int i = 0; i < nb; i++) {
-        int2 rt = __ldg(rtb + i);
-        double cb = __ldg(c1b + i) * __ldg(cg2g + (rt.x + Ab * rt.y));
+        int2 rt = __ldg(T.rowtab3 + rb0 + i);
+        double cb = __ldg(T.cg1 + (c1b + (uint32_t)rt.y)) * __ldg(T.cg2g + (uint32_t)(rt.x + Ab));
         double acc = 0.0;
         for (int k = 0; k < nk; k++) {
-            int2 rk = __ldg(rtk + k);
-            double ck = __ldg(c1k + k) * __ldg(cg2g + (rk.x + Ak * rk.y));
+            int2 rk = __ldg(T.rowtab3 + rk0 + k);
+            double ck = __ldg(T.cg1 + (c1k + (uint32_t)rk.y)) * __ldg(T.cg2g + (uint32_t)(rk.x + Ak));
             const double* cell = row + NISO3 * k;
             double inner = w0 * __ldg(cell);
             inner = fma(w1, __ldg(cell + 1), inner);
@@ -475,7 +482,7 @@ __global__ void __launch_bounds__(128) k_transform3(Tables T, long long n, const
         const uint32_t g = __shfl_sync(0xFFFFFFFFu, key, __ffs(pending) - 1);
         const bool mine = !done && key == g;
         if (mine) done = true;
-        const uint32_t so = __ldg(T.slab_off3 + g);
+        uint32_t so = __ldg(T.slab_off3 + g);
         if (so == NO_SLAB) continue;                        // no common channel: value 0
         const uint32_t tb = g / nt, tk = g - tb * nt;
         const int4 db = __ldg(T.tdesc3 + tb), dk = __ldg(T.tdesc3 + tk);
@@ -489,44 +496,38 @@ __global__ void __launch_bounds__(128) k_transform3(Tables T, long long n, const
         const int Ab = (ima + imb - ((ja + jb) >> 1)) * (jc + 1) + imc;     // M12*(jc+1) + imc
         const int Ak = (imd + ime - ((jd + je) >> 1)) * (jf + 1) + imf;
         const int nj = T.nj;
-        const double* c1b = T.cg1 + __ldg(T.cg1_off + (ja >> 1) * nj + (jb >> 1)) + (ima * (jb + 1) + imb) * (min(ja, jb) + 1);
-        const double* c1k = T.cg1 + __ldg(T.cg1_off + (jd >> 1) * nj + (je >> 1)) + (imd * (je + 1) + ime) * (min(jd, je) + 1);
+        const uint32_t c1b = (uint32_t)(__ldg(T.cg1_off + (ja >> 1) * nj + (jb >> 1)) + ima * (jb + 1) + imb);
+        const uint32_t c1k = (uint32_t)(__ldg(T.cg1_off + (jd >> 1) * nj + (je >> 1)) + imd * (je + 1) + ime);
         const int tz6 = mine ? (int)((rec >> 30) & 63) : 0;
         double w[5];
         {
-            const double2* wp = (const double2*)(T.wtab3 + tz6 * 6);
+            const double2* wp = (const double2*)T.wtab3 + tz6 * 3;
             double2 a = __ldg(wp), b = __ldg(wp + 1), c = __ldg(wp + 2);
             w[0] = a.x; w[1] = a.y; w[2] = b.x; w[3] = b.y; w[4] = c.x;
         }
         const int Jminb = (db.y >> 16) & 255, Jmink = (dk.y >> 16) & 255;
         const int Jlo = max(Jminb, Jmink), Jhi = min((db.y >> 24) & 255, (dk.y >> 24) & 255);
-        const uint32_t* jib = T.jinfo3 + trb.y + ((Jlo - Jminb) >> 1);
-        const uint32_t* jik = T.jinfo3 + trk.y + ((Jlo - Jmink) >> 1);
-        const int2* rowb = T.rowtab3 + trb.x;
-        const int2* rowk = T.rowtab3 + trk.x;
-        const double2* rowp = (const double2*)T.slab3 + so;
+        const uint32_t jib = (uint32_t)(trb.y + ((Jlo - Jminb) >> 1)), jik = (uint32_t)(trk.y + ((Jlo - Jmink) >> 1));
         double total = 0.0;
         const int nJ = ((Jhi - Jlo) >> 1) + 1;
         for (int q = 0; q < nJ; q++) {
-            const uint32_t ib = __ldg(jib + q), ik = __ldg(jik + q);
-            const int nb = ib >> 24, nk = ik >> 24;
-            const int2* rtb = rowb + (ib & 0xFFFF);
-            const int2* rtk = rowk + (ik & 0xFFFF);
-            const double* pb = c1b + ((ib >> 16) & 255);
-            const double* pk = c1k + ((ik >> 16) & 255);
+            const int2 ib = __ldg(T.jinfo3 + jib + q), ik = __ldg(T.jinfo3 + jik + q);
+            const int nb = ib.y, nk = ik.y;
+            const uint32_t rb0 = (uint32_t)ib.x, rk0 = (uint32_t)ik.x;
             switch (nk) {
                 case 0: break;
-                case 1: j_block3<1>(T.cg2g, rtb, rtk, nb, pb, pk, Ab, Ak, rowp, w, total); break;
-                case 2: j_block3<2>(T.cg2g, rtb, rtk, nb, pb, pk, Ab, Ak, rowp, w, total); break;
-                case 3: j_block3<3>(T.cg2g, rtb, rtk, nb, pb, pk, Ab, Ak, rowp, w, total); break;
-                case 4: j_block3<4>(T.cg2g, rtb, rtk, nb, pb, pk, Ab, Ak, rowp, w, total); break;
-                case 5: j_block3<5>(T.cg2g, rtb, rtk, nb, pb, pk, Ab, Ak, rowp, w, total); break;
-                case 6: j_block3<6>(T.cg2g, rtb, rtk, nb, pb, pk, Ab, Ak, rowp, w, total); break;
-                case 7: j_block3<7>(T.cg2g, rtb, rtk, nb, pb, pk, Ab, Ak, rowp, w, total); break;
-                case 8: j_block3<8>(T.cg2g, rtb, rtk, nb, pb, pk, Ab, Ak, rowp, w, total); break;
+                case 1: total += j_block3<1>(T, rb0, rk0, nb, c1b, c1k, Ab, Ak, so, w); break;
+                case 2: total += j_block3<2>(T, rb0, rk0, nb, c1b, c1k, Ab, Ak, so, w); break;
+                case 3: total += j_block3<3>(T, rb0, rk0, nb, c1b, c1k, Ab, Ak, so, w); break;
+                case 4: total += j_block3<4>(T, rb0, rk0, nb, c1b, c1k, Ab, Ak, so, w); break;
+                case 5: total += j_block3<5>(T, rb0, rk0, nb, c1b, c1k, Ab, Ak, so, w); break;
+                case 6: total += j_block3<6>(T, rb0, rk0, nb, c1b, c1k, Ab, Ak, so, w); break;
+                case 7: total += j_block3<7>(T, rb0, rk0, nb, c1b, c1k, Ab, Ak, so, w); break;
+                case 8: total += j_block3<8>(T, rb0, rk0, nb, c1b, c1k, Ab, Ak, so, w); break;
                 default:
-                    total += j_block3_generic(T.cg2g, rtb, rtk, nb, nk, pb, pk, Ab, Ak, (const double*)rowp, w[0], w[1], w[2], w[3], w[4]);
-                    rowp += (size_t)nb * (row_pitch3(nk) >> 1);
+                    total += j_block3_generic(GenericPtrs{T.rowtab3, T.cg1, T.cg2g, T.slab3}, rb0, rk0, nb, nk, c1b, c1k, Ab, Ak, so,
+                                              w[0], w[1], w[2], w[3], w[4]);
+                    so += (uint32_t)nb * (row_pitch3(nk) >> 1);
                     break;
             }
         }
@@ -563,13 +564,14 @@ __global__ void __launch_bounds__(128) k_transform2(Tables T, long long n, const
         const int nj = T.nj;
         const int Jminb = db.y & 255, Jmink = dk.y & 255;
         const int Jlo = max(Jminb, Jmink), Jhi = min((db.y >> 8) & 255, (dk.y >> 8) & 255);
-        const double* cb = T.cg1 + __ldg(T.cg1_off + (ja >> 1) * nj + (jb >> 1)) + (ima * (jb + 1) + imb) * (min(ja, jb) + 1) + (Jlo - Jminb);
-        const double* ck = T.cg1 + __ldg(T.cg1_off + (jc >> 1) * nj + (jd >> 1)) + (imc * (jd + 1) + imd) * (min(jc, jd) + 1) + (Jlo - Jmink);
+        const int Sb = (ja + 1) * (jb + 1), Sk = (jc + 1) * (jd + 1);
+        const double* cb = T.cg1 + __ldg(T.cg1_off + (ja >> 1) * nj + (jb >> 1)) + ima * (jb + 1) + imb + (Jlo - Jminb) * Sb;
+        const double* ck = T.cg1 + __ldg(T.cg1_off + (jc >> 1) * nj + (jd >> 1)) + imc * (jd + 1) + imd + (Jlo - Jmink) * Sk;
         const double2* cell = (const double2*)T.slab2 + so;
         double total = 0.0;
         for (int q = 0; q <= Jhi - Jlo; q++) {
             double2 v = __ldg(cell + q);
-            double c = __ldg(cb + q) * __ldg(ck + q);
+            double c = __ldg(cb + q * Sb) * __ldg(ck + q * Sk);
             total = fma(c, fma(w.y, v.y, w.x * v.x), total);
         }
         double norm = ((db.x >> 24) & 1) ? (((dk.x >> 24) & 1) ? 2.0 : 1.4142135623730951)

@@ -90,14 +90,14 @@ def test_cg_tables_match_exact(torch, B, emax):
             for tj2 in [2 * b + 1 for b in range(nj)]:
                 nJ = min(tj1, tj2) + 1
                 cnt = (tj1 + 1) * (tj2 + 1) * nJ
-                blk = tab[pos:pos + cnt].reshape(tj1 + 1, tj2 + 1, nJ)
+                blk = tab[pos:pos + cnt].reshape(nJ, tj1 + 1, tj2 + 1)
                 pos += cnt
                 # all entries for small blocks, a random sample for big ones (exact arithmetic is slow)
                 idx = np.ndindex(blk.shape) if cnt <= 400 else \
                     [np.unravel_index(k, blk.shape) for k in rng.choice(cnt, 150, replace=False)]
-                for (i1, i2, iJ) in idx:
+                for (iJ, i1, i2) in idx:
                     tm1, tm2, tJ = 2 * i1 - tj1, 2 * i2 - tj2, abs(tj1 - tj2) + 2 * iJ
-                    worst = max(worst, abs(blk[i1, i2, iJ] - cg_exact(tj1, tm1, tj2, tm2, tJ, tm1 + tm2)))
+                    worst = max(worst, abs(blk[iJ, i1, i2] - cg_exact(tj1, tm1, tj2, tm2, tJ, tm1 + tm2)))
         assert pos == len(tab)
         assert worst <= 1e-15, f"stage {stage}: max CG error {worst:.2e}"
     ctx.close()
@@ -189,8 +189,8 @@ def test_order_chunk_and_stream_invariance(torch, B):
     perm = rng.permutation(len(req))
     got, gmask = run_gpu(torch, ctx, req[perm], 0)
     assert np.array_equal(got, base[perm]) and np.array_equal(gmask, bmask[perm])
-    naive, nmask = run_gpu(torch, ctx, req, 2)
-    assert np.array_equal(naive, base) and np.array_equal(nmask, bmask)
+    naive, nmask = run_gpu(torch, ctx, req, 2)          # different kernel, different summation tree
+    assert np.max(np.abs(naive - base)) < 1e-13 and np.array_equal(nmask, bmask)
     # chunks of ~20 000 (the paper's buffer size) on two streams
     d_req = torch.from_numpy(req).cuda()
     out = torch.empty(len(req), dtype=torch.float64, device="cuda")
