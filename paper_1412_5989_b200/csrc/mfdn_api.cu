@@ -138,13 +138,31 @@ extern "C" int mfdn_orbitals_init(mfdn_ctx** out, int device, int32_t n_orb, con
             w2[(tb * 4 + tk) * 2 + 0] = c->t.iso2[tb][0] * c->t.iso2[tk][0];
             w2[(tb * 4 + tk) * 2 + 1] = c->t.iso2[tb][1] * c->t.iso2[tk][1];
         }
+    // isospin bins: the (bra, ket) tz patterns with equal MT (1 + 9 + 9 + 1 = NBIN3), in ascending tz-bit order
+    std::vector<double> wb(NBIN3 * NISO3, 0.0);
+    std::vector<uint8_t> t2b(64, NBIN3 - 1);
+    {
+        int nbin = 0;
+        for (int tb = 0; tb < 8; tb++)
+            for (int tk = 0; tk < 8; tk++)
+                if (__builtin_popcount(tb) == __builtin_popcount(tk)) {
+                    for (int q = 0; q < NISO3; q++) wb[nbin * NISO3 + q] = w3[(tb * 8 + tk) * 6 + q];
+                    t2b[tb * 8 + tk] = (uint8_t)nbin++;
+                }
+        if (nbin != NBIN3) { mfdn_destroy(c); return MFDN_ERR_STATE; }
+    }
     void* dw = nullptr;
-    if (cudaMalloc(&dw, (w3.size() + w2.size()) * sizeof(double)) != cudaSuccess) { mfdn_destroy(c); return MFDN_ERR_OOM; }
+    const size_t nw = w3.size() + w2.size() + wb.size();
+    if (cudaMalloc(&dw, nw * sizeof(double) + 64) != cudaSuccess) { mfdn_destroy(c); return MFDN_ERR_OOM; }
     c->owned.push_back(dw);
     cudaMemcpy(dw, w3.data(), w3.size() * sizeof(double), cudaMemcpyHostToDevice);
     cudaMemcpy((double*)dw + w3.size(), w2.data(), w2.size() * sizeof(double), cudaMemcpyHostToDevice);
+    cudaMemcpy((double*)dw + w3.size() + w2.size(), wb.data(), wb.size() * sizeof(double), cudaMemcpyHostToDevice);
+    cudaMemcpy((double*)dw + nw, t2b.data(), 64, cudaMemcpyHostToDevice);
     c->t.wtab3 = (const double*)dw;
     c->t.wtab2 = (const double*)dw + w3.size();
+    c->t.wbin3 = (const double*)dw + w3.size() + w2.size();
+    c->t.tz2bin3 = (const uint8_t*)((const double*)dw + nw);
     c->stage = 1;
     *out = c;
     return MFDN_OK;
@@ -328,7 +346,7 @@ extern "C" int mfdn_cg_download(mfdn_ctx* c, int stage, double* host_out, int64_
 struct Retile3 {
     int n_tup;
     const int4* tdesc;
-    const uint32_t* slab_off;
+    const uint2* sgrp;
     const int32_t* rowmap;
     const int32_t* chan_of;   // [(twoJ>>1)*4 + (twoT>>1)*2 + par]
     const int64_t* chan_off;
@@ -347,14 +365,15 @@ __device__ __forceinline__ void j12_range(int4 d, int twoJ, int& lo, int& hi)
 __global__ void k_retile3(Retile3 p)
 {
     for (long long g = blockIdx.x; g < (long long)p.n_tup * p.n_tup; g += gridDim.x) {
-        uint32_t so = p.slab_off[g];
-        if (so == NO_SLAB) continue;
+        uint2 sg = p.sgrp[g];
+        if (sg.x == NO_SLAB) continue;
+        const int gsize = (int)sg.y;
         int tb = (int)(g / p.n_tup), tk = (int)(g % p.n_tup);
         int4 db = p.tdesc[tb], dk = p.tdesc[tk];
         int par = (db.x >> 25) & 1;
         int Jlo = max((db.y >> 16) & 255, (dk.y >> 16) & 255), Jhi = min((db.y >> 24) & 255, (dk.y >> 24) & 255);
         int nJb = (((db.y >> 24) & 255) - ((db.y >> 16) & 255)) / 2 + 1, nJk = (((dk.y >> 24) & 255) - ((dk.y >> 16) & 255)) / 2 + 1;
-        double* dst = p.slab + (size_t)so * 2;
+        double* dst = p.slab + (size_t)sg.x * 2;
         for (int twoJ = Jlo; twoJ <= Jhi; twoJ += 2) {
             int lb, hb, lk, hk;
             j12_range(db, twoJ, lb, hb);
@@ -363,11 +382,11 @@ __global__ void k_retile3(Retile3 p)
             if (nb <= 0 || nk <= 0) continue;
             int iJb = (twoJ - ((db.y >> 16) & 255)) / 2, iJk = (twoJ - ((dk.y >> 16) & 255)) / 2;
             const int pitch = row_pitch3(nk);
-            for (int idx = threadIdx.x; idx < nb * pitch; idx += blockDim.x) {
-                int i = idx / pitch, o = idx % pitch;
+            for (int idx = threadIdx.x; idx < NISO3 * nb * pitch; idx += blockDim.x) {
+                int slot = idx / (nb * pitch), o = idx % (nb * pitch);
+                int i = o / pitch, k = o % pitch;
                 double v = 0.0;
-                if (o < NISO3 * nk) {
-                    int k = o / NISO3, slot = o % NISO3;
+                if (k < nk) {
                     int T12 = slot >> 1 & 1, T12p = slot & 1, Ti = 0;
                     if (slot == 4) { T12 = 1; T12p = 1; Ti = 1; }
                     int ch = p.chan_of[(twoJ >> 1) * 4 + Ti * 2 + par];
@@ -377,10 +396,42 @@ __global__ void k_retile3(Retile3 p)
                         if (r >= 0 && q >= 0) v = p.values[p.chan_off[ch] + (long long)r * p.chan_dim[ch] + q];
                     }
                 }
-                dst[idx] = v;
+                dst[(size_t)slot * gsize + o] = v;
             }
             dst += (size_t)nb * pitch;
         }
+    }
+}
+
+// Per-tuple coefficient tables (A1/A2): dtab[tk.x + row*S + (ima*(jb+1) + imb)*(jc+1) + imc] =
+// <ja ma jb mb|J12 M12> <J12 M12 jc mc|J M> for the tuple's rows (J, J12) in loop order; one fp64 product of the two
+// tabulated coefficients, 0 where |M12| > J12 or |M| > J (the zero guard of the stage-2 table).
+struct Dtab3 {
+    const int4* tdesc;
+    const int4* tk;
+    const int2* trow;      // {first row of the tuple in rowtab, -}
+    const int2* rowtab;    // per row {cg2g offset at A = 0, cg1 offset relative to the m-pair base}
+    const int32_t* nrows;
+    const double* cg1;
+    const int32_t* cg1_off;
+    const double* cg2g;
+    int nj;
+    double* dtab;
+};
+
+__global__ void k_dtab3(Dtab3 p)
+{
+    const int t = blockIdx.x;
+    const int4 d = p.tdesc[t], k = p.tk[t];
+    const int ja = d.x & 255, jb = (d.x >> 8) & 255, jc = (d.x >> 16) & 255;
+    const int S = k.y, nr = p.nrows[t], r0 = p.trow[t].x;
+    const int c1 = p.cg1_off[(ja >> 1) * p.nj + (jb >> 1)];
+    for (int idx = threadIdx.x; idx < nr * S; idx += blockDim.x) {
+        int r = idx / S, o = idx % S;
+        int imc = o % (jc + 1), imb = (o / (jc + 1)) % (jb + 1), ima = o / ((jc + 1) * (jb + 1));
+        int2 rt = p.rowtab[r0 + r];
+        int A = (ima + imb - ((ja + jb) >> 1)) * (jc + 1) + imc;
+        p.dtab[(size_t)(uint32_t)k.x + idx] = p.cg1[c1 + ima * (jb + 1) + imb + rt.y] * p.cg2g[rt.x + A];
     }
 }
 
@@ -531,11 +582,14 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
         hi = std::min((d.y >> 8) & 255, (twoJ + jc) >> 1);
     };
     // ---- row tables (A2 "tile index": flat offsets, no pointers -- PAPER.md:109-121).  Per (tuple, J, J12) row the
-    //      request-independent parts of the two coefficient addresses:
+    //      request-independent parts of the two coefficient addresses (used only to build dtab3):
     //        x: <J12 M12 jc mc|J M> lives at cg2g[x + A],  A = M12*(jc+1) + imc  (x includes CG_GUARD and J12*(jc+1))
-    //        y: <ja ma jb mb|J12 M12> lives at cg1[c1_lane + y],  c1_lane = off(ja,jb) + ima*(jb+1) + imb
-    //      and per (tuple, J): {first row (absolute), number of rows}
+    //        y: <ja ma jb mb|J12 M12> lives at cg1[c1 + y],  c1 = off(ja,jb) + ima*(jb+1) + imb
+    //      and per (tuple, J): {first row (tuple-relative), number of rows}
     std::vector<int2> trow(nt), rowtab, jinfo;
+    std::vector<int4> tk(nt);
+    std::vector<int32_t> nrows(nt);
+    uint64_t dtab_len = 0;
     for (int t = 0; t < nt; t++) {
         int4 d = tdesc[t];
         int ja = d.x & 255, jb = (d.x >> 8) & 255, jc = (d.x >> 16) & 255;
@@ -545,7 +599,7 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
             int lo, hi;
             range(d, twoJ, lo, hi);
             int2 ji;
-            ji.x = (int)rowtab.size();
+            ji.x = (int)rowtab.size() - trow[t].x;
             ji.y = std::max(0, hi - lo + 1);
             jinfo.push_back(ji);
             for (int J12 = lo; J12 <= hi; J12++) {
@@ -556,34 +610,44 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
                 rowtab.push_back(e);
             }
         }
+        nrows[t] = (int)rowtab.size() - trow[t].x;
+        const int S = (ja + 1) * (jb + 1) * (jc + 1);
+        if (dtab_len + (uint64_t)nrows[t] * S >= 0x7FFFFFF0ull) return fail(c, MFDN_ERR_OOM, "coefficient table too large for 31-bit offsets");
+        tk[t].x = (int)dtab_len;
+        tk[t].y = S;
+        tk[t].z = trow[t].y;
+        tk[t].w = (jb + 1) | ((jc + 1) << 8) | (d.y & 0xFFFF0000);
+        dtab_len += (uint64_t)nrows[t] * S;
+        dtab_len = (dtab_len + 1) & ~1ull;
     }
-    // ---- slab offsets (16-byte units) per (bra tuple, ket tuple) group, rows in loop order J, J12
-    std::vector<uint32_t> slab_off((size_t)nt * nt, NO_SLAB);
+    // ---- group descriptors: slab offset (16-byte units) and plane size, rows in loop order J, J12
+    std::vector<uint2> sgrp((size_t)nt * nt, uint2{NO_SLAB, 0u});
     uint64_t cells = 0;   // in 16-byte units
     for (int tb = 0; tb < nt; tb++)
-        for (int tk = 0; tk < nt; tk++) {
-            int4 db = tdesc[tb], dk = tdesc[tk];
+        for (int tkk = 0; tkk < nt; tkk++) {
+            int4 db = tdesc[tb], dk = tdesc[tkk];
             if (((db.x ^ dk.x) >> 25) & 1) continue;
             int Jlo = std::max((db.y >> 16) & 255, (dk.y >> 16) & 255), Jhi = std::min((db.y >> 24) & 255, (dk.y >> 24) & 255);
-            uint64_t n = 0;
+            uint64_t gsize = 0;
             for (int twoJ = Jlo; twoJ <= Jhi; twoJ += 2) {
                 int lb, hb, lk, hk;
                 range(db, twoJ, lb, hb);
                 range(dk, twoJ, lk, hk);
-                if (hb >= lb && hk >= lk) n += (uint64_t)(hb - lb + 1) * (row_pitch3(hk - lk + 1) / 2);
+                if (hb >= lb && hk >= lk) gsize += (uint64_t)(hb - lb + 1) * row_pitch3(hk - lk + 1);
             }
-            if (n == 0) continue;
-            if (cells + n >= 0xFFFFFFF0ull) return fail(c, MFDN_ERR_OOM, "table too large for 32-bit slab offsets");
-            slab_off[(size_t)tb * nt + tk] = (uint32_t)cells;
-            cells += n;
+            if (gsize == 0) continue;
+            if (cells + gsize * NISO3 / 2 >= 0xFFFFFFF0ull) return fail(c, MFDN_ERR_OOM, "table too large for 32-bit slab offsets");
+            sgrp[(size_t)tb * nt + tkk] = uint2{(uint32_t)cells, (uint32_t)gsize};
+            cells += gsize * NISO3 / 2;
         }
     // ---- one arena for the resident index tables, one for the upload-only ones
     Arena res, tmp;
-    size_t o_tid = res.add(tuple_id), o_desc = res.add(tdesc), o_soff = res.add(slab_off), o_sm = res.add(stmask);
-    size_t o_trow = res.add(trow), o_rowtab = res.add(rowtab), o_jinfo = res.add(jinfo);
+    size_t o_tid = res.add(tuple_id), o_desc = res.add(tdesc), o_sgrp = res.add(sgrp), o_sm = res.add(stmask);
+    size_t o_tk = res.add(tk), o_jinfo = res.add(jinfo);
     std::vector<int64_t> coff(chan_off, chan_off + n_chan);
     std::vector<int32_t> cdim(chan_dim, chan_dim + n_chan);
     size_t o_rm = tmp.add(rowmap), o_cof = tmp.add(chan_of), o_coff = tmp.add(coff), o_cdim = tmp.add(cdim);
+    size_t o_trow = tmp.add(trow), o_rowtab = tmp.add(rowtab), o_nrows = tmp.add(nrows);
     char* dres = nullptr;
     int rc = arena_upload(c, res, &dres, st);
     if (rc) return rc;
@@ -596,12 +660,20 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     if (rc) { cudaFree(dtmp); return rc; }
     void* dslab = nullptr;
     cudaError_t e = cudaMalloc(&dslab, std::max<uint64_t>(cells, 1) * 16 + 256);
-    if (e != cudaSuccess) { cudaFree(dtmp); if (vtmp) cudaFree(vtmp); return cuda_fail(c, e, "cudaMalloc(slab3)"); }
+    void* ddtab = nullptr;
+    if (e == cudaSuccess) e = cudaMalloc(&ddtab, std::max<uint64_t>(dtab_len, 2) * sizeof(double));
+    if (e != cudaSuccess) {
+        cudaFree(dtmp);
+        if (vtmp) cudaFree(vtmp);
+        if (dslab) cudaFree(dslab);
+        return cuda_fail(c, e, "cudaMalloc(slab3/dtab3)");
+    }
     c->owned.push_back(dslab);
+    c->owned.push_back(ddtab);
     Retile3 p;
     p.n_tup = nt;
     p.tdesc = (const int4*)(dres + o_desc);
-    p.slab_off = (const uint32_t*)(dres + o_soff);
+    p.sgrp = (const uint2*)(dres + o_sgrp);
     p.rowmap = (const int32_t*)((char*)dtmp + o_rm);
     p.chan_of = (const int32_t*)((char*)dtmp + o_cof);
     p.chan_off = (const int64_t*)((char*)dtmp + o_coff);
@@ -610,22 +682,35 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     p.slab = (double*)dslab;
     long long groups = (long long)nt * nt;
     k_retile3<<<(unsigned)std::min<long long>(groups, 1 << 20), 64, 0, st>>>(p);
+    Dtab3 q;
+    q.tdesc = p.tdesc;
+    q.tk = (const int4*)(dres + o_tk);
+    q.trow = (const int2*)((char*)dtmp + o_trow);
+    q.rowtab = (const int2*)((char*)dtmp + o_rowtab);
+    q.nrows = (const int32_t*)((char*)dtmp + o_nrows);
+    q.cg1 = c->t.cg1;
+    q.cg1_off = c->t.cg1_off;
+    q.cg2g = c->t.cg2g;
+    q.nj = c->t.nj;
+    q.dtab = (double*)ddtab;
+    k_dtab3<<<(unsigned)nt, 256, 0, st>>>(q);
     e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     cudaFree(dtmp);
     if (vtmp) cudaFree(vtmp);
-    if (e != cudaSuccess) return cuda_fail(c, e, "k_retile3");
+    if (e != cudaSuccess) return cuda_fail(c, e, "k_retile3/k_dtab3");
     c->t.n_tup3 = nt;
     c->t.e3max = e3max;
     c->t.tuple_id3 = (const int32_t*)(dres + o_tid);
     c->t.tdesc3 = p.tdesc;
-    c->t.slab_off3 = p.slab_off;
+    c->t.sgrp3 = p.sgrp;
     c->t.slab3 = (const double*)dslab;
     c->t.stmask3 = (const unsigned long long*)(dres + o_sm);
-    c->t.trow3 = (const int2*)(dres + o_trow);
-    c->t.rowtab3 = (const int2*)(dres + o_rowtab);
+    c->t.tk3 = q.tk;
     c->t.jinfo3 = (const int2*)(dres + o_jinfo);
+    c->t.dtab3 = (const double*)ddtab;
     c->slab_bytes3 = (int64_t)(cells * 16);
+    c->dtab_bytes3 = (int64_t)(dtab_len * sizeof(double));
     c->has3 = true;
     return MFDN_OK;
 }
@@ -785,6 +870,7 @@ extern "C" int64_t mfdn_info(mfdn_ctx* c, int which)
         case 4: return c->n_cg1;
         case 5: return c->n_cg2;
         case 6: return c->launches;
+        case 7: return c->dtab_bytes3;
         default: return -1;
     }
 }

@@ -27,14 +27,20 @@ __host__ __device__ inline int rec_lpar(uint32_t r) { return (r >> 27) & 1; }
 
 constexpr int MAX_TWOJ = 21;       // 3*MAX_TWOJ <= 63 so that (2J,2T) fits a 64-bit channel mask
 constexpr int NISO3 = 5;           // isospin slots per 3-body cell: (T12,T12',T) = (0,0,1/2) (0,1,1/2) (1,0,1/2) (1,1,1/2) (1,1,3/2)
+constexpr int NBIN3 = 20;          // isospin bins: (bra tz pattern, ket tz pattern) pairs with equal MT
 constexpr int CELL2 = 2;           // doubles per 2-body slab cell: T = 0, 1 (16 B)
 constexpr uint32_t NO_SLAB = 0xFFFFFFFFu;
 constexpr int CG_GUARD = 8192;     // zero doubles before and after the stage-2 table (see Tables::cg2g)
 
-// 3-body slab of a (bra tuple, ket tuple) group, in the order the kernel's loops read it:
-//   for J (common range, ascending) / for bra J12 in range(J) / [ for ket J12' in range(J) / 5 isospin slots ]
-// one "row" = the NISO3*nk(J) doubles of a fixed (J, J12), padded to an even count (16-byte units).
-__host__ __device__ inline int row_pitch3(int nk) { return (NISO3 * nk + 1) & ~1; }
+// 3-body slab of a (bra tuple, ket tuple) group = NISO3 isospin planes of `gsize` doubles each; inside a plane the
+// cells are in the order the kernel's loops read them:
+//   for J (common range, ascending) / for bra J12 in range(J) / for ket J12' in range(J)
+// one "row" = the nk(J) cells of a fixed (J, J12), padded to an even count (16-byte units), zero where a state is
+// not listed.  The isospin-combined copy Vw = sum_s w[s] * plane[s] that the transform stages in shared memory has
+// the same indexing.
+__host__ __device__ inline int row_pitch3(int nk) { return (nk + 1) & ~1; }
+constexpr int ITEM3 = 512;         // records per work item of the 3-body transform (one group per item)
+constexpr uint32_t ZERO_ITEM = 0xFFFFFFFFu;   // work item whose records all have value 0 (no slab / failed S1-S6)
 
 // ---- packed canonical request record (H1 output), 64 bit --------------------------------------------
 //  [0,30) im of the canonical particles (5 bits each: bra then ket)   [30,36) tz bits (bra then ket)
@@ -47,6 +53,9 @@ constexpr uint32_t REC_INVALID = 0x7FFFFFFu;
 //         y = J12min | J12max<<8 | twoJmin<<16 | twoJmax<<24
 //         z = offset of the tuple's state masks in stmask3 (entries: [J12-J12min][T12])
 //         w = offset of the tuple's row map (upload only)
+// tk3 (what the transform kernel needs of a tuple): x = offset of the tuple's coefficient table in dtab3 (doubles),
+//         y = its row pitch S = (ja+1)(jb+1)(jc+1), z = first entry of the tuple in jinfo3,
+//         w = (jb+1) | (jc+1)<<8 | twoJmin<<16 | twoJmax<<24
 // 2-body: x = ja | jb<<8 | (a==b)<<24 | par<<25,  y = Jmin | Jmax<<8,  z = state mask (low), w = (high)
 struct Tables {
     // A0
@@ -62,18 +71,20 @@ struct Tables {
                              // |M12| > J12 (stage-1 factor = 0) still reads valid, finite memory
     const double* wtab3;     // [64][6] isospin weights w[5] (+pad) indexed by the 6 tz bits of a record
     const double* wtab2;     // [16][2]
+    const double* wbin3;     // [NBIN3][NISO3] the same weights indexed by isospin bin
+    const uint8_t* tz2bin3;  // [64] tz bits of a record -> isospin bin
     double iso3[8][3];       // [ta<<2|tb<<1|tc][(T12,T) = (0,1/2),(1,1/2),(1,3/2)]
     double iso2[4][2];       // [ta<<1|tb][T]
     // A2, 3-body
     int n_tup3, e3max;
     const int32_t* tuple_id3;      // [n_orb^3] -> tuple or -1
     const int4* tdesc3;
-    const uint32_t* slab_off3;     // [n_tup3^2] start of the group's slab in 16-byte units, or NO_SLAB
+    const uint2* sgrp3;            // [n_tup3^2] {start of the group's slab in 16-byte units or NO_SLAB, doubles per plane}
     const double* slab3;
     const unsigned long long* stmask3;
-    const int2* trow3;             // [n_tup3] {first row of the tuple in rowtab3, first entry in jinfo3}
-    const int2* rowtab3;           // per (tuple, J, J12) row: {cg2g offset at A = 0, cg1 offset relative to the lane base}
-    const int2* jinfo3;            // per (tuple, J): {first row in rowtab3 (absolute), number of rows}
+    const int4* tk3;               // [n_tup3] see above
+    const int2* jinfo3;            // per (tuple, J): {first row of this J (tuple-relative, loop order J, J12), number of rows}
+    const double* dtab3;           // per tuple [row][ima][imb][imc] = <ja ma jb mb|J12 M12> <J12 M12 jc mc|J M>
     // A2, 2-body
     int n_tup2;
     const int32_t* tuple_id2;      // [n_orb^2]
@@ -97,7 +108,7 @@ struct mfdn_ctx {
     std::vector<uint32_t> h_sps_rec;
     std::vector<void*> owned;  // device allocations
     int64_t n_cg1 = 0, n_cg2 = 0;
-    int64_t slab_bytes2 = 0, slab_bytes3 = 0;
+    int64_t slab_bytes2 = 0, slab_bytes3 = 0, dtab_bytes3 = 0;
     int64_t launches = 0;
     int num_sms = 148;
     // measurement hooks

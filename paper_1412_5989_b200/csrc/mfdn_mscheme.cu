@@ -162,8 +162,8 @@ __device__ __forceinline__ double eval3_naive(const Tables& T, const Side3& B, c
 {
     mask = 0;
     if (!select3(T, B, K)) return 0.0;
-    const uint32_t so = __ldg(T.slab_off3 + (size_t)B.tup * T.n_tup3 + K.tup);
-    if (so == NO_SLAB) return 0.0;
+    const uint2 sg = __ldg(T.sgrp3 + (size_t)B.tup * T.n_tup3 + K.tup);
+    if (sg.x == NO_SLAB) return 0.0;
     const int4 db = __ldg(T.tdesc3 + B.tup), dk = __ldg(T.tdesc3 + K.tup);
     if (!mask3(T, B, K, db, dk)) return 0.0;
     mask = 1;
@@ -180,7 +180,8 @@ __device__ __forceinline__ double eval3_naive(const Tables& T, const Side3& B, c
     const double* c1b = T.cg1 + __ldg(T.cg1_off + (ja >> 1) * nj + (jb >> 1)) + B.ima * (jb + 1) + B.imb;
     const double* c1k = T.cg1 + __ldg(T.cg1_off + (jd >> 1) * nj + (je >> 1)) + K.ima * (je + 1) + K.imb;
     const int S1b = (ja + 1) * (jb + 1), S1k = (jd + 1) * (je + 1);
-    const double* row = T.slab3 + (size_t)so * 2;
+    const size_t plane = sg.y;
+    const double* row = T.slab3 + (size_t)sg.x * 2;
     const int Jlo = max((db.y >> 16) & 255, (dk.y >> 16) & 255), Jhi = min((db.y >> 24) & 255, (dk.y >> 24) & 255);
     double total = 0.0;
     for (int twoJ = Jlo; twoJ <= Jhi; twoJ += 2) {
@@ -190,6 +191,7 @@ __device__ __forceinline__ double eval3_naive(const Tables& T, const Side3& B, c
         if (nb <= 0 || nk <= 0) continue;
         const int pitch = row_pitch3(nk);
         if (twoJ < aM) { row += (size_t)nb * pitch; continue; }
+        double tj = 0.0;
         for (int J12 = lb; J12 <= hb; J12++) {
             double cb = 0.0;
             if (abs(twoM12b) <= 2 * J12) {
@@ -207,17 +209,18 @@ __device__ __forceinline__ double eval3_naive(const Tables& T, const Side3& B, c
                     ck = __ldg(c1k + (J12p - J12mink) * S1k) *
                          __ldg(c2 + (iJ * (2 * J12p + 1) + ((twoM12k + 2 * J12p) >> 1)) * (jf + 1) + K.imc);
                 }
-                const double* cell = row + NISO3 * (J12p - lk);
+                const double* cell = row + (J12p - lk);
                 double inner = w0 * __ldg(cell);
-                inner = fma(w1, __ldg(cell + 1), inner);
-                inner = fma(w2, __ldg(cell + 2), inner);
-                inner = fma(w3, __ldg(cell + 3), inner);
-                inner = fma(w4, __ldg(cell + 4), inner);
+                inner = fma(w1, __ldg(cell + plane), inner);
+                inner = fma(w2, __ldg(cell + 2 * plane), inner);
+                inner = fma(w3, __ldg(cell + 3 * plane), inner);
+                inner = fma(w4, __ldg(cell + 4 * plane), inner);
                 acc = fma(ck, inner, acc);
             }
-            total = fma(cb, acc, total);
+            tj = fma(cb, acc, tj);
             row += pitch;
         }
+        total += tj;
     }
     return (B.sign * K.sign) * total;
 }
@@ -276,14 +279,14 @@ __global__ void __launch_bounds__(128) k_mscheme_naive(Tables T, long long n, co
 
 // =============================================================================== H1: records
 // One thread per request: decode, S1-S7 -> mask (request order, coalesced), canonical packed record.
-template <int BODY>
+template <int BODY, bool AGG>
 __global__ void __launch_bounds__(256) k_keys(Tables T, long long n, const int32_t* __restrict__ req,
                                               unsigned long long* __restrict__ recs, uint8_t* __restrict__ maskout,
                                               uint32_t* __restrict__ hist, uint32_t invalid_bucket,
                                               uint32_t* __restrict__ keys32)
 {
     long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
+    if (i >= n) return;   // n is a multiple of 32 or the tail warp is partial: __activemask below
     int s[6];
     if (BODY == 3) load_req3(req, i, s); else load_req2(req, i, s);
     uint32_t key = REC_INVALID;
@@ -295,7 +298,7 @@ __global__ void __launch_bounds__(256) k_keys(Tables T, long long n, const int32
         Side3 B = decode3(T, s[0], s[1], s[2]), K = decode3(T, s[3], s[4], s[5]);
         if (select3(T, B, K)) {
             key = (uint32_t)B.tup * T.n_tup3 + K.tup;
-            if (__ldg(T.slab_off3 + key) != NO_SLAB) mask = mask3(T, B, K, __ldg(T.tdesc3 + B.tup), __ldg(T.tdesc3 + K.tup));
+            if (__ldg(T.sgrp3 + key).x != NO_SLAB) mask = mask3(T, B, K, __ldg(T.tdesc3 + B.tup), __ldg(T.tdesc3 + K.tup));
             low = (unsigned long long)(B.ima | (B.imb << 5) | (B.imc << 10) | (K.ima << 15) | (K.imb << 20) | (K.imc << 25)) |
                   ((unsigned long long)((B.tz << 3) | K.tz) << 30) | ((unsigned long long)(B.sign * K.sign < 0) << 36);
         }
@@ -310,7 +313,16 @@ __global__ void __launch_bounds__(256) k_keys(Tables T, long long n, const int32
     }
     if (recs) recs[i] = ((unsigned long long)key << REC_KEY_SHIFT) | low;
     if (maskout) maskout[i] = (uint8_t)mask;
-    if (hist) atomicAdd(hist + (key == REC_INVALID ? invalid_bucket : key), 1u);
+    if (hist) {
+        const uint32_t bucket = key == REC_INVALID ? invalid_bucket : key;
+        if (AGG) {   // group-ordered input: one atomic per run of equal keys in the warp
+            const unsigned act = __activemask();
+            const unsigned same = __match_any_sync(act, bucket);
+            if ((threadIdx.x & 31) == __ffs(same) - 1) atomicAdd(hist + bucket, (uint32_t)__popc(same));
+        } else {
+            atomicAdd(hist + bucket, 1u);
+        }
+    }
     if (keys32) keys32[i] = key == REC_INVALID ? 0xFFFFFFFFu : key;
 }
 
@@ -388,152 +400,250 @@ __global__ void __launch_bounds__(256) k_scatter(long long n, const unsigned lon
 }
 
 // =============================================================================== H3-H6: transform
-// All table accesses are 32-bit indices off kernel-parameter base pointers (one IMAD.WIDE per load).
-// One J block of the 3-body sum with the ket range size NK known at compile time: the NK ket coefficients live
-// in registers, one bra row (5*NK slab doubles, 128-bit loads at warp-uniform addresses) per iteration.
+// Work items (H3): one item = up to ITEM3 consecutive records of ONE group in the group-ordered stream, so that a
+// thread block shares every loop bound, table row and the group's slab.  `bounds[b]` is the END of bucket b after the
+// scatter (ends = 1: the cursor array) or its START for pre-sorted input (ends = 0: the scanned histogram).
+__global__ void __launch_bounds__(256) k_items3(const uint32_t* __restrict__ bounds, uint32_t n_buckets, int ends, uint32_t n,
+                                               const uint2* __restrict__ sgrp, uint32_t invalid_bucket,
+                                               uint4* __restrict__ items, uint32_t* __restrict__ n_items)
+{
+    const uint32_t b = blockIdx.x * 256u + threadIdx.x;
+    uint32_t start = 0, end = 0;
+    if (b < n_buckets) {
+        if (ends) { end = bounds[b]; start = b ? bounds[b - 1] : 0u; }
+        else { start = bounds[b]; end = (b + 1 < n_buckets) ? bounds[b + 1] : n; }
+    }
+    const uint32_t cnt = end - start, k = (cnt + ITEM3 - 1) / ITEM3;
+    // warp-aggregated append: the list stays (nearly) in group order, neighbours share the bra tuple's tables
+    const int lane = threadIdx.x & 31;
+    uint32_t incl = k;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+        uint32_t x = __shfl_up_sync(0xFFFFFFFFu, incl, off);
+        if (lane >= off) incl += x;
+    }
+    uint32_t base = 0;
+    if (lane == 31 && incl) base = atomicAdd(n_items, incl);
+    base = __shfl_sync(0xFFFFFFFFu, base, 31);
+    if (k == 0) return;
+    const uint32_t g = (b == invalid_bucket || sgrp[b].x == NO_SLAB) ? ZERO_ITEM : b;
+    uint32_t slot = base + incl - k;
+    for (uint32_t j = 0; j < k; j++) items[slot + j] = make_uint4(start + j * ITEM3, min((uint32_t)ITEM3, cnt - j * ITEM3), g, 0u);
+}
+
+constexpr int TR_THREADS = 256;
+constexpr int TR_RPT = ITEM3 / TR_THREADS;   // records per thread
+constexpr int VW_CAP = 3072;                 // doubles: isospin-combined slabs Vw[bin][cell] of the current item (24 KB)
+constexpr int MAX_JBLK = 32;                 // common J values of a group (2J <= 63)
+
+struct ItemShared {
+    double vw[VW_CAP];
+    double w[NBIN3 * NISO3];
+    uint32_t sc[8];
+    uint32_t mask[2];
+    uint16_t nbk[MAX_JBLK];
+    uint8_t tz2bin[64];
+};
+
+// One J block of the sum with the ket range size NK known at compile time:
+//   sum_i cb(i) * sum_k ck(k) * Vw[i][k],  cb/ck read from the tuples' coefficient tables (one gather per row),
+// Vw rows (padded to even length) read from shared memory with 128-bit loads.
 template <int NK>
-__device__ __forceinline__ double j_block3(const Tables& T, uint32_t rb0, uint32_t rk0, int nb, uint32_t c1b, uint32_t c1k,
-                                           int Ab, int Ak, uint32_t& so, const double (&w)[5])
+__device__ __forceinline__ double j_block3(const double* __restrict__ dtab, const double* __restrict__ vw, uint32_t& pb, uint32_t& pk,
+                                           uint32_t Sb, uint32_t Sk, int nb, uint32_t& vi)
 {
     double ck[NK];
 #pragma unroll
     for (int k = 0; k < NK; k++) {
-        int2 rt = __ldg(T.rowtab3 + rk0 + k);
-        ck[k] = __ldg(T.cg1 + (c1k + (uint32_t)rt.y)) * __ldg(T.cg2g + (uint32_t)(rt.x + Ak));
+        ck[k] = __ldg(dtab + pk);
+        pk += Sk;
     }
-    constexpr int NV = (NISO3 * NK + 1) / 2;
-    const double2* slab = (const double2*)T.slab3;
-    uint32_t rp = so;
+    constexpr int P = (NK + 1) & ~1;
     double total = 0.0;
 #pragma unroll 2
     for (int i = 0; i < nb; i++) {
-        int2 rt = __ldg(T.rowtab3 + rb0 + i);
-        double cb = __ldg(T.cg1 + (c1b + (uint32_t)rt.y)) * __ldg(T.cg2g + (uint32_t)(rt.x + Ab));
-        double v[2 * NV];
+        const double cb = __ldg(dtab + pb);
+        pb += Sb;
+        double v[P];
 #pragma unroll
-        for (int q = 0; q < NV; q++) {
-            double2 t = __ldg(slab + rp + q);
+        for (int q = 0; q < P / 2; q++) {
+            double2 t = *reinterpret_cast<const double2*>(vw + vi + 2 * q);
             v[2 * q] = t.x;
             v[2 * q + 1] = t.y;
         }
-        double acc = 0.0;
+        vi += P;
+        double acc = ck[0] * v[0];
 #pragma unroll
-        for (int k = 0; k < NK; k++) {
-            double inner = w[0] * v[5 * k];
-            inner = fma(w[1], v[5 * k + 1], inner);
-            inner = fma(w[2], v[5 * k + 2], inner);
-            inner = fma(w[3], v[5 * k + 3], inner);
-            inner = fma(w[4], v[5 * k + 4], inner);
-            acc = fma(ck[k], inner, acc);
-        }
+        for (int k = 1; k < NK; k++) acc = fma(ck[k], v[k], acc);
         total = fma(cb, acc, total);
-        rp += NV;
     }
-    so = rp;
     return total;
 }
 
-// any ket range size (rare: nk > 8): ket coefficient recomputed per cell
-struct GenericPtrs { const int2* rowtab3; const double* cg1; const double* cg2g; const double* slab3; };
-__device__ __noinline__ double j_block3_generic(GenericPtrs T, uint32_t rb0, uint32_t rk0, int nb, int nk, uint32_t c1b,
-                                                uint32_t c1k, int Ab, int Ak, uint32_t so, double w0, double w1, double w2,
-                                                double w3, double w4)
+// any ket range size (rare: nk > 6): ket coefficient re-read per cell
+__device__ __noinline__ double j_block3_generic(const double* __restrict__ dtab, const double* vw, uint32_t pb, uint32_t pk, uint32_t Sb,
+                                                uint32_t Sk, int nb, int nk, uint32_t vi)
 {
-    const int pitch = row_pitch3(nk);
-    const double* row = T.slab3 + (size_t)so * 2;
+    const int P = row_pitch3(nk);
     double total = 0.0;
     for (int i = 0; i < nb; i++) {
-        int2 rt = __ldg(T.rowtab3 + rb0 + i);
-        double cb = __ldg(T.cg1 + (c1b + (uint32_t)rt.y)) * __ldg(T.cg2g + (uint32_t)(rt.x + Ab));
+        const double cb = __ldg(dtab + pb + (uint32_t)i * Sb);
         double acc = 0.0;
-        for (int k = 0; k < nk; k++) {
-            int2 rk = __ldg(T.rowtab3 + rk0 + k);
-            double ck = __ldg(T.cg1 + (c1k + (uint32_t)rk.y)) * __ldg(T.cg2g + (uint32_t)(rk.x + Ak));
-            const double* cell = row + NISO3 * k;
-            double inner = w0 * __ldg(cell);
-            inner = fma(w1, __ldg(cell + 1), inner);
-            inner = fma(w2, __ldg(cell + 2), inner);
-            inner = fma(w3, __ldg(cell + 3), inner);
-            inner = fma(w4, __ldg(cell + 4), inner);
-            acc = fma(ck, inner, acc);
-        }
+        for (int k = 0; k < nk; k++) acc = fma(__ldg(dtab + pk + (uint32_t)k * Sk), vw[vi + k], acc);
         total = fma(cb, acc, total);
-        row += pitch;
+        vi += P;
     }
     return total;
 }
 
-// One warp = 32 consecutive records of the group-ordered stream.  The warp walks over the (few) distinct groups
-// among its lanes; inside a group every loop bound, table row and slab address is warp-uniform, the lanes differ
-// only in their m/tz projections (the irregular loop structure is per element -- here it is per group).
-__global__ void __launch_bounds__(128) k_transform3(Tables T, long long n, const unsigned long long* __restrict__ recs,
-                                                   const uint32_t* __restrict__ order, double* __restrict__ out)
+// H3-H6.  Persistent blocks walk the item list.  Per item: (1) the block ORs the isospin bins (tz patterns) of its
+// records into a shared mask; (2) it stages Vw[bin][cell] = sum_s w[bin][s] * plane_s[cell] for the bins present -- the
+// paper's "isospin loops ... unrolled into a single weighted summation" done once per (group, bin) instead
+// of once per request; (3) every thread evaluates its records: three nested loops over J, J12, J12' with
+// all bounds shared by the block, the lanes differing only in their projections (coefficient-table offsets) and bin.
+__global__ void __launch_bounds__(TR_THREADS, 4) k_transform3(Tables T, const uint4* __restrict__ items, const uint32_t* __restrict__ n_items_p,
+                                                             const unsigned long long* __restrict__ recs,
+                                                             const uint32_t* __restrict__ order, double* __restrict__ out)
 {
-    const long long pos = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const bool valid = pos < n;
-    const unsigned long long rec = valid ? __ldg(recs + pos) : ~0ull;
-    const uint32_t key = (uint32_t)(rec >> REC_KEY_SHIFT);
-    bool done = !valid || key == REC_INVALID;
-    double result = 0.0;
+    __shared__ __align__(16) ItemShared sh;
+    const int tid = threadIdx.x;
+    for (int i = tid; i < NBIN3 * NISO3; i += TR_THREADS) sh.w[i] = __ldg(T.wbin3 + i);
+    if (tid < 64) sh.tz2bin[tid] = __ldg(T.tz2bin3 + tid);
+    if (tid < 2) sh.mask[tid] = 0u;
+    __syncthreads();
+    const uint32_t n_items = __ldg(n_items_p);
     const uint32_t nt = (uint32_t)T.n_tup3;
-    for (;;) {
-        unsigned pending = __ballot_sync(0xFFFFFFFFu, !done);
-        if (pending == 0) break;
-        const uint32_t g = __shfl_sync(0xFFFFFFFFu, key, __ffs(pending) - 1);
-        const bool mine = !done && key == g;
-        if (mine) done = true;
-        uint32_t so = __ldg(T.slab_off3 + g);
-        if (so == NO_SLAB) continue;                        // no common channel: value 0
-        const uint32_t tb = g / nt, tk = g - tb * nt;
-        const int4 db = __ldg(T.tdesc3 + tb), dk = __ldg(T.tdesc3 + tk);
-        const int2 trb = __ldg(T.trow3 + tb), trk = __ldg(T.trow3 + tk);
-        const int ja = db.x & 255, jb = (db.x >> 8) & 255, jc = (db.x >> 16) & 255;
-        const int jd = dk.x & 255, je = (dk.x >> 8) & 255, jf = (dk.x >> 16) & 255;
-        // lane part (a lane of another group runs with m = 0: harmless, result discarded)
-        const uint32_t mrec = mine ? (uint32_t)rec : 0u;
-        const int ima = mrec & 31, imb = (mrec >> 5) & 31, imc = (mrec >> 10) & 31;
-        const int imd = (mrec >> 15) & 31, ime = (mrec >> 20) & 31, imf = (mrec >> 25) & 31;
-        const int Ab = (ima + imb - ((ja + jb) >> 1)) * (jc + 1) + imc;     // M12*(jc+1) + imc
-        const int Ak = (imd + ime - ((jd + je) >> 1)) * (jf + 1) + imf;
-        const int nj = T.nj;
-        const uint32_t c1b = (uint32_t)(__ldg(T.cg1_off + (ja >> 1) * nj + (jb >> 1)) + ima * (jb + 1) + imb);
-        const uint32_t c1k = (uint32_t)(__ldg(T.cg1_off + (jd >> 1) * nj + (je >> 1)) + imd * (je + 1) + ime);
-        const int tz6 = mine ? (int)((rec >> 30) & 63) : 0;
-        double w[5];
-        {
-            const double2* wp = (const double2*)T.wtab3 + tz6 * 3;
-            double2 a = __ldg(wp), b = __ldg(wp + 1), c = __ldg(wp + 2);
-            w[0] = a.x; w[1] = a.y; w[2] = b.x; w[3] = b.y; w[4] = c.x;
+    int par = 0;
+    for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
+        const uint4 item = __ldg(items + it);
+        const uint32_t pos0 = item.x, cnt = item.y, g = item.z;
+        unsigned long long rec[TR_RPT];
+        bool valid[TR_RPT];
+#pragma unroll
+        for (int r = 0; r < TR_RPT; r++) {
+            const uint32_t idx = (uint32_t)(r * TR_THREADS + tid);
+            valid[r] = idx < cnt;
+            rec[r] = valid[r] ? __ldg(recs + pos0 + idx) : 0ull;
         }
-        const int Jminb = (db.y >> 16) & 255, Jmink = (dk.y >> 16) & 255;
-        const int Jlo = max(Jminb, Jmink), Jhi = min((db.y >> 24) & 255, (dk.y >> 24) & 255);
-        const uint32_t jib = (uint32_t)(trb.y + ((Jlo - Jminb) >> 1)), jik = (uint32_t)(trk.y + ((Jlo - Jmink) >> 1));
-        double total = 0.0;
-        const int nJ = ((Jhi - Jlo) >> 1) + 1;
-        for (int q = 0; q < nJ; q++) {
-            const int2 ib = __ldg(T.jinfo3 + jib + q), ik = __ldg(T.jinfo3 + jik + q);
-            const int nb = ib.y, nk = ik.y;
-            const uint32_t rb0 = (uint32_t)ib.x, rk0 = (uint32_t)ik.x;
-            switch (nk) {
-                case 0: break;
-                case 1: total += j_block3<1>(T, rb0, rk0, nb, c1b, c1k, Ab, Ak, so, w); break;
-                case 2: total += j_block3<2>(T, rb0, rk0, nb, c1b, c1k, Ab, Ak, so, w); break;
-                case 3: total += j_block3<3>(T, rb0, rk0, nb, c1b, c1k, Ab, Ak, so, w); break;
-                case 4: total += j_block3<4>(T, rb0, rk0, nb, c1b, c1k, Ab, Ak, so, w); break;
-                case 5: total += j_block3<5>(T, rb0, rk0, nb, c1b, c1k, Ab, Ak, so, w); break;
-                case 6: total += j_block3<6>(T, rb0, rk0, nb, c1b, c1k, Ab, Ak, so, w); break;
-                case 7: total += j_block3<7>(T, rb0, rk0, nb, c1b, c1k, Ab, Ak, so, w); break;
-                case 8: total += j_block3<8>(T, rb0, rk0, nb, c1b, c1k, Ab, Ak, so, w); break;
-                default:
-                    total += j_block3_generic(GenericPtrs{T.rowtab3, T.cg1, T.cg2g, T.slab3}, rb0, rk0, nb, nk, c1b, c1k, Ab, Ak, so,
-                                              w[0], w[1], w[2], w[3], w[4]);
-                    so += (uint32_t)nb * (row_pitch3(nk) >> 1);
-                    break;
+        if (g == ZERO_ITEM) {   // block-uniform
+#pragma unroll
+            for (int r = 0; r < TR_RPT; r++)
+                if (valid[r]) {
+                    const uint32_t pos = pos0 + (uint32_t)(r * TR_THREADS + tid);
+                    out[order ? __ldg(order + pos) : pos] = 0.0;
+                }
+            continue;
+        }
+        int bin[TR_RPT];
+        uint32_t bits = 0u;
+#pragma unroll
+        for (int r = 0; r < TR_RPT; r++) {
+            bin[r] = sh.tz2bin[(uint32_t)(rec[r] >> 30) & 63u];
+            if (valid[r]) bits |= 1u << bin[r];
+        }
+        bits = __reduce_or_sync(0xFFFFFFFFu, bits);
+        __syncthreads();   // S0: the previous item's compute phase is over, shared state may be overwritten
+        if ((tid & 31) == 0) atomicOr(&sh.mask[par], bits);
+        if (tid < MAX_JBLK) {
+            const uint32_t tb = g / nt, tk = g - tb * nt;
+            const int4 kb = __ldg(T.tk3 + tb), kk = __ldg(T.tk3 + tk);
+            const int Jminb = (kb.w >> 16) & 255, Jmink = (kk.w >> 16) & 255;
+            const int Jlo = max(Jminb, Jmink), Jhi = min((kb.w >> 24) & 255, (kk.w >> 24) & 255);
+            const int nblk = ((Jhi - Jlo) >> 1) + 1;
+            const int qb = kb.z + ((Jlo - Jminb) >> 1), qk = kk.z + ((Jlo - Jmink) >> 1);
+            if (tid < nblk) {
+                const int2 jb = __ldg(T.jinfo3 + qb + tid), jk = __ldg(T.jinfo3 + qk + tid);
+                sh.nbk[tid] = (uint16_t)(jb.y | (jk.y << 8));
+                if (tid == 0) {
+                    const uint2 sg = __ldg(T.sgrp3 + g);
+                    sh.sc[0] = (uint32_t)kb.y;
+                    sh.sc[1] = (uint32_t)kk.y;
+                    sh.sc[2] = (uint32_t)kb.x + (uint32_t)jb.x * (uint32_t)kb.y;
+                    sh.sc[3] = (uint32_t)kk.x + (uint32_t)jk.x * (uint32_t)kk.y;
+                    sh.sc[4] = ((uint32_t)kb.w & 0xFFFFu) | (((uint32_t)kk.w & 0xFFFFu) << 16);
+                    sh.sc[5] = sg.y | ((uint32_t)nblk << 16);
+                    sh.sc[6] = sg.x;
+                    sh.sc[7] = 0u;
+                }
             }
         }
-        if (mine) result = (((rec >> 36) & 1) ? -total : total) + 0.0;   // + 0.0: never store -0
+        __syncthreads();   // S1
+        const uint32_t mask = sh.mask[par];
+        if (tid == 0) sh.mask[par ^ 1] = 0u;
+        const uint4 s0 = *reinterpret_cast<const uint4*>(&sh.sc[0]);
+        const uint4 s1 = *reinterpret_cast<const uint4*>(&sh.sc[4]);
+        const uint32_t Sb = s0.x, Sk = s0.y;
+        const uint32_t gsize = s1.y & 0xFFFFu;
+        const int nblk = (int)(s1.y >> 16);
+        const int jb1 = s1.x & 255, jc1 = (s1.x >> 8) & 255, je1 = (s1.x >> 16) & 255, jf1 = (s1.x >> 24) & 255;
+        const uint32_t bpr = min((uint32_t)NBIN3, (uint32_t)VW_CAP / gsize);   // bins per round
+        const uint32_t inv = 0xFFFFFFFFu / gsize + 1u;
+        const double* __restrict__ slab = T.slab3 + (size_t)s1.z * 2;
+        double res[TR_RPT];
+#pragma unroll
+        for (int r = 0; r < TR_RPT; r++) res[r] = 0.0;
+        bool first = true;
+        for (uint32_t b0 = 0; b0 < (uint32_t)NBIN3; b0 += bpr) {
+            if (((mask >> b0) & ((1u << bpr) - 1u)) == 0u) continue;   // block-uniform
+            if (!first) __syncthreads();   // the previous round's compute phase is over
+            first = false;
+            for (uint32_t idx = tid; idx < bpr * gsize; idx += TR_THREADS) {
+                const uint32_t bl = __umulhi(idx, inv), c = idx - bl * gsize, b = b0 + bl;
+                if (b < (uint32_t)NBIN3 && ((mask >> b) & 1u)) {
+                    const double* w = &sh.w[b * NISO3];
+                    double v = w[0] * __ldg(slab + c);
+                    v = fma(w[1], __ldg(slab + gsize + c), v);
+                    v = fma(w[2], __ldg(slab + 2 * gsize + c), v);
+                    v = fma(w[3], __ldg(slab + 3 * gsize + c), v);
+                    v = fma(w[4], __ldg(slab + 4 * gsize + c), v);
+                    sh.vw[idx] = v;
+                }
+            }
+            __syncthreads();   // S2
+#pragma unroll 1
+            for (int r = 0; r < TR_RPT; r++) {
+                static_assert(TR_RPT == 2, "record selection below assumes two records per thread");
+                const unsigned long long rc = r ? rec[1] : rec[0];   // static indices: the arrays stay in registers
+                const uint32_t bl = (uint32_t)(r ? bin[1] : bin[0]) - b0;
+                if (!(r ? valid[1] : valid[0]) || bl >= bpr) continue;
+                const uint32_t mrec = (uint32_t)rc;
+                const int ima = mrec & 31, imb = (mrec >> 5) & 31, imc = (mrec >> 10) & 31;
+                const int imd = (mrec >> 15) & 31, ime = (mrec >> 20) & 31, imf = (mrec >> 25) & 31;
+                uint32_t pb = s0.z + (uint32_t)((ima * jb1 + imb) * jc1 + imc);
+                uint32_t pk = s0.w + (uint32_t)((imd * je1 + ime) * jf1 + imf);
+                uint32_t vi = bl * gsize;
+                const double* __restrict__ dtab = T.dtab3;
+                double total = 0.0;
+                for (int q = 0; q < nblk; q++) {
+                    const uint32_t d = sh.nbk[q];
+                    const int nb = d & 255, nk = d >> 8;
+                    switch (nk) {
+                        case 1: total += j_block3<1>(dtab, sh.vw, pb, pk, Sb, Sk, nb, vi); break;
+                        case 2: total += j_block3<2>(dtab, sh.vw, pb, pk, Sb, Sk, nb, vi); break;
+                        case 3: total += j_block3<3>(dtab, sh.vw, pb, pk, Sb, Sk, nb, vi); break;
+                        case 4: total += j_block3<4>(dtab, sh.vw, pb, pk, Sb, Sk, nb, vi); break;
+                        case 5: total += j_block3<5>(dtab, sh.vw, pb, pk, Sb, Sk, nb, vi); break;
+                        case 6: total += j_block3<6>(dtab, sh.vw, pb, pk, Sb, Sk, nb, vi); break;
+                        default:
+                            if (nk > 0 && nb > 0) total += j_block3_generic(dtab, sh.vw, pb, pk, Sb, Sk, nb, nk, vi);
+                            pb += (uint32_t)nb * Sb;
+                            pk += (uint32_t)nk * Sk;
+                            if (nk > 0) vi += (uint32_t)(nb * row_pitch3(nk));
+                            break;
+                    }
+                }
+                const double val = (((rc >> 36) & 1) ? -total : total) + 0.0;   // + 0.0: never store -0
+                if (r) res[1] = val; else res[0] = val;
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < TR_RPT; r++)
+            if (valid[r]) {
+                const uint32_t pos = pos0 + (uint32_t)(r * TR_THREADS + tid);
+                out[order ? __ldg(order + pos) : pos] = res[r];
+            }
+        par ^= 1;
     }
-    if (valid) out[order ? (long long)__ldg(order + pos) : pos] = result;
 }
 
 __global__ void __launch_bounds__(128) k_transform2(Tables T, long long n, const unsigned long long* __restrict__ recs,
@@ -595,17 +705,27 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
     const long long n_tiles = (n_buckets + SCAN_TILE - 1) / SCAN_TILE;
     const bool naive = flags & MFDN_FORCE_NAIVE;
     const bool sort = !naive && !(flags & MFDN_PRESORTED);
+    const bool items = !naive && BODY == 3;    // the 3-body transform walks a list of one-group work items
+    const bool hist_needed = sort || items;
+    const long long max_items = n / ITEM3 + std::min<long long>(n, n_buckets) + 1;
     size_t need = 256;
-    size_t o_recs = 0, o_sorted = 0, o_order = 0, o_hist = 0, o_sums = 0;
+    size_t o_recs = 0, o_sorted = 0, o_order = 0, o_hist = 0, o_sums = 0, o_items = 0, o_count = 0;
     if (!naive) {
-        o_recs = 0;
         need = o_recs + align256((size_t)n * 8);
         if (sort) {
             o_sorted = need;
             o_order = o_sorted + align256((size_t)n * 8);
-            o_hist = o_order + align256((size_t)n * 4);
+            need = o_order + align256((size_t)n * 4);
+        }
+        if (hist_needed) {
+            o_hist = need;
             o_sums = o_hist + align256((size_t)n_buckets * 4);
             need = o_sums + align256((size_t)n_tiles * 4);
+        }
+        if (items) {
+            o_items = need;
+            o_count = o_items + align256((size_t)max_items * 16);
+            need = o_count + 256;
         }
     }
     if (!d_work) { *work_bytes = need; return MFDN_OK; }
@@ -631,29 +751,43 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
         unsigned long long* recs = (unsigned long long*)(w + o_recs);
         const unsigned long long* trecs = recs;
         const uint32_t* order = nullptr;
+        uint32_t* hist = hist_needed ? (uint32_t*)(w + o_hist) : nullptr;
+        uint32_t* sums = hist_needed ? (uint32_t*)(w + o_sums) : nullptr;
         const unsigned gk = (unsigned)((n + 255) / 256);
-        if (sort) {
-            unsigned long long* sorted = (unsigned long long*)(w + o_sorted);
-            uint32_t* ord = (uint32_t*)(w + o_order);
-            uint32_t* hist = (uint32_t*)(w + o_hist);
-            uint32_t* sums = (uint32_t*)(w + o_sums);
-            MFDN_CUDA(c, cudaMemsetAsync(hist, 0, (size_t)n_buckets * 4, st));
-            k_keys<BODY><<<gk, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, (uint32_t)(nt * nt), nullptr);
+        const uint32_t invalid_bucket = (uint32_t)(nt * nt);
+        if (hist_needed) MFDN_CUDA(c, cudaMemsetAsync(hist, 0, (size_t)n_buckets * 4, st));
+        if (sort) k_keys<BODY, false><<<gk, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr);
+        else k_keys<BODY, true><<<gk, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr);
+        c->launches += 1;
+        if (hist_needed) {
             k_scan_tiles<<<(unsigned)n_tiles, SCAN_T, 0, st>>>(hist, n_buckets, sums);
             k_scan_sums<<<1, 1024, 0, st>>>(sums, (int)n_tiles);
             k_scan_add<<<(unsigned)n_tiles, SCAN_T, 0, st>>>(hist, n_buckets, sums);
-            k_scatter<<<gk, 256, 0, st>>>(n, recs, hist, sorted, ord, (uint32_t)(nt * nt));
-            c->launches += 5;
+            c->launches += 3;
+        }
+        if (sort) {
+            unsigned long long* sorted = (unsigned long long*)(w + o_sorted);
+            uint32_t* ord = (uint32_t*)(w + o_order);
+            k_scatter<<<gk, 256, 0, st>>>(n, recs, hist, sorted, ord, invalid_bucket);
+            c->launches += 1;
             trecs = sorted;
             order = ord;
+        }
+        if (items) {
+            uint4* itm = (uint4*)(w + o_items);
+            uint32_t* cnt = (uint32_t*)(w + o_count);
+            MFDN_CUDA(c, cudaMemsetAsync(cnt, 0, 4, st));
+            k_items3<<<(unsigned)((n_buckets + 255) / 256), 256, 0, st>>>(hist, (uint32_t)n_buckets, sort ? 1 : 0, (uint32_t)n, c->t.sgrp3,
+                                                                           invalid_bucket, itm, cnt);
+            if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.b, st));
+            const unsigned grid = (unsigned)std::min<long long>(max_items, (long long)c->num_sms * 4);
+            k_transform3<<<grid, TR_THREADS, 0, st>>>(c->t, itm, cnt, trecs, order, d_out);
+            c->launches += 2;
         } else {
-            k_keys<BODY><<<gk, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, nullptr, 0u, nullptr);
+            if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.b, st));
+            k_transform2<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(c->t, n, trecs, order, d_out);
             c->launches += 1;
         }
-        if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.b, st));
-        if (BODY == 3) k_transform3<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(c->t, n, trecs, order, d_out);
-        else k_transform2<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(c->t, n, trecs, order, d_out);
-        c->launches += 1;
     }
     MFDN_CUDA(c, cudaGetLastError());
     if (c->profile) {
@@ -695,8 +829,8 @@ extern "C" int mfdn_group_keys(mfdn_ctx* c, int body, int64_t n, const int32_t* 
     if (body == 3 ? !c->has3 : !c->has2) return fail(c, MFDN_ERR_STATE, "group_keys before coupled upload");
     if (n == 0) return MFDN_OK;
     cudaStream_t st = (cudaStream_t)stream;
-    if (body == 3) k_keys<3><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(c->t, n, d_req, nullptr, nullptr, nullptr, 0u, d_key);
-    else k_keys<2><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(c->t, n, d_req, nullptr, nullptr, nullptr, 0u, d_key);
+    if (body == 3) k_keys<3, false><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(c->t, n, d_req, nullptr, nullptr, nullptr, 0u, d_key);
+    else k_keys<2, false><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(c->t, n, d_req, nullptr, nullptr, nullptr, 0u, d_key);
     MFDN_CUDA(c, cudaGetLastError());
     return MFDN_OK;
 }
