@@ -403,7 +403,7 @@ __global__ void k_retile3(Retile3 p)
     }
 }
 
-// Per-tuple coefficient tables (A1/A2): dtab[tk.x + row*S + (ima*(jb+1) + imb)*(jc+1) + imc] =
+// Per-tuple coefficient tables (A1/A2): dtab[tk.x + row*S + sigma(ima, imb, imc)] =
 // <ja ma jb mb|J12 M12> <J12 M12 jc mc|J M> for the tuple's rows (J, J12) in loop order; one fp64 product of the two
 // tabulated coefficients, 0 where |M12| > J12 or |M| > J (the zero guard of the stage-2 table).
 struct Dtab3 {
@@ -412,6 +412,8 @@ struct Dtab3 {
     const int2* trow;      // {first row of the tuple in rowtab, -}
     const int2* rowtab;    // per row {cg2g offset at A = 0, cg1 offset relative to the m-pair base}
     const int32_t* nrows;
+    const uint16_t* sig;
+    const int32_t* sigoff;
     const double* cg1;
     const int32_t* cg1_off;
     const double* cg2g;
@@ -431,7 +433,7 @@ __global__ void k_dtab3(Dtab3 p)
         int imc = o % (jc + 1), imb = (o / (jc + 1)) % (jb + 1), ima = o / ((jc + 1) * (jb + 1));
         int2 rt = p.rowtab[r0 + r];
         int A = (ima + imb - ((ja + jb) >> 1)) * (jc + 1) + imc;
-        p.dtab[(size_t)(uint32_t)k.x + idx] = p.cg1[c1 + ima * (jb + 1) + imb + rt.y] * p.cg2g[rt.x + A];
+        p.dtab[(size_t)(uint32_t)k.x + (size_t)r * S + p.sig[p.sigoff[t] + o]] = p.cg1[c1 + ima * (jb + 1) + imb + rt.y] * p.cg2g[rt.x + A];
     }
 }
 
@@ -588,7 +590,8 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     //      and per (tuple, J): {first row (tuple-relative), number of rows}
     std::vector<int2> trow(nt), rowtab, jinfo;
     std::vector<int4> tk(nt);
-    std::vector<int32_t> nrows(nt);
+    std::vector<int32_t> nrows(nt), sigoff(nt);
+    std::vector<uint16_t> sig;
     uint64_t dtab_len = 0;
     for (int t = 0; t < nt; t++) {
         int4 d = tdesc[t];
@@ -612,11 +615,23 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
         }
         nrows[t] = (int)rowtab.size() - trow[t].x;
         const int S = (ja + 1) * (jb + 1) * (jc + 1);
+        if (S > MAX_STATES3) return fail(c, MFDN_ERR_TABLE, "tuple with more than 4096 m-states");
+        // sigma: m-states of the tuple ordered by (iM = ima+imb+imc, ima, imb); counting sort over iM
+        sigoff[t] = (int32_t)sig.size();
+        {
+            std::vector<int> start(ja + jb + jc + 2, 0);
+            for (int a = 0; a <= ja; a++) for (int b = 0; b <= jb; b++) for (int m = 0; m <= jc; m++) start[a + b + m + 1]++;
+            for (size_t i = 1; i < start.size(); i++) start[i] += start[i - 1];
+            sig.resize(sig.size() + S);
+            uint16_t* sg = sig.data() + sigoff[t];
+            for (int a = 0; a <= ja; a++) for (int b = 0; b <= jb; b++) for (int m = 0; m <= jc; m++)
+                sg[(a * (jb + 1) + b) * (jc + 1) + m] = (uint16_t)start[a + b + m]++;
+        }
         if (dtab_len + (uint64_t)nrows[t] * S >= 0x7FFFFFF0ull) return fail(c, MFDN_ERR_OOM, "coefficient table too large for 31-bit offsets");
         tk[t].x = (int)dtab_len;
         tk[t].y = S;
         tk[t].z = trow[t].y;
-        tk[t].w = (jb + 1) | ((jc + 1) << 8) | (d.y & 0xFFFF0000);
+        tk[t].w = (ja + jb + jc) | (d.y & 0xFFFF0000);
         dtab_len += (uint64_t)nrows[t] * S;
         dtab_len = (dtab_len + 1) & ~1ull;
     }
@@ -643,7 +658,7 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     // ---- one arena for the resident index tables, one for the upload-only ones
     Arena res, tmp;
     size_t o_tid = res.add(tuple_id), o_desc = res.add(tdesc), o_sgrp = res.add(sgrp), o_sm = res.add(stmask);
-    size_t o_tk = res.add(tk), o_jinfo = res.add(jinfo);
+    size_t o_tk = res.add(tk), o_jinfo = res.add(jinfo), o_sig = res.add(sig), o_sigoff = res.add(sigoff);
     std::vector<int64_t> coff(chan_off, chan_off + n_chan);
     std::vector<int32_t> cdim(chan_dim, chan_dim + n_chan);
     size_t o_rm = tmp.add(rowmap), o_cof = tmp.add(chan_of), o_coff = tmp.add(coff), o_cdim = tmp.add(cdim);
@@ -688,6 +703,8 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     q.trow = (const int2*)((char*)dtmp + o_trow);
     q.rowtab = (const int2*)((char*)dtmp + o_rowtab);
     q.nrows = (const int32_t*)((char*)dtmp + o_nrows);
+    q.sig = (const uint16_t*)(dres + o_sig);
+    q.sigoff = (const int32_t*)(dres + o_sigoff);
     q.cg1 = c->t.cg1;
     q.cg1_off = c->t.cg1_off;
     q.cg2g = c->t.cg2g;
@@ -709,6 +726,8 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     c->t.tk3 = q.tk;
     c->t.jinfo3 = (const int2*)(dres + o_jinfo);
     c->t.dtab3 = (const double*)ddtab;
+    c->t.sig3 = q.sig;
+    c->t.sigoff3 = q.sigoff;
     c->slab_bytes3 = (int64_t)(cells * 16);
     c->dtab_bytes3 = (int64_t)(dtab_len * sizeof(double));
     c->has3 = true;

@@ -39,14 +39,18 @@ constexpr int CG_GUARD = 8192;     // zero doubles before and after the stage-2 
 // not listed.  The isospin-combined copy Vw = sum_s w[s] * plane[s] that the transform stages in shared memory has
 // the same indexing.
 __host__ __device__ inline int row_pitch3(int nk) { return (nk + 1) & ~1; }
-constexpr int ITEM3 = 512;         // records per work item of the 3-body transform (one group per item)
+constexpr int ITEM3 = 1024;        // max records per work item of the 3-body transform (one group per item)
 constexpr uint32_t ZERO_ITEM = 0xFFFFFFFFu;   // work item whose records all have value 0 (no slab / failed S1-S6)
 
 // ---- packed canonical request record (H1 output), 64 bit --------------------------------------------
-//  [0,30) im of the canonical particles (5 bits each: bra then ket)   [30,36) tz bits (bra then ket)
-//  [36] 1 = odd permutation (sign -1)                                  [37,64) group key, REC_INVALID if S1-S6 fail
+// 2-body: [0,30) im of the canonical particles (5 bits each: bra at 0,5; ket at 15,20)   [30,36) tz bits (bra then ket)
+//         [36] 1 = odd permutation (sign -1)                     [37,64) group key, REC_INVALID if S1-S6 fail
+// 3-body: [0,12) sigma_b  [12,24) sigma_k : index of the bra / ket m-state in its tuple's coefficient table (M-major)
+//         [24,29) isospin bin   [29] 1 = odd permutation   [30,36) iM = ima+imb+imc of the bra (M = iM - (ja+jb+jc)/2)
+//         [37,64) group key
 constexpr unsigned REC_KEY_SHIFT = 37;
 constexpr uint32_t REC_INVALID = 0x7FFFFFFu;
+constexpr int MAX_STATES3 = 4096;   // (ja+1)(jb+1)(jc+1) of a tuple must fit the 12-bit sigma fields
 
 // ---- per-tuple descriptor (A2), 16 bytes ---------------------------------------------------------
 // 3-body: x = ja | jb<<8 | jc<<16 | (a==b)<<24 | par<<25      (ja.. are 2j)
@@ -55,7 +59,7 @@ constexpr uint32_t REC_INVALID = 0x7FFFFFFu;
 //         w = offset of the tuple's row map (upload only)
 // tk3 (what the transform kernel needs of a tuple): x = offset of the tuple's coefficient table in dtab3 (doubles),
 //         y = its row pitch S = (ja+1)(jb+1)(jc+1), z = first entry of the tuple in jinfo3,
-//         w = (jb+1) | (jc+1)<<8 | twoJmin<<16 | twoJmax<<24
+//         w = (ja+jb+jc) | twoJmin<<16 | twoJmax<<24
 // 2-body: x = ja | jb<<8 | (a==b)<<24 | par<<25,  y = Jmin | Jmax<<8,  z = state mask (low), w = (high)
 struct Tables {
     // A0
@@ -84,7 +88,10 @@ struct Tables {
     const unsigned long long* stmask3;
     const int4* tk3;               // [n_tup3] see above
     const int2* jinfo3;            // per (tuple, J): {first row of this J (tuple-relative, loop order J, J12), number of rows}
-    const double* dtab3;           // per tuple [row][ima][imb][imc] = <ja ma jb mb|J12 M12> <J12 M12 jc mc|J M>
+    const double* dtab3;           // per tuple [row][sigma] = <ja ma jb mb|J12 M12> <J12 M12 jc mc|J M>
+    const uint16_t* sig3;          // per tuple [(ima*(jb+1)+imb)*(jc+1)+imc] -> sigma: m-states ordered by (M, ima, imb), so that
+                                   // requests with equal M (bra and ket always have equal M) read neighbouring entries
+    const int32_t* sigoff3;        // [n_tup3] start of the tuple's sigma table in sig3
     // A2, 2-body
     int n_tup2;
     const int32_t* tuple_id2;      // [n_orb^2]

@@ -298,9 +298,15 @@ __global__ void __launch_bounds__(256) k_keys(Tables T, long long n, const int32
         Side3 B = decode3(T, s[0], s[1], s[2]), K = decode3(T, s[3], s[4], s[5]);
         if (select3(T, B, K)) {
             key = (uint32_t)B.tup * T.n_tup3 + K.tup;
-            if (__ldg(T.sgrp3 + key).x != NO_SLAB) mask = mask3(T, B, K, __ldg(T.tdesc3 + B.tup), __ldg(T.tdesc3 + K.tup));
-            low = (unsigned long long)(B.ima | (B.imb << 5) | (B.imc << 10) | (K.ima << 15) | (K.imb << 20) | (K.imc << 25)) |
-                  ((unsigned long long)((B.tz << 3) | K.tz) << 30) | ((unsigned long long)(B.sign * K.sign < 0) << 36);
+            const int4 db = __ldg(T.tdesc3 + B.tup), dk = __ldg(T.tdesc3 + K.tup);
+            if (__ldg(T.sgrp3 + key).x != NO_SLAB) mask = mask3(T, B, K, db, dk);
+            const int jb1 = ((db.x >> 8) & 255) + 1, jc1 = ((db.x >> 16) & 255) + 1;
+            const int je1 = ((dk.x >> 8) & 255) + 1, jf1 = ((dk.x >> 16) & 255) + 1;
+            const uint32_t sb = __ldg(T.sig3 + __ldg(T.sigoff3 + B.tup) + (B.ima * jb1 + B.imb) * jc1 + B.imc);
+            const uint32_t sk = __ldg(T.sig3 + __ldg(T.sigoff3 + K.tup) + (K.ima * je1 + K.imb) * jf1 + K.imc);
+            const uint32_t bin = __ldg(T.tz2bin3 + ((B.tz << 3) | K.tz));
+            low = (unsigned long long)(sb | (sk << 12) | (bin << 24) | ((uint32_t)(B.sign * K.sign < 0) << 29)) |
+                  ((unsigned long long)(B.ima + B.imb + B.imc) << 30);
         }
     } else {
         Side2 B = decode2(T, s[0], s[1]), K = decode2(T, s[2], s[3]);
@@ -431,53 +437,114 @@ __global__ void __launch_bounds__(256) k_items3(const uint32_t* __restrict__ bou
     for (uint32_t j = 0; j < k; j++) items[slot + j] = make_uint4(start + j * ITEM3, min((uint32_t)ITEM3, cnt - j * ITEM3), g, 0u);
 }
 
-constexpr int TR_THREADS = 256;
-constexpr int TR_RPT = ITEM3 / TR_THREADS;   // records per thread
-constexpr int VW_CAP = 3072;                 // doubles: isospin-combined slabs Vw[bin][cell] of the current item (24 KB)
+constexpr int TR_THREADS = 128;
+constexpr int VW_CAP = 2048;                 // doubles: isospin-combined slabs Vw[bin][cell] of the current item (16 KB)
 constexpr int MAX_JBLK = 32;                 // common J values of a group (2J <= 63)
+constexpr int NM_MAX = 64;                   // iM = ima+imb+imc < 64 (3*MAX_TWOJ = 63)
 
 struct ItemShared {
     double vw[VW_CAP];
+    unsigned long long desc[MAX_JBLK];       // per J block: nb | nk<<8 | rows_b before<<16 | rows_k before<<24 | Vw doubles before<<32 | dispatch code<<48
     double w[NBIN3 * NISO3];
     uint32_t sc[8];
-    uint32_t mask[2];
-    uint16_t nbk[MAX_JBLK];
-    uint8_t tz2bin[64];
+    uint32_t hist[NM_MAX + 1];               // records per iM
+    uint32_t soff[NM_MAX + 1];
+    uint32_t mask;
+    uint16_t sidx[ITEM3];                    // position in the item of the record in M-sorted slot i
+    uint16_t srank[ITEM3];                   // per record: iM<<10 | rank among the item's records of equal iM
 };
 
-// One J block of the sum with the ket range size NK known at compile time:
+// bin stride of Vw: >= gsize, == 2 (mod 16) doubles, so that different bins fall into different bank quads
+__device__ __forceinline__ uint32_t vw_stride(uint32_t gsize) { return ((gsize + 13u) & ~15u) + 2u; }
+
+// One J block of the sum for TWO records of the group (A and B, 32 sorted slots apart) with the ket range size NK known
+// at compile time and a run-time loop over the bra rows (blocks with more than 4 rows or columns):
 //   sum_i cb(i) * sum_k ck(k) * Vw[i][k],  cb/ck read from the tuples' coefficient tables (one gather per row),
 // Vw rows (padded to even length) read from shared memory with 128-bit loads.
 template <int NK>
-__device__ __forceinline__ double j_block3(const double* __restrict__ dtab, const double* __restrict__ vw, uint32_t& pb, uint32_t& pk,
-                                           uint32_t Sb, uint32_t Sk, int nb, uint32_t& vi)
+__device__ __forceinline__ void j_block3x2_rows(const double* __restrict__ dtab, const double* __restrict__ vw, uint32_t& pbA, uint32_t& pkA,
+                                                uint32_t& pbB, uint32_t& pkB, uint32_t Sb, uint32_t Sk, int nb, uint32_t& viA,
+                                                uint32_t& viB, double& totA, double& totB)
 {
-    double ck[NK];
+    constexpr int P = (NK + 1) & ~1;
+    double ckA[NK], ckB[NK];
 #pragma unroll
     for (int k = 0; k < NK; k++) {
-        ck[k] = __ldg(dtab + pk);
-        pk += Sk;
+        ckA[k] = __ldg(dtab + pkA + (uint32_t)k * Sk);
+        ckB[k] = __ldg(dtab + pkB + (uint32_t)k * Sk);
     }
-    constexpr int P = (NK + 1) & ~1;
-    double total = 0.0;
+    pkA += NK * Sk; pkB += NK * Sk;
+    double tA = 0.0, tB = 0.0;
 #pragma unroll 2
     for (int i = 0; i < nb; i++) {
-        const double cb = __ldg(dtab + pb);
-        pb += Sb;
-        double v[P];
+        const double cbA = __ldg(dtab + pbA), cbB = __ldg(dtab + pbB);
+        pbA += Sb; pbB += Sb;
+        double vA[P], vB[P];
 #pragma unroll
         for (int q = 0; q < P / 2; q++) {
-            double2 t = *reinterpret_cast<const double2*>(vw + vi + 2 * q);
-            v[2 * q] = t.x;
-            v[2 * q + 1] = t.y;
+            const double2 a = *reinterpret_cast<const double2*>(vw + viA + 2 * q);
+            const double2 b = *reinterpret_cast<const double2*>(vw + viB + 2 * q);
+            vA[2 * q] = a.x; vA[2 * q + 1] = a.y;
+            vB[2 * q] = b.x; vB[2 * q + 1] = b.y;
         }
-        vi += P;
-        double acc = ck[0] * v[0];
+        viA += P; viB += P;
+        double accA = ckA[0] * vA[0], accB = ckB[0] * vB[0];
 #pragma unroll
-        for (int k = 1; k < NK; k++) acc = fma(ck[k], v[k], acc);
-        total = fma(cb, acc, total);
+        for (int k = 1; k < NK; k++) {
+            accA = fma(ckA[k], vA[k], accA);
+            accB = fma(ckB[k], vB[k], accB);
+        }
+        tA = fma(cbA, accA, tA);
+        tB = fma(cbB, accB, tB);
     }
-    return total;
+    totA += tA;
+    totB += tB;
+}
+
+// The same J block for TWO records of the group at once (A and B, 32 sorted slots apart), bra and ket range sizes
+// both known at compile time: every load of the block is issued before the first multiply, the loop control is shared.
+template <int NB, int NK>
+__device__ __forceinline__ void j_block3x2(const double* __restrict__ dtab, const double* __restrict__ vw, uint32_t& pbA, uint32_t& pkA,
+                                           uint32_t& pbB, uint32_t& pkB, uint32_t Sb, uint32_t Sk, uint32_t& viA, uint32_t& viB,
+                                           double& totA, double& totB)
+{
+    constexpr int P = (NK + 1) & ~1;
+    double ckA[NK], ckB[NK], cbA[NB], cbB[NB];
+#pragma unroll
+    for (int k = 0; k < NK; k++) {
+        ckA[k] = __ldg(dtab + pkA + (uint32_t)k * Sk);
+        ckB[k] = __ldg(dtab + pkB + (uint32_t)k * Sk);
+    }
+#pragma unroll
+    for (int i = 0; i < NB; i++) {
+        cbA[i] = __ldg(dtab + pbA + (uint32_t)i * Sb);
+        cbB[i] = __ldg(dtab + pbB + (uint32_t)i * Sb);
+    }
+    double tA = 0.0, tB = 0.0;
+#pragma unroll
+    for (int i = 0; i < NB; i++) {
+        double vA[P], vB[P];
+#pragma unroll
+        for (int q = 0; q < P / 2; q++) {
+            const double2 a = *reinterpret_cast<const double2*>(vw + viA + i * P + 2 * q);
+            const double2 b = *reinterpret_cast<const double2*>(vw + viB + i * P + 2 * q);
+            vA[2 * q] = a.x; vA[2 * q + 1] = a.y;
+            vB[2 * q] = b.x; vB[2 * q + 1] = b.y;
+        }
+        double accA = ckA[0] * vA[0], accB = ckB[0] * vB[0];
+#pragma unroll
+        for (int k = 1; k < NK; k++) {
+            accA = fma(ckA[k], vA[k], accA);
+            accB = fma(ckB[k], vB[k], accB);
+        }
+        tA = fma(cbA[i], accA, tA);
+        tB = fma(cbB[i], accB, tB);
+    }
+    pkA += NK * Sk; pkB += NK * Sk;
+    pbA += NB * Sb; pbB += NB * Sb;
+    viA += NB * P; viB += NB * P;
+    totA += tA;
+    totB += tB;
 }
 
 // any ket range size (rare: nk > 6): ket coefficient re-read per cell
@@ -496,97 +563,129 @@ __device__ __noinline__ double j_block3_generic(const double* __restrict__ dtab,
     return total;
 }
 
-// H3-H6.  Persistent blocks walk the item list.  Per item: (1) the block ORs the isospin bins (tz patterns) of its
-// records into a shared mask; (2) it stages Vw[bin][cell] = sum_s w[bin][s] * plane_s[cell] for the bins present -- the
-// paper's "isospin loops ... unrolled into a single weighted summation" done once per (group, bin) instead
-// of once per request; (3) every thread evaluates its records: three nested loops over J, J12, J12' with
-// all bounds shared by the block, the lanes differing only in their projections (coefficient-table offsets) and bin.
-__global__ void __launch_bounds__(TR_THREADS, 4) k_transform3(Tables T, const uint4* __restrict__ items, const uint32_t* __restrict__ n_items_p,
+// H3-H6.  Persistent blocks walk the item list.  Per item (<= ITEM3 records of one group):
+//  (1) the block histograms the item's records by iM (the bra's, = the ket's, M) and ORs their isospin bins into a mask;
+//      warp 0 meanwhile builds the J-block descriptors of the group;
+//  (2) it stages Vw[bin][cell] = sum_s w[bin][s] * plane_s[cell] for the bins present -- the paper's "isospin loops ...
+//      unrolled into a single weighted summation", done once per (item, bin) instead of once per request --
+//      and builds the M-sorted order of the records: the coefficient tables are M-major, so the 32 gathers of a warp
+//      fall into one or two cache lines on the bra AND on the ket side;
+//  (3) every thread evaluates records in sorted order: three nested loops over J, J12, J12' whose bounds
+//      are shared by the block; lanes differ in their table offsets (sigma), bin and first J block (J >= |M|).
+__global__ void __launch_bounds__(TR_THREADS, 6) k_transform3(Tables T, const uint4* __restrict__ items, const uint32_t* __restrict__ n_items_p,
                                                              const unsigned long long* __restrict__ recs,
                                                              const uint32_t* __restrict__ order, double* __restrict__ out)
 {
     __shared__ __align__(16) ItemShared sh;
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31;
     for (int i = tid; i < NBIN3 * NISO3; i += TR_THREADS) sh.w[i] = __ldg(T.wbin3 + i);
-    if (tid < 64) sh.tz2bin[tid] = __ldg(T.tz2bin3 + tid);
-    if (tid < 2) sh.mask[tid] = 0u;
+    if (tid <= NM_MAX) sh.hist[tid] = 0u;
+    if (tid == 0) sh.mask = 0u;
     __syncthreads();
     const uint32_t n_items = __ldg(n_items_p);
     const uint32_t nt = (uint32_t)T.n_tup3;
-    int par = 0;
+    const double* __restrict__ dtab = T.dtab3;
     for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
         const uint4 item = __ldg(items + it);
         const uint32_t pos0 = item.x, cnt = item.y, g = item.z;
-        unsigned long long rec[TR_RPT];
-        bool valid[TR_RPT];
-#pragma unroll
-        for (int r = 0; r < TR_RPT; r++) {
-            const uint32_t idx = (uint32_t)(r * TR_THREADS + tid);
-            valid[r] = idx < cnt;
-            rec[r] = valid[r] ? __ldg(recs + pos0 + idx) : 0ull;
-        }
+        const unsigned long long* __restrict__ irec = recs + pos0;
         if (g == ZERO_ITEM) {   // block-uniform
-#pragma unroll
-            for (int r = 0; r < TR_RPT; r++)
-                if (valid[r]) {
-                    const uint32_t pos = pos0 + (uint32_t)(r * TR_THREADS + tid);
-                    out[order ? __ldg(order + pos) : pos] = 0.0;
-                }
+            for (uint32_t idx = tid; idx < cnt; idx += TR_THREADS) out[order ? __ldg(order + pos0 + idx) : pos0 + idx] = 0.0;
             continue;
         }
-        int bin[TR_RPT];
-        uint32_t bits = 0u;
+        __syncthreads();   // B0: the previous item is finished, shared state may be overwritten
+        {   // (1) histogram over iM (each record keeps its rank inside its iM bucket), mask of the isospin bins present
+            uint32_t bits = 0u;
+            constexpr int U = 4;   // records in flight per thread
+            for (uint32_t base = 0; base < cnt; base += U * TR_THREADS) {
+                unsigned long long rec[U];
 #pragma unroll
-        for (int r = 0; r < TR_RPT; r++) {
-            bin[r] = sh.tz2bin[(uint32_t)(rec[r] >> 30) & 63u];
-            if (valid[r]) bits |= 1u << bin[r];
+                for (int u = 0; u < U; u++) {
+                    const uint32_t idx = base + u * TR_THREADS + tid;
+                    rec[u] = idx < cnt ? __ldg(irec + idx) : 0ull;
+                }
+#pragma unroll
+                for (int u = 0; u < U; u++) {
+                    const uint32_t idx = base + u * TR_THREADS + tid;
+                    if (base + u * TR_THREADS + (uint32_t)(tid & ~31) >= cnt) break;   // warp-uniform
+                    const bool valid = idx < cnt;
+                    const uint32_t key = valid ? (uint32_t)(rec[u] >> 30) & 63u : (uint32_t)NM_MAX;
+                    if (valid) bits |= 1u << ((uint32_t)(rec[u] >> 24) & 31u);
+                    const unsigned same = __match_any_sync(0xFFFFFFFFu, key);
+                    const int leader = __ffs(same) - 1;
+                    uint32_t rank = 0u;
+                    if (lane == leader) rank = atomicAdd(&sh.hist[key], (uint32_t)__popc(same));
+                    rank = __shfl_sync(0xFFFFFFFFu, rank, leader) + (uint32_t)__popc(same & ((1u << lane) - 1u));
+                    if (valid) sh.srank[idx] = (uint16_t)((key << 10) | rank);
+                }
+            }
+            bits = __reduce_or_sync(0xFFFFFFFFu, bits);
+            if (lane == 0 && bits) atomicOr(&sh.mask, bits);
         }
-        bits = __reduce_or_sync(0xFFFFFFFFu, bits);
-        __syncthreads();   // S0: the previous item's compute phase is over, shared state may be overwritten
-        if ((tid & 31) == 0) atomicOr(&sh.mask[par], bits);
-        if (tid < MAX_JBLK) {
+        if (tid < 32) {   // warp 0: item scalars and J-block descriptors
             const uint32_t tb = g / nt, tk = g - tb * nt;
             const int4 kb = __ldg(T.tk3 + tb), kk = __ldg(T.tk3 + tk);
             const int Jminb = (kb.w >> 16) & 255, Jmink = (kk.w >> 16) & 255;
             const int Jlo = max(Jminb, Jmink), Jhi = min((kb.w >> 24) & 255, (kk.w >> 24) & 255);
             const int nblk = ((Jhi - Jlo) >> 1) + 1;
             const int qb = kb.z + ((Jlo - Jminb) >> 1), qk = kk.z + ((Jlo - Jmink) >> 1);
-            if (tid < nblk) {
-                const int2 jb = __ldg(T.jinfo3 + qb + tid), jk = __ldg(T.jinfo3 + qk + tid);
-                sh.nbk[tid] = (uint16_t)(jb.y | (jk.y << 8));
-                if (tid == 0) {
-                    const uint2 sg = __ldg(T.sgrp3 + g);
-                    sh.sc[0] = (uint32_t)kb.y;
-                    sh.sc[1] = (uint32_t)kk.y;
-                    sh.sc[2] = (uint32_t)kb.x + (uint32_t)jb.x * (uint32_t)kb.y;
-                    sh.sc[3] = (uint32_t)kk.x + (uint32_t)jk.x * (uint32_t)kk.y;
-                    sh.sc[4] = ((uint32_t)kb.w & 0xFFFFu) | (((uint32_t)kk.w & 0xFFFFu) << 16);
-                    sh.sc[5] = sg.y | ((uint32_t)nblk << 16);
-                    sh.sc[6] = sg.x;
-                    sh.sc[7] = 0u;
-                }
+            int2 jb = make_int2(0, 0), jk = make_int2(0, 0);
+            if (tid < nblk) { jb = __ldg(T.jinfo3 + qb + tid); jk = __ldg(T.jinfo3 + qk + tid); }
+            // exclusive prefix sums over the blocks: bra rows, ket rows, Vw doubles
+            const uint32_t rb = (uint32_t)jb.y, rk = (uint32_t)jk.y, vv = (uint32_t)(jb.y * row_pitch3(jk.y));
+            uint32_t ib = rb, ik = rk, iv = vv;
+#pragma unroll
+            for (int off = 1; off < 32; off <<= 1) {
+                uint32_t xb = __shfl_up_sync(0xFFFFFFFFu, ib, off), xk = __shfl_up_sync(0xFFFFFFFFu, ik, off), xv = __shfl_up_sync(0xFFFFFFFFu, iv, off);
+                if (lane >= off) { ib += xb; ik += xk; iv += xv; }
             }
+            if (tid < nblk) {
+                // dispatch code: 0..15 fully unrolled (nb, nk <= 4); 16 + nk row-loop templates (nk <= 8); 25 generic
+                const uint32_t code = (rb - 1u < 4u && rk - 1u < 4u) ? (rb - 1u) * 4u + (rk - 1u) : (rk - 1u < 8u && rb > 0u) ? 16u + rk : 25u;
+                sh.desc[tid] = (unsigned long long)(rb | (rk << 8) | ((ib - rb) << 16) | ((ik - rk) << 24)) |
+                               ((unsigned long long)((iv - vv) | (code << 16)) << 32);
+            }
+            if (tid == 0) {
+                const uint2 sg = __ldg(T.sgrp3 + g);
+                sh.sc[0] = (uint32_t)kb.y;
+                sh.sc[1] = (uint32_t)kk.y;
+                sh.sc[2] = (uint32_t)kb.x + (uint32_t)jb.x * (uint32_t)kb.y;
+                sh.sc[3] = (uint32_t)kk.x + (uint32_t)jk.x * (uint32_t)kk.y;
+                sh.sc[4] = ((uint32_t)kb.w & 0xFFu) | ((uint32_t)Jlo << 8) | ((uint32_t)nblk << 16);
+                sh.sc[5] = sg.y;
+                sh.sc[6] = sg.x;
+            }
+            if (tid == nblk - 1) sh.sc[7] = ib | (ik << 8);   // rows of the common J range: bra | ket<<8
         }
-        __syncthreads();   // S1
-        const uint32_t mask = sh.mask[par];
-        if (tid == 0) sh.mask[par ^ 1] = 0u;
+        __syncthreads();   // B1: histogram, mask, descriptors complete
+        const uint32_t mask = sh.mask;
         const uint4 s0 = *reinterpret_cast<const uint4*>(&sh.sc[0]);
         const uint4 s1 = *reinterpret_cast<const uint4*>(&sh.sc[4]);
         const uint32_t Sb = s0.x, Sk = s0.y;
-        const uint32_t gsize = s1.y & 0xFFFFu;
-        const int nblk = (int)(s1.y >> 16);
-        const int jb1 = s1.x & 255, jc1 = (s1.x >> 8) & 255, je1 = (s1.x >> 16) & 255, jf1 = (s1.x >> 24) & 255;
-        const uint32_t bpr = min((uint32_t)NBIN3, (uint32_t)VW_CAP / gsize);   // bins per round
+        const uint32_t gsize = s1.y, vstride = vw_stride(gsize);
+        const int sumj = s1.x & 255, Jlo = (s1.x >> 8) & 255, nblk = (int)(s1.x >> 16);
+        const uint32_t bpr = min((uint32_t)NBIN3, (uint32_t)VW_CAP / vstride);   // bins per round
         const uint32_t inv = 0xFFFFFFFFu / gsize + 1u;
         const double* __restrict__ slab = T.slab3 + (size_t)s1.z * 2;
-        double res[TR_RPT];
+        if (tid < 32) {   // warp 0: exclusive scan of the iM histogram -> cursors, then clear it for the next item
+            const uint32_t a = sh.hist[2 * lane], b = sh.hist[2 * lane + 1];
+            uint32_t incl = a + b;
 #pragma unroll
-        for (int r = 0; r < TR_RPT; r++) res[r] = 0.0;
+            for (int off = 1; off < 32; off <<= 1) {
+                uint32_t x = __shfl_up_sync(0xFFFFFFFFu, incl, off);
+                if (lane >= off) incl += x;
+            }
+            sh.soff[2 * lane] = incl - a - b;
+            sh.soff[2 * lane + 1] = incl - b;
+            sh.hist[2 * lane] = 0u;
+            sh.hist[2 * lane + 1] = 0u;
+            if (lane == 0) sh.hist[NM_MAX] = 0u;
+        }
         bool first = true;
         for (uint32_t b0 = 0; b0 < (uint32_t)NBIN3; b0 += bpr) {
             if (((mask >> b0) & ((1u << bpr) - 1u)) == 0u) continue;   // block-uniform
             if (!first) __syncthreads();   // the previous round's compute phase is over
-            first = false;
+            // (2) stage the isospin-combined slabs of the bins of this round
             for (uint32_t idx = tid; idx < bpr * gsize; idx += TR_THREADS) {
                 const uint32_t bl = __umulhi(idx, inv), c = idx - bl * gsize, b = b0 + bl;
                 if (b < (uint32_t)NBIN3 && ((mask >> b) & 1u)) {
@@ -596,53 +695,74 @@ __global__ void __launch_bounds__(TR_THREADS, 4) k_transform3(Tables T, const ui
                     v = fma(w[2], __ldg(slab + 2 * gsize + c), v);
                     v = fma(w[3], __ldg(slab + 3 * gsize + c), v);
                     v = fma(w[4], __ldg(slab + 4 * gsize + c), v);
-                    sh.vw[idx] = v;
+                    sh.vw[bl * vstride + c] = v;
                 }
             }
-            __syncthreads();   // S2
-#pragma unroll 1
-            for (int r = 0; r < TR_RPT; r++) {
-                static_assert(TR_RPT == 2, "record selection below assumes two records per thread");
-                const unsigned long long rc = r ? rec[1] : rec[0];   // static indices: the arrays stay in registers
-                const uint32_t bl = (uint32_t)(r ? bin[1] : bin[0]) - b0;
-                if (!(r ? valid[1] : valid[0]) || bl >= bpr) continue;
-                const uint32_t mrec = (uint32_t)rc;
-                const int ima = mrec & 31, imb = (mrec >> 5) & 31, imc = (mrec >> 10) & 31;
-                const int imd = (mrec >> 15) & 31, ime = (mrec >> 20) & 31, imf = (mrec >> 25) & 31;
-                uint32_t pb = s0.z + (uint32_t)((ima * jb1 + imb) * jc1 + imc);
-                uint32_t pk = s0.w + (uint32_t)((imd * je1 + ime) * jf1 + imf);
-                uint32_t vi = bl * gsize;
-                const double* __restrict__ dtab = T.dtab3;
-                double total = 0.0;
-                for (int q = 0; q < nblk; q++) {
-                    const uint32_t d = sh.nbk[q];
-                    const int nb = d & 255, nk = d >> 8;
-                    switch (nk) {
-                        case 1: total += j_block3<1>(dtab, sh.vw, pb, pk, Sb, Sk, nb, vi); break;
-                        case 2: total += j_block3<2>(dtab, sh.vw, pb, pk, Sb, Sk, nb, vi); break;
-                        case 3: total += j_block3<3>(dtab, sh.vw, pb, pk, Sb, Sk, nb, vi); break;
-                        case 4: total += j_block3<4>(dtab, sh.vw, pb, pk, Sb, Sk, nb, vi); break;
-                        case 5: total += j_block3<5>(dtab, sh.vw, pb, pk, Sb, Sk, nb, vi); break;
-                        case 6: total += j_block3<6>(dtab, sh.vw, pb, pk, Sb, Sk, nb, vi); break;
-                        default:
-                            if (nk > 0 && nb > 0) total += j_block3_generic(dtab, sh.vw, pb, pk, Sb, Sk, nb, nk, vi);
-                            pb += (uint32_t)nb * Sb;
-                            pk += (uint32_t)nk * Sk;
-                            if (nk > 0) vi += (uint32_t)(nb * row_pitch3(nk));
-                            break;
-                    }
+            if (first) {
+                __syncthreads();   // B2: cursors ready; every thread has read the mask
+                if (tid == 0) sh.mask = 0u;
+                for (uint32_t idx = tid; idx < cnt; idx += TR_THREADS) {   // M-sorted order of the records
+                    const uint32_t kr = sh.srank[idx];
+                    sh.sidx[sh.soff[kr >> 10] + (kr & 1023u)] = (uint16_t)idx;
                 }
-                const double val = (((rc >> 36) & 1) ? -total : total) + 0.0;   // + 0.0: never store -0
-                if (r) res[1] = val; else res[0] = val;
+                first = false;
+            }
+            __syncthreads();   // B3: Vw and the sorted order are in place
+            // (3) evaluate.  Warp-uniform loop over pairs of 32 sorted slots: lane l takes slots base+l (A) and base+32+l
+            //     (B); lanes past the end of the item redo its last record and skip the store.
+            for (uint32_t base = (uint32_t)(tid & ~31) * 2u; base < cnt; base += 2u * TR_THREADS) {
+                const uint32_t slotA = base + lane, slotB = slotA + 32u;
+                const uint32_t idxA = sh.sidx[min(slotA, cnt - 1u)], idxB = sh.sidx[min(slotB, cnt - 1u)];
+                const unsigned long long rcA = __ldg(irec + idxA), rcB = __ldg(irec + idxB);
+                const uint32_t loA = (uint32_t)rcA, loB = (uint32_t)rcB;
+                const uint32_t blA = ((loA >> 24) & 31u) - b0, blB = ((loB >> 24) & 31u) - b0;
+                const int aMA = abs(2 * ((int)(rcA >> 30) & 63) - sumj), aMB = abs(2 * ((int)(rcB >> 30) & 63) - sumj);
+                const int q0 = max(0, (min(aMA, aMB) - Jlo + 1) >> 1);   // first block with J >= |M| of either record
+                uint32_t pbA = s0.z + (loA & 0xFFFu), pkA = s0.w + ((loA >> 12) & 0xFFFu), viA = min(blA, bpr - 1u) * vstride;
+                uint32_t pbB = s0.z + (loB & 0xFFFu), pkB = s0.w + ((loB >> 12) & 0xFFFu), viB = min(blB, bpr - 1u) * vstride;
+                if (q0 > 0 && q0 < nblk) {
+                    const unsigned long long d = sh.desc[q0];
+                    const uint32_t rb = ((uint32_t)d >> 16) & 255u, rk = (uint32_t)d >> 24, dv = (uint32_t)(d >> 32) & 0xFFFFu;
+                    pbA += rb * Sb; pbB += rb * Sb;
+                    pkA += rk * Sk; pkB += rk * Sk;
+                    viA += dv; viB += dv;
+                }
+                double totA = 0.0, totB = 0.0;
+                for (int q = q0; q < nblk; q++) {
+                    const unsigned long long d = sh.desc[q];
+                    const int nb = (uint32_t)d & 255, nk = ((uint32_t)d >> 8) & 255;
+#define MFDN_BLK(NB, NK) case ((NB) - 1) * 4 + ((NK) - 1): j_block3x2<NB, NK>(dtab, sh.vw, pbA, pkA, pbB, pkB, Sb, Sk, viA, viB, totA, totB); break;
+#define MFDN_ROWS(NK) case 16 + (NK): j_block3x2_rows<NK>(dtab, sh.vw, pbA, pkA, pbB, pkB, Sb, Sk, nb, viA, viB, totA, totB); break;
+                    switch ((uint32_t)(d >> 48)) {
+                        MFDN_BLK(1, 1) MFDN_BLK(1, 2) MFDN_BLK(1, 3) MFDN_BLK(1, 4)
+                        MFDN_BLK(2, 1) MFDN_BLK(2, 2) MFDN_BLK(2, 3) MFDN_BLK(2, 4)
+                        MFDN_BLK(3, 1) MFDN_BLK(3, 2) MFDN_BLK(3, 3) MFDN_BLK(3, 4)
+                        MFDN_BLK(4, 1) MFDN_BLK(4, 2) MFDN_BLK(4, 3) MFDN_BLK(4, 4)
+                        MFDN_ROWS(1) MFDN_ROWS(2) MFDN_ROWS(3) MFDN_ROWS(4) MFDN_ROWS(5) MFDN_ROWS(6) MFDN_ROWS(7) MFDN_ROWS(8)
+                        default: {
+                            if (nk > 0 && nb > 0) {
+                                totA += j_block3_generic(dtab, sh.vw, pbA, pkA, Sb, Sk, nb, nk, viA);
+                                totB += j_block3_generic(dtab, sh.vw, pbB, pkB, Sb, Sk, nb, nk, viB);
+                            }
+                            pbA += (uint32_t)nb * Sb; pbB += (uint32_t)nb * Sb;
+                            pkA += (uint32_t)nk * Sk; pkB += (uint32_t)nk * Sk;
+                            if (nk > 0) { viA += (uint32_t)(nb * row_pitch3(nk)); viB += (uint32_t)(nb * row_pitch3(nk)); }
+                            break;
+                        }
+                    }
+#undef MFDN_BLK
+#undef MFDN_ROWS
+                }
+                if (slotA < cnt && blA < bpr) {   // else: past the end / bin staged in another round
+                    const uint32_t pos = pos0 + idxA;
+                    out[order ? __ldg(order + pos) : pos] = (((loA >> 29) & 1u) ? -totA : totA) + 0.0;   // + 0.0: never store -0
+                }
+                if (slotB < cnt && blB < bpr) {
+                    const uint32_t pos = pos0 + idxB;
+                    out[order ? __ldg(order + pos) : pos] = (((loB >> 29) & 1u) ? -totB : totB) + 0.0;
+                }
             }
         }
-#pragma unroll
-        for (int r = 0; r < TR_RPT; r++)
-            if (valid[r]) {
-                const uint32_t pos = pos0 + (uint32_t)(r * TR_THREADS + tid);
-                out[order ? __ldg(order + pos) : pos] = res[r];
-            }
-        par ^= 1;
     }
 }
 
@@ -780,7 +900,7 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
             k_items3<<<(unsigned)((n_buckets + 255) / 256), 256, 0, st>>>(hist, (uint32_t)n_buckets, sort ? 1 : 0, (uint32_t)n, c->t.sgrp3,
                                                                            invalid_bucket, itm, cnt);
             if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.b, st));
-            const unsigned grid = (unsigned)std::min<long long>(max_items, (long long)c->num_sms * 4);
+            const unsigned grid = (unsigned)std::min<long long>(max_items, (long long)c->num_sms * 6);
             k_transform3<<<grid, TR_THREADS, 0, st>>>(c->t, itm, cnt, trecs, order, d_out);
             c->launches += 2;
         } else {
