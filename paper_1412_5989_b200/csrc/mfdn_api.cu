@@ -578,6 +578,11 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
                 stmask[d.z + i12 * 2 + T12] |= 1ull << ((chan_twoJ[ch] >> 1) * 2 + Ti);
             }
     }
+    // stmask -> suffix OR over J12 (per T12): entry [i12][T12] = channels of all listed states with J12 >= J12min + i12,
+    // so that S7's "some admissible J12 >= |M12|" is ONE 16-byte look-up per side
+    for (int t = 0; t < nt; t++)
+        for (int i = nJ12v[t] - 2; i >= 0; i--)
+            for (int T12 = 0; T12 < 2; T12++) stmask[tdesc[t].z + i * 2 + T12] |= stmask[tdesc[t].z + (i + 1) * 2 + T12];
     auto range = [&](int4 d, int twoJ, int& lo, int& hi) {
         int jc = (d.x >> 16) & 255;
         lo = std::max(d.y & 255, std::abs(twoJ - jc) >> 1);
@@ -657,7 +662,10 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
         }
     // ---- one arena for the resident index tables, one for the upload-only ones
     Arena res, tmp;
-    size_t o_tid = res.add(tuple_id), o_desc = res.add(tdesc), o_sgrp = res.add(sgrp), o_sm = res.add(stmask);
+    std::vector<int4> tdesc_rt = tdesc;   // run-time copy: w = start of the tuple's sigma table (the row-map offset is upload-only)
+    for (int t = 0; t < nt; t++) tdesc_rt[t].w = sigoff[t];
+    size_t o_tid = res.add(tuple_id), o_desc_rt = res.add(tdesc_rt), o_sgrp = res.add(sgrp), o_sm = res.add(stmask);
+    size_t o_desc = tmp.add(tdesc);
     size_t o_tk = res.add(tk), o_jinfo = res.add(jinfo), o_sig = res.add(sig), o_sigoff = res.add(sigoff);
     std::vector<int64_t> coff(chan_off, chan_off + n_chan);
     std::vector<int32_t> cdim(chan_dim, chan_dim + n_chan);
@@ -687,7 +695,7 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     c->owned.push_back(ddtab);
     Retile3 p;
     p.n_tup = nt;
-    p.tdesc = (const int4*)(dres + o_desc);
+    p.tdesc = (const int4*)((char*)dtmp + o_desc);
     p.sgrp = (const uint2*)(dres + o_sgrp);
     p.rowmap = (const int32_t*)((char*)dtmp + o_rm);
     p.chan_of = (const int32_t*)((char*)dtmp + o_cof);
@@ -719,7 +727,7 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     c->t.n_tup3 = nt;
     c->t.e3max = e3max;
     c->t.tuple_id3 = (const int32_t*)(dres + o_tid);
-    c->t.tdesc3 = p.tdesc;
+    c->t.tdesc3 = (const int4*)(dres + o_desc_rt);
     c->t.sgrp3 = p.sgrp;
     c->t.slab3 = (const double*)dslab;
     c->t.stmask3 = (const unsigned long long*)(dres + o_sm);
@@ -727,7 +735,6 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     c->t.jinfo3 = (const int2*)(dres + o_jinfo);
     c->t.dtab3 = (const double*)ddtab;
     c->t.sig3 = q.sig;
-    c->t.sigoff3 = q.sigoff;
     c->slab_bytes3 = (int64_t)(cells * 16);
     c->dtab_bytes3 = (int64_t)(dtab_len * sizeof(double));
     c->has3 = true;

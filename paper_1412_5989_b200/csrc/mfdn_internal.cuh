@@ -55,8 +55,8 @@ constexpr int MAX_STATES3 = 4096;   // (ja+1)(jb+1)(jc+1) of a tuple must fit th
 // ---- per-tuple descriptor (A2), 16 bytes ---------------------------------------------------------
 // 3-body: x = ja | jb<<8 | jc<<16 | (a==b)<<24 | par<<25      (ja.. are 2j)
 //         y = J12min | J12max<<8 | twoJmin<<16 | twoJmax<<24
-//         z = offset of the tuple's state masks in stmask3 (entries: [J12-J12min][T12])
-//         w = offset of the tuple's row map (upload only)
+//         z = offset of the tuple's state masks in stmask3 (entries: [J12-J12min][T12], suffix-ORed over J12)
+//         w = start of the tuple's sigma table in sig3 (during the upload: offset of the tuple's row map)
 // tk3 (what the transform kernel needs of a tuple): x = offset of the tuple's coefficient table in dtab3 (doubles),
 //         y = its row pitch S = (ja+1)(jb+1)(jc+1), z = first entry of the tuple in jinfo3,
 //         w = (ja+jb+jc) | twoJmin<<16 | twoJmax<<24
@@ -91,7 +91,6 @@ struct Tables {
     const double* dtab3;           // per tuple [row][sigma] = <ja ma jb mb|J12 M12> <J12 M12 jc mc|J M>
     const uint16_t* sig3;          // per tuple [(ima*(jb+1)+imb)*(jc+1)+imc] -> sigma: m-states ordered by (M, ima, imb), so that
                                    // requests with equal M (bra and ket always have equal M) read neighbouring entries
-    const int32_t* sigoff3;        // [n_tup3] start of the tuple's sigma table in sig3
     // A2, 2-body
     int n_tup2;
     const int32_t* tuple_id2;      // [n_orb^2]

@@ -44,10 +44,11 @@ __device__ __forceinline__ void cswap(uint32_t& ka, uint32_t& kb, uint32_t& ra, 
 }
 
 // canonicalise three particles: stable sort by (orbital, SPS) ascending, sign of the permutation
-__device__ __forceinline__ Side3 decode3(const Tables& T, int s0, int s1, int s2)
+template <bool SMEM>
+__device__ __forceinline__ Side3 decode3(const Tables& T, const uint32_t* sps, int s0, int s1, int s2)
 {
     Side3 S;
-    uint32_t r0 = __ldg(T.sps_rec + s0), r1 = __ldg(T.sps_rec + s1), r2 = __ldg(T.sps_rec + s2);
+    uint32_t r0 = SMEM ? sps[s0] : __ldg(sps + s0), r1 = SMEM ? sps[s1] : __ldg(sps + s1), r2 = SMEM ? sps[s2] : __ldg(sps + s2);
     uint32_t k0 = (rec_orb(r0) << 16) | s0, k1 = (rec_orb(r1) << 16) | s1, k2 = (rec_orb(r2) << 16) | s2;
     S.distinct = (s0 != s1) && (s0 != s2) && (s1 != s2);
     S.sign = 1;
@@ -70,10 +71,11 @@ struct Side2 {
     bool distinct;
 };
 
-__device__ __forceinline__ Side2 decode2(const Tables& T, int s0, int s1)
+template <bool SMEM>
+__device__ __forceinline__ Side2 decode2(const Tables& T, const uint32_t* sps, int s0, int s1)
 {
     Side2 S;
-    uint32_t r0 = __ldg(T.sps_rec + s0), r1 = __ldg(T.sps_rec + s1);
+    uint32_t r0 = SMEM ? sps[s0] : __ldg(sps + s0), r1 = SMEM ? sps[s1] : __ldg(sps + s1);
     uint32_t k0 = (rec_orb(r0) << 16) | s0, k1 = (rec_orb(r1) << 16) | s1;
     S.distinct = s0 != s1;
     S.sign = 1;
@@ -111,15 +113,12 @@ __device__ __forceinline__ bool select2(const Side2& B, const Side2& K)
 // S7 helper: set of (J,T) channels in which this side has an admissible listed state
 __device__ __forceinline__ unsigned long long chanmask3(const Tables& T, int4 d, int twoM12, int twoMT12)
 {
-    int J12min = d.y & 255, J12max = (d.y >> 8) & 255;
-    unsigned long long m = 0;
-    int lo = max(J12min, (abs(twoM12) + 1) >> 1);   // 2*J12 >= |2*M12|
-    for (int J12 = lo; J12 <= J12max; J12++) {
-        const unsigned long long* p = T.stmask3 + d.z + (J12 - J12min) * 2;
-        if (twoMT12 == 0) m |= __ldg(p);
-        m |= __ldg(p + 1);
-    }
-    return m;
+    const int J12min = d.y & 255, J12max = (d.y >> 8) & 255;
+    const int lo = max(J12min, (abs(twoM12) + 1) >> 1);   // 2*J12 >= |2*M12|
+    if (lo > J12max) return 0ull;
+    // stmask3 holds suffix ORs over J12: one 16-byte entry {T12 = 0, T12 = 1} covers all J12 >= lo
+    const ulonglong2 m = __ldg(reinterpret_cast<const ulonglong2*>(T.stmask3 + d.z + (lo - J12min) * 2));
+    return (twoMT12 == 0 ? m.x : 0ull) | m.y;
 }
 
 // S7 for a decoded 3-body request that passed S1-S6: at least one admissible channel term
@@ -267,10 +266,10 @@ __global__ void __launch_bounds__(128) k_mscheme_naive(Tables T, long long n, co
     if (!in_range(T, s, 2 * BODY)) {
         atomicAdd(T.bad_count, 1ull);
     } else if (BODY == 3) {
-        Side3 B = decode3(T, s[0], s[1], s[2]), K = decode3(T, s[3], s[4], s[5]);
+        Side3 B = decode3<false>(T, T.sps_rec, s[0], s[1], s[2]), K = decode3<false>(T, T.sps_rec, s[3], s[4], s[5]);
         v = eval3_naive(T, B, K, mask);
     } else {
-        Side2 B = decode2(T, s[0], s[1]), K = decode2(T, s[2], s[3]);
+        Side2 B = decode2<false>(T, T.sps_rec, s[0], s[1]), K = decode2<false>(T, T.sps_rec, s[2], s[3]);
         v = eval2_naive(T, B, K, mask);
     }
     out[i] = mask ? v : 0.0;
@@ -279,14 +278,22 @@ __global__ void __launch_bounds__(128) k_mscheme_naive(Tables T, long long n, co
 
 // =============================================================================== H1: records
 // One thread per request: decode, S1-S7 -> mask (request order, coalesced), canonical packed record.
-template <int BODY, bool AGG>
+constexpr int KEYS_SPS_SMEM = 2048;   // SPS records held in shared memory by k_keys when the basis is this small
+
+template <int BODY, bool AGG, bool SMEM>
 __global__ void __launch_bounds__(256) k_keys(Tables T, long long n, const int32_t* __restrict__ req,
                                               unsigned long long* __restrict__ recs, uint8_t* __restrict__ maskout,
                                               uint32_t* __restrict__ hist, uint32_t invalid_bucket,
                                               uint32_t* __restrict__ keys32)
 {
+    __shared__ uint32_t s_sps[SMEM ? KEYS_SPS_SMEM : 1];
+    if (SMEM) {
+        for (int k = threadIdx.x; k < T.n_sps; k += blockDim.x) s_sps[k] = __ldg(T.sps_rec + k);
+        __syncthreads();
+    }
+    const uint32_t* sps = SMEM ? s_sps : T.sps_rec;
     long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;   // n is a multiple of 32 or the tail warp is partial: __activemask below
+    if (i >= n) return;   // partial tail warp: __activemask below
     int s[6];
     if (BODY == 3) load_req3(req, i, s); else load_req2(req, i, s);
     uint32_t key = REC_INVALID;
@@ -295,21 +302,21 @@ __global__ void __launch_bounds__(256) k_keys(Tables T, long long n, const int32
     if (!in_range(T, s, 2 * BODY)) {
         if (recs) atomicAdd(T.bad_count, 1ull);
     } else if (BODY == 3) {
-        Side3 B = decode3(T, s[0], s[1], s[2]), K = decode3(T, s[3], s[4], s[5]);
+        Side3 B = decode3<SMEM>(T, sps, s[0], s[1], s[2]), K = decode3<SMEM>(T, sps, s[3], s[4], s[5]);
         if (select3(T, B, K)) {
             key = (uint32_t)B.tup * T.n_tup3 + K.tup;
             const int4 db = __ldg(T.tdesc3 + B.tup), dk = __ldg(T.tdesc3 + K.tup);
             if (__ldg(T.sgrp3 + key).x != NO_SLAB) mask = mask3(T, B, K, db, dk);
             const int jb1 = ((db.x >> 8) & 255) + 1, jc1 = ((db.x >> 16) & 255) + 1;
             const int je1 = ((dk.x >> 8) & 255) + 1, jf1 = ((dk.x >> 16) & 255) + 1;
-            const uint32_t sb = __ldg(T.sig3 + __ldg(T.sigoff3 + B.tup) + (B.ima * jb1 + B.imb) * jc1 + B.imc);
-            const uint32_t sk = __ldg(T.sig3 + __ldg(T.sigoff3 + K.tup) + (K.ima * je1 + K.imb) * jf1 + K.imc);
+            const uint32_t sb = __ldg(T.sig3 + db.w + (B.ima * jb1 + B.imb) * jc1 + B.imc);
+            const uint32_t sk = __ldg(T.sig3 + dk.w + (K.ima * je1 + K.imb) * jf1 + K.imc);
             const uint32_t bin = __ldg(T.tz2bin3 + ((B.tz << 3) | K.tz));
             low = (unsigned long long)(sb | (sk << 12) | (bin << 24) | ((uint32_t)(B.sign * K.sign < 0) << 29)) |
                   ((unsigned long long)(B.ima + B.imb + B.imc) << 30);
         }
     } else {
-        Side2 B = decode2(T, s[0], s[1]), K = decode2(T, s[2], s[3]);
+        Side2 B = decode2<SMEM>(T, sps, s[0], s[1]), K = decode2<SMEM>(T, sps, s[2], s[3]);
         if (select2(B, K)) {
             key = (uint32_t)B.tup * T.n_tup2 + K.tup;
             if (__ldg(T.slab_off2 + key) != NO_SLAB) mask = mask2(B, __ldg(T.tdesc2 + B.tup), __ldg(T.tdesc2 + K.tup));
@@ -392,20 +399,56 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_add(uint32_t* __restrict__ data
         if (base + k < m) data[base + k] += add;
 }
 
+// H2 scatter: records -> group order.  posof[i] = position of request i in the group-ordered stream (coalesced write);
+// the results are computed in group order and gathered back by k_unpermute (random 8-byte READS are far cheaper
+// than the random 8-byte WRITES of a direct out[original index] store: no read-modify-write of DRAM sectors).
+constexpr int SC_PER_THREAD = 4;
 __global__ void __launch_bounds__(256) k_scatter(long long n, const unsigned long long* __restrict__ recs,
                                                  uint32_t* __restrict__ cursor, unsigned long long* __restrict__ sorted,
-                                                 uint32_t* __restrict__ order, uint32_t invalid_bucket)
+                                                 uint32_t* __restrict__ posof, uint32_t invalid_bucket)
 {
-    long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    unsigned long long r = recs[i];
-    uint32_t key = (uint32_t)(r >> REC_KEY_SHIFT);
-    uint32_t pos = atomicAdd(cursor + (key == REC_INVALID ? invalid_bucket : key), 1u);
-    sorted[pos] = r;
-    order[pos] = (uint32_t)i;
+    const long long base = (long long)blockIdx.x * (256 * SC_PER_THREAD) + threadIdx.x;
+    unsigned long long r[SC_PER_THREAD];
+    uint32_t pos[SC_PER_THREAD];
+#pragma unroll
+    for (int u = 0; u < SC_PER_THREAD; u++) {
+        const long long i = base + u * 256;
+        r[u] = i < n ? __ldg(recs + i) : 0ull;
+    }
+#pragma unroll
+    for (int u = 0; u < SC_PER_THREAD; u++) {   // SC_PER_THREAD independent atomics in flight per thread
+        const long long i = base + u * 256;
+        const uint32_t key = (uint32_t)(r[u] >> REC_KEY_SHIFT);
+        pos[u] = i < n ? atomicAdd(cursor + (key == REC_INVALID ? invalid_bucket : key), 1u) : 0u;
+    }
+#pragma unroll
+    for (int u = 0; u < SC_PER_THREAD; u++) {
+        const long long i = base + u * 256;
+        if (i < n) {
+            sorted[pos[u]] = r[u];
+            posof[i] = pos[u];
+        }
+    }
 }
 
-// =============================================================================== H3-H6: transform
+// H6 (sort path): results from group order back to request order
+__global__ void __launch_bounds__(256) k_unpermute(long long n, const double* __restrict__ vals, const uint32_t* __restrict__ posof,
+                                                   double* __restrict__ out)
+{
+    const long long base = (long long)blockIdx.x * (256 * SC_PER_THREAD) + threadIdx.x;
+    uint32_t p[SC_PER_THREAD];
+#pragma unroll
+    for (int u = 0; u < SC_PER_THREAD; u++) {
+        const long long i = base + u * 256;
+        p[u] = i < n ? __ldg(posof + i) : 0u;
+    }
+#pragma unroll
+    for (int u = 0; u < SC_PER_THREAD; u++) {
+        const long long i = base + u * 256;
+        if (i < n) out[i] = __ldg(vals + p[u]);
+    }
+}
+
 // Work items (H3): one item = up to ITEM3 consecutive records of ONE group in the group-ordered stream, so that a
 // thread block shares every loop bound, table row and the group's slab.  `bounds[b]` is the END of bucket b after the
 // scatter (ends = 1: the cursor array) or its START for pre-sorted input (ends = 0: the scanned histogram).
@@ -579,7 +622,7 @@ __global__ void __launch_bounds__(TR_THREADS, 6) k_transform3(Tables T, const ui
     __shared__ __align__(16) ItemShared sh;
     const int tid = threadIdx.x, lane = tid & 31;
     for (int i = tid; i < NBIN3 * NISO3; i += TR_THREADS) sh.w[i] = __ldg(T.wbin3 + i);
-    if (tid <= NM_MAX) sh.hist[tid] = 0u;
+    for (int i = tid; i <= NM_MAX; i += TR_THREADS) sh.hist[i] = 0u;
     if (tid == 0) sh.mask = 0u;
     __syncthreads();
     const uint32_t n_items = __ldg(n_items_p);
@@ -592,6 +635,20 @@ __global__ void __launch_bounds__(TR_THREADS, 6) k_transform3(Tables T, const ui
         if (g == ZERO_ITEM) {   // block-uniform
             for (uint32_t idx = tid; idx < cnt; idx += TR_THREADS) out[order ? __ldg(order + pos0 + idx) : pos0 + idx] = 0.0;
             continue;
+        }
+        {   // prefetch what the NEXT item of this block will read first: its records (and their output order) into L2,
+            // the two tuple descriptors and the group descriptor into L1
+            const uint32_t nit = it + gridDim.x;
+            if (nit < n_items) {
+                const uint4 nx = __ldg(items + nit);
+                if ((uint32_t)tid * 16u < nx.y) asm volatile("prefetch.global.L2 [%0];" ::"l"(recs + nx.x + tid * 16));
+                if (order && (uint32_t)tid * 32u < nx.y) asm volatile("prefetch.global.L2 [%0];" ::"l"(order + nx.x + tid * 32));
+                if (nx.z != ZERO_ITEM && tid >= 32 && tid < 35) {
+                    const uint32_t tb = nx.z / nt, tk = nx.z - tb * nt;
+                    const void* a = tid == 32 ? (const void*)(T.tk3 + tb) : tid == 33 ? (const void*)(T.tk3 + tk) : (const void*)(T.sgrp3 + nx.z);
+                    asm volatile("prefetch.global.L1 [%0];" ::"l"(a));
+                }
+            }
         }
         __syncthreads();   // B0: the previous item is finished, shared state may be overwritten
         {   // (1) histogram over iM (each record keeps its rank inside its iM bucket), mask of the isospin bins present
@@ -870,14 +927,19 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
         char* w = (char*)d_work;
         unsigned long long* recs = (unsigned long long*)(w + o_recs);
         const unsigned long long* trecs = recs;
-        const uint32_t* order = nullptr;
         uint32_t* hist = hist_needed ? (uint32_t*)(w + o_hist) : nullptr;
         uint32_t* sums = hist_needed ? (uint32_t*)(w + o_sums) : nullptr;
         const unsigned gk = (unsigned)((n + 255) / 256);
         const uint32_t invalid_bucket = (uint32_t)(nt * nt);
         if (hist_needed) MFDN_CUDA(c, cudaMemsetAsync(hist, 0, (size_t)n_buckets * 4, st));
-        if (sort) k_keys<BODY, false><<<gk, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr);
-        else k_keys<BODY, true><<<gk, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr);
+        const bool sm = c->t.n_sps <= KEYS_SPS_SMEM;
+        if (sort) {
+            if (sm) k_keys<BODY, false, true><<<gk, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr);
+            else k_keys<BODY, false, false><<<gk, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr);
+        } else {
+            if (sm) k_keys<BODY, true, true><<<gk, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr);
+            else k_keys<BODY, true, false><<<gk, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr);
+        }
         c->launches += 1;
         if (hist_needed) {
             k_scan_tiles<<<(unsigned)n_tiles, SCAN_T, 0, st>>>(hist, n_buckets, sums);
@@ -885,13 +947,16 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
             k_scan_add<<<(unsigned)n_tiles, SCAN_T, 0, st>>>(hist, n_buckets, sums);
             c->launches += 3;
         }
+        double* tout = d_out;   // where the transform writes: request order if pre-sorted, else group order (scratch)
+        const uint32_t* posof = nullptr;
         if (sort) {
             unsigned long long* sorted = (unsigned long long*)(w + o_sorted);
-            uint32_t* ord = (uint32_t*)(w + o_order);
-            k_scatter<<<gk, 256, 0, st>>>(n, recs, hist, sorted, ord, invalid_bucket);
+            uint32_t* po = (uint32_t*)(w + o_order);
+            k_scatter<<<(unsigned)((n + 256 * SC_PER_THREAD - 1) / (256 * SC_PER_THREAD)), 256, 0, st>>>(n, recs, hist, sorted, po, invalid_bucket);
             c->launches += 1;
             trecs = sorted;
-            order = ord;
+            posof = po;
+            tout = (double*)recs;   // the request-order records are dead after the scatter: reuse them for the values
         }
         if (items) {
             uint4* itm = (uint4*)(w + o_items);
@@ -901,11 +966,15 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
                                                                            invalid_bucket, itm, cnt);
             if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.b, st));
             const unsigned grid = (unsigned)std::min<long long>(max_items, (long long)c->num_sms * 6);
-            k_transform3<<<grid, TR_THREADS, 0, st>>>(c->t, itm, cnt, trecs, order, d_out);
+            k_transform3<<<grid, TR_THREADS, 0, st>>>(c->t, itm, cnt, trecs, nullptr, tout);
             c->launches += 2;
         } else {
             if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.b, st));
-            k_transform2<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(c->t, n, trecs, order, d_out);
+            k_transform2<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(c->t, n, trecs, nullptr, tout);
+            c->launches += 1;
+        }
+        if (sort) {
+            k_unpermute<<<(unsigned)((n + 256 * SC_PER_THREAD - 1) / (256 * SC_PER_THREAD)), 256, 0, st>>>(n, tout, posof, d_out);
             c->launches += 1;
         }
     }
@@ -949,8 +1018,8 @@ extern "C" int mfdn_group_keys(mfdn_ctx* c, int body, int64_t n, const int32_t* 
     if (body == 3 ? !c->has3 : !c->has2) return fail(c, MFDN_ERR_STATE, "group_keys before coupled upload");
     if (n == 0) return MFDN_OK;
     cudaStream_t st = (cudaStream_t)stream;
-    if (body == 3) k_keys<3, false><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(c->t, n, d_req, nullptr, nullptr, nullptr, 0u, d_key);
-    else k_keys<2, false><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(c->t, n, d_req, nullptr, nullptr, nullptr, 0u, d_key);
+    if (body == 3) k_keys<3, false, false><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(c->t, n, d_req, nullptr, nullptr, nullptr, 0u, d_key);
+    else k_keys<2, false, false><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(c->t, n, d_req, nullptr, nullptr, nullptr, 0u, d_key);
     MFDN_CUDA(c, cudaGetLastError());
     return MFDN_OK;
 }
