@@ -2,7 +2,7 @@
 """bench.py -- coupled-JT -> M-scheme transformation throughput on B200 (BASELINE.json metric).
 
 One "step" = one pass of the whole hot path (H1 decode/selection/canonicalise/key, H2 group sort,
-H3-H6 locate/stage/channel-sum/store) over one batch of synthetic requests:
+H3-H6 locate/stage/channel-sum/store incl. the gather back to request order) over one batch of synthetic requests:
 config 3 = 3-body, E3max = 8, 2^26 requests sampled uniformly from the conserving pairs, arriving
 UNSORTED and device-resident.  Prints ONE JSON line (see README/DESIGN.md "Measurement").
 
@@ -61,7 +61,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.gpu}", f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
         except Exception:
             self.proc = None
@@ -120,6 +120,7 @@ def run_reference(args):
         return
     from paper_1412_5989_b200 import workloads as W
     cfg = W.make_config(args.config)
+    args.ref_log2n = 21 if args.ref_log2n is None else args.ref_log2n
     n_sample = 1 << args.ref_log2n
     from oracle import mscheme_c
     req = host_requests(cfg, n_sample, 0)
@@ -146,12 +147,13 @@ def run_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--log2n", type=int, default=26)
-    ap.add_argument("--ref-log2n", type=int, default=21)
+    ap.add_argument("--ref-log2n", type=int, default=None,
+                    help="log2 of the CPU-oracle sample (default: 25 for the cpu_baseline leg, 21 per step of --impl reference)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -160,7 +162,7 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_1412_5989_b200 import binding as B, build, workloads as W
+    from paper_1412_5989_b200 import binding as B, build, shard, workloads as W
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -177,7 +179,7 @@ def main():
     body = cfg.body
     n = 1 << args.log2n
     ctx = B.Context(cfg.basis, local).upload(cfg.table)
-    h_req = torch.from_numpy(host_requests(cfg, n, rank * n)).pin_memory()
+    h_req = torch.from_numpy(host_requests(cfg, n, shard.rank_window(rank, world, n)[0])).pin_memory()
     d_req = h_req.cuda(non_blocking=True)
     d_out = torch.empty(n, dtype=torch.float64, device="cuda")
     d_mask = torch.empty(n, dtype=torch.uint8, device="cuda")
@@ -193,11 +195,11 @@ def main():
             torch.cuda.synchronize()
 
     def timed(flags, req, steps, warmup, sampler=None):
+        if sampler:
+            sampler.start()          # nvidia-smi needs a few 100 ms to come up: start before the warm-up steps
         for _ in range(warmup):
             ctx.mscheme(req, d_out, d_mask, flags, work)
         sync_all()
-        if sampler:
-            sampler.start()
         l0 = B.mfdn_info(ctx.ctx, 6)
         B.mfdn_profile(ctx.ctx, 1)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -208,17 +210,14 @@ def main():
         sync_all()
         clocks = sampler.stop() if sampler else None
         B.mfdn_profile(ctx.ctx, 0)
-        ms_sort, ms_tr, calls = B.mfdn_profile_read(ctx.ctx)
-        ms = e0.elapsed_time(e1) / steps
-        if world > 1:
-            t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
-        return ms, ms_sort / max(calls, 1), ms_tr / max(calls, 1), B.mfdn_info(ctx.ctx, 6) - l0, clocks
+        ms_sort, ms_tr, ms_un, calls = B.mfdn_profile_read(ctx.ctx)
+        ms = shard.max_over_ranks(e0.elapsed_time(e1) / steps, "cuda")
+        k = max(calls, 1)
+        return ms, ms_sort / k, ms_tr / k, ms_un / k, B.mfdn_info(ctx.ctx, 6) - l0, clocks
 
     # ---- headline: whole path on unsorted device-resident input
     sampler = ClockSampler(local)
-    ms, ms_sort, ms_tr, launches, clocks = timed(0, d_req, args.steps, args.warmup, sampler)
+    ms, ms_sort, ms_tr, ms_un, launches, clocks = timed(0, d_req, args.steps, args.warmup, sampler)
     n_mask = int(d_mask.sum(dtype=torch.int64).item())
     frac_mask = n_mask / n
     # ---- the same multiset pre-ordered by the library's group key (MFDN_PRESORTED): transform proper
@@ -226,7 +225,7 @@ def main():
     order = torch.argsort(keys.to(torch.int64) & 0xFFFFFFFF)
     d_sorted = d_req[order].contiguous()
     del keys, order
-    ms_p, _, ms_tr_p, _, _ = timed(B.MFDN_PRESORTED, d_sorted, args.steps, args.warmup)
+    ms_p, ms_sort_p, ms_tr_p, _, _, _ = timed(B.MFDN_PRESORTED, d_sorted, args.steps, args.warmup)
     del d_sorted
     # ---- end to end through the C ABI with HOST buffers (H2D + D2H inside the timed region)
     h_out = torch.empty(n, dtype=torch.float64).pin_memory()
@@ -237,10 +236,7 @@ def main():
     for _ in range(args.e2e_steps):
         ctx.mscheme_host(h_req, h_out, h_mask)
     e2e_s = (time.perf_counter() - t0) / args.e2e_steps
-    if world > 1:
-        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = shard.max_over_ranks(e2e_s, "cuda")
     assert int(h_mask.sum(dtype=torch.int64).item()) == n_mask, "host-buffer path disagrees with device path"
     fp64_peak = B.mfdn_fp64_peak(ctx.ctx)
 
@@ -274,10 +270,11 @@ def main():
         "e2e": {"value": world * n / e2e_s, "unit": UNIT, "h2d_bytes_per_step": n * 8 * body,
                 "d2h_bytes_per_step": n * 9, "ms_per_step": e2e_s * 1e3, "steps": args.e2e_steps,
                 "api": "mfdn_mscheme_host (pinned host buffers, 2 streams, 2^22-request chunks)"},
-        "breakdown_ms": {"group_sort_H1_H2": ms_sort, "transform_H3_H6": ms_tr},
+        "breakdown_ms": {"group_sort_H1_H2": ms_sort, "transform_H3_H5": ms_tr, "gather_to_request_order_H6": ms_un,
+                         "presorted": {"keys_items_H1_H3": ms_sort_p, "transform_H3_H6": ms_tr_p}},
         "presorted": {"value": world * n / (ms_p * 1e-3), "unit": UNIT, "ms_per_step": ms_p,
                       "note": "same multiset pre-ordered by mfdn_group_keys, flag MFDN_PRESORTED"},
-        "roofline": {"kernel": f"k_mscheme<{body}> (transform, inside the unsorted step)", "bound": "alu",
+        "roofline": {"kernel": f"k_transform{body} (dominant kernel of the unsorted step; CUDA events on the launch stream)", "bound": "alu",
                      "achieved": flops_rate, "peak": fp64_peak, "unit": "TFLOP/s", "frac": flops_rate / fp64_peak,
                      "traffic": traffic, "flops_per_request": alg["flops"],
                      "peak_source": "measured DFMA micro-benchmark (mfdn_fp64_peak); nominal %.1f" % FP64_NOMINAL_TFLOPS,
@@ -288,6 +285,7 @@ def main():
                      "presorted_frac_alu": alg["flops"] * n / (ms_tr_p * 1e-3) / 1e12 / fp64_peak},
     }
     if not args.no_cpu_baseline:
+        args.ref_log2n = 25 if args.ref_log2n is None else args.ref_log2n
         n_s = 1 << args.ref_log2n
         v, cores, dt = cpu_baseline(cfg, n_s)
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",

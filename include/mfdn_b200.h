@@ -112,20 +112,22 @@ int mfdn_mscheme_3b(mfdn_ctx*, int64_t n, const int32_t* d_req, double* d_out, u
 int mfdn_mscheme_host(mfdn_ctx*, int body, int64_t n, const int32_t* h_req, double* h_out, uint8_t* h_mask,
                       void* d_work, size_t* work_bytes, uint32_t flags, int64_t chunk);
 
-/* Measurement hooks.  mfdn_profile(ctx, 1) makes every later mfdn_mscheme_2b/3b call bracket its group-sort
- * kernels (H1-H2) and its transform kernel (H3-H6) with CUDA events on the call's stream; mfdn_profile_read
- * synchronises those events, returns the accumulated milliseconds and call count since the last read and resets
- * them.  mfdn_fp64_peak runs a register-resident DFMA micro-benchmark on all SMs (the fp64 roofline
- * denominator; MEASURED_PEAKS.json has no fp64 entry) and returns TFLOP/s (2 flops per FMA); synchronises. */
+/* Measurement hooks.  mfdn_profile(ctx, 1) makes every later mfdn_mscheme_2b/3b call record CUDA events on the
+ * call's stream around (1) its group-sort kernels (H1-H2: keys, scans, scatter, work-item list), (2) its transform
+ * kernel (H3-H6) and (3) the gather of the results back into request order (sort path only; 0 for MFDN_PRESORTED
+ * and MFDN_FORCE_NAIVE).  mfdn_profile_read synchronises those events, returns the accumulated milliseconds of the
+ * three parts and the call count since the last read, and resets them.  mfdn_fp64_peak runs a register-resident
+ * DFMA micro-benchmark on all SMs (the fp64 roofline denominator; MEASURED_PEAKS.json has no fp64 entry) and
+ * returns TFLOP/s (2 flops per FMA); synchronises. */
 int mfdn_profile(mfdn_ctx*, int enable);
-int mfdn_profile_read(mfdn_ctx*, double* ms_sort, double* ms_transform, int64_t* calls);
+int mfdn_profile_read(mfdn_ctx*, double* ms_sort, double* ms_transform, double* ms_unpermute, int64_t* calls);
 int mfdn_fp64_peak(mfdn_ctx*, double* tflops);
 
 /* Number of requests with an out-of-range SPS index seen so far (synchronises `stream`). */
 int64_t mfdn_bad_request_count(mfdn_ctx*, void* stream);
 
 /* Sizes of what was uploaded, for reports: which = 0 tuples (2b), 1 tuples (3b), 2 slab bytes (2b),
- * 3 slab bytes (3b), 4 CG entries stage 1, 5 CG entries stage 2, 6 kernels launched so far by mscheme_*. */
+ * 3 slab bytes (3b), 4 CG entries stage 1, 5 CG entries stage 2, 6 kernels launched so far by mscheme_*, 7 bytes of the 3-body coefficient tables. */
 int64_t mfdn_info(mfdn_ctx*, int which);
 
 /* Group key of every request, for producing MFDN_PRESORTED input: d_key[i] = bra_tuple * n_tuples +

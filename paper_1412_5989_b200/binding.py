@@ -51,7 +51,7 @@ def lib():
             f.argtypes = [vp, i64, vp, vp, vp, vp, C.POINTER(C.c_size_t), u32, vp]
         L.mfdn_mscheme_host.argtypes = [vp, C.c_int, i64, vp, vp, vp, vp, C.POINTER(C.c_size_t), u32, i64]
         L.mfdn_profile.argtypes = [vp, C.c_int]
-        L.mfdn_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(i64)]
+        L.mfdn_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(i64)]
         L.mfdn_fp64_peak.argtypes = [vp, C.POINTER(C.c_double)]
         L.mfdn_bad_request_count.argtypes = [vp, vp]
         L.mfdn_bad_request_count.restype = i64
@@ -167,9 +167,9 @@ def mfdn_profile(ctx, enable):
 
 
 def mfdn_profile_read(ctx):
-    a, b, n = C.c_double(0), C.c_double(0), C.c_int64(0)
-    _check(ctx, lib().mfdn_profile_read(ctx, C.byref(a), C.byref(b), C.byref(n)))
-    return a.value, b.value, n.value
+    a, b, u, n = C.c_double(0), C.c_double(0), C.c_double(0), C.c_int64(0)
+    _check(ctx, lib().mfdn_profile_read(ctx, C.byref(a), C.byref(b), C.byref(u), C.byref(n)))
+    return a.value, b.value, u.value, n.value
 
 
 def mfdn_fp64_peak(ctx):

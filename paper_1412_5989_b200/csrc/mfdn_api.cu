@@ -908,7 +908,7 @@ extern "C" void mfdn_destroy(mfdn_ctx* c)
     if (!c) return;
     cudaSetDevice(c->device);
     for (void* p : c->owned) cudaFree(p);
-    for (auto& ev : c->ev_pending) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); cudaEventDestroy(ev.c); }
+    for (auto& ev : c->ev_pending) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); cudaEventDestroy(ev.d); cudaEventDestroy(ev.c); }
     for (auto e : c->ev_pool) cudaEventDestroy(e);
     for (auto s : c->hs) if (s) cudaStreamDestroy(s);
     delete c;

@@ -119,7 +119,7 @@ struct mfdn_ctx {
     int num_sms = 148;
     // measurement hooks
     bool profile = false;
-    struct EvTriple { cudaEvent_t a, b, c; bool has_sort; };
+    struct EvTriple { cudaEvent_t a, b, d, c; bool has_sort; };   // start | transform kernel start | its end | end of call
     std::vector<EvTriple> ev_pending;
     std::vector<cudaEvent_t> ev_pool;
     // host-buffer wrapper

@@ -910,9 +910,9 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
     if (n == 0) return MFDN_OK;
     if (!d_req || !d_out) return fail(c, MFDN_ERR_ARG, "null request/output pointer");
     cudaStream_t st = (cudaStream_t)stream;
-    mfdn_ctx::EvTriple ev{nullptr, nullptr, nullptr, sort};
+    mfdn_ctx::EvTriple ev{nullptr, nullptr, nullptr, nullptr, sort};
     if (c->profile) {
-        cudaEvent_t* e3[3] = {&ev.a, &ev.b, &ev.c};
+        cudaEvent_t* e3[4] = {&ev.a, &ev.b, &ev.d, &ev.c};
         for (auto pe : e3) {
             if (!c->ev_pool.empty()) { *pe = c->ev_pool.back(); c->ev_pool.pop_back(); }
             else MFDN_CUDA(c, cudaEventCreate(pe));
@@ -923,6 +923,7 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
         if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.b, st));
         k_mscheme_naive<BODY><<<(unsigned)((n + 127) / 128), 128, 0, st>>>(c->t, n, d_req, d_out, d_mask);
         c->launches += 1;
+        if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.d, st));
     } else {
         char* w = (char*)d_work;
         unsigned long long* recs = (unsigned long long*)(w + o_recs);
@@ -973,6 +974,7 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
             k_transform2<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(c->t, n, trecs, nullptr, tout);
             c->launches += 1;
         }
+        if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.d, st));
         if (sort) {
             k_unpermute<<<(unsigned)((n + 256 * SC_PER_THREAD - 1) / (256 * SC_PER_THREAD)), 256, 0, st>>>(n, tout, posof, d_out);
             c->launches += 1;
@@ -1031,20 +1033,22 @@ extern "C" int mfdn_profile(mfdn_ctx* c, int enable)
     return MFDN_OK;
 }
 
-extern "C" int mfdn_profile_read(mfdn_ctx* c, double* ms_sort, double* ms_transform, int64_t* calls)
+extern "C" int mfdn_profile_read(mfdn_ctx* c, double* ms_sort, double* ms_transform, double* ms_unpermute, int64_t* calls)
 {
-    if (!c || !ms_sort || !ms_transform || !calls) return MFDN_ERR_ARG;
-    *ms_sort = *ms_transform = 0.0;
+    if (!c || !ms_sort || !ms_transform || !ms_unpermute || !calls) return MFDN_ERR_ARG;
+    *ms_sort = *ms_transform = *ms_unpermute = 0.0;
     *calls = 0;
     for (auto& ev : c->ev_pending) {
         MFDN_CUDA(c, cudaEventSynchronize(ev.c));
-        float t1 = 0.f, t2 = 0.f;
+        float t1 = 0.f, t2 = 0.f, t3 = 0.f;
         MFDN_CUDA(c, cudaEventElapsedTime(&t1, ev.a, ev.b));
-        MFDN_CUDA(c, cudaEventElapsedTime(&t2, ev.b, ev.c));
+        MFDN_CUDA(c, cudaEventElapsedTime(&t2, ev.b, ev.d));
+        MFDN_CUDA(c, cudaEventElapsedTime(&t3, ev.d, ev.c));
         *ms_sort += t1;
         *ms_transform += t2;
+        *ms_unpermute += t3;
         *calls += 1;
-        c->ev_pool.push_back(ev.a); c->ev_pool.push_back(ev.b); c->ev_pool.push_back(ev.c);
+        c->ev_pool.push_back(ev.a); c->ev_pool.push_back(ev.b); c->ev_pool.push_back(ev.d); c->ev_pool.push_back(ev.c);
     }
     c->ev_pending.clear();
     return MFDN_OK;
