@@ -39,8 +39,11 @@ typedef enum {
 
 /* flags of mfdn_mscheme_2b/3b */
 enum {
-    MFDN_PRESORTED = 1,   /* requests are already ordered by orbital-tuple group (bra tuple, ket tuple):
-                             skip the internal group sort (step H2) */
+    MFDN_PRESORTED = 1,   /* requests are already ordered by orbital-tuple group: NON-DECREASING mfdn_group_keys value
+                             (requests failing S1-S6, key 0xFFFFFFFF, last).  Skips the scatter of step H2 and the
+                             gather of step H6; 3-body still histograms the keys to cut the stream into one-group
+                             work items.  Input that is not so ordered gives undefined VALUES (never a fault);
+                             the mask stays correct */
     MFDN_FORCE_NAIVE = 2, /* one thread per request in request order, no sort, no staging: the paper's own
                              kernel design; kept as on-device reference */
     MFDN_FORCE_DENSE = 4  /* reserved for the dense-block path; currently ignored */
