@@ -662,10 +662,23 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
         }
     // ---- one arena for the resident index tables, one for the upload-only ones
     Arena res, tmp;
+    // (a,b) -> tuple map: the sorted tuple list keeps the tuples of one (a,b) together with ascending c; if every such run
+    // is a dense c range (true for any E3max truncation of an energy-ordered orbital list) k_keys finds a tuple with one
+    // 8-byte shared-memory look-up instead of a random read of the n_orb^3 table
+    std::vector<int2> ab((size_t)No * No, int2{-1, 0});
+    bool ab_dense = No * No <= 65535 * 16;
+    for (int t = 0; t < nt && ab_dense; t++) {
+        int64_t k = tuples[t];
+        int a = (int)(k / ((int64_t)No * No)), b = (int)((k / No) % No), cc = (int)(k % No);
+        int2& e = ab[(size_t)a * No + b];
+        if (e.x < 0) { e.x = t; e.y = cc | (1 << 16); }
+        else if (cc == (e.y & 0xFFFF) + (e.y >> 16) && (e.y >> 16) < 32767) e.y += 1 << 16;
+        else ab_dense = false;
+    }
     std::vector<int4> tdesc_rt = tdesc;   // run-time copy: w = start of the tuple's sigma table (the row-map offset is upload-only)
     for (int t = 0; t < nt; t++) tdesc_rt[t].w = sigoff[t];
     size_t o_tid = res.add(tuple_id), o_desc_rt = res.add(tdesc_rt), o_sgrp = res.add(sgrp), o_sm = res.add(stmask);
-    size_t o_desc = tmp.add(tdesc);
+    size_t o_desc = tmp.add(tdesc), o_ab = res.add(ab);
     size_t o_tk = res.add(tk), o_jinfo = res.add(jinfo), o_sig = res.add(sig), o_sigoff = res.add(sigoff);
     std::vector<int64_t> coff(chan_off, chan_off + n_chan);
     std::vector<int32_t> cdim(chan_dim, chan_dim + n_chan);
@@ -684,7 +697,7 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     void* dslab = nullptr;
     cudaError_t e = cudaMalloc(&dslab, std::max<uint64_t>(cells, 1) * 16 + 256);
     void* ddtab = nullptr;
-    if (e == cudaSuccess) e = cudaMalloc(&ddtab, std::max<uint64_t>(dtab_len, 2) * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(&ddtab, (dtab_len + 2 * MAX_STATES3) * sizeof(double));   // slack: a mis-ordered MFDN_PRESORTED stream may index past a tuple
     if (e != cudaSuccess) {
         cudaFree(dtmp);
         if (vtmp) cudaFree(vtmp);
@@ -729,6 +742,7 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     c->t.tuple_id3 = (const int32_t*)(dres + o_tid);
     c->t.tdesc3 = (const int4*)(dres + o_desc_rt);
     c->t.sgrp3 = p.sgrp;
+    c->t.ab3 = ab_dense ? (const int2*)(dres + o_ab) : nullptr;
     c->t.slab3 = (const double*)dslab;
     c->t.stmask3 = (const unsigned long long*)(dres + o_sm);
     c->t.tk3 = q.tk;

@@ -82,6 +82,7 @@ struct Tables {
     // A2, 3-body
     int n_tup3, e3max;
     const int32_t* tuple_id3;      // [n_orb^3] -> tuple or -1
+    const int2* ab3;               // [n_orb^2] {first tuple of (a,b,*), cmin | count<<16} if every (a,b) has a dense c range, else NULL
     const int4* tdesc3;
     const uint2* sgrp3;            // [n_tup3^2] {start of the group's slab in 16-byte units or NO_SLAB, doubles per plane}
     const double* slab3;

@@ -45,7 +45,7 @@ __device__ __forceinline__ void cswap(uint32_t& ka, uint32_t& kb, uint32_t& ra, 
 
 // canonicalise three particles: stable sort by (orbital, SPS) ascending, sign of the permutation
 template <bool SMEM>
-__device__ __forceinline__ Side3 decode3(const Tables& T, const uint32_t* sps, int s0, int s1, int s2)
+__device__ __forceinline__ Side3 decode3(const Tables& T, const uint32_t* sps, const int2* ab, int s0, int s1, int s2)
 {
     Side3 S;
     uint32_t r0 = SMEM ? sps[s0] : __ldg(sps + s0), r1 = SMEM ? sps[s1] : __ldg(sps + s1), r2 = SMEM ? sps[s2] : __ldg(sps + s2);
@@ -56,7 +56,13 @@ __device__ __forceinline__ Side3 decode3(const Tables& T, const uint32_t* sps, i
     cswap(k1, k2, r1, r2, S.sign);
     cswap(k0, k1, r0, r1, S.sign);
     int a = rec_orb(r0), b = rec_orb(r1), c = rec_orb(r2);
-    S.tup = __ldg(T.tuple_id3 + (a * T.n_orb + b) * T.n_orb + c);
+    if (ab) {   // tuples of a fixed (a, b) are consecutive and their c's form a dense range: {first tuple, cmin | count<<16}
+        const int2 e = ab[a * T.n_orb + b];
+        const int d = c - (e.y & 0xFFFF);
+        S.tup = (e.x >= 0 && (unsigned)d < (unsigned)(e.y >> 16)) ? e.x + d : -1;
+    } else {
+        S.tup = __ldg(T.tuple_id3 + (a * T.n_orb + b) * T.n_orb + c);
+    }
     S.ima = rec_im(r0); S.imb = rec_im(r1); S.imc = rec_im(r2);
     S.tz = (rec_tz(r0) << 2) | (rec_tz(r1) << 1) | rec_tz(r2);
     S.twoM = 2 * (S.ima + S.imb + S.imc) - rec_twoj(r0) - rec_twoj(r1) - rec_twoj(r2);
@@ -124,6 +130,7 @@ __device__ __forceinline__ unsigned long long chanmask3(const Tables& T, int4 d,
 // S7 for a decoded 3-body request that passed S1-S6: at least one admissible channel term
 __device__ __forceinline__ bool mask3(const Tables& T, const Side3& B, const Side3& K, int4 db, int4 dk)
 {
+    if (max((db.y >> 16) & 255, (dk.y >> 16) & 255) > min((db.y >> 24) & 255, (dk.y >> 24) & 255)) return false;   // no common J: no slab
     const int ja = db.x & 255, jb = (db.x >> 8) & 255, jd = dk.x & 255, je = (dk.x >> 8) & 255;
     const int twoM12b = 2 * (B.ima + B.imb) - ja - jb, twoM12k = 2 * (K.ima + K.imb) - jd - je;
     const int tzb12 = (B.tz >> 2) + ((B.tz >> 1) & 1) - 1, tzk12 = (K.tz >> 2) + ((K.tz >> 1) & 1) - 1;  // MT12
@@ -266,7 +273,7 @@ __global__ void __launch_bounds__(128) k_mscheme_naive(Tables T, long long n, co
     if (!in_range(T, s, 2 * BODY)) {
         atomicAdd(T.bad_count, 1ull);
     } else if (BODY == 3) {
-        Side3 B = decode3<false>(T, T.sps_rec, s[0], s[1], s[2]), K = decode3<false>(T, T.sps_rec, s[3], s[4], s[5]);
+        Side3 B = decode3<false>(T, T.sps_rec, nullptr, s[0], s[1], s[2]), K = decode3<false>(T, T.sps_rec, nullptr, s[3], s[4], s[5]);
         v = eval3_naive(T, B, K, mask);
     } else {
         Side2 B = decode2<false>(T, T.sps_rec, s[0], s[1]), K = decode2<false>(T, T.sps_rec, s[2], s[3]);
@@ -278,7 +285,11 @@ __global__ void __launch_bounds__(128) k_mscheme_naive(Tables T, long long n, co
 
 // =============================================================================== H1: records
 // One thread per request: decode, S1-S7 -> mask (request order, coalesced), canonical packed record.
-constexpr int KEYS_SPS_SMEM = 2048;   // SPS records held in shared memory by k_keys when the basis is this small
+// Blocks walk KEYS_PER_BLOCK consecutive requests.  With SMEM the small per-basis tables every request needs (SPS
+// records, the (a,b) -> tuple map) are copied to shared memory once per block: a random 4..16-byte
+// look-up there costs a few bank-conflict wavefronts instead of up to 32 L1 tag look-ups (ncu: k_keys was bound by
+// the L1 data pipe, 81 % of peak).
+constexpr int KEYS_SPS_SMEM = 2048, KEYS_AB_SMEM = 2048, KEYS_PER_BLOCK = 256 * 32;
 
 template <int BODY, bool AGG, bool SMEM>
 __global__ void __launch_bounds__(256) k_keys(Tables T, long long n, const int32_t* __restrict__ req,
@@ -287,56 +298,63 @@ __global__ void __launch_bounds__(256) k_keys(Tables T, long long n, const int32
                                               uint32_t* __restrict__ keys32)
 {
     __shared__ uint32_t s_sps[SMEM ? KEYS_SPS_SMEM : 1];
+    __shared__ int2 s_ab[SMEM && BODY == 3 ? KEYS_AB_SMEM : 1];
     if (SMEM) {
         for (int k = threadIdx.x; k < T.n_sps; k += blockDim.x) s_sps[k] = __ldg(T.sps_rec + k);
+        if (BODY == 3) {
+            for (int k = threadIdx.x; k < T.n_orb * T.n_orb; k += blockDim.x) s_ab[k] = __ldg(T.ab3 + k);
+        }
         __syncthreads();
     }
     const uint32_t* sps = SMEM ? s_sps : T.sps_rec;
-    long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;   // partial tail warp: __activemask below
-    int s[6];
-    if (BODY == 3) load_req3(req, i, s); else load_req2(req, i, s);
-    uint32_t key = REC_INVALID;
-    unsigned long long low = 0;
-    int mask = 0;
-    if (!in_range(T, s, 2 * BODY)) {
-        if (recs) atomicAdd(T.bad_count, 1ull);
-    } else if (BODY == 3) {
-        Side3 B = decode3<SMEM>(T, sps, s[0], s[1], s[2]), K = decode3<SMEM>(T, sps, s[3], s[4], s[5]);
-        if (select3(T, B, K)) {
-            key = (uint32_t)B.tup * T.n_tup3 + K.tup;
-            const int4 db = __ldg(T.tdesc3 + B.tup), dk = __ldg(T.tdesc3 + K.tup);
-            if (__ldg(T.sgrp3 + key).x != NO_SLAB) mask = mask3(T, B, K, db, dk);
-            const int jb1 = ((db.x >> 8) & 255) + 1, jc1 = ((db.x >> 16) & 255) + 1;
-            const int je1 = ((dk.x >> 8) & 255) + 1, jf1 = ((dk.x >> 16) & 255) + 1;
-            const uint32_t sb = __ldg(T.sig3 + db.w + (B.ima * jb1 + B.imb) * jc1 + B.imc);
-            const uint32_t sk = __ldg(T.sig3 + dk.w + (K.ima * je1 + K.imb) * jf1 + K.imc);
-            const uint32_t bin = __ldg(T.tz2bin3 + ((B.tz << 3) | K.tz));
-            low = (unsigned long long)(sb | (sk << 12) | (bin << 24) | ((uint32_t)(B.sign * K.sign < 0) << 29)) |
-                  ((unsigned long long)(B.ima + B.imb + B.imc) << 30);
-        }
-    } else {
-        Side2 B = decode2<SMEM>(T, sps, s[0], s[1]), K = decode2<SMEM>(T, sps, s[2], s[3]);
-        if (select2(B, K)) {
-            key = (uint32_t)B.tup * T.n_tup2 + K.tup;
-            if (__ldg(T.slab_off2 + key) != NO_SLAB) mask = mask2(B, __ldg(T.tdesc2 + B.tup), __ldg(T.tdesc2 + K.tup));
-            low = (unsigned long long)(B.ima | (B.imb << 5) | (K.ima << 15) | (K.imb << 20)) |
-                  ((unsigned long long)((B.tz << 3) | K.tz) << 30) | ((unsigned long long)(B.sign * K.sign < 0) << 36);
-        }
-    }
-    if (recs) recs[i] = ((unsigned long long)key << REC_KEY_SHIFT) | low;
-    if (maskout) maskout[i] = (uint8_t)mask;
-    if (hist) {
-        const uint32_t bucket = key == REC_INVALID ? invalid_bucket : key;
-        if (AGG) {   // group-ordered input: one atomic per run of equal keys in the warp
-            const unsigned act = __activemask();
-            const unsigned same = __match_any_sync(act, bucket);
-            if ((threadIdx.x & 31) == __ffs(same) - 1) atomicAdd(hist + bucket, (uint32_t)__popc(same));
+    const int2* ab = (SMEM && BODY == 3) ? s_ab : nullptr;
+    const long long i0 = (long long)blockIdx.x * KEYS_PER_BLOCK + threadIdx.x;
+    const long long i1 = min(n, (long long)(blockIdx.x + 1) * KEYS_PER_BLOCK);
+    for (long long i = i0; i < i1; i += 256) {
+        int s[6];
+        if (BODY == 3) load_req3(req, i, s); else load_req2(req, i, s);
+        uint32_t key = REC_INVALID;
+        unsigned long long low = 0;
+        int mask = 0;
+        if (!in_range(T, s, 2 * BODY)) {
+            if (recs) atomicAdd(T.bad_count, 1ull);
+        } else if (BODY == 3) {
+            Side3 B = decode3<SMEM>(T, sps, ab, s[0], s[1], s[2]), K = decode3<SMEM>(T, sps, ab, s[3], s[4], s[5]);
+            if (select3(T, B, K)) {
+                key = (uint32_t)B.tup * T.n_tup3 + K.tup;
+                const int4 db = __ldg(T.tdesc3 + B.tup), dk = __ldg(T.tdesc3 + K.tup);
+                mask = mask3(T, B, K, db, dk);
+                const int jb1 = ((db.x >> 8) & 255) + 1, jc1 = ((db.x >> 16) & 255) + 1;
+                const int je1 = ((dk.x >> 8) & 255) + 1, jf1 = ((dk.x >> 16) & 255) + 1;
+                const uint32_t sb = __ldg(T.sig3 + db.w + (B.ima * jb1 + B.imb) * jc1 + B.imc);
+                const uint32_t sk = __ldg(T.sig3 + dk.w + (K.ima * je1 + K.imb) * jf1 + K.imc);
+                const uint32_t bin = __ldg(T.tz2bin3 + ((B.tz << 3) | K.tz));
+                low = (unsigned long long)(sb | (sk << 12) | (bin << 24) | ((uint32_t)(B.sign * K.sign < 0) << 29)) |
+                      ((unsigned long long)(B.ima + B.imb + B.imc) << 30);
+            }
         } else {
-            atomicAdd(hist + bucket, 1u);
+            Side2 B = decode2<SMEM>(T, sps, s[0], s[1]), K = decode2<SMEM>(T, sps, s[2], s[3]);
+            if (select2(B, K)) {
+                key = (uint32_t)B.tup * T.n_tup2 + K.tup;
+                if (__ldg(T.slab_off2 + key) != NO_SLAB) mask = mask2(B, __ldg(T.tdesc2 + B.tup), __ldg(T.tdesc2 + K.tup));
+                low = (unsigned long long)(B.ima | (B.imb << 5) | (K.ima << 15) | (K.imb << 20)) |
+                      ((unsigned long long)((B.tz << 3) | K.tz) << 30) | ((unsigned long long)(B.sign * K.sign < 0) << 36);
+            }
         }
+        if (recs) recs[i] = ((unsigned long long)key << REC_KEY_SHIFT) | low;
+        if (maskout) maskout[i] = (uint8_t)mask;
+        if (hist) {
+            const uint32_t bucket = key == REC_INVALID ? invalid_bucket : key;
+            if (AGG) {   // group-ordered input: one atomic per run of equal keys in the warp
+                const unsigned act = __activemask();
+                const unsigned same = __match_any_sync(act, bucket);
+                if ((threadIdx.x & 31) == __ffs(same) - 1) atomicAdd(hist + bucket, (uint32_t)__popc(same));
+            } else {
+                atomicAdd(hist + bucket, 1u);
+            }
+        }
+        if (keys32) keys32[i] = key == REC_INVALID ? 0xFFFFFFFFu : key;
     }
-    if (keys32) keys32[i] = key == REC_INVALID ? 0xFFFFFFFFu : key;
 }
 
 // =============================================================================== H2: group sort
@@ -399,9 +417,11 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_add(uint32_t* __restrict__ data
         if (base + k < m) data[base + k] += add;
 }
 
-// H2 scatter: records -> group order.  posof[i] = position of request i in the group-ordered stream (coalesced write);
-// the results are computed in group order and gathered back by k_unpermute (random 8-byte READS are far cheaper
-// than the random 8-byte WRITES of a direct out[original index] store: no read-modify-write of DRAM sectors).
+// H2 scatter: records -> group order; the cursor array (scanned histogram) ends up holding the END of every bucket.
+// posof[i] = position of request i in the group-ordered stream (coalesced write); the results are computed in group
+// order and gathered back by k_unpermute.  Measured alternatives: ranks from a returning histogram atomic in k_keys
+// (scatter without atomics) made k_keys 1.3 ms slower and the scatter no faster -- it is bound by the scattered
+// 8-byte writes, not by the atomics.
 constexpr int SC_PER_THREAD = 4;
 __global__ void __launch_bounds__(256) k_scatter(long long n, const unsigned long long* __restrict__ recs,
                                                  uint32_t* __restrict__ cursor, unsigned long long* __restrict__ sorted,
@@ -930,16 +950,16 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
         const unsigned long long* trecs = recs;
         uint32_t* hist = hist_needed ? (uint32_t*)(w + o_hist) : nullptr;
         uint32_t* sums = hist_needed ? (uint32_t*)(w + o_sums) : nullptr;
-        const unsigned gk = (unsigned)((n + 255) / 256);
         const uint32_t invalid_bucket = (uint32_t)(nt * nt);
         if (hist_needed) MFDN_CUDA(c, cudaMemsetAsync(hist, 0, (size_t)n_buckets * 4, st));
-        const bool sm = c->t.n_sps <= KEYS_SPS_SMEM;
+        const bool sm = c->t.n_sps <= KEYS_SPS_SMEM && (BODY == 2 || (c->t.ab3 && c->t.n_orb * c->t.n_orb <= KEYS_AB_SMEM));
+        const unsigned gkb = (unsigned)((n + KEYS_PER_BLOCK - 1) / KEYS_PER_BLOCK);
         if (sort) {
-            if (sm) k_keys<BODY, false, true><<<gk, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr);
-            else k_keys<BODY, false, false><<<gk, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr);
+            if (sm) k_keys<BODY, false, true><<<gkb, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr);
+            else k_keys<BODY, false, false><<<gkb, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr);
         } else {
-            if (sm) k_keys<BODY, true, true><<<gk, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr);
-            else k_keys<BODY, true, false><<<gk, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr);
+            if (sm) k_keys<BODY, true, true><<<gkb, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr);
+            else k_keys<BODY, true, false><<<gkb, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr);
         }
         c->launches += 1;
         if (hist_needed) {
@@ -1020,8 +1040,8 @@ extern "C" int mfdn_group_keys(mfdn_ctx* c, int body, int64_t n, const int32_t* 
     if (body == 3 ? !c->has3 : !c->has2) return fail(c, MFDN_ERR_STATE, "group_keys before coupled upload");
     if (n == 0) return MFDN_OK;
     cudaStream_t st = (cudaStream_t)stream;
-    if (body == 3) k_keys<3, false, false><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(c->t, n, d_req, nullptr, nullptr, nullptr, 0u, d_key);
-    else k_keys<2, false, false><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(c->t, n, d_req, nullptr, nullptr, nullptr, 0u, d_key);
+    if (body == 3) k_keys<3, false, false><<<(unsigned)((n + KEYS_PER_BLOCK - 1) / KEYS_PER_BLOCK), 256, 0, st>>>(c->t, n, d_req, nullptr, nullptr, nullptr, 0u, d_key);
+    else k_keys<2, false, false><<<(unsigned)((n + KEYS_PER_BLOCK - 1) / KEYS_PER_BLOCK), 256, 0, st>>>(c->t, n, d_req, nullptr, nullptr, nullptr, 0u, d_key);
     MFDN_CUDA(c, cudaGetLastError());
     return MFDN_OK;
 }
