@@ -517,8 +517,9 @@ struct ItemShared {
     uint16_t srank[ITEM3];                   // per record: iM<<10 | rank among the item's records of equal iM
 };
 
-// bin stride of Vw: >= gsize, == 2 (mod 16) doubles, so that different bins fall into different bank quads
-__device__ __forceinline__ uint32_t vw_stride(uint32_t gsize) { return ((gsize + 13u) & ~15u) + 2u; }
+// bin stride of Vw: odd, so that with 64-bit loads the 16 lanes of a half warp that sit in 16 different isospin bins
+// hit 16 different bank pairs (ncu: 128-bit loads with an even stride ran at 1.8x their ideal wavefront count)
+__device__ __forceinline__ uint32_t vw_stride(uint32_t gsize) { return gsize | 1u; }
 
 // One J block of the sum for TWO records of the group (A and B, 32 sorted slots apart) with the ket range size NK known
 // at compile time and a run-time loop over the bra rows (blocks with more than 4 rows or columns):
@@ -544,11 +545,9 @@ __device__ __forceinline__ void j_block3x2_rows(const double* __restrict__ dtab,
         pbA += Sb; pbB += Sb;
         double vA[P], vB[P];
 #pragma unroll
-        for (int q = 0; q < P / 2; q++) {
-            const double2 a = *reinterpret_cast<const double2*>(vw + viA + 2 * q);
-            const double2 b = *reinterpret_cast<const double2*>(vw + viB + 2 * q);
-            vA[2 * q] = a.x; vA[2 * q + 1] = a.y;
-            vB[2 * q] = b.x; vB[2 * q + 1] = b.y;
+        for (int k = 0; k < NK; k++) {
+            vA[k] = vw[viA + k];
+            vB[k] = vw[viB + k];
         }
         viA += P; viB += P;
         double accA = ckA[0] * vA[0], accB = ckB[0] * vB[0];
@@ -588,11 +587,9 @@ __device__ __forceinline__ void j_block3x2(const double* __restrict__ dtab, cons
     for (int i = 0; i < NB; i++) {
         double vA[P], vB[P];
 #pragma unroll
-        for (int q = 0; q < P / 2; q++) {
-            const double2 a = *reinterpret_cast<const double2*>(vw + viA + i * P + 2 * q);
-            const double2 b = *reinterpret_cast<const double2*>(vw + viB + i * P + 2 * q);
-            vA[2 * q] = a.x; vA[2 * q + 1] = a.y;
-            vB[2 * q] = b.x; vB[2 * q + 1] = b.y;
+        for (int k = 0; k < NK; k++) {
+            vA[k] = vw[viA + i * P + k];
+            vB[k] = vw[viB + i * P + k];
         }
         double accA = ckA[0] * vA[0], accB = ckB[0] * vB[0];
 #pragma unroll
