@@ -472,9 +472,13 @@ __global__ void __launch_bounds__(256) k_unpermute(long long n, const double* __
 // Work items (H3): one item = up to ITEM3 consecutive records of ONE group in the group-ordered stream, so that a
 // thread block shares every loop bound, table row and the group's slab.  `bounds[b]` is the END of bucket b after the
 // scatter (ends = 1: the cursor array) or its START for pre-sorted input (ends = 0: the scanned histogram).
+// Groups with at most SMALL_ITEM3 records go to a second list (filled from the END of the item array, counted in
+// n_items[1]): for them the per-item prologue of k_transform3 (block-wide staging, M sort) costs more than it saves, a
+// single warp evaluates them directly (k_transform3_small).
+constexpr uint32_t SMALL_ITEM3 = 64;
 __global__ void __launch_bounds__(256) k_items3(const uint32_t* __restrict__ bounds, uint32_t n_buckets, int ends, uint32_t n,
                                                const uint2* __restrict__ sgrp, uint32_t invalid_bucket,
-                                               uint4* __restrict__ items, uint32_t* __restrict__ n_items)
+                                               uint4* __restrict__ items, uint32_t last_slot, uint32_t* __restrict__ n_items)
 {
     const uint32_t b = blockIdx.x * 256u + threadIdx.x;
     uint32_t start = 0, end = 0;
@@ -482,22 +486,98 @@ __global__ void __launch_bounds__(256) k_items3(const uint32_t* __restrict__ bou
         if (ends) { end = bounds[b]; start = b ? bounds[b - 1] : 0u; }
         else { start = bounds[b]; end = (b + 1 < n_buckets) ? bounds[b + 1] : n; }
     }
-    const uint32_t cnt = end - start, k = (cnt + ITEM3 - 1) / ITEM3;
-    // warp-aggregated append: the list stays (nearly) in group order, neighbours share the bra tuple's tables
+    const uint32_t cnt = end - start;
+    const bool small = cnt <= SMALL_ITEM3;
+    const uint32_t k = small ? 0u : (cnt + ITEM3 - 1) / ITEM3, ks = (small && cnt) ? 1u : 0u;
+    // warp-aggregated append: the lists stay (nearly) in group order, neighbours share the bra tuple's tables
     const int lane = threadIdx.x & 31;
-    uint32_t incl = k;
+    uint32_t incl = k, incs = ks;
 #pragma unroll
     for (int off = 1; off < 32; off <<= 1) {
-        uint32_t x = __shfl_up_sync(0xFFFFFFFFu, incl, off);
-        if (lane >= off) incl += x;
+        uint32_t x = __shfl_up_sync(0xFFFFFFFFu, incl, off), y = __shfl_up_sync(0xFFFFFFFFu, incs, off);
+        if (lane >= off) { incl += x; incs += y; }
     }
-    uint32_t base = 0;
+    uint32_t base = 0, bases = 0;
     if (lane == 31 && incl) base = atomicAdd(n_items, incl);
+    if (lane == 31 && incs) bases = atomicAdd(n_items + 1, incs);
     base = __shfl_sync(0xFFFFFFFFu, base, 31);
-    if (k == 0) return;
+    bases = __shfl_sync(0xFFFFFFFFu, bases, 31);
+    if (cnt == 0) return;
     const uint32_t g = (b == invalid_bucket || sgrp[b].x == NO_SLAB) ? ZERO_ITEM : b;
+    if (small) {
+        items[last_slot - (bases + incs - 1u)] = make_uint4(start, cnt, g, 0u);
+        return;
+    }
     uint32_t slot = base + incl - k;
     for (uint32_t j = 0; j < k; j++) items[slot + j] = make_uint4(start + j * ITEM3, min((uint32_t)ITEM3, cnt - j * ITEM3), g, 0u);
+}
+
+// H3-H6 for small groups: one warp per item, lane = record.  The group's loop bounds, table rows and slab addresses
+// are warp-uniform, the lanes differ in their projections (sigma) and isospin weights.  Same operations in the same
+// order as the staged path of k_transform3 (Vw first, then ck, then cb, then the sum over J), so a request's value
+// does not depend on which of the two kernels its group happened to go to.
+__global__ void __launch_bounds__(128) k_transform3_small(Tables T, const uint4* __restrict__ items, uint32_t last_slot,
+                                                          const uint32_t* __restrict__ n_items_p,
+                                                          const unsigned long long* __restrict__ recs, double* __restrict__ out)
+{
+    const int lane = threadIdx.x & 31;
+    const uint32_t gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
+    const uint32_t n_small = __ldg(n_items_p + 1);
+    const uint32_t nt = (uint32_t)T.n_tup3;
+    const double* __restrict__ dtab = T.dtab3;
+    for (uint32_t it = gw; it < n_small; it += nw) {
+        const uint4 item = __ldg(items + (last_slot - it));
+        const uint32_t pos0 = item.x, cnt = item.y, g = item.z;
+        if (g == ZERO_ITEM) {
+            for (uint32_t r = lane; r < cnt; r += 32) out[pos0 + r] = 0.0;
+            continue;
+        }
+        const uint32_t tb = g / nt, tk = g - tb * nt;
+        const int4 kb = __ldg(T.tk3 + tb), kk = __ldg(T.tk3 + tk);
+        const uint2 sg = __ldg(T.sgrp3 + g);
+        const int Jminb = (kb.w >> 16) & 255, Jmink = (kk.w >> 16) & 255;
+        const int Jlo = max(Jminb, Jmink), Jhi = min((kb.w >> 24) & 255, (kk.w >> 24) & 255);
+        const int nblk = ((Jhi - Jlo) >> 1) + 1;
+        const int2* __restrict__ jib = T.jinfo3 + kb.z + ((Jlo - Jminb) >> 1);
+        const int2* __restrict__ jik = T.jinfo3 + kk.z + ((Jlo - Jmink) >> 1);
+        const uint32_t Sb = (uint32_t)kb.y, Sk = (uint32_t)kk.y, gsize = sg.y;
+        const uint32_t pb0 = (uint32_t)kb.x + (uint32_t)__ldg(jib).x * Sb, pk0 = (uint32_t)kk.x + (uint32_t)__ldg(jik).x * Sk;
+        for (uint32_t r0 = 0; r0 < cnt; r0 += 32) {   // 32 records per pass
+            const bool valid = r0 + lane < cnt;
+            const unsigned long long rec = __ldg(recs + pos0 + (valid ? r0 + lane : r0));
+            const uint32_t lo = (uint32_t)rec;
+            const double* wp = T.wbin3 + ((lo >> 24) & 31u) * NISO3;
+            const double w0 = __ldg(wp), w1 = __ldg(wp + 1), w2 = __ldg(wp + 2), w3 = __ldg(wp + 3), w4 = __ldg(wp + 4);
+            uint32_t pb = pb0 + (lo & 0xFFFu), pk = pk0 + ((lo >> 12) & 0xFFFu);
+            const double* __restrict__ row = T.slab3 + (size_t)sg.x * 2;
+            double total = 0.0;
+            for (int q = 0; q < nblk; q++) {
+                const int nb = __ldg(jib + q).y, nk = __ldg(jik + q).y;
+                const int P = row_pitch3(nk);
+                double t = 0.0;
+                for (int i = 0; i < nb; i++) {
+                    const double cb = __ldg(dtab + pb);
+                    pb += Sb;
+                    double acc = 0.0;
+                    for (int k = 0; k < nk; k++) {
+                        const double ck = __ldg(dtab + pk + (uint32_t)k * Sk);
+                        const double* cell = row + k;
+                        double v = w0 * __ldg(cell);
+                        v = fma(w1, __ldg(cell + gsize), v);
+                        v = fma(w2, __ldg(cell + 2 * gsize), v);
+                        v = fma(w3, __ldg(cell + 3 * gsize), v);
+                        v = fma(w4, __ldg(cell + 4 * gsize), v);
+                        acc = k ? fma(ck, v, acc) : ck * v;
+                    }
+                    t = fma(cb, acc, t);
+                    row += P;
+                }
+                pk += (uint32_t)nk * Sk;
+                total += t;
+            }
+            if (valid) out[pos0 + r0 + lane] = (((lo >> 29) & 1u) ? -total : total) + 0.0;   // + 0.0: never store -0
+        }
+    }
 }
 
 constexpr int TR_THREADS = 128;
@@ -979,13 +1059,16 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
         if (items) {
             uint4* itm = (uint4*)(w + o_items);
             uint32_t* cnt = (uint32_t*)(w + o_count);
-            MFDN_CUDA(c, cudaMemsetAsync(cnt, 0, 4, st));
+            MFDN_CUDA(c, cudaMemsetAsync(cnt, 0, 8, st));
+            const uint32_t last_slot = (uint32_t)(max_items - 1);
             k_items3<<<(unsigned)((n_buckets + 255) / 256), 256, 0, st>>>(hist, (uint32_t)n_buckets, sort ? 1 : 0, (uint32_t)n, c->t.sgrp3,
-                                                                           invalid_bucket, itm, cnt);
+                                                                           invalid_bucket, itm, last_slot, cnt);
             if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.b, st));
             const unsigned grid = (unsigned)std::min<long long>(max_items, (long long)c->num_sms * 6);
             k_transform3<<<grid, TR_THREADS, 0, st>>>(c->t, itm, cnt, trecs, nullptr, tout);
-            c->launches += 2;
+            const unsigned grid_s = (unsigned)std::min<long long>((std::min<long long>(n, n_buckets) + 3) / 4, (long long)c->num_sms * 16);
+            k_transform3_small<<<grid_s, 128, 0, st>>>(c->t, itm, last_slot, cnt, trecs, tout);
+            c->launches += 3;
         } else {
             if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.b, st));
             k_transform2<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(c->t, n, trecs, nullptr, tout);
