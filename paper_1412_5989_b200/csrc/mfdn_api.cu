@@ -83,7 +83,7 @@ extern "C" int mfdn_orbitals_init(mfdn_ctx** out, int device, int32_t n_orb, con
         if (o < 0 || o >= n_orb) { delete c; return MFDN_ERR_ARG; }
         int tm = sps_twom[s], tz = sps_twotz[s];
         if (std::abs(tm) > twoj[o] || !(tm & 1) || (tz != 1 && tz != -1)) { delete c; return MFDN_ERR_ARG; }
-        c->h_sps_rec[s] = sps_pack(o, (tm + twoj[o]) / 2, tz == 1, twoj[o], 2 * n[o] + l[o], l[o] & 1);
+        c->h_sps_rec[s] = sps_pack(o, (tm + twoj[o]) / 2, tz == 1, twoj[o], l[o] & 1);
     }
     void* d = nullptr;
     if (cudaMalloc(&d, n_sps * sizeof(uint32_t) + 256) != cudaSuccess) { delete c; return MFDN_ERR_OOM; }

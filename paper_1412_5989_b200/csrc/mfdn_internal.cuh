@@ -11,19 +11,25 @@
 namespace mfdn {
 
 // ---- SPS record (A0): one 32-bit word per single-particle state -------------------------------
-//  [0,10) orbital   [10,15) im = (2m+2j)/2   [15] tz bit (1 <=> 2tz = +1)
-//  [16,21) 2j       [21,27) e = 2n+l         [27] l & 1
-__host__ __device__ inline uint32_t sps_pack(int orb, int im, int tzbit, int twoj, int e, int lpar)
+//  [0,10) orbital   [10,17) im = (2m+2j)/2   [17,24) 2j   [24,26) tz bit (1 <=> 2tz = +1)   [26,28) l & 1
+// The fields above bit 10 are two bits wider than their values: (r0 >> 10) + (r1 >> 10) + (r2 >> 10) is the packed
+// sum of every field over up to three particles (M, Tz and parity conservation from one addition).  e = 2n+l is
+// not kept: S5 (sum of e <= E3max) is implied by S6 (the tuple is listed), because the upload rejects listed
+// states above E3max.
+__host__ __device__ inline uint32_t sps_pack(int orb, int im, int tzbit, int twoj, int lpar)
 {
-    return (uint32_t)orb | ((uint32_t)im << 10) | ((uint32_t)tzbit << 15) | ((uint32_t)twoj << 16) |
-           ((uint32_t)e << 21) | ((uint32_t)lpar << 27);
+    return (uint32_t)orb | ((uint32_t)im << 10) | ((uint32_t)twoj << 17) | ((uint32_t)tzbit << 24) | ((uint32_t)lpar << 26);
 }
 __host__ __device__ inline int rec_orb(uint32_t r) { return r & 1023; }
 __host__ __device__ inline int rec_im(uint32_t r) { return (r >> 10) & 31; }
-__host__ __device__ inline int rec_tz(uint32_t r) { return (r >> 15) & 1; }
-__host__ __device__ inline int rec_twoj(uint32_t r) { return (r >> 16) & 31; }
-__host__ __device__ inline int rec_e(uint32_t r) { return (r >> 21) & 63; }
-__host__ __device__ inline int rec_lpar(uint32_t r) { return (r >> 27) & 1; }
+__host__ __device__ inline int rec_twoj(uint32_t r) { return (r >> 17) & 31; }
+__host__ __device__ inline int rec_tz(uint32_t r) { return (r >> 24) & 1; }
+__host__ __device__ inline int rec_lpar(uint32_t r) { return (r >> 26) & 1; }
+// fields of a packed sum (r0 >> 10) + (r1 >> 10) [+ (r2 >> 10)]
+__host__ __device__ inline int sum_im(uint32_t s) { return s & 127; }
+__host__ __device__ inline int sum_twoj(uint32_t s) { return (s >> 7) & 127; }
+__host__ __device__ inline int sum_tz(uint32_t s) { return (s >> 14) & 3; }
+__host__ __device__ inline int sum_lpar(uint32_t s) { return (s >> 16) & 3; }
 
 constexpr int MAX_TWOJ = 21;       // 3*MAX_TWOJ <= 63 so that (2J,2T) fits a 64-bit channel mask
 constexpr int NISO3 = 5;           // isospin slots per 3-body cell: (T12,T12',T) = (0,0,1/2) (0,1,1/2) (1,0,1/2) (1,1,1/2) (1,1,3/2)

@@ -11,10 +11,15 @@
 // The slab of a (bra tuple, ket tuple) group is stored in exactly this loop order (A2).
 //
 // Pipeline of one call:
-//   k_keys      H1  decode, selection S1-S7 -> mask, canonicalise -> 64-bit record (group key | sign | tz | m)
-//   k_scan_*    H2  exclusive scan of the group histogram            (skipped if MFDN_PRESORTED)
-//   k_scatter   H2  records -> group order (+ original index)        (skipped if MFDN_PRESORTED)
-//   k_transform H3-H6  one warp per 32 consecutive records of the group-ordered stream
+//   k_keys        H1  decode, selection S1-S7 -> mask, canonicalise -> 64-bit record; histogram of the group keys
+//   k_scan_*      H2  exclusive scan of the histogram -> bucket bounds
+//   k_scatter     H2  records -> group order, posof[request] = position        (skipped if MFDN_PRESORTED)
+//   k_items3      H3  one-group work items from the bucket bounds (3-body); groups of <= 64 records on a second list
+//   k_transform3  H3-H5  block per item: staged isospin-combined slab, records ordered by M, paired channel sums
+//   k_transform3_small   warp per small group, direct sums in the same operation order
+//   k_transform2  H3-H5  2-body: warp per 32 records of the group-ordered stream
+//   k_unpermute   H6  values from group order back to request order            (skipped if MFDN_PRESORTED)
+//   k_mscheme_naive      MFDN_FORCE_NAIVE: the paper's design, thread per request in request order
 #include <algorithm>
 #include <cstdio>
 
@@ -29,7 +34,7 @@ struct Side3 {
     int tup;       // tuple id or -1
     int ima, imb, imc;
     int tz;        // ta<<2 | tb<<1 | tc
-    int twoM, twoMT, par, e;
+    int twoM, twoMT, par;
     int sign;      // +1 / -1
     bool distinct;
 };
@@ -65,10 +70,10 @@ __device__ __forceinline__ Side3 decode3(const Tables& T, const uint32_t* sps, c
     }
     S.ima = rec_im(r0); S.imb = rec_im(r1); S.imc = rec_im(r2);
     S.tz = (rec_tz(r0) << 2) | (rec_tz(r1) << 1) | rec_tz(r2);
-    S.twoM = 2 * (S.ima + S.imb + S.imc) - rec_twoj(r0) - rec_twoj(r1) - rec_twoj(r2);
-    S.twoMT = 2 * (rec_tz(r0) + rec_tz(r1) + rec_tz(r2)) - 3;
-    S.par = (rec_lpar(r0) + rec_lpar(r1) + rec_lpar(r2)) & 1;
-    S.e = rec_e(r0) + rec_e(r1) + rec_e(r2);
+    const uint32_t sum = (r0 >> 10) + (r1 >> 10) + (r2 >> 10);   // every field summed over the three particles at once
+    S.twoM = 2 * sum_im(sum) - sum_twoj(sum);
+    S.twoMT = 2 * sum_tz(sum) - 3;
+    S.par = sum_lpar(sum) & 1;
     return S;
 }
 
@@ -89,9 +94,10 @@ __device__ __forceinline__ Side2 decode2(const Tables& T, const uint32_t* sps, i
     S.tup = __ldg(T.tuple_id2 + rec_orb(r0) * T.n_orb + rec_orb(r1));
     S.ima = rec_im(r0); S.imb = rec_im(r1);
     S.tz = (rec_tz(r0) << 1) | rec_tz(r1);
-    S.twoM = 2 * (S.ima + S.imb) - rec_twoj(r0) - rec_twoj(r1);
-    S.twoMT = 2 * (rec_tz(r0) + rec_tz(r1)) - 2;
-    S.par = (rec_lpar(r0) + rec_lpar(r1)) & 1;
+    const uint32_t sum = (r0 >> 10) + (r1 >> 10);
+    S.twoM = 2 * sum_im(sum) - sum_twoj(sum);
+    S.twoMT = 2 * sum_tz(sum) - 2;
+    S.par = sum_lpar(sum) & 1;
     return S;
 }
 
@@ -108,7 +114,7 @@ __device__ __forceinline__ bool in_range(const Tables& T, const int* s, int k)
 __device__ __forceinline__ bool select3(const Tables& T, const Side3& B, const Side3& K)
 {
     return B.distinct && K.distinct && B.twoM == K.twoM && B.twoMT == K.twoMT && B.par == K.par &&
-           B.e <= T.e3max && K.e <= T.e3max && B.tup >= 0 && K.tup >= 0;
+           B.tup >= 0 && K.tup >= 0;   // S5 is implied by S6: listed tuples are within E3max (checked at upload)
 }
 __device__ __forceinline__ bool select2(const Side2& B, const Side2& K)
 {
@@ -310,9 +316,13 @@ __global__ void __launch_bounds__(256) k_keys(Tables T, long long n, const int32
     const int2* ab = (SMEM && BODY == 3) ? s_ab : nullptr;
     const long long i0 = (long long)blockIdx.x * KEYS_PER_BLOCK + threadIdx.x;
     const long long i1 = min(n, (long long)(blockIdx.x + 1) * KEYS_PER_BLOCK);
+    int nx[6];
+    if (i0 < i1) { if (BODY == 3) load_req3(req, i0, nx); else load_req2(req, i0, nx); }
     for (long long i = i0; i < i1; i += 256) {
         int s[6];
-        if (BODY == 3) load_req3(req, i, s); else load_req2(req, i, s);
+#pragma unroll
+        for (int k = 0; k < 6; k++) s[k] = nx[k];
+        if (i + 256 < i1) { if (BODY == 3) load_req3(req, i + 256, nx); else load_req2(req, i + 256, nx); }   // next request in flight
         uint32_t key = REC_INVALID;
         unsigned long long low = 0;
         int mask = 0;
@@ -713,8 +723,7 @@ __device__ __noinline__ double j_block3_generic(const double* __restrict__ dtab,
 //  (3) every thread evaluates records in sorted order: three nested loops over J, J12, J12' whose bounds
 //      are shared by the block; lanes differ in their table offsets (sigma), bin and first J block (J >= |M|).
 __global__ void __launch_bounds__(TR_THREADS, 6) k_transform3(Tables T, const uint4* __restrict__ items, const uint32_t* __restrict__ n_items_p,
-                                                             const unsigned long long* __restrict__ recs,
-                                                             const uint32_t* __restrict__ order, double* __restrict__ out)
+                                                             const unsigned long long* __restrict__ recs, double* __restrict__ out)
 {
     __shared__ __align__(16) ItemShared sh;
     const int tid = threadIdx.x, lane = tid & 31;
@@ -730,16 +739,15 @@ __global__ void __launch_bounds__(TR_THREADS, 6) k_transform3(Tables T, const ui
         const uint32_t pos0 = item.x, cnt = item.y, g = item.z;
         const unsigned long long* __restrict__ irec = recs + pos0;
         if (g == ZERO_ITEM) {   // block-uniform
-            for (uint32_t idx = tid; idx < cnt; idx += TR_THREADS) out[order ? __ldg(order + pos0 + idx) : pos0 + idx] = 0.0;
+            for (uint32_t idx = tid; idx < cnt; idx += TR_THREADS) out[pos0 + idx] = 0.0;
             continue;
         }
-        {   // prefetch what the NEXT item of this block will read first: its records (and their output order) into L2,
+        {   // prefetch what the NEXT item of this block will read first: its records into L2,
             // the two tuple descriptors and the group descriptor into L1
             const uint32_t nit = it + gridDim.x;
             if (nit < n_items) {
                 const uint4 nx = __ldg(items + nit);
                 if ((uint32_t)tid * 16u < nx.y) asm volatile("prefetch.global.L2 [%0];" ::"l"(recs + nx.x + tid * 16));
-                if (order && (uint32_t)tid * 32u < nx.y) asm volatile("prefetch.global.L2 [%0];" ::"l"(order + nx.x + tid * 32));
                 if (nx.z != ZERO_ITEM && tid >= 32 && tid < 35) {
                     const uint32_t tb = nx.z / nt, tk = nx.z - tb * nt;
                     const void* a = tid == 32 ? (const void*)(T.tk3 + tb) : tid == 33 ? (const void*)(T.tk3 + tk) : (const void*)(T.sgrp3 + nx.z);
@@ -907,21 +915,16 @@ __global__ void __launch_bounds__(TR_THREADS, 6) k_transform3(Tables T, const ui
 #undef MFDN_BLK
 #undef MFDN_ROWS
                 }
-                if (slotA < cnt && blA < bpr) {   // else: past the end / bin staged in another round
-                    const uint32_t pos = pos0 + idxA;
-                    out[order ? __ldg(order + pos) : pos] = (((loA >> 29) & 1u) ? -totA : totA) + 0.0;   // + 0.0: never store -0
-                }
-                if (slotB < cnt && blB < bpr) {
-                    const uint32_t pos = pos0 + idxB;
-                    out[order ? __ldg(order + pos) : pos] = (((loB >> 29) & 1u) ? -totB : totB) + 0.0;
-                }
+                // store unless past the end of the item or the bin is staged in another round; + 0.0: never store -0
+                if (slotA < cnt && blA < bpr) out[pos0 + idxA] = (((loA >> 29) & 1u) ? -totA : totA) + 0.0;
+                if (slotB < cnt && blB < bpr) out[pos0 + idxB] = (((loB >> 29) & 1u) ? -totB : totB) + 0.0;
             }
         }
     }
 }
 
 __global__ void __launch_bounds__(128) k_transform2(Tables T, long long n, const unsigned long long* __restrict__ recs,
-                                                   const uint32_t* __restrict__ order, double* __restrict__ out)
+                                                   double* __restrict__ out)
 {
     const long long pos = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const bool valid = pos < n;
@@ -962,7 +965,7 @@ __global__ void __launch_bounds__(128) k_transform2(Tables T, long long n, const
                                          : (((dk.x >> 24) & 1) ? 1.4142135623730951 : 1.0);
         if (mine) result = (((rec >> 36) & 1) ? -(norm * total) : norm * total) + 0.0;
     }
-    if (valid) out[order ? (long long)__ldg(order + pos) : pos] = result;
+    if (valid) out[pos] = result;
 }
 
 size_t align256(size_t x) { return (x + 255) & ~size_t(255); }
@@ -1065,13 +1068,13 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
                                                                            invalid_bucket, itm, last_slot, cnt);
             if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.b, st));
             const unsigned grid = (unsigned)std::min<long long>(max_items, (long long)c->num_sms * 6);
-            k_transform3<<<grid, TR_THREADS, 0, st>>>(c->t, itm, cnt, trecs, nullptr, tout);
+            k_transform3<<<grid, TR_THREADS, 0, st>>>(c->t, itm, cnt, trecs, tout);
             const unsigned grid_s = (unsigned)std::min<long long>((std::min<long long>(n, n_buckets) + 3) / 4, (long long)c->num_sms * 16);
             k_transform3_small<<<grid_s, 128, 0, st>>>(c->t, itm, last_slot, cnt, trecs, tout);
             c->launches += 3;
         } else {
             if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.b, st));
-            k_transform2<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(c->t, n, trecs, nullptr, tout);
+            k_transform2<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(c->t, n, trecs, tout);
             c->launches += 1;
         }
         if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.d, st));
