@@ -755,6 +755,25 @@ __global__ void __launch_bounds__(TR_THREADS, 6) k_transform3(Tables T, const ui
                 }
             }
         }
+        // group descriptors: loads issued here, used by warp 0 after its share of the histogram pass (their two
+        // dependent latencies overlap that pass instead of extending the B0 -> B1 phase)
+        int4 kb = make_int4(0, 0, 0, 0), kk = kb;
+        uint2 sg = make_uint2(0u, 0u);
+        int2 jb = make_int2(0, 0), jk = make_int2(0, 0);
+        int gJlo = 0, gnblk = 0;
+        if (tid < 32) {
+            const uint32_t tb = g / nt, tk = g - tb * nt;
+            kb = __ldg(T.tk3 + tb);
+            kk = __ldg(T.tk3 + tk);
+            sg = __ldg(T.sgrp3 + g);
+            const int Jminb = (kb.w >> 16) & 255, Jmink = (kk.w >> 16) & 255;
+            gJlo = max(Jminb, Jmink);
+            gnblk = ((min((kb.w >> 24) & 255, (kk.w >> 24) & 255) - gJlo) >> 1) + 1;
+            if (tid < gnblk) {
+                jb = __ldg(T.jinfo3 + kb.z + ((gJlo - Jminb) >> 1) + tid);
+                jk = __ldg(T.jinfo3 + kk.z + ((gJlo - Jmink) >> 1) + tid);
+            }
+        }
         __syncthreads();   // B0: the previous item is finished, shared state may be overwritten
         {   // (1) histogram over iM (each record keeps its rank inside its iM bucket), mask of the isospin bins present
             uint32_t bits = 0u;
@@ -785,14 +804,6 @@ __global__ void __launch_bounds__(TR_THREADS, 6) k_transform3(Tables T, const ui
             if (lane == 0 && bits) atomicOr(&sh.mask, bits);
         }
         if (tid < 32) {   // warp 0: item scalars and J-block descriptors
-            const uint32_t tb = g / nt, tk = g - tb * nt;
-            const int4 kb = __ldg(T.tk3 + tb), kk = __ldg(T.tk3 + tk);
-            const int Jminb = (kb.w >> 16) & 255, Jmink = (kk.w >> 16) & 255;
-            const int Jlo = max(Jminb, Jmink), Jhi = min((kb.w >> 24) & 255, (kk.w >> 24) & 255);
-            const int nblk = ((Jhi - Jlo) >> 1) + 1;
-            const int qb = kb.z + ((Jlo - Jminb) >> 1), qk = kk.z + ((Jlo - Jmink) >> 1);
-            int2 jb = make_int2(0, 0), jk = make_int2(0, 0);
-            if (tid < nblk) { jb = __ldg(T.jinfo3 + qb + tid); jk = __ldg(T.jinfo3 + qk + tid); }
             // exclusive prefix sums over the blocks: bra rows, ket rows, Vw doubles
             const uint32_t rb = (uint32_t)jb.y, rk = (uint32_t)jk.y, vv = (uint32_t)(jb.y * row_pitch3(jk.y));
             uint32_t ib = rb, ik = rk, iv = vv;
@@ -801,23 +812,22 @@ __global__ void __launch_bounds__(TR_THREADS, 6) k_transform3(Tables T, const ui
                 uint32_t xb = __shfl_up_sync(0xFFFFFFFFu, ib, off), xk = __shfl_up_sync(0xFFFFFFFFu, ik, off), xv = __shfl_up_sync(0xFFFFFFFFu, iv, off);
                 if (lane >= off) { ib += xb; ik += xk; iv += xv; }
             }
-            if (tid < nblk) {
+            if (tid < gnblk) {
                 // dispatch code: 0..15 fully unrolled (nb, nk <= 4); 16 + nk row-loop templates (nk <= 8); 25 generic
                 const uint32_t code = (rb - 1u < 4u && rk - 1u < 4u) ? (rb - 1u) * 4u + (rk - 1u) : (rk - 1u < 8u && rb > 0u) ? 16u + rk : 25u;
                 sh.desc[tid] = (unsigned long long)(rb | (rk << 8) | ((ib - rb) << 16) | ((ik - rk) << 24)) |
                                ((unsigned long long)((iv - vv) | (code << 16)) << 32);
             }
             if (tid == 0) {
-                const uint2 sg = __ldg(T.sgrp3 + g);
                 sh.sc[0] = (uint32_t)kb.y;
                 sh.sc[1] = (uint32_t)kk.y;
                 sh.sc[2] = (uint32_t)kb.x + (uint32_t)jb.x * (uint32_t)kb.y;
                 sh.sc[3] = (uint32_t)kk.x + (uint32_t)jk.x * (uint32_t)kk.y;
-                sh.sc[4] = ((uint32_t)kb.w & 0xFFu) | ((uint32_t)Jlo << 8) | ((uint32_t)nblk << 16);
+                sh.sc[4] = ((uint32_t)kb.w & 0xFFu) | ((uint32_t)gJlo << 8) | ((uint32_t)gnblk << 16);
                 sh.sc[5] = sg.y;
                 sh.sc[6] = sg.x;
             }
-            if (tid == nblk - 1) sh.sc[7] = ib | (ik << 8);   // rows of the common J range: bra | ket<<8
+            if (tid == gnblk - 1) sh.sc[7] = ib | (ik << 8);   // rows of the common J range: bra | ket<<8
         }
         __syncthreads();   // B1: histogram, mask, descriptors complete
         const uint32_t mask = sh.mask;
