@@ -601,7 +601,7 @@ struct ItemShared {
     double w[NBIN3 * NISO3];
     uint32_t sc[8];
     uint32_t hist[NM_MAX + 1];               // records per iM
-    uint32_t soff[NM_MAX + 1];
+    uint32_t soff[TR_THREADS / 32][NM_MAX + 1];   // every warp keeps its own copy of the scanned histogram
     uint32_t mask;
     uint16_t sidx[ITEM3];                    // position in the item of the record in M-sorted slot i
     uint16_t srank[ITEM3];                   // per record: iM<<10 | rank among the item's records of equal iM
@@ -839,7 +839,8 @@ __global__ void __launch_bounds__(TR_THREADS, 6) k_transform3(Tables T, const ui
         const uint32_t bpr = min((uint32_t)NBIN3, (uint32_t)VW_CAP / vstride);   // bins per round
         const uint32_t inv = 0xFFFFFFFFu / gsize + 1u;
         const double* __restrict__ slab = T.slab3 + (size_t)s1.z * 2;
-        if (tid < 32) {   // warp 0: exclusive scan of the iM histogram -> cursors, then clear it for the next item
+        uint32_t* soff = sh.soff[tid >> 5];
+        {   // every warp: exclusive scan of the iM histogram into its own cursor array (no block barrier needed before (2b))
             const uint32_t a = sh.hist[2 * lane], b = sh.hist[2 * lane + 1];
             uint32_t incl = a + b;
 #pragma unroll
@@ -847,11 +848,9 @@ __global__ void __launch_bounds__(TR_THREADS, 6) k_transform3(Tables T, const ui
                 uint32_t x = __shfl_up_sync(0xFFFFFFFFu, incl, off);
                 if (lane >= off) incl += x;
             }
-            sh.soff[2 * lane] = incl - a - b;
-            sh.soff[2 * lane + 1] = incl - b;
-            sh.hist[2 * lane] = 0u;
-            sh.hist[2 * lane + 1] = 0u;
-            if (lane == 0) sh.hist[NM_MAX] = 0u;
+            soff[2 * lane] = incl - a - b;
+            soff[2 * lane + 1] = incl - b;
+            __syncwarp();
         }
         bool first = true;
         for (uint32_t b0 = 0; b0 < (uint32_t)NBIN3; b0 += bpr) {
@@ -870,16 +869,20 @@ __global__ void __launch_bounds__(TR_THREADS, 6) k_transform3(Tables T, const ui
                     sh.vw[bl * vstride + c] = v;
                 }
             }
-            if (first) {
-                __syncthreads();   // B2: cursors ready; every thread has read the mask
-                if (tid == 0) sh.mask = 0u;
-                for (uint32_t idx = tid; idx < cnt; idx += TR_THREADS) {   // M-sorted order of the records
+            const bool was_first = first;
+            if (first) {   // (2b) M-sorted order of the records (a thread reads the ranks it wrote itself)
+                for (uint32_t idx = tid; idx < cnt; idx += TR_THREADS) {
                     const uint32_t kr = sh.srank[idx];
-                    sh.sidx[sh.soff[kr >> 10] + (kr & 1023u)] = (uint16_t)idx;
+                    sh.sidx[soff[kr >> 10] + (kr & 1023u)] = (uint16_t)idx;
                 }
                 first = false;
             }
-            __syncthreads();   // B3: Vw and the sorted order are in place
+            __syncthreads();   // B3: Vw and the sorted order are in place; every warp has read the histogram and the mask
+            if (was_first && tid < 32) {   // clear them for the next item (its atomics come after its B0)
+                sh.hist[2 * lane] = 0u;
+                sh.hist[2 * lane + 1] = 0u;
+                if (lane == 0) { sh.hist[NM_MAX] = 0u; sh.mask = 0u; }
+            }
             // (3) evaluate.  Warp-uniform loop over pairs of 32 sorted slots: lane l takes slots base+l (A) and base+32+l
             //     (B); lanes past the end of the item redo its last record and skip the store.
             for (uint32_t base = (uint32_t)(tid & ~31) * 2u; base < cnt; base += 2u * TR_THREADS) {
