@@ -74,10 +74,11 @@ int mfdn_cg_download(mfdn_ctx*, int stage, double* host_out, int64_t cap, int64_
  * orbital combination).  chan_* have length n_chan; state_* have length sum(chan_dim), listed channel by
  * channel; channel c is a row-major chan_dim[c] x chan_dim[c] fp64 square at values + chan_off[c].
  * Index arrays are HOST; `values` is HOST or DEVICE (values_on_device != 0).  The library copies and
- * re-tiles (group-major, in the order the kernel's nested loops read them); the caller keeps
- * ownership.  Structural rules (else MFDN_ERR_TABLE): orbitals in range and a <= b (<= c); triangle rules;
+ * re-tiles (group-major, in the order the kernel's nested loops read them) and, for 3-body tables,
+ * builds the per-tuple coefficient tables <ja ma jb mb|J12 M12><J12 M12 jc mc|J M>; the caller keeps ownership.  Structural rules (else MFDN_ERR_TABLE): orbitals in range and a <= b (<= c); triangle rules;
  * channel parity = parity of the state's orbitals; a == b only with J+T (2-body) resp. J12+T12 (3-body) odd;
- * 3-body: e_a+e_b+e_c <= e3max, 2T in {1,3}, T12 in {0,1}; no duplicate channel or state.
+ * 3-body: e_a+e_b+e_c <= e3max, 2T in {1,3}, T12 in {0,1}; no duplicate channel or state; (2ja+1)(2jb+1)(2jc+1) <= 4096
+ * for every listed orbital triple (12-bit m-state index of the packed request record).
  * 2-body: chan_J, chan_T are J and T; 3-body: chan_twoJ, chan_twoT are 2J and 2T.  chan_par: 0 even, 1 odd.
  * Synchronises `stream` before returning. */
 int mfdn_coupled_upload_2b(mfdn_ctx*, int32_t n_chan, const int32_t* chan_J, const int32_t* chan_T,
