@@ -268,3 +268,26 @@ def test_full_size_config3_sampled(torch, B, oracle):
     out3, mask3 = ctx.mscheme(d_sorted, flags=B.MFDN_PRESORTED)
     torch.cuda.synchronize()
     assert bool((out3 == out[order]).all()) and bool((mask3 == mask[order]).all())
+
+
+def test_3b_upload_rules(torch, B):
+    """3-body upload validation: a tuple with more than 4096 m-states does not fit the 12-bit state index of the
+    packed record and is refused; a state above E3max is refused; the context stays usable."""
+    b = W.ho_basis(8)
+    ctx = B.mfdn_orbitals_init(0, b.n, b.l, b.twoj, b.sps_orb, b.sps_twom, b.sps_twotz)
+    B.mfdn_cg_build(ctx)
+    big = int(np.argmax(b.twoj))                      # 0k17/2: (2j+1)^3 = 5832 m-states for the triple (big, big, big)
+    assert (int(b.twoj[big]) + 1) ** 3 > 4096
+    one = np.array([1], np.int32)
+    args = dict(chan_twoJ=[17], chan_twoT=[1], chan_par=[0], chan_dim=one, chan_off=np.array([0], np.int64),
+                state_a=[big], state_b=[big], state_c=[big], state_J12=[0], state_T12=[1], values=np.ones(1))
+    with pytest.raises(B.MfdnError) as e:
+        B.mfdn_coupled_upload_3b(ctx, 24, **args)
+    assert e.value.code == B.MFDN_ERR_TABLE
+    with pytest.raises(B.MfdnError) as e:
+        B.mfdn_coupled_upload_3b(ctx, 8, **args)      # e_a + e_b + e_c = 24 > E3max = 8
+    assert e.value.code == B.MFDN_ERR_TABLE
+    small = W.coupled_3b(b, 2, 5)                     # a failed upload leaves the context usable
+    B.mfdn_coupled_upload_3b(ctx, 2, small.chan_twoJ, small.chan_twoT, small.chan_par, small.chan_dim, small.chan_off,
+                             small.state_a, small.state_b, small.state_c, small.state_J12, small.state_T12, small.values)
+    B.mfdn_destroy(ctx)
