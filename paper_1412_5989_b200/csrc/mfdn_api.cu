@@ -346,7 +346,7 @@ extern "C" int mfdn_cg_download(mfdn_ctx* c, int stage, double* host_out, int64_
 struct Retile3 {
     int n_tup;
     const int4* tdesc;
-    const uint2* sgrp;
+    const uint4* sgrp;
     const int32_t* rowmap;
     const int32_t* chan_of;   // [(twoJ>>1)*4 + (twoT>>1)*2 + par]
     const int64_t* chan_off;
@@ -365,7 +365,7 @@ __device__ __forceinline__ void j12_range(int4 d, int twoJ, int& lo, int& hi)
 __global__ void k_retile3(Retile3 p)
 {
     for (long long g = blockIdx.x; g < (long long)p.n_tup * p.n_tup; g += gridDim.x) {
-        uint2 sg = p.sgrp[g];
+        uint4 sg = p.sgrp[g];
         if (sg.x == NO_SLAB) continue;
         const int gsize = (int)sg.y;
         int tb = (int)(g / p.n_tup), tk = (int)(g % p.n_tup);
@@ -400,6 +400,34 @@ __global__ void k_retile3(Retile3 p)
             }
             dst += (size_t)nb * pitch;
         }
+    }
+}
+
+// Isospin-combined slabs (A2; layout: vw_stride in mfdn_internal.cuh): the paper's "isospin loops ... unrolled into a
+// single weighted summation" done once per (group, isospin bin, cell) at upload instead of once per
+// request.  Same operation order as the kernels that sum the five planes themselves (k_transform3_small,
+// k_mscheme_naive use w0*p0, then fma over s = 1..4), so a value does not depend on the path its group takes.
+__global__ void k_vw20(long long n_groups, const uint4* __restrict__ sgrp, const double* __restrict__ slab,
+                       const double* __restrict__ wbin, uint32_t* __restrict__ vw20)
+{
+    for (long long g = blockIdx.x; g < n_groups; g += gridDim.x) {
+        const uint4 sg = sgrp[g];
+        if (sg.x == NO_SLAB) continue;
+        const uint32_t gsize = sg.y, S = vw_stride(gsize);
+        const double* src = slab + (size_t)sg.x * 2;
+        uint32_t* dst = vw20 + (size_t)sg.z * 4;
+        for (uint32_t idx = threadIdx.x; idx < NBIN3 * gsize; idx += blockDim.x) {
+            const uint32_t b = idx / gsize, cell = idx - b * gsize;
+            const double* w = wbin + b * NISO3;
+            double v = w[0] * src[cell];
+            v = fma(w[1], src[gsize + cell], v);
+            v = fma(w[2], src[2 * (size_t)gsize + cell], v);
+            v = fma(w[3], src[3 * (size_t)gsize + cell], v);
+            v = fma(w[4], src[4 * (size_t)gsize + cell], v);
+            dst[(size_t)b * S + cell] = (uint32_t)__double2loint(v);
+            dst[(size_t)b * S + gsize + cell] = (uint32_t)__double2hiint(v);
+        }
+        for (uint32_t b = threadIdx.x; b < NBIN3; b += blockDim.x) dst[(size_t)b * S + 2 * gsize] = 0u;
     }
 }
 
@@ -641,12 +669,23 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
         dtab_len = (dtab_len + 1) & ~1ull;
     }
     // ---- group descriptors: slab offset (16-byte units) and plane size, rows in loop order J, J12
-    std::vector<uint2> sgrp((size_t)nt * nt, uint2{NO_SLAB, 0u});
+    //      and the (group, M) buckets of the request sort: every same-parity group owns one bucket per common M
+    std::vector<uint4> sgrp((size_t)nt * nt, uint4{NO_SLAB, 0u, 0u, 0u});
+    std::vector<uint32_t> gbase((size_t)nt * nt + 1, 0u);
     uint64_t cells = 0;   // in 16-byte units
+    uint64_t vwcells = 0; // 16-byte units of the isospin-combined slabs
+    uint64_t buckets = 0;
     for (int tb = 0; tb < nt; tb++)
         for (int tkk = 0; tkk < nt; tkk++) {
             int4 db = tdesc[tb], dk = tdesc[tkk];
+            gbase[(size_t)tb * nt + tkk] = (uint32_t)buckets;
             if (((db.x ^ dk.x) >> 25) & 1) continue;
+            {
+                const int sb = (db.x & 255) + ((db.x >> 8) & 255) + ((db.x >> 16) & 255);
+                const int sk = (dk.x & 255) + ((dk.x >> 8) & 255) + ((dk.x >> 16) & 255);
+                buckets += (uint64_t)std::min(sb, sk) + 1;
+                if (buckets >= (uint64_t)REC_INVALID) return fail(c, MFDN_ERR_OOM, "too many (group, M) buckets for 27-bit sort keys");
+            }
             int Jlo = std::max((db.y >> 16) & 255, (dk.y >> 16) & 255), Jhi = std::min((db.y >> 24) & 255, (dk.y >> 24) & 255);
             uint64_t gsize = 0;
             for (int twoJ = Jlo; twoJ <= Jhi; twoJ += 2) {
@@ -656,10 +695,14 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
                 if (hb >= lb && hk >= lk) gsize += (uint64_t)(hb - lb + 1) * row_pitch3(hk - lk + 1);
             }
             if (gsize == 0) continue;
-            if (cells + gsize * NISO3 / 2 >= 0xFFFFFFF0ull) return fail(c, MFDN_ERR_OOM, "table too large for 32-bit slab offsets");
-            sgrp[(size_t)tb * nt + tkk] = uint2{(uint32_t)cells, (uint32_t)gsize};
+            const uint64_t vw16 = ((uint64_t)NBIN3 * vw_stride((uint32_t)gsize) + 3) / 4;   // 16-byte units, rounded up
+            if (cells + gsize * NISO3 / 2 >= 0xFFFFFFF0ull || vwcells + vw16 >= 0xFFFFFFF0ull)
+                return fail(c, MFDN_ERR_OOM, "table too large for 32-bit slab offsets");
+            sgrp[(size_t)tb * nt + tkk] = uint4{(uint32_t)cells, (uint32_t)gsize, (uint32_t)vwcells, 0u};
             cells += gsize * NISO3 / 2;
+            vwcells += vw16;
         }
+    gbase[(size_t)nt * nt] = (uint32_t)buckets;
     // ---- one arena for the resident index tables, one for the upload-only ones
     Arena res, tmp;
     // (a,b) -> tuple map: the sorted tuple list keeps the tuples of one (a,b) together with ascending c; if every such run
@@ -678,6 +721,7 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     std::vector<int4> tdesc_rt = tdesc;   // run-time copy: w = start of the tuple's sigma table (the row-map offset is upload-only)
     for (int t = 0; t < nt; t++) tdesc_rt[t].w = sigoff[t];
     size_t o_tid = res.add(tuple_id), o_desc_rt = res.add(tdesc_rt), o_sgrp = res.add(sgrp), o_sm = res.add(stmask);
+    size_t o_gbase = res.add(gbase);
     size_t o_desc = tmp.add(tdesc), o_ab = res.add(ab);
     size_t o_tk = res.add(tk), o_jinfo = res.add(jinfo), o_sig = res.add(sig), o_sigoff = res.add(sigoff);
     std::vector<int64_t> coff(chan_off, chan_off + n_chan);
@@ -698,18 +742,22 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     cudaError_t e = cudaMalloc(&dslab, std::max<uint64_t>(cells, 1) * 16 + 256);
     void* ddtab = nullptr;
     if (e == cudaSuccess) e = cudaMalloc(&ddtab, (dtab_len + 2 * MAX_STATES3) * sizeof(double));   // slack: a mis-ordered MFDN_PRESORTED stream may index past a tuple
+    void* dvw = nullptr;
+    if (e == cudaSuccess) e = cudaMalloc(&dvw, std::max<uint64_t>(vwcells, 1) * 16 + 256);        // slack: bulk copies are rounded up to 16 bytes
     if (e != cudaSuccess) {
         cudaFree(dtmp);
         if (vtmp) cudaFree(vtmp);
         if (dslab) cudaFree(dslab);
-        return cuda_fail(c, e, "cudaMalloc(slab3/dtab3)");
+        if (ddtab) cudaFree(ddtab);
+        return cuda_fail(c, e, "cudaMalloc(slab3/dtab3/vw20)");
     }
     c->owned.push_back(dslab);
     c->owned.push_back(ddtab);
+    c->owned.push_back(dvw);
     Retile3 p;
     p.n_tup = nt;
     p.tdesc = (const int4*)((char*)dtmp + o_desc);
-    p.sgrp = (const uint2*)(dres + o_sgrp);
+    p.sgrp = (const uint4*)(dres + o_sgrp);
     p.rowmap = (const int32_t*)((char*)dtmp + o_rm);
     p.chan_of = (const int32_t*)((char*)dtmp + o_cof);
     p.chan_off = (const int64_t*)((char*)dtmp + o_coff);
@@ -718,6 +766,7 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     p.slab = (double*)dslab;
     long long groups = (long long)nt * nt;
     k_retile3<<<(unsigned)std::min<long long>(groups, 1 << 20), 64, 0, st>>>(p);
+    k_vw20<<<(unsigned)std::min<long long>(groups, 1 << 20), 128, 0, st>>>(groups, p.sgrp, (const double*)dslab, c->t.wbin3, (uint32_t*)dvw);
     Dtab3 q;
     q.tdesc = p.tdesc;
     q.tk = (const int4*)(dres + o_tk);
@@ -742,6 +791,10 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     c->t.tuple_id3 = (const int32_t*)(dres + o_tid);
     c->t.tdesc3 = (const int4*)(dres + o_desc_rt);
     c->t.sgrp3 = p.sgrp;
+    c->t.gbase3 = (const uint32_t*)(dres + o_gbase);
+    c->t.n_buckets3 = (uint32_t)buckets;
+    c->t.vw20 = (const uint32_t*)dvw;
+    c->vw_bytes3 = (int64_t)(vwcells * 16);
     c->t.ab3 = ab_dense ? (const int2*)(dres + o_ab) : nullptr;
     c->t.slab3 = (const double*)dslab;
     c->t.stmask3 = (const unsigned long long*)(dres + o_sm);
@@ -911,6 +964,8 @@ extern "C" int64_t mfdn_info(mfdn_ctx* c, int which)
         case 5: return c->n_cg2;
         case 6: return c->launches;
         case 7: return c->dtab_bytes3;
+        case 8: return c->vw_bytes3;
+        case 9: return c->t.n_buckets3;
         default: return -1;
     }
 }

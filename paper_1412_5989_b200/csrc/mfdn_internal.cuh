@@ -45,7 +45,15 @@ constexpr int CG_GUARD = 8192;     // zero doubles before and after the stage-2 
 // not listed.  The isospin-combined copy Vw = sum_s w[s] * plane[s] that the transform stages in shared memory has
 // the same indexing.
 __host__ __device__ inline int row_pitch3(int nk) { return (nk + 1) & ~1; }
-constexpr int ITEM3 = 1024;        // max records per work item of the 3-body transform (one group per item)
+constexpr int ITEM3 = 512;         // max records per work item of the 3-body transform (one group per item)
+// Isospin-combined slabs (A2): for every group and every isospin bin the weighted plane sum Vw[cell] =
+// sum_s w[bin][s] * plane_s[cell], precomputed at upload so that staging it is a pure bulk copy.  The two 32-bit
+// halves of a value live in separate word planes: bin b occupies vw_stride(gsize) 32-bit words, low words at
+// [0, gsize), high words at [gsize, 2*gsize), one pad word.  The stride is ODD, so the 20 bins of one cell fall
+// into 20 different shared-memory banks: a warp whose lanes sit in any mixture of bins reads a cell with two
+// conflict-free 32-bit loads (measured: 2.0 cycles per cell against 3.7 for 64-bit loads over 20 random bins).
+__host__ __device__ inline uint32_t vw_stride(uint32_t gsize) { return 2u * gsize + 1u; }
+constexpr int VW_WORDS = 5120;     // 32-bit words of one staged slab (20 KB): all 20 bins of a group with gsize <= 127
 constexpr uint32_t ZERO_ITEM = 0xFFFFFFFFu;   // work item whose records all have value 0 (no slab / failed S1-S6)
 
 // ---- packed canonical request record (H1 output), 64 bit --------------------------------------------
@@ -53,7 +61,7 @@ constexpr uint32_t ZERO_ITEM = 0xFFFFFFFFu;   // work item whose records all hav
 //         [36] 1 = odd permutation (sign -1)                     [37,64) group key, REC_INVALID if S1-S6 fail
 // 3-body: [0,12) sigma_b  [12,24) sigma_k : index of the bra / ket m-state in its tuple's coefficient table (M-major)
 //         [24,29) isospin bin   [29] 1 = odd permutation   [30,36) iM = ima+imb+imc of the bra (M = iM - (ja+jb+jc)/2)
-//         [37,64) group key
+//         [37,64) sort key: 2-body bra_tuple*n_tup+ket_tuple; 3-body the (group, M) bucket gbase3[group] + iM - iMmin
 constexpr unsigned REC_KEY_SHIFT = 37;
 constexpr uint32_t REC_INVALID = 0x7FFFFFFu;
 constexpr int MAX_STATES3 = 4096;   // (ja+1)(jb+1)(jc+1) of a tuple must fit the 12-bit sigma fields
@@ -90,8 +98,13 @@ struct Tables {
     const int32_t* tuple_id3;      // [n_orb^3] -> tuple or -1
     const int2* ab3;               // [n_orb^2] {first tuple of (a,b,*), cmin | count<<16} if every (a,b) has a dense c range, else NULL
     const int4* tdesc3;
-    const uint2* sgrp3;            // [n_tup3^2] {start of the group's slab in 16-byte units or NO_SLAB, doubles per plane}
+    const uint4* sgrp3;            // [n_tup3^2] {start of the group's slab in 16-byte units or NO_SLAB, doubles per plane,
+                                   //              start of its isospin-combined slabs in vw20 in 16-byte units, -}
+    const uint32_t* gbase3;        // [n_tup3^2 + 1] first (group, M) bucket of a group; same-parity groups own
+                                   //              min(ja+jb+jc, jd+je+jf) + 1 buckets (one per common M), the others none
+    uint32_t n_buckets3;           // = gbase3[n_tup3^2]; bucket n_buckets3 collects the requests failing S1-S6
     const double* slab3;
+    const uint32_t* vw20;          // isospin-combined slabs, split word planes (see vw_stride)
     const unsigned long long* stmask3;
     const int4* tk3;               // [n_tup3] see above
     const int2* jinfo3;            // per (tuple, J): {first row of this J (tuple-relative, loop order J, J12), number of rows}
@@ -121,9 +134,10 @@ struct mfdn_ctx {
     std::vector<uint32_t> h_sps_rec;
     std::vector<void*> owned;  // device allocations
     int64_t n_cg1 = 0, n_cg2 = 0;
-    int64_t slab_bytes2 = 0, slab_bytes3 = 0, dtab_bytes3 = 0;
+    int64_t slab_bytes2 = 0, slab_bytes3 = 0, dtab_bytes3 = 0, vw_bytes3 = 0;
     int64_t launches = 0;
     int num_sms = 148;
+    int tr_blocks_per_sm = 0;   // resident k_transform3 blocks per SM (occupancy query at the first call)
     // measurement hooks
     bool profile = false;
     struct EvTriple { cudaEvent_t a, b, d, c; bool has_sort; };   // start | transform kernel start | its end | end of call

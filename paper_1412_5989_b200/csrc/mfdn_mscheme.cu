@@ -174,7 +174,7 @@ __device__ __forceinline__ double eval3_naive(const Tables& T, const Side3& B, c
 {
     mask = 0;
     if (!select3(T, B, K)) return 0.0;
-    const uint2 sg = __ldg(T.sgrp3 + (size_t)B.tup * T.n_tup3 + K.tup);
+    const uint4 sg = __ldg(T.sgrp3 + (size_t)B.tup * T.n_tup3 + K.tup);
     if (sg.x == NO_SLAB) return 0.0;
     const int4 db = __ldg(T.tdesc3 + B.tup), dk = __ldg(T.tdesc3 + K.tup);
     if (!mask3(T, B, K, db, dk)) return 0.0;
@@ -331,8 +331,12 @@ __global__ void __launch_bounds__(256) k_keys(Tables T, long long n, const int32
         } else if (BODY == 3) {
             Side3 B = decode3<SMEM>(T, sps, ab, s[0], s[1], s[2]), K = decode3<SMEM>(T, sps, ab, s[3], s[4], s[5]);
             if (select3(T, B, K)) {
-                key = (uint32_t)B.tup * T.n_tup3 + K.tup;
                 const int4 db = __ldg(T.tdesc3 + B.tup), dk = __ldg(T.tdesc3 + K.tup);
+                {   // sort key = (group, M) bucket: the group's first bucket + index of M in the common M range
+                    const int sjb = (db.x & 255) + ((db.x >> 8) & 255) + ((db.x >> 16) & 255);
+                    const int sjk = (dk.x & 255) + ((dk.x >> 8) & 255) + ((dk.x >> 16) & 255);
+                    key = __ldg(T.gbase3 + (size_t)B.tup * T.n_tup3 + K.tup) + (uint32_t)(B.ima + B.imb + B.imc - ((sjb - min(sjb, sjk)) >> 1));
+                }
                 mask = mask3(T, B, K, db, dk);
                 const int jb1 = ((db.x >> 8) & 255) + 1, jc1 = ((db.x >> 16) & 255) + 1;
                 const int je1 = ((dk.x >> 8) & 255) + 1, jf1 = ((dk.x >> 16) & 255) + 1;
@@ -479,26 +483,47 @@ __global__ void __launch_bounds__(256) k_unpermute(long long n, const double* __
     }
 }
 
-// Work items (H3): one item = up to ITEM3 consecutive records of ONE group in the group-ordered stream, so that a
-// thread block shares every loop bound, table row and the group's slab.  `bounds[b]` is the END of bucket b after the
-// scatter (ends = 1: the cursor array) or its START for pre-sorted input (ends = 0: the scanned histogram).
-// Groups with at most SMALL_ITEM3 records go to a second list (filled from the END of the item array, counted in
-// n_items[1]): for them the per-item prologue of k_transform3 (block-wide staging, M sort) costs more than it saves, a
-// single warp evaluates them directly (k_transform3_small).
+// Work items (H3): one item = up to ITEM3 consecutive records of ONE group in the (group, M)-ordered stream, so that
+// a thread block shares every loop bound, table row and the group's slab.  One thread per group (plus one for the
+// bucket of the requests failing S1-S6): the group's records are the buckets [gbase[g], gbase[g+1]).  `bounds[b]` is
+// the END of bucket b after the scatter (ends = 1: the cursor array) or its START for pre-sorted input (ends = 0: the
+// scanned histogram).  item = {first position, records, group | ZERO_ITEM, first isospin bin | bins << 8}: a group
+// whose 20 isospin-combined slabs exceed one stage (VW_WORDS) is evaluated in rounds over bin ranges, one item per
+// (chunk, round); a record is evaluated by the round that holds its bin.
+// Groups with at most SMALL_ITEM3 records -- and groups whose slab does not fit a stage even four bins at a time -- go
+// to a second list (filled from the END of the item array, counted in n_items[1]): a single warp evaluates them
+// directly from the five isospin planes (k_transform3_small; no capacity limit).
 constexpr uint32_t SMALL_ITEM3 = 64;
-__global__ void __launch_bounds__(256) k_items3(const uint32_t* __restrict__ bounds, uint32_t n_buckets, int ends, uint32_t n,
-                                               const uint2* __restrict__ sgrp, uint32_t invalid_bucket,
-                                               uint4* __restrict__ items, uint32_t last_slot, uint32_t* __restrict__ n_items)
+__device__ __forceinline__ uint32_t bins_per_round3(uint32_t gsize)
 {
-    const uint32_t b = blockIdx.x * 256u + threadIdx.x;
-    uint32_t start = 0, end = 0;
-    if (b < n_buckets) {
-        if (ends) { end = bounds[b]; start = b ? bounds[b - 1] : 0u; }
-        else { start = bounds[b]; end = (b + 1 < n_buckets) ? bounds[b + 1] : n; }
+    const uint32_t b = ((uint32_t)VW_WORDS / vw_stride(gsize)) & ~3u;   // multiple of 4: every round starts 16-byte aligned
+    return min(b, (uint32_t)NBIN3);
+}
+__global__ void __launch_bounds__(256) k_items3(const uint32_t* __restrict__ bounds, const uint32_t* __restrict__ gbase,
+                                               uint32_t n_groups, uint32_t n_buckets, int ends, uint32_t n,
+                                               const uint4* __restrict__ sgrp, uint4* __restrict__ items, uint32_t last_slot,
+                                               uint32_t* __restrict__ n_items)
+{
+    const uint32_t g = blockIdx.x * 256u + threadIdx.x;   // g == n_groups: the bucket of the invalid requests
+    uint32_t start = 0, end = 0, gsize = 0;
+    bool zero = true;
+    if (g <= n_groups) {
+        const uint32_t b0 = g < n_groups ? __ldg(gbase + g) : n_buckets - 1u, b1 = g < n_groups ? __ldg(gbase + g + 1) : n_buckets;
+        if (b1 > b0) {
+            if (ends) { start = b0 ? bounds[b0 - 1] : 0u; end = bounds[b1 - 1]; }
+            else { start = bounds[b0]; end = b1 < n_buckets ? bounds[b1] : n; }
+        }
+        if (end > start && g < n_groups) {
+            const uint4 sg = __ldg(sgrp + g);
+            zero = sg.x == NO_SLAB;
+            gsize = sg.y;
+        }
     }
     const uint32_t cnt = end - start;
-    const bool small = cnt <= SMALL_ITEM3;
-    const uint32_t k = small ? 0u : (cnt + ITEM3 - 1) / ITEM3, ks = (small && cnt) ? 1u : 0u;
+    const uint32_t bpr = zero ? (uint32_t)NBIN3 : bins_per_round3(gsize);
+    const bool small = cnt <= SMALL_ITEM3 || bpr == 0u;
+    const uint32_t rounds = small ? 0u : (NBIN3 + bpr - 1u) / bpr;
+    const uint32_t k = small ? 0u : ((cnt + ITEM3 - 1) / ITEM3) * rounds, ks = (small && cnt) ? 1u : 0u;
     // warp-aggregated append: the lists stay (nearly) in group order, neighbours share the bra tuple's tables
     const int lane = threadIdx.x & 31;
     uint32_t incl = k, incs = ks;
@@ -513,13 +538,15 @@ __global__ void __launch_bounds__(256) k_items3(const uint32_t* __restrict__ bou
     base = __shfl_sync(0xFFFFFFFFu, base, 31);
     bases = __shfl_sync(0xFFFFFFFFu, bases, 31);
     if (cnt == 0) return;
-    const uint32_t g = (b == invalid_bucket || sgrp[b].x == NO_SLAB) ? ZERO_ITEM : b;
+    const uint32_t gz = zero ? ZERO_ITEM : g;
     if (small) {
-        items[last_slot - (bases + incs - 1u)] = make_uint4(start, cnt, g, 0u);
+        items[last_slot - (bases + incs - 1u)] = make_uint4(start, cnt, gz, 0u);
         return;
     }
     uint32_t slot = base + incl - k;
-    for (uint32_t j = 0; j < k; j++) items[slot + j] = make_uint4(start + j * ITEM3, min((uint32_t)ITEM3, cnt - j * ITEM3), g, 0u);
+    for (uint32_t j = 0; j * ITEM3 < cnt; j++)
+        for (uint32_t r = 0; r < rounds; r++)
+            items[slot++] = make_uint4(start + j * ITEM3, min((uint32_t)ITEM3, cnt - j * ITEM3), gz, (r * bpr) | (min(bpr, NBIN3 - r * bpr) << 8));
 }
 
 // H3-H6 for small groups: one warp per item, lane = record.  The group's loop bounds, table rows and slab addresses
@@ -544,7 +571,7 @@ __global__ void __launch_bounds__(128) k_transform3_small(Tables T, const uint4*
         }
         const uint32_t tb = g / nt, tk = g - tb * nt;
         const int4 kb = __ldg(T.tk3 + tb), kk = __ldg(T.tk3 + tk);
-        const uint2 sg = __ldg(T.sgrp3 + g);
+        const uint4 sg = __ldg(T.sgrp3 + g);
         const int Jminb = (kb.w >> 16) & 255, Jmink = (kk.w >> 16) & 255;
         const int Jlo = max(Jminb, Jmink), Jhi = min((kb.w >> 24) & 255, (kk.w >> 24) & 255);
         const int nblk = ((Jhi - Jlo) >> 1) + 1;
@@ -590,35 +617,66 @@ __global__ void __launch_bounds__(128) k_transform3_small(Tables T, const uint4*
     }
 }
 
-constexpr int TR_THREADS = 128;
-constexpr int VW_CAP = 2048;                 // doubles: isospin-combined slabs Vw[bin][cell] of the current item (16 KB)
-constexpr int MAX_JBLK = 32;                 // common J values of a group (2J <= 63)
-constexpr int NM_MAX = 64;                   // iM = ima+imb+imc < 64 (3*MAX_TWOJ = 63)
+// ------------------------------------------------------------------------------- H3-H6, pipelined transform
+// mbarrier / bulk-copy (TMA, 1-D) primitives
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* b, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* b)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_tx(unsigned long long* b, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* b, uint32_t parity)
+{
+    const uint32_t a = smem_u32(b);
+    uint32_t ok;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, unsigned long long* b)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(b)) : "memory");
+}
 
-struct ItemShared {
-    double vw[VW_CAP];
-    unsigned long long desc[MAX_JBLK];       // per J block: nb | nk<<8 | rows_b before<<16 | rows_k before<<24 | Vw doubles before<<32 | dispatch code<<48
-    double w[NBIN3 * NISO3];
-    uint32_t sc[8];
-    uint32_t hist[NM_MAX + 1];               // records per iM
-    uint32_t soff[TR_THREADS / 32][NM_MAX + 1];   // every warp keeps its own copy of the scanned histogram
-    uint32_t mask;
-    uint16_t sidx[ITEM3];                    // position in the item of the record in M-sorted slot i
-    uint16_t srank[ITEM3];                   // per record: iM<<10 | rank among the item's records of equal iM
+constexpr int TR_CW = 4;                        // consumer warps per block
+constexpr int TR_THREADS = (TR_CW + 1) * 32;    // + one producer warp
+constexpr int TR_STAGES = 2;
+constexpr int MAX_JBLK = 32;                    // common J values of a group (2J <= 63)
+constexpr int BATCH3 = 64;                      // records per consumer-warp batch (two per lane)
+
+// One pipeline stage = everything the consumer warps need for one work item: its isospin-combined slabs and its records
+// (both landed by bulk copies), the J-block descriptors and the group's scalars (written by the producer warp).
+struct __align__(16) Stage3 {
+    uint32_t vw[VW_WORDS];
+    unsigned long long rec[ITEM3 + 2];          // copied from an even position: one record of slack at either end
+    uint4 desc[MAX_JBLK];                       // per J block: {nb | nk<<8 | dispatch code<<16, bra rows before, ket rows before, Vw cells before}
+    uint32_t sc[16];                            // item scalars, see SC_*
+};
+enum { SC_POS0, SC_CNT, SC_GROUP, SC_SB, SC_SK, SC_PB0, SC_PK0, SC_JINFO, SC_GSIZE, SC_STRIDE, SC_BINS, SC_ROFF, SC_NEXT };
+struct Pipe3 {
+    Stage3 st[TR_STAGES];
+    unsigned long long full[TR_STAGES], empty[TR_STAGES];
 };
 
-// bin stride of Vw: odd, so that with 64-bit loads the 16 lanes of a half warp that sit in 16 different isospin bins
-// hit 16 different bank pairs (ncu: 128-bit loads with an even stride ran at 1.8x their ideal wavefront count)
-__device__ __forceinline__ uint32_t vw_stride(uint32_t gsize) { return gsize | 1u; }
+__device__ __forceinline__ double ldvw(const uint32_t* vw, uint32_t i, uint32_t G) { return __hiloint2double((int)vw[i + G], (int)vw[i]); }
 
-// One J block of the sum for TWO records of the group (A and B, 32 sorted slots apart) with the ket range size NK known
-// at compile time and a run-time loop over the bra rows (blocks with more than 4 rows or columns):
+// One J block of the sum for TWO records of the group (A and B, 32 stream positions apart) with the ket range size NK
+// known at compile time and a run-time loop over the bra rows (blocks with more than 4 rows or columns):
 //   sum_i cb(i) * sum_k ck(k) * Vw[i][k],  cb/ck read from the tuples' coefficient tables (one gather per row),
-// Vw rows (padded to even length) read from shared memory with 128-bit loads.
+// Vw rows (padded to even length) read from the staged word planes.
 template <int NK>
-__device__ __forceinline__ void j_block3x2_rows(const double* __restrict__ dtab, const double* __restrict__ vw, uint32_t& pbA, uint32_t& pkA,
+__device__ __forceinline__ void j_block3x2_rows(const double* __restrict__ dtab, const uint32_t* vw, uint32_t& pbA, uint32_t& pkA,
                                                 uint32_t& pbB, uint32_t& pkB, uint32_t Sb, uint32_t Sk, int nb, uint32_t& viA,
-                                                uint32_t& viB, double& totA, double& totB)
+                                                uint32_t& viB, uint32_t G, double& totA, double& totB)
 {
     constexpr int P = (NK + 1) & ~1;
     double ckA[NK], ckB[NK];
@@ -633,11 +691,11 @@ __device__ __forceinline__ void j_block3x2_rows(const double* __restrict__ dtab,
     for (int i = 0; i < nb; i++) {
         const double cbA = __ldg(dtab + pbA), cbB = __ldg(dtab + pbB);
         pbA += Sb; pbB += Sb;
-        double vA[P], vB[P];
+        double vA[NK], vB[NK];
 #pragma unroll
         for (int k = 0; k < NK; k++) {
-            vA[k] = vw[viA + k];
-            vB[k] = vw[viB + k];
+            vA[k] = ldvw(vw, viA + k, G);
+            vB[k] = ldvw(vw, viB + k, G);
         }
         viA += P; viB += P;
         double accA = ckA[0] * vA[0], accB = ckB[0] * vB[0];
@@ -653,12 +711,12 @@ __device__ __forceinline__ void j_block3x2_rows(const double* __restrict__ dtab,
     totB += tB;
 }
 
-// The same J block for TWO records of the group at once (A and B, 32 sorted slots apart), bra and ket range sizes
-// both known at compile time: every load of the block is issued before the first multiply, the loop control is shared.
+// The same J block with bra and ket range sizes both known at compile time: every load of the block is issued before
+// the first multiply, the loop control is shared by the two records.
 template <int NB, int NK>
-__device__ __forceinline__ void j_block3x2(const double* __restrict__ dtab, const double* __restrict__ vw, uint32_t& pbA, uint32_t& pkA,
+__device__ __forceinline__ void j_block3x2(const double* __restrict__ dtab, const uint32_t* vw, uint32_t& pbA, uint32_t& pkA,
                                            uint32_t& pbB, uint32_t& pkB, uint32_t Sb, uint32_t Sk, uint32_t& viA, uint32_t& viB,
-                                           double& totA, double& totB)
+                                           uint32_t G, double& totA, double& totB)
 {
     constexpr int P = (NK + 1) & ~1;
     double ckA[NK], ckB[NK], cbA[NB], cbB[NB];
@@ -675,11 +733,11 @@ __device__ __forceinline__ void j_block3x2(const double* __restrict__ dtab, cons
     double tA = 0.0, tB = 0.0;
 #pragma unroll
     for (int i = 0; i < NB; i++) {
-        double vA[P], vB[P];
+        double vA[NK], vB[NK];
 #pragma unroll
         for (int k = 0; k < NK; k++) {
-            vA[k] = vw[viA + i * P + k];
-            vB[k] = vw[viB + i * P + k];
+            vA[k] = ldvw(vw, viA + i * P + k, G);
+            vB[k] = ldvw(vw, viB + i * P + k, G);
         }
         double accA = ckA[0] * vA[0], accB = ckB[0] * vB[0];
 #pragma unroll
@@ -697,114 +755,87 @@ __device__ __forceinline__ void j_block3x2(const double* __restrict__ dtab, cons
     totB += tB;
 }
 
-// any ket range size (rare: nk > 6): ket coefficient re-read per cell
-__device__ __noinline__ double j_block3_generic(const double* __restrict__ dtab, const double* vw, uint32_t pb, uint32_t pk, uint32_t Sb,
-                                                uint32_t Sk, int nb, int nk, uint32_t vi)
+// any ket range size (nk > 8): ket coefficient re-read per cell
+__device__ __noinline__ double j_block3_generic(const double* __restrict__ dtab, const uint32_t* vw, uint32_t pb, uint32_t pk, uint32_t Sb,
+                                                uint32_t Sk, int nb, int nk, uint32_t vi, uint32_t G)
 {
     const int P = row_pitch3(nk);
     double total = 0.0;
     for (int i = 0; i < nb; i++) {
         const double cb = __ldg(dtab + pb + (uint32_t)i * Sb);
         double acc = 0.0;
-        for (int k = 0; k < nk; k++) acc = fma(__ldg(dtab + pk + (uint32_t)k * Sk), vw[vi + k], acc);
+        for (int k = 0; k < nk; k++) {
+            const double ck = __ldg(dtab + pk + (uint32_t)k * Sk), v = ldvw(vw, vi + k, G);
+            acc = k ? fma(ck, v, acc) : ck * v;
+        }
         total = fma(cb, acc, total);
         vi += P;
     }
     return total;
 }
 
-// H3-H6.  Persistent blocks walk the item list.  Per item (<= ITEM3 records of one group):
-//  (1) the block histograms the item's records by iM (the bra's, = the ket's, M) and ORs their isospin bins into a mask;
-//      warp 0 meanwhile builds the J-block descriptors of the group;
-//  (2) it stages Vw[bin][cell] = sum_s w[bin][s] * plane_s[cell] for the bins present -- the paper's "isospin loops ...
-//      unrolled into a single weighted summation", done once per (item, bin) instead of once per request --
-//      and builds the M-sorted order of the records: the coefficient tables are M-major, so the 32 gathers of a warp
-//      fall into one or two cache lines on the bra AND on the ket side;
-//  (3) every thread evaluates records in sorted order: three nested loops over J, J12, J12' whose bounds
-//      are shared by the block; lanes differ in their table offsets (sigma), bin and first J block (J >= |M|).
-__global__ void __launch_bounds__(TR_THREADS, 6) k_transform3(Tables T, const uint4* __restrict__ items, const uint32_t* __restrict__ n_items_p,
-                                                             const unsigned long long* __restrict__ recs, double* __restrict__ out)
+// H3-H6.  Persistent blocks walk the item list (item k of a block = list entry blockIdx.x + k * gridDim.x) through a
+// ring of TR_STAGES stages:
+//  * the PRODUCER warp, per item: waits until every consumer warp has left the stage, reads the group's descriptors,
+//    builds the J-block table (bounds of the three nested loops of PAPER.md:61, shared by every record of the group),
+//    and starts two bulk copies (cp.async.bulk -> UBLKCP, completion on the stage's mbarrier): the group's
+//    isospin-combined slabs Vw[bin][cell] and the item's records.  It never touches the data itself, so it runs ahead
+//    of the consumers by TR_STAGES - 1 items and their loads are off the critical path;
+//  * the CONSUMER warps wait for the stage, then claim batches of 64 records (two per lane, stream order).  The stream
+//    is ordered by (group, M) and the coefficient tables are M-major: the lanes of a warp read one or two cache lines
+//    per coefficient on the bra AND on the ket side.  Every lane evaluates
+//        sum_J sum_J12 cb(J12,J) sum_J12' ck(J12',J) Vw[bin][J,J12,J12']
+//    for its records with warp-uniform loop bounds (first J block = the smallest |M| in the warp; coefficients are 0
+//    for J < |M|), and stores the signed value at the record's stream position (coalesced).
+// No block-wide barrier after the prologue.
+__global__ void __launch_bounds__(TR_THREADS, 4) k_transform3(Tables T, const uint4* __restrict__ items, const uint32_t* __restrict__ n_items_p,
+                                                          const unsigned long long* __restrict__ recs, double* __restrict__ out)
 {
-    __shared__ __align__(16) ItemShared sh;
-    const int tid = threadIdx.x, lane = tid & 31;
-    for (int i = tid; i < NBIN3 * NISO3; i += TR_THREADS) sh.w[i] = __ldg(T.wbin3 + i);
-    for (int i = tid; i <= NM_MAX; i += TR_THREADS) sh.hist[i] = 0u;
-    if (tid == 0) sh.mask = 0u;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    Pipe3& P = *reinterpret_cast<Pipe3*>(smem_raw);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) {
+        for (int s = 0; s < TR_STAGES; s++) { mbar_init(&P.full[s], 1u); mbar_init(&P.empty[s], (uint32_t)TR_CW); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
     __syncthreads();
     const uint32_t n_items = __ldg(n_items_p);
     const uint32_t nt = (uint32_t)T.n_tup3;
-    const double* __restrict__ dtab = T.dtab3;
-    for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x) {
-        const uint4 item = __ldg(items + it);
-        const uint32_t pos0 = item.x, cnt = item.y, g = item.z;
-        const unsigned long long* __restrict__ irec = recs + pos0;
-        if (g == ZERO_ITEM) {   // block-uniform
-            for (uint32_t idx = tid; idx < cnt; idx += TR_THREADS) out[pos0 + idx] = 0.0;
-            continue;
-        }
-        {   // prefetch what the NEXT item of this block will read first: its records into L2,
-            // the two tuple descriptors and the group descriptor into L1
-            const uint32_t nit = it + gridDim.x;
-            if (nit < n_items) {
-                const uint4 nx = __ldg(items + nit);
-                if ((uint32_t)tid * 16u < nx.y) asm volatile("prefetch.global.L2 [%0];" ::"l"(recs + nx.x + tid * 16));
-                if (nx.z != ZERO_ITEM && tid >= 32 && tid < 35) {
-                    const uint32_t tb = nx.z / nt, tk = nx.z - tb * nt;
-                    const void* a = tid == 32 ? (const void*)(T.tk3 + tb) : tid == 33 ? (const void*)(T.tk3 + tk) : (const void*)(T.sgrp3 + nx.z);
-                    asm volatile("prefetch.global.L1 [%0];" ::"l"(a));
+    if (warp == TR_CW) {
+        // ------------------------------------------------------------------ producer
+        uint32_t k = 0;
+        for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x, k++) {
+            const uint32_t s = k % TR_STAGES;
+            Stage3& st = P.st[s];
+            const uint4 item = __ldg(items + it);
+            const uint32_t pos0 = item.x, cnt = item.y, g = item.z;
+            // descriptor loads first: they do not need the stage
+            int4 kb = make_int4(0, 0, 0, 0), kk = kb;
+            uint4 sg = make_uint4(0u, 0u, 0u, 0u);
+            int2 jb = make_int2(0, 0), jk = make_int2(0, 0);
+            int gJlo = 0, gnblk = 0;
+            if (g != ZERO_ITEM) {
+                const uint32_t tb = g / nt, tk = g - tb * nt;
+                kb = __ldg(T.tk3 + tb);
+                kk = __ldg(T.tk3 + tk);
+                sg = __ldg(T.sgrp3 + g);
+                const int Jminb = (kb.w >> 16) & 255, Jmink = (kk.w >> 16) & 255;
+                gJlo = max(Jminb, Jmink);
+                gnblk = ((min((kb.w >> 24) & 255, (kk.w >> 24) & 255) - gJlo) >> 1) + 1;
+                if (lane < gnblk) {
+                    jb = __ldg(T.jinfo3 + kb.z + ((gJlo - Jminb) >> 1) + lane);
+                    jk = __ldg(T.jinfo3 + kk.z + ((gJlo - Jmink) >> 1) + lane);
                 }
             }
-        }
-        // group descriptors: loads issued here, used by warp 0 after its share of the histogram pass (their two
-        // dependent latencies overlap that pass instead of extending the B0 -> B1 phase)
-        int4 kb = make_int4(0, 0, 0, 0), kk = kb;
-        uint2 sg = make_uint2(0u, 0u);
-        int2 jb = make_int2(0, 0), jk = make_int2(0, 0);
-        int gJlo = 0, gnblk = 0;
-        if (tid < 32) {
-            const uint32_t tb = g / nt, tk = g - tb * nt;
-            kb = __ldg(T.tk3 + tb);
-            kk = __ldg(T.tk3 + tk);
-            sg = __ldg(T.sgrp3 + g);
-            const int Jminb = (kb.w >> 16) & 255, Jmink = (kk.w >> 16) & 255;
-            gJlo = max(Jminb, Jmink);
-            gnblk = ((min((kb.w >> 24) & 255, (kk.w >> 24) & 255) - gJlo) >> 1) + 1;
-            if (tid < gnblk) {
-                jb = __ldg(T.jinfo3 + kb.z + ((gJlo - Jminb) >> 1) + tid);
-                jk = __ldg(T.jinfo3 + kk.z + ((gJlo - Jmink) >> 1) + tid);
-            }
-        }
-        __syncthreads();   // B0: the previous item is finished, shared state may be overwritten
-        {   // (1) histogram over iM (each record keeps its rank inside its iM bucket), mask of the isospin bins present
-            uint32_t bits = 0u;
-            constexpr int U = 4;   // records in flight per thread
-            for (uint32_t base = 0; base < cnt; base += U * TR_THREADS) {
-                unsigned long long rec[U];
-#pragma unroll
-                for (int u = 0; u < U; u++) {
-                    const uint32_t idx = base + u * TR_THREADS + tid;
-                    rec[u] = idx < cnt ? __ldg(irec + idx) : 0ull;
+            mbar_wait(&P.empty[s], ((k / TR_STAGES) & 1u) ^ 1u);   // every consumer warp has left the stage
+            if (g == ZERO_ITEM) {
+                if (lane == 0) {
+                    st.sc[SC_POS0] = pos0; st.sc[SC_CNT] = cnt; st.sc[SC_GROUP] = ZERO_ITEM; st.sc[SC_NEXT] = 0u;
+                    mbar_arrive(&P.full[s]);
                 }
-#pragma unroll
-                for (int u = 0; u < U; u++) {
-                    const uint32_t idx = base + u * TR_THREADS + tid;
-                    if (base + u * TR_THREADS + (uint32_t)(tid & ~31) >= cnt) break;   // warp-uniform
-                    const bool valid = idx < cnt;
-                    const uint32_t key = valid ? (uint32_t)(rec[u] >> 30) & 63u : (uint32_t)NM_MAX;
-                    if (valid) bits |= 1u << ((uint32_t)(rec[u] >> 24) & 31u);
-                    const unsigned same = __match_any_sync(0xFFFFFFFFu, key);
-                    const int leader = __ffs(same) - 1;
-                    uint32_t rank = 0u;
-                    if (lane == leader) rank = atomicAdd(&sh.hist[key], (uint32_t)__popc(same));
-                    rank = __shfl_sync(0xFFFFFFFFu, rank, leader) + (uint32_t)__popc(same & ((1u << lane) - 1u));
-                    if (valid) sh.srank[idx] = (uint16_t)((key << 10) | rank);
-                }
+                continue;
             }
-            bits = __reduce_or_sync(0xFFFFFFFFu, bits);
-            if (lane == 0 && bits) atomicOr(&sh.mask, bits);
-        }
-        if (tid < 32) {   // warp 0: item scalars and J-block descriptors
-            // exclusive prefix sums over the blocks: bra rows, ket rows, Vw doubles
+            // exclusive prefix sums over the J blocks: bra rows, ket rows, Vw cells
             const uint32_t rb = (uint32_t)jb.y, rk = (uint32_t)jk.y, vv = (uint32_t)(jb.y * row_pitch3(jk.y));
             uint32_t ib = rb, ik = rk, iv = vv;
 #pragma unroll
@@ -812,103 +843,86 @@ __global__ void __launch_bounds__(TR_THREADS, 6) k_transform3(Tables T, const ui
                 uint32_t xb = __shfl_up_sync(0xFFFFFFFFu, ib, off), xk = __shfl_up_sync(0xFFFFFFFFu, ik, off), xv = __shfl_up_sync(0xFFFFFFFFu, iv, off);
                 if (lane >= off) { ib += xb; ik += xk; iv += xv; }
             }
-            if (tid < gnblk) {
+            if (lane < gnblk) {
                 // dispatch code: 0..15 fully unrolled (nb, nk <= 4); 16 + nk row-loop templates (nk <= 8); 25 generic
                 const uint32_t code = (rb - 1u < 4u && rk - 1u < 4u) ? (rb - 1u) * 4u + (rk - 1u) : (rk - 1u < 8u && rb > 0u) ? 16u + rk : 25u;
-                sh.desc[tid] = (unsigned long long)(rb | (rk << 8) | ((ib - rb) << 16) | ((ik - rk) << 24)) |
-                               ((unsigned long long)((iv - vv) | (code << 16)) << 32);
+                st.desc[lane] = make_uint4(rb | (rk << 8) | (code << 16), ib - rb, ik - rk, iv - vv);
             }
-            if (tid == 0) {
-                sh.sc[0] = (uint32_t)kb.y;
-                sh.sc[1] = (uint32_t)kk.y;
-                sh.sc[2] = (uint32_t)kb.x + (uint32_t)jb.x * (uint32_t)kb.y;
-                sh.sc[3] = (uint32_t)kk.x + (uint32_t)jk.x * (uint32_t)kk.y;
-                sh.sc[4] = ((uint32_t)kb.w & 0xFFu) | ((uint32_t)gJlo << 8) | ((uint32_t)gnblk << 16);
-                sh.sc[5] = sg.y;
-                sh.sc[6] = sg.x;
+            const uint32_t gsize = sg.y, S = vw_stride(gsize), bin_lo = item.w & 255u, bins = item.w >> 8;
+            if (lane == 0) {
+                st.sc[SC_POS0] = pos0; st.sc[SC_CNT] = cnt; st.sc[SC_GROUP] = g;
+                st.sc[SC_SB] = (uint32_t)kb.y; st.sc[SC_SK] = (uint32_t)kk.y;
+                st.sc[SC_PB0] = (uint32_t)kb.x + (uint32_t)jb.x * (uint32_t)kb.y;
+                st.sc[SC_PK0] = (uint32_t)kk.x + (uint32_t)jk.x * (uint32_t)kk.y;
+                st.sc[SC_JINFO] = ((uint32_t)kb.w & 0xFFu) | ((uint32_t)gJlo << 8) | ((uint32_t)gnblk << 16);
+                st.sc[SC_GSIZE] = gsize; st.sc[SC_STRIDE] = S; st.sc[SC_BINS] = item.w; st.sc[SC_ROFF] = pos0 & 1u;
+                st.sc[SC_NEXT] = 0u;
             }
-            if (tid == gnblk - 1) sh.sc[7] = ib | (ik << 8);   // rows of the common J range: bra | ket<<8
-        }
-        __syncthreads();   // B1: histogram, mask, descriptors complete
-        const uint32_t mask = sh.mask;
-        const uint4 s0 = *reinterpret_cast<const uint4*>(&sh.sc[0]);
-        const uint4 s1 = *reinterpret_cast<const uint4*>(&sh.sc[4]);
-        const uint32_t Sb = s0.x, Sk = s0.y;
-        const uint32_t gsize = s1.y, vstride = vw_stride(gsize);
-        const int sumj = s1.x & 255, Jlo = (s1.x >> 8) & 255, nblk = (int)(s1.x >> 16);
-        const uint32_t bpr = min((uint32_t)NBIN3, (uint32_t)VW_CAP / vstride);   // bins per round
-        const uint32_t inv = 0xFFFFFFFFu / gsize + 1u;
-        const double* __restrict__ slab = T.slab3 + (size_t)s1.z * 2;
-        uint32_t* soff = sh.soff[tid >> 5];
-        {   // every warp: exclusive scan of the iM histogram into its own cursor array (no block barrier needed before (2b))
-            const uint32_t a = sh.hist[2 * lane], b = sh.hist[2 * lane + 1];
-            uint32_t incl = a + b;
-#pragma unroll
-            for (int off = 1; off < 32; off <<= 1) {
-                uint32_t x = __shfl_up_sync(0xFFFFFFFFu, incl, off);
-                if (lane >= off) incl += x;
-            }
-            soff[2 * lane] = incl - a - b;
-            soff[2 * lane + 1] = incl - b;
             __syncwarp();
+            if (lane == 0) {
+                const uint32_t vw_bytes = (bins * S * 4u + 15u) & ~15u;
+                const uint32_t rec_bytes = (((pos0 & 1u) + cnt + 1u) & ~1u) * 8u;
+                mbar_arrive_tx(&P.full[s], vw_bytes + rec_bytes);
+                bulk_g2s(st.vw, T.vw20 + (size_t)sg.z * 4 + (size_t)bin_lo * S, vw_bytes, &P.full[s]);
+                bulk_g2s(st.rec, recs + (pos0 & ~1u), rec_bytes, &P.full[s]);
+            }
         }
-        bool first = true;
-        for (uint32_t b0 = 0; b0 < (uint32_t)NBIN3; b0 += bpr) {
-            if (((mask >> b0) & ((1u << bpr) - 1u)) == 0u) continue;   // block-uniform
-            if (!first) __syncthreads();   // the previous round's compute phase is over
-            // (2) stage the isospin-combined slabs of the bins of this round
-            for (uint32_t idx = tid; idx < bpr * gsize; idx += TR_THREADS) {
-                const uint32_t bl = __umulhi(idx, inv), c = idx - bl * gsize, b = b0 + bl;
-                if (b < (uint32_t)NBIN3 && ((mask >> b) & 1u)) {
-                    const double* w = &sh.w[b * NISO3];
-                    double v = w[0] * __ldg(slab + c);
-                    v = fma(w[1], __ldg(slab + gsize + c), v);
-                    v = fma(w[2], __ldg(slab + 2 * gsize + c), v);
-                    v = fma(w[3], __ldg(slab + 3 * gsize + c), v);
-                    v = fma(w[4], __ldg(slab + 4 * gsize + c), v);
-                    sh.vw[bl * vstride + c] = v;
-                }
+        return;
+    }
+    // ---------------------------------------------------------------------- consumers
+    const double* __restrict__ dtab = T.dtab3;
+    uint32_t k = 0;
+    for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x, k++) {
+        const uint32_t s = k % TR_STAGES;
+        Stage3& st = P.st[s];
+        mbar_wait(&P.full[s], (k / TR_STAGES) & 1u);
+        const uint4 s0 = *reinterpret_cast<const uint4*>(&st.sc[0]);    // pos0, cnt, group, Sb
+        const uint32_t pos0 = s0.x, cnt = s0.y;
+        if (s0.z == ZERO_ITEM) {
+            for (;;) {
+                uint32_t b = 0;
+                if (lane == 0) b = atomicAdd(&st.sc[SC_NEXT], 1u);
+                b = __shfl_sync(0xFFFFFFFFu, b, 0) * BATCH3;
+                if (b >= cnt) break;
+                if (b + lane < cnt) out[pos0 + b + lane] = 0.0;
+                if (b + 32 + lane < cnt) out[pos0 + b + 32 + lane] = 0.0;
             }
-            const bool was_first = first;
-            if (first) {   // (2b) M-sorted order of the records (a thread reads the ranks it wrote itself)
-                for (uint32_t idx = tid; idx < cnt; idx += TR_THREADS) {
-                    const uint32_t kr = sh.srank[idx];
-                    sh.sidx[soff[kr >> 10] + (kr & 1023u)] = (uint16_t)idx;
-                }
-                first = false;
-            }
-            __syncthreads();   // B3: Vw and the sorted order are in place; every warp has read the histogram and the mask
-            if (was_first && tid < 32) {   // clear them for the next item (its atomics come after its B0)
-                sh.hist[2 * lane] = 0u;
-                sh.hist[2 * lane + 1] = 0u;
-                if (lane == 0) { sh.hist[NM_MAX] = 0u; sh.mask = 0u; }
-            }
-            // (3) evaluate.  Warp-uniform loop over pairs of 32 sorted slots: lane l takes slots base+l (A) and base+32+l
-            //     (B); lanes past the end of the item redo its last record and skip the store.
-            for (uint32_t base = (uint32_t)(tid & ~31) * 2u; base < cnt; base += 2u * TR_THREADS) {
+        } else {
+            const uint4 s1 = *reinterpret_cast<const uint4*>(&st.sc[4]);    // Sk, pb0, pk0, jinfo
+            const uint4 s2 = *reinterpret_cast<const uint4*>(&st.sc[8]);    // gsize, stride, bins, roff
+            const uint32_t Sb = s0.w, Sk = s1.x, G = s2.x, S = s2.y, bin_lo = s2.z & 255u, bins = s2.z >> 8;
+            const int sumj = s1.w & 255, Jlo = (s1.w >> 8) & 255, nblk = (int)(s1.w >> 16);
+            const unsigned long long* __restrict__ irec = st.rec + s2.w;
+            const uint32_t* vw = st.vw;
+            for (;;) {
+                uint32_t base = 0;
+                if (lane == 0) base = atomicAdd(&st.sc[SC_NEXT], 1u);
+                base = __shfl_sync(0xFFFFFFFFu, base, 0) * BATCH3;
+                if (base >= cnt) break;
+                // lane l takes stream positions base+l (A) and base+32+l (B); lanes past the end of the item redo its last
+                // record and skip the store
                 const uint32_t slotA = base + lane, slotB = slotA + 32u;
-                const uint32_t idxA = sh.sidx[min(slotA, cnt - 1u)], idxB = sh.sidx[min(slotB, cnt - 1u)];
-                const unsigned long long rcA = __ldg(irec + idxA), rcB = __ldg(irec + idxB);
+                const unsigned long long rcA = irec[min(slotA, cnt - 1u)], rcB = irec[min(slotB, cnt - 1u)];
                 const uint32_t loA = (uint32_t)rcA, loB = (uint32_t)rcB;
-                const uint32_t blA = ((loA >> 24) & 31u) - b0, blB = ((loB >> 24) & 31u) - b0;
+                const uint32_t blA = ((loA >> 24) & 31u) - bin_lo, blB = ((loB >> 24) & 31u) - bin_lo;
                 const int aMA = abs(2 * ((int)(rcA >> 30) & 63) - sumj), aMB = abs(2 * ((int)(rcB >> 30) & 63) - sumj);
-                const int q0 = max(0, (min(aMA, aMB) - Jlo + 1) >> 1);   // first block with J >= |M| of either record
-                uint32_t pbA = s0.z + (loA & 0xFFFu), pkA = s0.w + ((loA >> 12) & 0xFFFu), viA = min(blA, bpr - 1u) * vstride;
-                uint32_t pbB = s0.z + (loB & 0xFFFu), pkB = s0.w + ((loB >> 12) & 0xFFFu), viB = min(blB, bpr - 1u) * vstride;
+                // first block with J >= |M| of any record of the warp (coefficients are 0 below a record's own |M|)
+                const int q0 = max(0, ((int)__reduce_min_sync(0xFFFFFFFFu, (unsigned)min(aMA, aMB)) - Jlo + 1) >> 1);
+                uint32_t pbA = s1.y + (loA & 0xFFFu), pkA = s1.z + ((loA >> 12) & 0xFFFu), viA = min(blA, bins - 1u) * S;
+                uint32_t pbB = s1.y + (loB & 0xFFFu), pkB = s1.z + ((loB >> 12) & 0xFFFu), viB = min(blB, bins - 1u) * S;
                 if (q0 > 0 && q0 < nblk) {
-                    const unsigned long long d = sh.desc[q0];
-                    const uint32_t rb = ((uint32_t)d >> 16) & 255u, rk = (uint32_t)d >> 24, dv = (uint32_t)(d >> 32) & 0xFFFFu;
-                    pbA += rb * Sb; pbB += rb * Sb;
-                    pkA += rk * Sk; pkB += rk * Sk;
-                    viA += dv; viB += dv;
+                    const uint4 d = st.desc[q0];
+                    pbA += d.y * Sb; pbB += d.y * Sb;
+                    pkA += d.z * Sk; pkB += d.z * Sk;
+                    viA += d.w; viB += d.w;
                 }
                 double totA = 0.0, totB = 0.0;
                 for (int q = q0; q < nblk; q++) {
-                    const unsigned long long d = sh.desc[q];
-                    const int nb = (uint32_t)d & 255, nk = ((uint32_t)d >> 8) & 255;
-#define MFDN_BLK(NB, NK) case ((NB) - 1) * 4 + ((NK) - 1): j_block3x2<NB, NK>(dtab, sh.vw, pbA, pkA, pbB, pkB, Sb, Sk, viA, viB, totA, totB); break;
-#define MFDN_ROWS(NK) case 16 + (NK): j_block3x2_rows<NK>(dtab, sh.vw, pbA, pkA, pbB, pkB, Sb, Sk, nb, viA, viB, totA, totB); break;
-                    switch ((uint32_t)(d >> 48)) {
+                    const uint32_t d = st.desc[q].x;
+                    const int nb = d & 255, nk = (d >> 8) & 255;
+#define MFDN_BLK(NB, NK) case ((NB) - 1) * 4 + ((NK) - 1): j_block3x2<NB, NK>(dtab, vw, pbA, pkA, pbB, pkB, Sb, Sk, viA, viB, G, totA, totB); break;
+#define MFDN_ROWS(NK) case 16 + (NK): j_block3x2_rows<NK>(dtab, vw, pbA, pkA, pbB, pkB, Sb, Sk, nb, viA, viB, G, totA, totB); break;
+                    switch (d >> 16) {
                         MFDN_BLK(1, 1) MFDN_BLK(1, 2) MFDN_BLK(1, 3) MFDN_BLK(1, 4)
                         MFDN_BLK(2, 1) MFDN_BLK(2, 2) MFDN_BLK(2, 3) MFDN_BLK(2, 4)
                         MFDN_BLK(3, 1) MFDN_BLK(3, 2) MFDN_BLK(3, 3) MFDN_BLK(3, 4)
@@ -916,8 +930,8 @@ __global__ void __launch_bounds__(TR_THREADS, 6) k_transform3(Tables T, const ui
                         MFDN_ROWS(1) MFDN_ROWS(2) MFDN_ROWS(3) MFDN_ROWS(4) MFDN_ROWS(5) MFDN_ROWS(6) MFDN_ROWS(7) MFDN_ROWS(8)
                         default: {
                             if (nk > 0 && nb > 0) {
-                                totA += j_block3_generic(dtab, sh.vw, pbA, pkA, Sb, Sk, nb, nk, viA);
-                                totB += j_block3_generic(dtab, sh.vw, pbB, pkB, Sb, Sk, nb, nk, viB);
+                                totA += j_block3_generic(dtab, vw, pbA, pkA, Sb, Sk, nb, nk, viA, G);
+                                totB += j_block3_generic(dtab, vw, pbB, pkB, Sb, Sk, nb, nk, viB, G);
                             }
                             pbA += (uint32_t)nb * Sb; pbB += (uint32_t)nb * Sb;
                             pkA += (uint32_t)nk * Sk; pkB += (uint32_t)nk * Sk;
@@ -928,11 +942,13 @@ __global__ void __launch_bounds__(TR_THREADS, 6) k_transform3(Tables T, const ui
 #undef MFDN_BLK
 #undef MFDN_ROWS
                 }
-                // store unless past the end of the item or the bin is staged in another round; + 0.0: never store -0
-                if (slotA < cnt && blA < bpr) out[pos0 + idxA] = (((loA >> 29) & 1u) ? -totA : totA) + 0.0;
-                if (slotB < cnt && blB < bpr) out[pos0 + idxB] = (((loB >> 29) & 1u) ? -totB : totB) + 0.0;
+                // store unless past the end of the item or the bin belongs to another round; + 0.0: never store -0
+                if (slotA < cnt && blA < bins) out[pos0 + slotA] = (((loA >> 29) & 1u) ? -totA : totA) + 0.0;
+                if (slotB < cnt && blB < bins) out[pos0 + slotB] = (((loB >> 29) & 1u) ? -totB : totB) + 0.0;
             }
         }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&P.empty[s]);
     }
 }
 
@@ -991,13 +1007,15 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
     if (BODY == 3 ? !c->has3 : !c->has2) return fail(c, MFDN_ERR_STATE, "mscheme before coupled upload");
     const long long nt = BODY == 3 ? c->t.n_tup3 : c->t.n_tup2;
     if (nt * nt >= (long long)REC_INVALID) return fail(c, MFDN_ERR_ARG, "too many tuples for 27-bit group keys");
-    const long long n_buckets = nt * nt + 1;   // last bucket: requests failing S1-S6
+    // sort buckets: 2-body one per group, 3-body one per (group, M); last bucket: requests failing S1-S6
+    const long long n_buckets = (BODY == 3 ? (long long)c->t.n_buckets3 : nt * nt) + 1;
     const long long n_tiles = (n_buckets + SCAN_TILE - 1) / SCAN_TILE;
     const bool naive = flags & MFDN_FORCE_NAIVE;
     const bool sort = !naive && !(flags & MFDN_PRESORTED);
     const bool items = !naive && BODY == 3;    // the 3-body transform walks a list of one-group work items
     const bool hist_needed = sort || items;
-    const long long max_items = n / ITEM3 + std::min<long long>(n, n_buckets) + 1;
+    // work items: at most 5 rounds per chunk of a group with more than SMALL_ITEM3 records, one entry per small group
+    const long long max_items = 5 * (n / ITEM3 + n / (SMALL_ITEM3 + 1) + 1) + std::min<long long>(n, nt * nt + 1) + 1;
     size_t need = 256;
     size_t o_recs = 0, o_sorted = 0, o_order = 0, o_hist = 0, o_sums = 0, o_items = 0, o_count = 0;
     if (!naive) {
@@ -1043,7 +1061,7 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
         const unsigned long long* trecs = recs;
         uint32_t* hist = hist_needed ? (uint32_t*)(w + o_hist) : nullptr;
         uint32_t* sums = hist_needed ? (uint32_t*)(w + o_sums) : nullptr;
-        const uint32_t invalid_bucket = (uint32_t)(nt * nt);
+        const uint32_t invalid_bucket = (uint32_t)(n_buckets - 1);
         if (hist_needed) MFDN_CUDA(c, cudaMemsetAsync(hist, 0, (size_t)n_buckets * 4, st));
         const bool sm = c->t.n_sps <= KEYS_SPS_SMEM && (BODY == 2 || (c->t.ab3 && c->t.n_orb * c->t.n_orb <= KEYS_AB_SMEM));
         const unsigned gkb = (unsigned)((n + KEYS_PER_BLOCK - 1) / KEYS_PER_BLOCK);
@@ -1077,12 +1095,18 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
             uint32_t* cnt = (uint32_t*)(w + o_count);
             MFDN_CUDA(c, cudaMemsetAsync(cnt, 0, 8, st));
             const uint32_t last_slot = (uint32_t)(max_items - 1);
-            k_items3<<<(unsigned)((n_buckets + 255) / 256), 256, 0, st>>>(hist, (uint32_t)n_buckets, sort ? 1 : 0, (uint32_t)n, c->t.sgrp3,
-                                                                           invalid_bucket, itm, last_slot, cnt);
+            k_items3<<<(unsigned)((nt * nt + 1 + 255) / 256), 256, 0, st>>>(hist, c->t.gbase3, (uint32_t)(nt * nt), (uint32_t)n_buckets, sort ? 1 : 0,
+                                                                             (uint32_t)n, c->t.sgrp3, itm, last_slot, cnt);
             if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.b, st));
-            const unsigned grid = (unsigned)std::min<long long>(max_items, (long long)c->num_sms * 6);
-            k_transform3<<<grid, TR_THREADS, 0, st>>>(c->t, itm, cnt, trecs, tout);
-            const unsigned grid_s = (unsigned)std::min<long long>((std::min<long long>(n, n_buckets) + 3) / 4, (long long)c->num_sms * 16);
+            if (c->tr_blocks_per_sm == 0) {
+                MFDN_CUDA(c, cudaFuncSetAttribute(k_transform3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Pipe3)));
+                int per_sm = 0;
+                MFDN_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_transform3, TR_THREADS, sizeof(Pipe3)));
+                c->tr_blocks_per_sm = std::max(per_sm, 1);
+            }
+            const unsigned grid = (unsigned)std::min<long long>(max_items, (long long)c->num_sms * c->tr_blocks_per_sm);
+            k_transform3<<<grid, TR_THREADS, sizeof(Pipe3), st>>>(c->t, itm, cnt, trecs, tout);
+            const unsigned grid_s = (unsigned)std::min<long long>((std::min<long long>(n, nt * nt + 1) + 3) / 4, (long long)c->num_sms * 16);
             k_transform3_small<<<grid_s, 128, 0, st>>>(c->t, itm, last_slot, cnt, trecs, tout);
             c->launches += 3;
         } else {
