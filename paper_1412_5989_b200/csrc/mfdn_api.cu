@@ -431,7 +431,7 @@ __global__ void k_vw20(long long n_groups, const uint4* __restrict__ sgrp, const
     }
 }
 
-// Per-tuple coefficient tables (A1/A2): dtab[tk.x + row*S + sigma(ima, imb, imc)] =
+// Per-tuple coefficient tables (A1/A2), one block per J of the tuple: dtab[tk.x + block(J) + sigma(ima, imb, imc)*nb(J) + i] =
 // <ja ma jb mb|J12 M12> <J12 M12 jc mc|J M> for the tuple's rows (J, J12) in loop order; one fp64 product of the two
 // tabulated coefficients, 0 where |M12| > J12 or |M| > J (the zero guard of the stage-2 table).
 struct Dtab3 {
@@ -439,6 +439,7 @@ struct Dtab3 {
     const int4* tk;
     const int2* trow;      // {first row of the tuple in rowtab, -}
     const int2* rowtab;    // per row {cg2g offset at A = 0, cg1 offset relative to the m-pair base}
+    const int2* rowdst;    // per row {offset of its J block in the tuple's table, rows of the block << 8 | row within the block}
     const int32_t* nrows;
     const uint16_t* sig;
     const int32_t* sigoff;
@@ -461,7 +462,9 @@ __global__ void k_dtab3(Dtab3 p)
         int imc = o % (jc + 1), imb = (o / (jc + 1)) % (jb + 1), ima = o / ((jc + 1) * (jb + 1));
         int2 rt = p.rowtab[r0 + r];
         int A = (ima + imb - ((ja + jb) >> 1)) * (jc + 1) + imc;
-        p.dtab[(size_t)(uint32_t)k.x + (size_t)r * S + p.sig[p.sigoff[t] + o]] = p.cg1[c1 + ima * (jb + 1) + imb + rt.y] * p.cg2g[rt.x + A];
+        int2 rd = p.rowdst[r0 + r];
+        p.dtab[(size_t)(uint32_t)k.x + (size_t)rd.x + (size_t)p.sig[p.sigoff[t] + o] * (rd.y >> 8) + (rd.y & 255)] =
+            p.cg1[c1 + ima * (jb + 1) + imb + rt.y] * p.cg2g[rt.x + A];
     }
 }
 
@@ -620,8 +623,10 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     //      request-independent parts of the two coefficient addresses (used only to build dtab3):
     //        x: <J12 M12 jc mc|J M> lives at cg2g[x + A],  A = M12*(jc+1) + imc  (x includes CG_GUARD and J12*(jc+1))
     //        y: <ja ma jb mb|J12 M12> lives at cg1[c1 + y],  c1 = off(ja,jb) + ima*(jb+1) + imb
-    //      and per (tuple, J): {first row (tuple-relative), number of rows}
-    std::vector<int2> trow(nt), rowtab, jinfo;
+    //      and per (tuple, J): {offset of the J block in the tuple's coefficient table, number of rows nb(J)}.  Inside a
+    //      block the nb coefficients of one m-state are contiguous ([sigma][row]): a request reads all its coefficients of
+    //      a J block with one address computation and vector loads, and neighbouring m-states stay neighbours in memory.
+    std::vector<int2> trow(nt), rowtab, rowdst, jinfo;
     std::vector<int4> tk(nt);
     std::vector<int32_t> nrows(nt), sigoff(nt);
     std::vector<uint16_t> sig;
@@ -631,12 +636,16 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
         int ja = d.x & 255, jb = (d.x >> 8) & 255, jc = (d.x >> 16) & 255;
         trow[t].x = (int)rowtab.size();
         trow[t].y = (int)jinfo.size();
+        const int S = (ja + 1) * (jb + 1) * (jc + 1);
+        if (S > MAX_STATES3) return fail(c, MFDN_ERR_TABLE, "tuple with more than 4096 m-states");
+        uint64_t tlen = 0;   // doubles of this tuple's table so far (every block starts 16-byte aligned)
         for (int twoJ = (d.y >> 16) & 255; twoJ <= ((d.y >> 24) & 255); twoJ += 2) {
             int lo, hi;
             range(d, twoJ, lo, hi);
             int2 ji;
-            ji.x = (int)rowtab.size() - trow[t].x;
+            ji.x = (int)tlen;
             ji.y = std::max(0, hi - lo + 1);
+            if (ji.y > 255) return fail(c, MFDN_ERR_TABLE, "more than 255 J12 values in one J block");
             jinfo.push_back(ji);
             for (int J12 = lo; J12 <= hi; J12++) {
                 int iJ = (twoJ - std::abs(2 * J12 - jc)) / 2;
@@ -644,11 +653,11 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
                 e.x = CG_GUARD + c->h_cg2_off[J12 * c->t.nj + (jc >> 1)] + (iJ * (2 * J12 + 1) + J12) * (jc + 1);
                 e.y = (J12 - (d.y & 255)) * (ja + 1) * (jb + 1);
                 rowtab.push_back(e);
+                rowdst.push_back(int2{ji.x, (ji.y << 8) | (J12 - lo)});
             }
+            tlen = (tlen + (uint64_t)S * ji.y + 1) & ~1ull;
         }
         nrows[t] = (int)rowtab.size() - trow[t].x;
-        const int S = (ja + 1) * (jb + 1) * (jc + 1);
-        if (S > MAX_STATES3) return fail(c, MFDN_ERR_TABLE, "tuple with more than 4096 m-states");
         // sigma: m-states of the tuple ordered by (iM = ima+imb+imc, ima, imb); counting sort over iM
         sigoff[t] = (int32_t)sig.size();
         {
@@ -660,13 +669,12 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
             for (int a = 0; a <= ja; a++) for (int b = 0; b <= jb; b++) for (int m = 0; m <= jc; m++)
                 sg[(a * (jb + 1) + b) * (jc + 1) + m] = (uint16_t)start[a + b + m]++;
         }
-        if (dtab_len + (uint64_t)nrows[t] * S >= 0x7FFFFFF0ull) return fail(c, MFDN_ERR_OOM, "coefficient table too large for 31-bit offsets");
+        if (dtab_len + tlen >= 0x7FFFFFF0ull) return fail(c, MFDN_ERR_OOM, "coefficient table too large for 31-bit offsets");
         tk[t].x = (int)dtab_len;
         tk[t].y = S;
         tk[t].z = trow[t].y;
         tk[t].w = (ja + jb + jc) | (d.y & 0xFFFF0000);
-        dtab_len += (uint64_t)nrows[t] * S;
-        dtab_len = (dtab_len + 1) & ~1ull;
+        dtab_len += tlen;
     }
     // ---- group descriptors: slab offset (16-byte units) and plane size, rows in loop order J, J12
     //      and the (group, M) buckets of the request sort: every same-parity group owns one bucket per common M
@@ -727,7 +735,7 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     std::vector<int64_t> coff(chan_off, chan_off + n_chan);
     std::vector<int32_t> cdim(chan_dim, chan_dim + n_chan);
     size_t o_rm = tmp.add(rowmap), o_cof = tmp.add(chan_of), o_coff = tmp.add(coff), o_cdim = tmp.add(cdim);
-    size_t o_trow = tmp.add(trow), o_rowtab = tmp.add(rowtab), o_nrows = tmp.add(nrows);
+    size_t o_trow = tmp.add(trow), o_rowtab = tmp.add(rowtab), o_rowdst = tmp.add(rowdst), o_nrows = tmp.add(nrows);
     char* dres = nullptr;
     int rc = arena_upload(c, res, &dres, st);
     if (rc) return rc;
@@ -741,7 +749,9 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     void* dslab = nullptr;
     cudaError_t e = cudaMalloc(&dslab, std::max<uint64_t>(cells, 1) * 16 + 256);
     void* ddtab = nullptr;
-    if (e == cudaSuccess) e = cudaMalloc(&ddtab, (dtab_len + 2 * MAX_STATES3) * sizeof(double));   // slack: a mis-ordered MFDN_PRESORTED stream may index past a tuple
+    // slack: in a mis-ordered MFDN_PRESORTED stream a record may meet the tables of another tuple and index up to
+    // MAX_STATES3 * 32 doubles past its block
+    if (e == cudaSuccess) e = cudaMalloc(&ddtab, (dtab_len + 32 * (uint64_t)MAX_STATES3) * sizeof(double));
     void* dvw = nullptr;
     if (e == cudaSuccess) e = cudaMalloc(&dvw, std::max<uint64_t>(vwcells, 1) * 16 + 256);        // slack: bulk copies are rounded up to 16 bytes
     if (e != cudaSuccess) {
@@ -772,6 +782,7 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     q.tk = (const int4*)(dres + o_tk);
     q.trow = (const int2*)((char*)dtmp + o_trow);
     q.rowtab = (const int2*)((char*)dtmp + o_rowtab);
+    q.rowdst = (const int2*)((char*)dtmp + o_rowdst);
     q.nrows = (const int32_t*)((char*)dtmp + o_nrows);
     q.sig = (const uint16_t*)(dres + o_sig);
     q.sigoff = (const int32_t*)(dres + o_sigoff);

@@ -72,7 +72,7 @@ constexpr int MAX_STATES3 = 4096;   // (ja+1)(jb+1)(jc+1) of a tuple must fit th
 //         z = offset of the tuple's state masks in stmask3 (entries: [J12-J12min][T12], suffix-ORed over J12)
 //         w = start of the tuple's sigma table in sig3 (during the upload: offset of the tuple's row map)
 // tk3 (what the transform kernel needs of a tuple): x = offset of the tuple's coefficient table in dtab3 (doubles),
-//         y = its row pitch S = (ja+1)(jb+1)(jc+1), z = first entry of the tuple in jinfo3,
+//         y = its m-state count S = (ja+1)(jb+1)(jc+1), z = first entry of the tuple in jinfo3,
 //         w = (ja+jb+jc) | twoJmin<<16 | twoJmax<<24
 // 2-body: x = ja | jb<<8 | (a==b)<<24 | par<<25,  y = Jmin | Jmax<<8,  z = state mask (low), w = (high)
 struct Tables {
@@ -107,8 +107,8 @@ struct Tables {
     const uint32_t* vw20;          // isospin-combined slabs, split word planes (see vw_stride)
     const unsigned long long* stmask3;
     const int4* tk3;               // [n_tup3] see above
-    const int2* jinfo3;            // per (tuple, J): {first row of this J (tuple-relative, loop order J, J12), number of rows}
-    const double* dtab3;           // per tuple [row][sigma] = <ja ma jb mb|J12 M12> <J12 M12 jc mc|J M>
+    const int2* jinfo3;            // per (tuple, J): {offset of the J block in the tuple's coefficient table (doubles, even), rows nb(J)}
+    const double* dtab3;           // per tuple and J block [sigma][row] = <ja ma jb mb|J12 M12> <J12 M12 jc mc|J M>, rows = J12 ascending
     const uint16_t* sig3;          // per tuple [(ima*(jb+1)+imb)*(jc+1)+imc] -> sigma: m-states ordered by (M, ima, imb), so that
                                    // requests with equal M (bra and ket always have equal M) read neighbouring entries
     // A2, 2-body

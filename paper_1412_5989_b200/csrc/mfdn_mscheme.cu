@@ -577,27 +577,28 @@ __global__ void __launch_bounds__(128) k_transform3_small(Tables T, const uint4*
         const int nblk = ((Jhi - Jlo) >> 1) + 1;
         const int2* __restrict__ jib = T.jinfo3 + kb.z + ((Jlo - Jminb) >> 1);
         const int2* __restrict__ jik = T.jinfo3 + kk.z + ((Jlo - Jmink) >> 1);
-        const uint32_t Sb = (uint32_t)kb.y, Sk = (uint32_t)kk.y, gsize = sg.y;
-        const uint32_t pb0 = (uint32_t)kb.x + (uint32_t)__ldg(jib).x * Sb, pk0 = (uint32_t)kk.x + (uint32_t)__ldg(jik).x * Sk;
+        const uint32_t gsize = sg.y;
         for (uint32_t r0 = 0; r0 < cnt; r0 += 32) {   // 32 records per pass
             const bool valid = r0 + lane < cnt;
             const unsigned long long rec = __ldg(recs + pos0 + (valid ? r0 + lane : r0));
             const uint32_t lo = (uint32_t)rec;
             const double* wp = T.wbin3 + ((lo >> 24) & 31u) * NISO3;
             const double w0 = __ldg(wp), w1 = __ldg(wp + 1), w2 = __ldg(wp + 2), w3 = __ldg(wp + 3), w4 = __ldg(wp + 4);
-            uint32_t pb = pb0 + (lo & 0xFFFu), pk = pk0 + ((lo >> 12) & 0xFFFu);
+            const uint32_t sb = lo & 0xFFFu, sk = (lo >> 12) & 0xFFFu;
             const double* __restrict__ row = T.slab3 + (size_t)sg.x * 2;
             double total = 0.0;
             for (int q = 0; q < nblk; q++) {
-                const int nb = __ldg(jib + q).y, nk = __ldg(jik + q).y;
+                const int2 ib = __ldg(jib + q), ik = __ldg(jik + q);
+                const int nb = ib.y, nk = ik.y;
                 const int P = row_pitch3(nk);
+                const double* __restrict__ cbp = dtab + (uint32_t)kb.x + (uint32_t)ib.x + sb * (uint32_t)nb;
+                const double* __restrict__ ckp = dtab + (uint32_t)kk.x + (uint32_t)ik.x + sk * (uint32_t)nk;
                 double t = 0.0;
                 for (int i = 0; i < nb; i++) {
-                    const double cb = __ldg(dtab + pb);
-                    pb += Sb;
+                    const double cb = __ldg(cbp + i);
                     double acc = 0.0;
                     for (int k = 0; k < nk; k++) {
-                        const double ck = __ldg(dtab + pk + (uint32_t)k * Sk);
+                        const double ck = __ldg(ckp + k);
                         const double* cell = row + k;
                         double v = w0 * __ldg(cell);
                         v = fma(w1, __ldg(cell + gsize), v);
@@ -607,9 +608,8 @@ __global__ void __launch_bounds__(128) k_transform3_small(Tables T, const uint4*
                         acc = k ? fma(ck, v, acc) : ck * v;
                     }
                     t = fma(cb, acc, t);
-                    row += P;
+                    if (nk > 0) row += P;
                 }
-                pk += (uint32_t)nk * Sk;
                 total += t;
             }
             if (valid) out[pos0 + r0 + lane] = (((lo >> 29) & 1u) ? -total : total) + 0.0;   // + 0.0: never store -0
@@ -637,8 +637,9 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* b, uint32_t parity
     const uint32_t a = smem_u32(b);
     uint32_t ok;
     do {
-        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+        // the last operand lets the hardware suspend the warp until the phase completes (or the time hint, ns, runs out)
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(a), "r"(parity), "r"(1000000u) : "memory");
     } while (!ok);
 }
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, unsigned long long* b)
@@ -647,57 +648,141 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(b)) : "memory");
 }
 
-constexpr int TR_CW = 4;                        // consumer warps per block
+#ifndef MFDN_TR_CW
+#define MFDN_TR_CW 4
+#endif
+#ifndef MFDN_TR_SLOTS
+#define MFDN_TR_SLOTS 8
+#endif
+#ifndef MFDN_TR_MINB
+#define MFDN_TR_MINB 4
+#endif
+#ifndef MFDN_TR_RING
+#define MFDN_TR_RING 6656
+#endif
+constexpr int TR_CW = MFDN_TR_CW;               // consumer warps per block
 constexpr int TR_THREADS = (TR_CW + 1) * 32;    // + one producer warp
-constexpr int TR_STAGES = 2;
+constexpr int TR_SLOTS = MFDN_TR_SLOTS;         // work items in flight per block
 constexpr int MAX_JBLK = 32;                    // common J values of a group (2J <= 63)
 constexpr int BATCH3 = 64;                      // records per consumer-warp batch (two per lane)
-
-// One pipeline stage = everything the consumer warps need for one work item: its isospin-combined slabs and its records
-// (both landed by bulk copies), the J-block descriptors and the group's scalars (written by the producer warp).
-struct __align__(16) Stage3 {
-    uint32_t vw[VW_WORDS];
-    unsigned long long rec[ITEM3 + 2];          // copied from an even position: one record of slack at either end
-    uint4 desc[MAX_JBLK];                       // per J block: {nb | nk<<8 | dispatch code<<16, bra rows before, ket rows before, Vw cells before}
-    uint32_t sc[16];                            // item scalars, see SC_*
+constexpr int REC_WORDS_MAX = (ITEM3 + 2) * 2;  // records are copied from an even position: one record of slack at either end
+// Ring of 32-bit words holding, per work item in flight, everything its consumer warps read: the isospin-combined slabs
+// and the records (both landed by bulk copies) and the J-block descriptors (written by the producer warp).  Sized for
+// one item of maximal size; typical items (4 KB of slabs, 3 KB of records) leave room for three to four in flight.  A
+// small ring keeps most of the SM's 228 KB as L1 for the coefficient tables (ncu: with two fixed 25 KB stages per
+// block the L1 hit rate of the coefficient gathers was 60 %).
+constexpr int RING_WORDS = MFDN_TR_RING;
+static_assert(RING_WORDS >= VW_WORDS + REC_WORDS_MAX + MAX_JBLK * 4, "ring must hold one maximal work item");
+enum { SC_POS0, SC_CNT, SC_GROUP, SC_SB, SC_SK, SC_PB0, SC_PK0, SC_JINFO, SC_GSIZE, SC_STRIDE, SC_BINS, SC_ROFF, SC_VW, SC_REC, SC_DESC, SC_NEXT };
+struct __align__(16) Pipe3 {
+    uint32_t ring[RING_WORDS];
+    uint32_t sc[TR_SLOTS][16];                  // item scalars, see SC_* (SC_VW, SC_REC, SC_DESC: ring offsets in words)
+    unsigned long long full[TR_SLOTS], empty[TR_SLOTS];
+    uint32_t start_of[TR_SLOTS];                // ring offset of the item in each slot (producer's bookkeeping)
 };
-enum { SC_POS0, SC_CNT, SC_GROUP, SC_SB, SC_SK, SC_PB0, SC_PK0, SC_JINFO, SC_GSIZE, SC_STRIDE, SC_BINS, SC_ROFF, SC_NEXT };
-struct Pipe3 {
-    Stage3 st[TR_STAGES];
-    unsigned long long full[TR_STAGES], empty[TR_STAGES];
-};
 
-__device__ __forceinline__ double ldvw(const uint32_t* vw, uint32_t i, uint32_t G) { return __hiloint2double((int)vw[i + G], (int)vw[i]); }
+// one Vw value from its two staged 32-bit words: `lo` / `hi` are shared-space byte addresses of word 0 of the low / high plane
+// of the record's bin, OFF the compile-time word offset of the cell
+template <int OFF>
+__device__ __forceinline__ double ldvw(uint32_t lo, uint32_t hi)
+{
+    uint32_t a, b;
+    asm("ld.shared.u32 %0, [%1+%2];" : "=r"(a) : "r"(lo), "n"(OFF * 4));
+    asm("ld.shared.u32 %0, [%1+%2];" : "=r"(b) : "r"(hi), "n"(OFF * 4));
+    return __hiloint2double((int)b, (int)a);
+}
 
-// One J block of the sum for TWO records of the group (A and B, 32 stream positions apart) with the ket range size NK
-// known at compile time and a run-time loop over the bra rows (blocks with more than 4 rows or columns):
-//   sum_i cb(i) * sum_k ck(k) * Vw[i][k],  cb/ck read from the tuples' coefficient tables (one gather per row),
-// Vw rows (padded to even length) read from the staged word planes.
+// N consecutive coefficients of one m-state in a J block (16-byte aligned when N is even)
+template <int N>
+__device__ __forceinline__ void ldcoef(const double* __restrict__ p, double (&c)[N])
+{
+    if constexpr (N % 2 == 0) {
+#pragma unroll
+        for (int i = 0; i < N / 2; i++) {
+            const double2 v = __ldg(reinterpret_cast<const double2*>(p) + i);
+            c[2 * i] = v.x;
+            c[2 * i + 1] = v.y;
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < N; i++) c[i] = __ldg(p + i);
+    }
+}
+
+// One J block of the sum for TWO records of the group (A and B, 32 stream positions apart):
+//   sum_i cb(i) * sum_k ck(k) * Vw[i][k],   cb = bq[sigma_b * nb + i],  ck = kq[sigma_k * nk + k]
+// (bq, kq: the J block of the bra / ket tuple's coefficient table), Vw rows (padded to even length) read from the staged
+// word planes at vi + i * P + k.  Bra and ket range sizes known at compile time: every load of the block is issued before
+// the first multiply, the loop control is shared by the two records.
+template <int NB, int NK, int I>
+__device__ __forceinline__ void vw_row(uint32_t lo, uint32_t hi, double (&v)[NK])
+{
+    constexpr int P = (NK + 1) & ~1;
+    if constexpr (NK >= 1) v[0] = ldvw<I * P + 0>(lo, hi);
+    if constexpr (NK >= 2) v[1] = ldvw<I * P + 1>(lo, hi);
+    if constexpr (NK >= 3) v[2] = ldvw<I * P + 2>(lo, hi);
+    if constexpr (NK >= 4) v[3] = ldvw<I * P + 3>(lo, hi);
+    if constexpr (NK >= 5) v[4] = ldvw<I * P + 4>(lo, hi);
+    if constexpr (NK >= 6) v[5] = ldvw<I * P + 5>(lo, hi);
+    if constexpr (NK >= 7) v[6] = ldvw<I * P + 6>(lo, hi);
+    if constexpr (NK >= 8) v[7] = ldvw<I * P + 7>(lo, hi);
+}
+template <int NB, int NK, int I>
+__device__ __forceinline__ void j_rows(const double (&ckA)[NK], const double (&ckB)[NK], const double (&cbA)[NB], const double (&cbB)[NB],
+                                       uint32_t loA, uint32_t hiA, uint32_t loB, uint32_t hiB, double& tA, double& tB)
+{
+    if constexpr (I < NB) {
+        double vA[NK], vB[NK];
+        vw_row<NB, NK, I>(loA, hiA, vA);
+        vw_row<NB, NK, I>(loB, hiB, vB);
+        double accA = ckA[0] * vA[0], accB = ckB[0] * vB[0];
+#pragma unroll
+        for (int k = 1; k < NK; k++) {
+            accA = fma(ckA[k], vA[k], accA);
+            accB = fma(ckB[k], vB[k], accB);
+        }
+        tA = fma(cbA[I], accA, tA);
+        tB = fma(cbB[I], accB, tB);
+        j_rows<NB, NK, I + 1>(ckA, ckB, cbA, cbB, loA, hiA, loB, hiB, tA, tB);
+    }
+}
+// boff / koff: offsets (doubles) of the J block in the bra / ket tuple's coefficient table; loA.. : shared-space byte addresses
+// of the block's first Vw cell in the low / high word plane of record A's / B's bin
+template <int NB, int NK>
+__device__ __forceinline__ void j_block3x2(const double* __restrict__ dtab, uint32_t boff, uint32_t koff, uint32_t sbA,
+                                           uint32_t skA, uint32_t sbB, uint32_t skB, uint32_t loA, uint32_t hiA, uint32_t loB, uint32_t hiB,
+                                           double& totA, double& totB)
+{
+    double ckA[NK], ckB[NK], cbA[NB], cbB[NB];
+    ldcoef<NK>(dtab + (koff + skA * NK), ckA);
+    ldcoef<NK>(dtab + (koff + skB * NK), ckB);
+    ldcoef<NB>(dtab + (boff + sbA * NB), cbA);
+    ldcoef<NB>(dtab + (boff + sbB * NB), cbB);
+    double tA = 0.0, tB = 0.0;
+    j_rows<NB, NK, 0>(ckA, ckB, cbA, cbB, loA, hiA, loB, hiB, tA, tB);
+    totA += tA;
+    totB += tB;
+}
+// The same with a run-time loop over the bra rows (blocks with more than 4 rows or columns, NK <= 8)
 template <int NK>
-__device__ __forceinline__ void j_block3x2_rows(const double* __restrict__ dtab, const uint32_t* vw, uint32_t& pbA, uint32_t& pkA,
-                                                uint32_t& pbB, uint32_t& pkB, uint32_t Sb, uint32_t Sk, int nb, uint32_t& viA,
-                                                uint32_t& viB, uint32_t G, double& totA, double& totB)
+__device__ __forceinline__ void j_block3x2_rows(const double* __restrict__ dtab, uint32_t boff, uint32_t koff, uint32_t sbA,
+                                                uint32_t skA, uint32_t sbB, uint32_t skB, int nb, uint32_t loA, uint32_t hiA, uint32_t loB,
+                                                uint32_t hiB, double& totA, double& totB)
 {
     constexpr int P = (NK + 1) & ~1;
     double ckA[NK], ckB[NK];
-#pragma unroll
-    for (int k = 0; k < NK; k++) {
-        ckA[k] = __ldg(dtab + pkA + (uint32_t)k * Sk);
-        ckB[k] = __ldg(dtab + pkB + (uint32_t)k * Sk);
-    }
-    pkA += NK * Sk; pkB += NK * Sk;
+    ldcoef<NK>(dtab + (koff + skA * NK), ckA);
+    ldcoef<NK>(dtab + (koff + skB * NK), ckB);
+    const double* __restrict__ bA = dtab + (boff + sbA * (uint32_t)nb);
+    const double* __restrict__ bB = dtab + (boff + sbB * (uint32_t)nb);
     double tA = 0.0, tB = 0.0;
 #pragma unroll 2
     for (int i = 0; i < nb; i++) {
-        const double cbA = __ldg(dtab + pbA), cbB = __ldg(dtab + pbB);
-        pbA += Sb; pbB += Sb;
+        const double cbA = __ldg(bA + i), cbB = __ldg(bB + i);
         double vA[NK], vB[NK];
-#pragma unroll
-        for (int k = 0; k < NK; k++) {
-            vA[k] = ldvw(vw, viA + k, G);
-            vB[k] = ldvw(vw, viB + k, G);
-        }
-        viA += P; viB += P;
+        vw_row<1, NK, 0>(loA, hiA, vA);
+        vw_row<1, NK, 0>(loB, hiB, vB);
+        loA += P * 4; hiA += P * 4; loB += P * 4; hiB += P * 4;
         double accA = ckA[0] * vA[0], accB = ckB[0] * vB[0];
 #pragma unroll
         for (int k = 1; k < NK; k++) {
@@ -711,110 +796,69 @@ __device__ __forceinline__ void j_block3x2_rows(const double* __restrict__ dtab,
     totB += tB;
 }
 
-// The same J block with bra and ket range sizes both known at compile time: every load of the block is issued before
-// the first multiply, the loop control is shared by the two records.
-template <int NB, int NK>
-__device__ __forceinline__ void j_block3x2(const double* __restrict__ dtab, const uint32_t* vw, uint32_t& pbA, uint32_t& pkA,
-                                           uint32_t& pbB, uint32_t& pkB, uint32_t Sb, uint32_t Sk, uint32_t& viA, uint32_t& viB,
-                                           uint32_t G, double& totA, double& totB)
-{
-    constexpr int P = (NK + 1) & ~1;
-    double ckA[NK], ckB[NK], cbA[NB], cbB[NB];
-#pragma unroll
-    for (int k = 0; k < NK; k++) {
-        ckA[k] = __ldg(dtab + pkA + (uint32_t)k * Sk);
-        ckB[k] = __ldg(dtab + pkB + (uint32_t)k * Sk);
-    }
-#pragma unroll
-    for (int i = 0; i < NB; i++) {
-        cbA[i] = __ldg(dtab + pbA + (uint32_t)i * Sb);
-        cbB[i] = __ldg(dtab + pbB + (uint32_t)i * Sb);
-    }
-    double tA = 0.0, tB = 0.0;
-#pragma unroll
-    for (int i = 0; i < NB; i++) {
-        double vA[NK], vB[NK];
-#pragma unroll
-        for (int k = 0; k < NK; k++) {
-            vA[k] = ldvw(vw, viA + i * P + k, G);
-            vB[k] = ldvw(vw, viB + i * P + k, G);
-        }
-        double accA = ckA[0] * vA[0], accB = ckB[0] * vB[0];
-#pragma unroll
-        for (int k = 1; k < NK; k++) {
-            accA = fma(ckA[k], vA[k], accA);
-            accB = fma(ckB[k], vB[k], accB);
-        }
-        tA = fma(cbA[i], accA, tA);
-        tB = fma(cbB[i], accB, tB);
-    }
-    pkA += NK * Sk; pkB += NK * Sk;
-    pbA += NB * Sb; pbB += NB * Sb;
-    viA += NB * P; viB += NB * P;
-    totA += tA;
-    totB += tB;
-}
-
 // any ket range size (nk > 8): ket coefficient re-read per cell
-__device__ __noinline__ double j_block3_generic(const double* __restrict__ dtab, const uint32_t* vw, uint32_t pb, uint32_t pk, uint32_t Sb,
-                                                uint32_t Sk, int nb, int nk, uint32_t vi, uint32_t G)
+__device__ __noinline__ double j_block3_generic(const double* __restrict__ bp, const double* __restrict__ kp, int nb, int nk, uint32_t lo,
+                                                uint32_t hi)
 {
     const int P = row_pitch3(nk);
     double total = 0.0;
     for (int i = 0; i < nb; i++) {
-        const double cb = __ldg(dtab + pb + (uint32_t)i * Sb);
+        const double cb = __ldg(bp + i);
         double acc = 0.0;
         for (int k = 0; k < nk; k++) {
-            const double ck = __ldg(dtab + pk + (uint32_t)k * Sk), v = ldvw(vw, vi + k, G);
+            uint32_t a, b;
+            asm("ld.shared.u32 %0, [%1];" : "=r"(a) : "r"(lo + 4u * k));
+            asm("ld.shared.u32 %0, [%1];" : "=r"(b) : "r"(hi + 4u * k));
+            const double ck = __ldg(kp + k), v = __hiloint2double((int)b, (int)a);
             acc = k ? fma(ck, v, acc) : ck * v;
         }
         total = fma(cb, acc, total);
-        vi += P;
+        lo += 4u * P; hi += 4u * P;
     }
     return total;
 }
 
-// H3-H6.  Persistent blocks walk the item list (item k of a block = list entry blockIdx.x + k * gridDim.x) through a
-// ring of TR_STAGES stages:
-//  * the PRODUCER warp, per item: waits until every consumer warp has left the stage, reads the group's descriptors,
-//    builds the J-block table (bounds of the three nested loops of PAPER.md:61, shared by every record of the group),
-//    and starts two bulk copies (cp.async.bulk -> UBLKCP, completion on the stage's mbarrier): the group's
-//    isospin-combined slabs Vw[bin][cell] and the item's records.  It never touches the data itself, so it runs ahead
-//    of the consumers by TR_STAGES - 1 items and their loads are off the critical path;
-//  * the CONSUMER warps wait for the stage, then claim batches of 64 records (two per lane, stream order).  The stream
+// H3-H6.  Persistent blocks walk the item list (item k of a block = list entry blockIdx.x + k * gridDim.x) with up to
+// TR_SLOTS items in flight:
+//  * the PRODUCER warp, per item: reads the group's descriptors, reserves room in the block's shared-memory ring (FIFO;
+//    it waits for the oldest items to be released when the ring or the slot table is full), builds the J-block table
+//    (bounds of the three nested loops of PAPER.md:61, shared by every record of the group) and starts two bulk copies
+//    (cp.async.bulk -> UBLKCP, completion on the slot's mbarrier): the group's isospin-combined slabs Vw[bin][cell] and
+//    the item's records.  It never touches the data itself, so it runs several items ahead of the consumers and every
+//    global latency of the prologue is off their critical path;
+//  * the CONSUMER warps wait for the slot, then claim batches of 64 records (two per lane, stream order).  The stream
 //    is ordered by (group, M) and the coefficient tables are M-major: the lanes of a warp read one or two cache lines
 //    per coefficient on the bra AND on the ket side.  Every lane evaluates
 //        sum_J sum_J12 cb(J12,J) sum_J12' ck(J12',J) Vw[bin][J,J12,J12']
 //    for its records with warp-uniform loop bounds (first J block = the smallest |M| in the warp; coefficients are 0
 //    for J < |M|), and stores the signed value at the record's stream position (coalesced).
 // No block-wide barrier after the prologue.
-__global__ void __launch_bounds__(TR_THREADS, 4) k_transform3(Tables T, const uint4* __restrict__ items, const uint32_t* __restrict__ n_items_p,
-                                                          const unsigned long long* __restrict__ recs, double* __restrict__ out)
+__global__ void __launch_bounds__(TR_THREADS, MFDN_TR_MINB) k_transform3(Tables T, const uint4* __restrict__ items, const uint32_t* __restrict__ n_items_p,
+                                                                     const unsigned long long* __restrict__ recs, double* __restrict__ out)
 {
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    Pipe3& P = *reinterpret_cast<Pipe3*>(smem_raw);
+    __shared__ Pipe3 P;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) {
-        for (int s = 0; s < TR_STAGES; s++) { mbar_init(&P.full[s], 1u); mbar_init(&P.empty[s], (uint32_t)TR_CW); }
+        for (int s = 0; s < TR_SLOTS; s++) { mbar_init(&P.full[s], 1u); mbar_init(&P.empty[s], (uint32_t)TR_CW); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
     const uint32_t n_items = __ldg(n_items_p);
     const uint32_t nt = (uint32_t)T.n_tup3;
     if (warp == TR_CW) {
-        // ------------------------------------------------------------------ producer
-        uint32_t k = 0;
+        // ------------------------------------------------------------------ producer (all lanes run the same control flow)
+        uint32_t k = 0, rel = 0, head = 0;       // items issued, items released (FIFO), next free ring word
         for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x, k++) {
-            const uint32_t s = k % TR_STAGES;
-            Stage3& st = P.st[s];
+            const uint32_t s = k % TR_SLOTS;
             const uint4 item = __ldg(items + it);
             const uint32_t pos0 = item.x, cnt = item.y, g = item.z;
-            // descriptor loads first: they do not need the stage
+            const bool zero = g == ZERO_ITEM;
+            // descriptor loads first: they do not need the slot
             int4 kb = make_int4(0, 0, 0, 0), kk = kb;
             uint4 sg = make_uint4(0u, 0u, 0u, 0u);
             int2 jb = make_int2(0, 0), jk = make_int2(0, 0);
             int gJlo = 0, gnblk = 0;
-            if (g != ZERO_ITEM) {
+            if (!zero) {
                 const uint32_t tb = g / nt, tk = g - tb * nt;
                 kb = __ldg(T.tk3 + tb);
                 kk = __ldg(T.tk3 + tk);
@@ -827,44 +871,67 @@ __global__ void __launch_bounds__(TR_THREADS, 4) k_transform3(Tables T, const ui
                     jk = __ldg(T.jinfo3 + kk.z + ((gJlo - Jmink) >> 1) + lane);
                 }
             }
-            mbar_wait(&P.empty[s], ((k / TR_STAGES) & 1u) ^ 1u);   // every consumer warp has left the stage
-            if (g == ZERO_ITEM) {
+            const uint32_t gsize = sg.y, S = vw_stride(gsize), bin_lo = item.w & 255u, bins = item.w >> 8;
+            const uint32_t vw_words = zero ? 0u : (bins * S + 3u) & ~3u;
+            const uint32_t rec_words = zero ? 0u : (((pos0 & 1u) + cnt + 1u) & ~1u) * 2u;
+            const uint32_t need = vw_words + rec_words + (uint32_t)gnblk * 4u;
+            // reserve `need` contiguous words: the live region is [start_of[rel], head), possibly wrapped
+            uint32_t at;
+            for (;;) {
+                bool ok = false;
+                at = head;
+                if (k - rel < (uint32_t)TR_SLOTS) {
+                    if (rel == k) { at = 0u; ok = true; }     // nothing in flight
+                    else {
+                        const uint32_t tail = P.start_of[rel % TR_SLOTS];
+                        if (head > tail) {
+                            if (head + need <= (uint32_t)RING_WORDS) ok = true;
+                            else if (need < tail) { at = 0u; ok = true; }
+                        } else if (head + need < tail) ok = true;
+                    }
+                }
+                if (ok) break;
+                mbar_wait(&P.empty[rel % TR_SLOTS], (rel / TR_SLOTS) & 1u);   // every consumer warp has left the oldest item
+                rel++;
+            }
+            head = at + need;
+            if (lane == 0) P.start_of[s] = at;
+            __syncwarp();
+            uint32_t* sc = P.sc[s];
+            if (zero) {
                 if (lane == 0) {
-                    st.sc[SC_POS0] = pos0; st.sc[SC_CNT] = cnt; st.sc[SC_GROUP] = ZERO_ITEM; st.sc[SC_NEXT] = 0u;
+                    sc[SC_POS0] = pos0; sc[SC_CNT] = cnt; sc[SC_GROUP] = ZERO_ITEM; sc[SC_NEXT] = 0u;
                     mbar_arrive(&P.full[s]);
                 }
                 continue;
             }
-            // exclusive prefix sums over the J blocks: bra rows, ket rows, Vw cells
+            // exclusive prefix sum of the Vw cells over the J blocks
             const uint32_t rb = (uint32_t)jb.y, rk = (uint32_t)jk.y, vv = (uint32_t)(jb.y * row_pitch3(jk.y));
-            uint32_t ib = rb, ik = rk, iv = vv;
+            uint32_t iv = vv;
 #pragma unroll
             for (int off = 1; off < 32; off <<= 1) {
-                uint32_t xb = __shfl_up_sync(0xFFFFFFFFu, ib, off), xk = __shfl_up_sync(0xFFFFFFFFu, ik, off), xv = __shfl_up_sync(0xFFFFFFFFu, iv, off);
-                if (lane >= off) { ib += xb; ik += xk; iv += xv; }
+                uint32_t xv = __shfl_up_sync(0xFFFFFFFFu, iv, off);
+                if (lane >= off) iv += xv;
             }
+            const uint32_t o_vw = at, o_rec = at + vw_words, o_desc = o_rec + rec_words;
             if (lane < gnblk) {
                 // dispatch code: 0..15 fully unrolled (nb, nk <= 4); 16 + nk row-loop templates (nk <= 8); 25 generic
                 const uint32_t code = (rb - 1u < 4u && rk - 1u < 4u) ? (rb - 1u) * 4u + (rk - 1u) : (rk - 1u < 8u && rb > 0u) ? 16u + rk : 25u;
-                st.desc[lane] = make_uint4(rb | (rk << 8) | (code << 16), ib - rb, ik - rk, iv - vv);
+                *reinterpret_cast<uint4*>(&P.ring[o_desc + 4u * lane]) =
+                    make_uint4(rb | (rk << 8) | (code << 16), (uint32_t)kb.x + (uint32_t)jb.x, (uint32_t)kk.x + (uint32_t)jk.x, iv - vv);
             }
-            const uint32_t gsize = sg.y, S = vw_stride(gsize), bin_lo = item.w & 255u, bins = item.w >> 8;
             if (lane == 0) {
-                st.sc[SC_POS0] = pos0; st.sc[SC_CNT] = cnt; st.sc[SC_GROUP] = g;
-                st.sc[SC_SB] = (uint32_t)kb.y; st.sc[SC_SK] = (uint32_t)kk.y;
-                st.sc[SC_PB0] = (uint32_t)kb.x + (uint32_t)jb.x * (uint32_t)kb.y;
-                st.sc[SC_PK0] = (uint32_t)kk.x + (uint32_t)jk.x * (uint32_t)kk.y;
-                st.sc[SC_JINFO] = ((uint32_t)kb.w & 0xFFu) | ((uint32_t)gJlo << 8) | ((uint32_t)gnblk << 16);
-                st.sc[SC_GSIZE] = gsize; st.sc[SC_STRIDE] = S; st.sc[SC_BINS] = item.w; st.sc[SC_ROFF] = pos0 & 1u;
-                st.sc[SC_NEXT] = 0u;
+                sc[SC_POS0] = pos0; sc[SC_CNT] = cnt; sc[SC_GROUP] = g;
+                sc[SC_SB] = 0u; sc[SC_SK] = 0u; sc[SC_PB0] = 0u; sc[SC_PK0] = 0u;
+                sc[SC_JINFO] = ((uint32_t)kb.w & 0xFFu) | ((uint32_t)gJlo << 8) | ((uint32_t)gnblk << 16);
+                sc[SC_GSIZE] = gsize; sc[SC_STRIDE] = S; sc[SC_BINS] = item.w; sc[SC_ROFF] = pos0 & 1u;
+                sc[SC_VW] = o_vw; sc[SC_REC] = o_rec; sc[SC_DESC] = o_desc; sc[SC_NEXT] = 0u;
             }
             __syncwarp();
             if (lane == 0) {
-                const uint32_t vw_bytes = (bins * S * 4u + 15u) & ~15u;
-                const uint32_t rec_bytes = (((pos0 & 1u) + cnt + 1u) & ~1u) * 8u;
-                mbar_arrive_tx(&P.full[s], vw_bytes + rec_bytes);
-                bulk_g2s(st.vw, T.vw20 + (size_t)sg.z * 4 + (size_t)bin_lo * S, vw_bytes, &P.full[s]);
-                bulk_g2s(st.rec, recs + (pos0 & ~1u), rec_bytes, &P.full[s]);
+                mbar_arrive_tx(&P.full[s], (vw_words + rec_words) * 4u);
+                bulk_g2s(&P.ring[o_vw], T.vw20 + (size_t)sg.z * 4 + (size_t)bin_lo * S, vw_words * 4u, &P.full[s]);
+                bulk_g2s(&P.ring[o_rec], recs + (pos0 & ~1u), rec_words * 4u, &P.full[s]);
             }
         }
         return;
@@ -873,30 +940,32 @@ __global__ void __launch_bounds__(TR_THREADS, 4) k_transform3(Tables T, const ui
     const double* __restrict__ dtab = T.dtab3;
     uint32_t k = 0;
     for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x, k++) {
-        const uint32_t s = k % TR_STAGES;
-        Stage3& st = P.st[s];
-        mbar_wait(&P.full[s], (k / TR_STAGES) & 1u);
-        const uint4 s0 = *reinterpret_cast<const uint4*>(&st.sc[0]);    // pos0, cnt, group, Sb
+        const uint32_t s = k % TR_SLOTS;
+        uint32_t* sc = P.sc[s];
+        mbar_wait(&P.full[s], (k / TR_SLOTS) & 1u);
+        const uint4 s0 = *reinterpret_cast<const uint4*>(&sc[0]);    // pos0, cnt, group, -
         const uint32_t pos0 = s0.x, cnt = s0.y;
         if (s0.z == ZERO_ITEM) {
             for (;;) {
                 uint32_t b = 0;
-                if (lane == 0) b = atomicAdd(&st.sc[SC_NEXT], 1u);
+                if (lane == 0) b = atomicAdd(&sc[SC_NEXT], 1u);
                 b = __shfl_sync(0xFFFFFFFFu, b, 0) * BATCH3;
                 if (b >= cnt) break;
                 if (b + lane < cnt) out[pos0 + b + lane] = 0.0;
                 if (b + 32 + lane < cnt) out[pos0 + b + 32 + lane] = 0.0;
             }
         } else {
-            const uint4 s1 = *reinterpret_cast<const uint4*>(&st.sc[4]);    // Sk, pb0, pk0, jinfo
-            const uint4 s2 = *reinterpret_cast<const uint4*>(&st.sc[8]);    // gsize, stride, bins, roff
-            const uint32_t Sb = s0.w, Sk = s1.x, G = s2.x, S = s2.y, bin_lo = s2.z & 255u, bins = s2.z >> 8;
+            const uint4 s1 = *reinterpret_cast<const uint4*>(&sc[4]);    // -, -, -, jinfo
+            const uint4 s2 = *reinterpret_cast<const uint4*>(&sc[8]);    // gsize, stride, bins, roff
+            const uint4 s3 = *reinterpret_cast<const uint4*>(&sc[12]);   // ring offsets: vw, rec, desc
+            const uint32_t G = s2.x, S = s2.y, bin_lo = s2.z & 255u, bins = s2.z >> 8;
             const int sumj = s1.w & 255, Jlo = (s1.w >> 8) & 255, nblk = (int)(s1.w >> 16);
-            const unsigned long long* __restrict__ irec = st.rec + s2.w;
-            const uint32_t* vw = st.vw;
+            const unsigned long long* irec = reinterpret_cast<const unsigned long long*>(&P.ring[s3.y]) + s2.w;
+            const uint32_t vw0 = smem_u32(&P.ring[s3.x]), G4 = G * 4u;
+            const uint4* desc = reinterpret_cast<const uint4*>(&P.ring[s3.z]);
             for (;;) {
                 uint32_t base = 0;
-                if (lane == 0) base = atomicAdd(&st.sc[SC_NEXT], 1u);
+                if (lane == 0) base = atomicAdd(&sc[SC_NEXT], 1u);
                 base = __shfl_sync(0xFFFFFFFFu, base, 0) * BATCH3;
                 if (base >= cnt) break;
                 // lane l takes stream positions base+l (A) and base+32+l (B); lanes past the end of the item redo its last
@@ -908,21 +977,16 @@ __global__ void __launch_bounds__(TR_THREADS, 4) k_transform3(Tables T, const ui
                 const int aMA = abs(2 * ((int)(rcA >> 30) & 63) - sumj), aMB = abs(2 * ((int)(rcB >> 30) & 63) - sumj);
                 // first block with J >= |M| of any record of the warp (coefficients are 0 below a record's own |M|)
                 const int q0 = max(0, ((int)__reduce_min_sync(0xFFFFFFFFu, (unsigned)min(aMA, aMB)) - Jlo + 1) >> 1);
-                uint32_t pbA = s1.y + (loA & 0xFFFu), pkA = s1.z + ((loA >> 12) & 0xFFFu), viA = min(blA, bins - 1u) * S;
-                uint32_t pbB = s1.y + (loB & 0xFFFu), pkB = s1.z + ((loB >> 12) & 0xFFFu), viB = min(blB, bins - 1u) * S;
-                if (q0 > 0 && q0 < nblk) {
-                    const uint4 d = st.desc[q0];
-                    pbA += d.y * Sb; pbB += d.y * Sb;
-                    pkA += d.z * Sk; pkB += d.z * Sk;
-                    viA += d.w; viB += d.w;
-                }
+                const uint32_t sbA = loA & 0xFFFu, skA = (loA >> 12) & 0xFFFu, wA = vw0 + min(blA, bins - 1u) * S * 4u;
+                const uint32_t sbB = loB & 0xFFFu, skB = (loB >> 12) & 0xFFFu, wB = vw0 + min(blB, bins - 1u) * S * 4u;
                 double totA = 0.0, totB = 0.0;
                 for (int q = q0; q < nblk; q++) {
-                    const uint32_t d = st.desc[q].x;
-                    const int nb = d & 255, nk = (d >> 8) & 255;
-#define MFDN_BLK(NB, NK) case ((NB) - 1) * 4 + ((NK) - 1): j_block3x2<NB, NK>(dtab, vw, pbA, pkA, pbB, pkB, Sb, Sk, viA, viB, G, totA, totB); break;
-#define MFDN_ROWS(NK) case 16 + (NK): j_block3x2_rows<NK>(dtab, vw, pbA, pkA, pbB, pkB, Sb, Sk, nb, viA, viB, G, totA, totB); break;
-                    switch (d >> 16) {
+                    const uint4 d = desc[q];
+                    const int nb = d.x & 255, nk = (d.x >> 8) & 255;
+                    const uint32_t vlA = wA + d.w * 4u, vlB = wB + d.w * 4u, vhA = vlA + G4, vhB = vlB + G4;
+#define MFDN_BLK(NB, NK) case ((NB) - 1) * 4 + ((NK) - 1): j_block3x2<NB, NK>(dtab, d.y, d.z, sbA, skA, sbB, skB, vlA, vhA, vlB, vhB, totA, totB); break;
+#define MFDN_ROWS(NK) case 16 + (NK): j_block3x2_rows<NK>(dtab, d.y, d.z, sbA, skA, sbB, skB, nb, vlA, vhA, vlB, vhB, totA, totB); break;
+                    switch (d.x >> 16) {
                         MFDN_BLK(1, 1) MFDN_BLK(1, 2) MFDN_BLK(1, 3) MFDN_BLK(1, 4)
                         MFDN_BLK(2, 1) MFDN_BLK(2, 2) MFDN_BLK(2, 3) MFDN_BLK(2, 4)
                         MFDN_BLK(3, 1) MFDN_BLK(3, 2) MFDN_BLK(3, 3) MFDN_BLK(3, 4)
@@ -930,12 +994,9 @@ __global__ void __launch_bounds__(TR_THREADS, 4) k_transform3(Tables T, const ui
                         MFDN_ROWS(1) MFDN_ROWS(2) MFDN_ROWS(3) MFDN_ROWS(4) MFDN_ROWS(5) MFDN_ROWS(6) MFDN_ROWS(7) MFDN_ROWS(8)
                         default: {
                             if (nk > 0 && nb > 0) {
-                                totA += j_block3_generic(dtab, vw, pbA, pkA, Sb, Sk, nb, nk, viA, G);
-                                totB += j_block3_generic(dtab, vw, pbB, pkB, Sb, Sk, nb, nk, viB, G);
+                                totA += j_block3_generic(dtab + (d.y + sbA * (uint32_t)nb), dtab + (d.z + skA * (uint32_t)nk), nb, nk, vlA, vhA);
+                                totB += j_block3_generic(dtab + (d.y + sbB * (uint32_t)nb), dtab + (d.z + skB * (uint32_t)nk), nb, nk, vlB, vhB);
                             }
-                            pbA += (uint32_t)nb * Sb; pbB += (uint32_t)nb * Sb;
-                            pkA += (uint32_t)nk * Sk; pkB += (uint32_t)nk * Sk;
-                            if (nk > 0) { viA += (uint32_t)(nb * row_pitch3(nk)); viB += (uint32_t)(nb * row_pitch3(nk)); }
                             break;
                         }
                     }
@@ -1099,13 +1160,12 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
                                                                              (uint32_t)n, c->t.sgrp3, itm, last_slot, cnt);
             if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.b, st));
             if (c->tr_blocks_per_sm == 0) {
-                MFDN_CUDA(c, cudaFuncSetAttribute(k_transform3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Pipe3)));
                 int per_sm = 0;
-                MFDN_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_transform3, TR_THREADS, sizeof(Pipe3)));
+                MFDN_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_transform3, TR_THREADS, 0));
                 c->tr_blocks_per_sm = std::max(per_sm, 1);
             }
             const unsigned grid = (unsigned)std::min<long long>(max_items, (long long)c->num_sms * c->tr_blocks_per_sm);
-            k_transform3<<<grid, TR_THREADS, sizeof(Pipe3), st>>>(c->t, itm, cnt, trecs, tout);
+            k_transform3<<<grid, TR_THREADS, 0, st>>>(c->t, itm, cnt, trecs, tout);
             const unsigned grid_s = (unsigned)std::min<long long>((std::min<long long>(n, nt * nt + 1) + 3) / 4, (long long)c->num_sms * 16);
             k_transform3_small<<<grid_s, 128, 0, st>>>(c->t, itm, last_slot, cnt, trecs, tout);
             c->launches += 3;
