@@ -447,7 +447,7 @@ __global__ void __launch_bounds__(256) k_scatter(long long n, const unsigned lon
 #pragma unroll
     for (int u = 0; u < SC_PER_THREAD; u++) {
         const long long i = base + u * 256;
-        r[u] = i < n ? __ldg(recs + i) : 0ull;
+        r[u] = i < n ? __ldcs(recs + i) : 0ull;   // streamed once: evict first, keep the write frontier of `sorted` in L2
     }
 #pragma unroll
     for (int u = 0; u < SC_PER_THREAD; u++) {   // SC_PER_THREAD independent atomics in flight per thread
@@ -460,7 +460,7 @@ __global__ void __launch_bounds__(256) k_scatter(long long n, const unsigned lon
         const long long i = base + u * 256;
         if (i < n) {
             sorted[pos[u]] = r[u];
-            posof[i] = pos[u];
+            __stcs(posof + i, pos[u]);
         }
     }
 }
@@ -474,12 +474,12 @@ __global__ void __launch_bounds__(256) k_unpermute(long long n, const double* __
 #pragma unroll
     for (int u = 0; u < SC_PER_THREAD; u++) {
         const long long i = base + u * 256;
-        p[u] = i < n ? __ldg(posof + i) : 0u;
+        p[u] = i < n ? __ldcs(posof + i) : 0u;
     }
 #pragma unroll
     for (int u = 0; u < SC_PER_THREAD; u++) {
         const long long i = base + u * 256;
-        if (i < n) out[i] = __ldg(vals + p[u]);
+        if (i < n) __stcs(out + i, __ldg(vals + p[u]));
     }
 }
 
@@ -490,9 +490,11 @@ __global__ void __launch_bounds__(256) k_unpermute(long long n, const double* __
 // scanned histogram).  item = {first position, records, group | ZERO_ITEM, first isospin bin | bins << 8}: a group
 // whose 20 isospin-combined slabs exceed one stage (VW_WORDS) is evaluated in rounds over bin ranges, one item per
 // (chunk, round); a record is evaluated by the round that holds its bin.
-// Groups with at most SMALL_ITEM3 records -- and groups whose slab does not fit a stage even four bins at a time -- go
-// to a second list (filled from the END of the item array, counted in n_items[1]): a single warp evaluates them
-// directly from the five isospin planes (k_transform3_small; no capacity limit).
+// Groups with at most SMALL_ITEM3 records go to a second list (filled from the END of the item array, counted in
+// n_items[1]): a single warp evaluates them directly from the five isospin planes (k_transform3_small).  Groups whose
+// slab does not fit a stage even four bins at a time (gsize > 639: no such group in the five workloads, but tuples
+// of three j = 15/2 orbitals have one) go to the same list in chunks of SMALL_ITEM3 records: that path has no
+// capacity limit.
 constexpr uint32_t SMALL_ITEM3 = 64;
 __device__ __forceinline__ uint32_t bins_per_round3(uint32_t gsize)
 {
@@ -523,7 +525,7 @@ __global__ void __launch_bounds__(256) k_items3(const uint32_t* __restrict__ bou
     const uint32_t bpr = zero ? (uint32_t)NBIN3 : bins_per_round3(gsize);
     const bool small = cnt <= SMALL_ITEM3 || bpr == 0u;
     const uint32_t rounds = small ? 0u : (NBIN3 + bpr - 1u) / bpr;
-    const uint32_t k = small ? 0u : ((cnt + ITEM3 - 1) / ITEM3) * rounds, ks = (small && cnt) ? 1u : 0u;
+    const uint32_t k = small ? 0u : ((cnt + ITEM3 - 1) / ITEM3) * rounds, ks = small ? (cnt + SMALL_ITEM3 - 1) / SMALL_ITEM3 : 0u;
     // warp-aggregated append: the lists stay (nearly) in group order, neighbours share the bra tuple's tables
     const int lane = threadIdx.x & 31;
     uint32_t incl = k, incs = ks;
@@ -540,7 +542,8 @@ __global__ void __launch_bounds__(256) k_items3(const uint32_t* __restrict__ bou
     if (cnt == 0) return;
     const uint32_t gz = zero ? ZERO_ITEM : g;
     if (small) {
-        items[last_slot - (bases + incs - 1u)] = make_uint4(start, cnt, gz, 0u);
+        uint32_t slot = last_slot - (bases + incs - ks);
+        for (uint32_t j = 0; j * SMALL_ITEM3 < cnt; j++) items[slot--] = make_uint4(start + j * SMALL_ITEM3, min(SMALL_ITEM3, cnt - j * SMALL_ITEM3), gz, 0u);
         return;
     }
     uint32_t slot = base + incl - k;
@@ -1075,8 +1078,9 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
     const bool sort = !naive && !(flags & MFDN_PRESORTED);
     const bool items = !naive && BODY == 3;    // the 3-body transform walks a list of one-group work items
     const bool hist_needed = sort || items;
-    // work items: at most 5 rounds per chunk of a group with more than SMALL_ITEM3 records, one entry per small group
-    const long long max_items = 5 * (n / ITEM3 + n / (SMALL_ITEM3 + 1) + 1) + std::min<long long>(n, nt * nt + 1) + 1;
+    // work items: at most 5 rounds per chunk of a group with more than SMALL_ITEM3 records; one entry per small group
+    // or per SMALL_ITEM3 records of an oversized one
+    const long long max_items = 5 * (n / ITEM3 + n / (SMALL_ITEM3 + 1) + 1) + n / SMALL_ITEM3 + std::min<long long>(n, nt * nt + 1) + 1;
     size_t need = 256;
     size_t o_recs = 0, o_sorted = 0, o_order = 0, o_hist = 0, o_sums = 0, o_items = 0, o_count = 0;
     if (!naive) {

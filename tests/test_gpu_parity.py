@@ -291,3 +291,123 @@ def test_3b_upload_rules(torch, B):
     B.mfdn_coupled_upload_3b(ctx, 2, small.chan_twoJ, small.chan_twoT, small.chan_par, small.chan_dim, small.chan_off,
                              small.state_a, small.state_b, small.state_c, small.state_J12, small.state_T12, small.values)
     B.mfdn_destroy(ctx)
+
+
+# --------------------------------------------------------------------------------- synthetic bases: rarely taken kernel paths
+def _custom_basis(orbs):
+    """Basis of the listed (n, l, 2j) orbitals, SPS laid out like workloads.ho_basis."""
+    n = np.array([o[0] for o in orbs], np.int32)
+    l = np.array([o[1] for o in orbs], np.int32)
+    tj = np.array([o[2] for o in orbs], np.int32)
+    so, sm, st = [], [], []
+    for o, (_, _, twoj) in enumerate(orbs):
+        for twotz in (1, -1):
+            for twom in range(-twoj, twoj + 1, 2):
+                so.append(o)
+                sm.append(twom)
+                st.append(twotz)
+    return W.Basis(n, l, tj, np.array(so, np.int32), np.array(sm, np.int32), np.array(st, np.int32))
+
+
+def _check_all_modes(torch, B, oracle, basis, table, req):
+    cfg = type("Cfg", (), {"table": table})
+    ctx = B.Context(basis, 0).upload(table)
+    want, wmask, _, _ = oracle.mscheme(basis, table, req)
+    assert wmask.mean() > 0.5
+    for flags in (0, B.MFDN_FORCE_NAIVE):
+        got, gmask = run_gpu(torch, ctx, req, flags)
+        check(cfg, got, gmask, want, wmask)
+    sreq, order = presort(torch, ctx, req)
+    got, gmask = run_gpu(torch, ctx, sreq, B.MFDN_PRESORTED)
+    check(cfg, got, gmask, want[order], wmask[order])
+    ctx.close()
+
+
+def test_wide_j_blocks_generic_branch(torch, B, oracle):
+    """Tuples (0g9/2, 0g9/2, 0g9/2) and (0g9/2, 0g9/2, 0h11/2) have TEN J12 rows at J = 9/2 resp. 11/2: the J blocks
+    wider than 8 take the generic branch of k_transform3 (dispatch code 25), and their isospin-combined slabs
+    (about 600 cells per bin) are staged four bins at a time (five rounds per work item).  No config of
+    BASELINE.json reaches either path (at most 8 rows per (tuple, J))."""
+    basis = _custom_basis([(0, 4, 9), (0, 5, 11)])
+    table = W.coupled_3b(basis, 13, 11)
+    ms = W.mstates(basis, 3, 13)
+    req = W.sampled_pairs(ms, 60000, 2011, permute_frac=0.02)
+    _check_all_modes(torch, B, oracle, basis, table, req)
+
+
+def test_oversized_group_plane(torch, B, oracle):
+    """The triple of three 0j15/2 orbitals has 4096 m-states (accepted) and a group plane of more than 2000 cells:
+    too large for the staged path even four bins at a time.  Such groups are evaluated in chunks by the
+    direct kernel (k_transform3_small) -- an error-free, capacity-free route, never a hang."""
+    basis = _custom_basis([(0, 7, 15)])
+    table = W.coupled_3b(basis, 21, 12)
+    ms = W.mstates(basis, 3, 21)
+    req = W.sampled_pairs(ms, 20000, 2012, permute_frac=0.02)
+    _check_all_modes(torch, B, oracle, basis, table, req)
+
+
+# --------------------------------------------------------------------------------- full size, bench launch configs of configs 1 and 4
+def test_full_size_config1_sampled(torch, B, oracle):
+    """BASELINE.json config 1 at its full size: 2^26 two-body requests, unsorted and MFDN_PRESORTED, checked on 2^16
+    sampled outputs the oracle computes one by one."""
+    cfg = get_cfg(1)
+    ctx = get_ctx(B, 1)
+    n = 1 << 26
+    req = cfg.requests(n)
+    d_req = torch.from_numpy(req).cuda()
+    out, mask = ctx.mscheme(d_req, flags=0)
+    torch.cuda.synchronize()
+    sample = np.sort(np.random.default_rng(78).choice(n, 1 << 16, replace=False))
+    want, wmask, _, _ = oracle.mscheme(cfg.basis, cfg.table, req[sample])
+    ds = torch.from_numpy(sample).cuda()
+    check(cfg, out[ds].cpu().numpy(), mask[ds].cpu().numpy(), want, wmask)
+    assert 0.93 < float(mask.float().mean()) < 0.955       # SURVEY.md 8(a): ~94.3% of sampled pairs have mask 1
+    assert bool((out[mask == 0] == 0).all())
+    keys = ctx.group_keys(d_req)
+    order = torch.argsort(keys.view(torch.int32).to(torch.int64) & 0xFFFFFFFF)
+    del keys
+    d_sorted = d_req[order].contiguous()
+    del d_req
+    out3, mask3 = ctx.mscheme(d_sorted, flags=B.MFDN_PRESORTED)
+    torch.cuda.synchronize()
+    assert bool((out3 == out[order]).all()) and bool((mask3 == mask[order]).all())
+
+
+def test_full_size_config4_batches(torch, B, oracle):
+    """BASELINE.json config 4 in the shape bench/report time it: 2^28 requests as 16 batches of 2^24, issued round-robin
+    on two streams with their own scratch; every batch checked on 2^16 sampled outputs against the oracle."""
+    cfg = get_cfg(4)
+    ctx = get_ctx(B, 4)
+    nb, n = 16, 1 << 24
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    need = ctx.work_bytes(3, n)
+    bufs = [dict(req=torch.empty((n, 6), dtype=torch.int32, device="cuda"), out=torch.empty(n, dtype=torch.float64, device="cuda"),
+                 mask=torch.empty(n, dtype=torch.uint8, device="cuda"), work=torch.empty(need, dtype=torch.uint8, device="cuda"))
+            for _ in streams]
+    pending = [None, None]
+    rng = np.random.default_rng(79)
+    mask_frac = []
+
+    def verify(slot):
+        b, req, sample = pending[slot]
+        streams[slot].synchronize()
+        ds = torch.from_numpy(sample).cuda()
+        want, wmask, _, _ = oracle.mscheme(cfg.basis, cfg.table, req[sample])
+        check(cfg, bufs[slot]["out"][ds].cpu().numpy(), bufs[slot]["mask"][ds].cpu().numpy(), want, wmask)
+        mask_frac.append(float(bufs[slot]["mask"].float().mean()))
+        pending[slot] = None
+
+    for b in range(nb):
+        slot = b % 2
+        if pending[slot] is not None:
+            verify(slot)
+        req = cfg.requests(n, start=b * n)
+        s = streams[slot]
+        with torch.cuda.stream(s):
+            bufs[slot]["req"].copy_(torch.from_numpy(req), non_blocking=False)
+            ctx.mscheme(bufs[slot]["req"], bufs[slot]["out"], bufs[slot]["mask"], 0, bufs[slot]["work"], s.cuda_stream)
+        pending[slot] = (b, req, np.sort(rng.choice(n, 1 << 16, replace=False)))
+    for slot in range(2):
+        if pending[slot] is not None:
+            verify(slot)
+    assert len(mask_frac) == nb and all(0.98 < f <= 1.0 for f in mask_frac)   # SURVEY.md 8(a): ~99.4%
