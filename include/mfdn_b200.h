@@ -39,14 +39,19 @@ typedef enum {
 
 /* flags of mfdn_mscheme_2b/3b */
 enum {
-    MFDN_PRESORTED = 1,   /* requests are already ordered by orbital-tuple group: NON-DECREASING mfdn_group_keys value
-                             (requests failing S1-S6, key 0xFFFFFFFF, last).  Skips the scatter of step H2 and the
-                             gather of step H6; 3-body still histograms the keys to cut the stream into one-group
-                             work items.  Input that is not so ordered gives undefined VALUES (never a fault);
-                             the mask stays correct */
+    MFDN_PRESORTED = 1,   /* requests are already ordered by the library's sort key: NON-DECREASING mfdn_group_keys value
+                             (2-body: orbital-tuple group; 3-body: group, then M; requests failing S1-S6, key
+                             0xFFFFFFFF, last).  Skips the scatter of step H2 and the gather of step H6; 3-body still
+                             histograms the keys to cut the stream into one-group work items.  Input that is not so
+                             ordered gives undefined VALUES (never a fault); the mask stays correct */
     MFDN_FORCE_NAIVE = 2, /* one thread per request in request order, no sort, no staging: the paper's own
                              kernel design; kept as on-device reference */
-    MFDN_FORCE_DENSE = 4  /* reserved for the dense-block path; currently ignored */
+    MFDN_FORCE_DENSE = 4  /* 3-body: every group whose blocks fit takes the dense-block path (step H5'): per (group, M,
+                             isospin pattern) the whole block C_bra * V * C_ket^T of m-scheme elements (PAPER.md:55
+                             A' = D^T A D, Fig. 1) is formed with fp64 tensor-core products (mma.sync m8n8k4) and the
+                             requested entries are picked from it; the other groups take the default path.  Values
+                             agree with the default path to rounding (another summation order), the mask bit for bit.
+                             MFDN_ERR_ARG for 2-body calls and together with MFDN_FORCE_NAIVE */
 };
 
 /* A0. Single-particle basis (quantum numbers flattened into one linear SPS index).
@@ -131,11 +136,15 @@ int mfdn_fp64_peak(mfdn_ctx*, double* tflops);
 int64_t mfdn_bad_request_count(mfdn_ctx*, void* stream);
 
 /* Sizes of what was uploaded, for reports: which = 0 tuples (2b), 1 tuples (3b), 2 slab bytes (2b),
- * 3 slab bytes (3b), 4 CG entries stage 1, 5 CG entries stage 2, 6 kernels launched so far by mscheme_*, 7 bytes of the 3-body coefficient tables. */
+ * 3 slab bytes (3b), 4 CG entries stage 1, 5 CG entries stage 2, 6 kernels launched so far by mscheme_*, 7 bytes of the
+ * 3-body coefficient tables, 8 bytes of the 3-body isospin-combined slabs, 9 number of 3-body (group, M) sort buckets. */
 int64_t mfdn_info(mfdn_ctx*, int which);
 
-/* Group key of every request, for producing MFDN_PRESORTED input: d_key[i] = bra_tuple * n_tuples +
- * ket_tuple, or 0xFFFFFFFF for requests that fail S1-S6.  body = 2 or 3.  Asynchronous on `stream`. */
+/* Sort key of every request, for producing MFDN_PRESORTED input (sort ascending by it): 2-body d_key[i] = bra_tuple *
+ * n_tuples + ket_tuple; 3-body the (group, M) bucket = first bucket of the group bra_tuple * n_tuples + ket_tuple + index
+ * of the request's M in the group's common M range (requests of one group are contiguous, ordered by M: the
+ * coefficient tables are M-major, so neighbouring requests read neighbouring entries).  0xFFFFFFFF for requests that
+ * fail S1-S6.  body = 2 or 3.  Asynchronous on `stream`. */
 int mfdn_group_keys(mfdn_ctx*, int body, int64_t n, const int32_t* d_req, uint32_t* d_key, void* stream);
 
 const char* mfdn_last_error(mfdn_ctx*);

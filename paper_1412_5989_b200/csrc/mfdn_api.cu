@@ -628,8 +628,8 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     //      a J block with one address computation and vector loads, and neighbouring m-states stay neighbours in memory.
     std::vector<int2> trow(nt), rowtab, rowdst, jinfo;
     std::vector<int4> tk(nt);
-    std::vector<int32_t> nrows(nt), sigoff(nt);
-    std::vector<uint16_t> sig;
+    std::vector<int32_t> nrows(nt), sigoff(nt), mstoff(nt);
+    std::vector<uint16_t> sig, mstart;   // mstart: per tuple, first sigma of every iM (prefix counts; sumj + 2 entries)
     uint64_t dtab_len = 0;
     for (int t = 0; t < nt; t++) {
         int4 d = tdesc[t];
@@ -664,6 +664,8 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
             std::vector<int> start(ja + jb + jc + 2, 0);
             for (int a = 0; a <= ja; a++) for (int b = 0; b <= jb; b++) for (int m = 0; m <= jc; m++) start[a + b + m + 1]++;
             for (size_t i = 1; i < start.size(); i++) start[i] += start[i - 1];
+            mstoff[t] = (int32_t)mstart.size();
+            for (int v : start) mstart.push_back((uint16_t)v);
             sig.resize(sig.size() + S);
             uint16_t* sg = sig.data() + sigoff[t];
             for (int a = 0; a <= ja; a++) for (int b = 0; b <= jb; b++) for (int m = 0; m <= jc; m++)
@@ -706,7 +708,33 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
             const uint64_t vw16 = ((uint64_t)NBIN3 * vw_stride((uint32_t)gsize) + 3) / 4;   // 16-byte units, rounded up
             if (cells + gsize * NISO3 / 2 >= 0xFFFFFFF0ull || vwcells + vw16 >= 0xFFFFFFF0ull)
                 return fail(c, MFDN_ERR_OOM, "table too large for 32-bit slab offsets");
-            sgrp[(size_t)tb * nt + tkk] = uint4{(uint32_t)cells, (uint32_t)gsize, (uint32_t)vwcells, 0u};
+            // dense-block path (H5'): feasible if every (M) block of m-states fits one warp's tile buffer and the
+            // flattened ket rows fit its row map; w = feasible << 31 | number of (bra, ket) m-state pairs with equal M
+            uint32_t dense = 0u;
+            {
+                const int sb = (db.x & 255) + ((db.x >> 8) & 255) + ((db.x >> 16) & 255);
+                const int sk = (dk.x & 255) + ((dk.x >> 8) & 255) + ((dk.x >> 16) & 255);
+                const int mm = std::min(sb, sk);
+                const uint16_t* msb = mstart.data() + mstoff[tb];
+                const uint16_t* msk = mstart.data() + mstoff[tkk];
+                uint64_t pairs = 0;
+                bool ok = true;
+                for (int mi = 0; mi <= mm; mi++) {
+                    const int ib = mi + (sb - mm) / 2, ik = mi + (sk - mm) / 2;
+                    const int nmb = msb[ib + 1] - msb[ib], nmk = msk[ik + 1] - msk[ik];
+                    pairs += (uint64_t)nmb * nmk;
+                    if (((nmb + 7) & ~7) * ((nmk + 7) & ~7) > DENSE_CAP) ok = false;
+                }
+                int rk = 0;
+                for (int twoJ = Jlo; twoJ <= Jhi; twoJ += 2) {
+                    int lk, hk;
+                    range(dk, twoJ, lk, hk);
+                    rk += std::max(0, hk - lk + 1);
+                }
+                if (rk > DENSE_RMAX) ok = false;
+                dense = (ok ? 0x80000000u : 0u) | (uint32_t)std::min<uint64_t>(pairs, 0x7FFFFFFFull);
+            }
+            sgrp[(size_t)tb * nt + tkk] = uint4{(uint32_t)cells, (uint32_t)gsize, (uint32_t)vwcells, dense};
             cells += gsize * NISO3 / 2;
             vwcells += vw16;
         }
@@ -732,6 +760,7 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     size_t o_gbase = res.add(gbase);
     size_t o_desc = tmp.add(tdesc), o_ab = res.add(ab);
     size_t o_tk = res.add(tk), o_jinfo = res.add(jinfo), o_sig = res.add(sig), o_sigoff = res.add(sigoff);
+    size_t o_mstart = res.add(mstart), o_mstoff = res.add(mstoff);
     std::vector<int64_t> coff(chan_off, chan_off + n_chan);
     std::vector<int32_t> cdim(chan_dim, chan_dim + n_chan);
     size_t o_rm = tmp.add(rowmap), o_cof = tmp.add(chan_of), o_coff = tmp.add(coff), o_cdim = tmp.add(cdim);
@@ -813,6 +842,8 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     c->t.jinfo3 = (const int2*)(dres + o_jinfo);
     c->t.dtab3 = (const double*)ddtab;
     c->t.sig3 = q.sig;
+    c->t.mstart3 = (const uint16_t*)(dres + o_mstart);
+    c->t.mstoff3 = (const int32_t*)(dres + o_mstoff);
     c->slab_bytes3 = (int64_t)(cells * 16);
     c->dtab_bytes3 = (int64_t)(dtab_len * sizeof(double));
     c->has3 = true;

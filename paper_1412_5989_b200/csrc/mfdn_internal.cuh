@@ -53,6 +53,8 @@ constexpr int ITEM3 = 512;         // max records per work item of the 3-body tr
 // into 20 different shared-memory banks: a warp whose lanes sit in any mixture of bins reads a cell with two
 // conflict-free 32-bit loads (measured: 2.0 cycles per cell against 3.7 for 64-bit loads over 20 random bins).
 __host__ __device__ inline uint32_t vw_stride(uint32_t gsize) { return 2u * gsize + 1u; }
+constexpr int DENSE_CAP = 1024;    // doubles of one (group, M, bin) block of the dense path, both dimensions padded to 8 (one warp's tile buffer)
+constexpr int DENSE_RMAX = 64;     // flattened ket rows (J, J12') of a group on the dense path
 constexpr int VW_WORDS = 5120;     // 32-bit words of one staged slab (20 KB): all 20 bins of a group with gsize <= 127
 constexpr uint32_t ZERO_ITEM = 0xFFFFFFFFu;   // work item whose records all have value 0 (no slab / failed S1-S6)
 
@@ -99,7 +101,8 @@ struct Tables {
     const int2* ab3;               // [n_orb^2] {first tuple of (a,b,*), cmin | count<<16} if every (a,b) has a dense c range, else NULL
     const int4* tdesc3;
     const uint4* sgrp3;            // [n_tup3^2] {start of the group's slab in 16-byte units or NO_SLAB, doubles per plane,
-                                   //              start of its isospin-combined slabs in vw20 in 16-byte units, -}
+                                   //              start of its isospin-combined slabs in vw20 in 16-byte units,
+                                   //              dense-block path feasible << 31 | (bra, ket) m-state pairs with equal M}
     const uint32_t* gbase3;        // [n_tup3^2 + 1] first (group, M) bucket of a group; same-parity groups own
                                    //              min(ja+jb+jc, jd+je+jf) + 1 buckets (one per common M), the others none
     uint32_t n_buckets3;           // = gbase3[n_tup3^2]; bucket n_buckets3 collects the requests failing S1-S6
@@ -109,6 +112,8 @@ struct Tables {
     const int4* tk3;               // [n_tup3] see above
     const int2* jinfo3;            // per (tuple, J): {offset of the J block in the tuple's coefficient table (doubles, even), rows nb(J)}
     const double* dtab3;           // per tuple and J block [sigma][row] = <ja ma jb mb|J12 M12> <J12 M12 jc mc|J M>, rows = J12 ascending
+    const uint16_t* mstart3;       // per tuple (at mstoff3[tuple]): first sigma of every iM, sumj + 2 entries (M-major order of the m-states)
+    const int32_t* mstoff3;
     const uint16_t* sig3;          // per tuple [(ima*(jb+1)+imb)*(jc+1)+imc] -> sigma: m-states ordered by (M, ima, imb), so that
                                    // requests with equal M (bra and ket always have equal M) read neighbouring entries
     // A2, 2-body

@@ -501,16 +501,20 @@ __device__ __forceinline__ uint32_t bins_per_round3(uint32_t gsize)
     const uint32_t b = ((uint32_t)VW_WORDS / vw_stride(gsize)) & ~3u;   // multiple of 4: every round starts 16-byte aligned
     return min(b, (uint32_t)NBIN3);
 }
+// dense_tau < 0: no group takes the dense-block path (H5'); otherwise a feasible group does if its records number at
+// least dense_tau * (its (bra, ket) m-state pairs with equal M) -- 0 = every feasible group (MFDN_FORCE_DENSE).  Such a
+// group gets one entry per non-empty (group, M) bucket in `ditems` {first position, records, group, index of M}.
 __global__ void __launch_bounds__(256) k_items3(const uint32_t* __restrict__ bounds, const uint32_t* __restrict__ gbase,
                                                uint32_t n_groups, uint32_t n_buckets, int ends, uint32_t n,
                                                const uint4* __restrict__ sgrp, uint4* __restrict__ items, uint32_t last_slot,
-                                               uint32_t* __restrict__ n_items)
+                                               uint32_t* __restrict__ n_items, float dense_tau, uint4* __restrict__ ditems)
 {
     const uint32_t g = blockIdx.x * 256u + threadIdx.x;   // g == n_groups: the bucket of the invalid requests
-    uint32_t start = 0, end = 0, gsize = 0;
-    bool zero = true;
+    uint32_t start = 0, end = 0, gsize = 0, b0 = 0, b1 = 0;
+    bool zero = true, dense = false;
     if (g <= n_groups) {
-        const uint32_t b0 = g < n_groups ? __ldg(gbase + g) : n_buckets - 1u, b1 = g < n_groups ? __ldg(gbase + g + 1) : n_buckets;
+        b0 = g < n_groups ? __ldg(gbase + g) : n_buckets - 1u;
+        b1 = g < n_groups ? __ldg(gbase + g + 1) : n_buckets;
         if (b1 > b0) {
             if (ends) { start = b0 ? bounds[b0 - 1] : 0u; end = bounds[b1 - 1]; }
             else { start = bounds[b0]; end = b1 < n_buckets ? bounds[b1] : n; }
@@ -519,7 +523,16 @@ __global__ void __launch_bounds__(256) k_items3(const uint32_t* __restrict__ bou
             const uint4 sg = __ldg(sgrp + g);
             zero = sg.x == NO_SLAB;
             gsize = sg.y;
+            dense = !zero && dense_tau >= 0.f && (sg.w >> 31) && (float)(end - start) >= dense_tau * (float)(sg.w & 0x7FFFFFFFu);
         }
+    }
+    if (dense) {   // one entry per non-empty bucket; the group is left out of the two lists below
+        for (uint32_t b = b0; b < b1; b++) {
+            const uint32_t s0 = ends ? (b ? bounds[b - 1] : 0u) : bounds[b];
+            const uint32_t s1 = ends ? bounds[b] : (b + 1 < n_buckets ? bounds[b + 1] : n);
+            if (s1 > s0) ditems[atomicAdd(n_items + 2, 1u)] = make_uint4(s0, s1 - s0, g, b - b0);
+        }
+        start = end = 0;
     }
     const uint32_t cnt = end - start;
     const uint32_t bpr = zero ? (uint32_t)NBIN3 : bins_per_round3(gsize);
@@ -1016,6 +1029,131 @@ __global__ void __launch_bounds__(TR_THREADS, MFDN_TR_MINB) k_transform3(Tables 
     }
 }
 
+// ------------------------------------------------------------------------------- H5': dense blocks on the fp64 tensor cores
+// The block view A' = D^T A D (Fig. 1 at :69) for one (group, M) run and one isospin bin:
+//     Vm[mu, mu'] = sum_{J >= |M|} sum_{J12, J12'} Cb[mu; J,J12] * Vw_bin[J; J12,J12'] * Ck[mu'; J,J12']
+// over ALL bra m-states mu and ket m-states mu' of that M (the M-major order of the coefficient tables makes them index
+// ranges), evaluated as two chained products:
+//     T[mu, r] = sum_i Cb[mu; q(r), i] * Vw[q(r); i, k(r)]        r = flattened ket rows (J block q, J12' index k)
+//     Vm       = T * Ck^T                                         8 x 8 tiles of mma.sync.m8n8k4.f64, K = r in chunks of 4
+// One warp per run.  Per bin present in the run it fills Vm in its shared-memory buffer, then every record of that bin
+// picks its entry.  T entries are computed directly in the A-fragment layout (lane = (mu, r mod 4)) and reused for all
+// mu' tiles.  Pays only where most pairs of a block are requested (config 2, "ALL pairs"); see DESIGN.md for the
+// measured break-even.  Summation order differs from the direct kernels: values agree to rounding, not bitwise.
+constexpr int DN_WARPS = 4;
+constexpr int DN_CHUNKS = DENSE_RMAX / 4;
+struct DenseWarp3 {
+    double vm[DENSE_CAP];
+    uint4 rmap[DENSE_RMAX];   // per flattened ket row: {bra block offset, nb | nk<<8 | k<<16, first Vw cell (i = 0), ket block offset}
+};
+__global__ void __launch_bounds__(DN_WARPS * 32) k_dense3(Tables T, const uint4* __restrict__ ditems, const uint32_t* __restrict__ n_items_p,
+                                                         const unsigned long long* __restrict__ recs, double* __restrict__ out)
+{
+    __shared__ DenseWarp3 shw[DN_WARPS];
+    DenseWarp3& W = shw[threadIdx.x >> 5];
+    const int lane = threadIdx.x & 31;
+    const uint32_t gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
+    const uint32_t n_runs = __ldg(n_items_p + 2);
+    const uint32_t nt = (uint32_t)T.n_tup3;
+    const double* __restrict__ dtab = T.dtab3;
+    for (uint32_t it = gw; it < n_runs; it += nw) {
+        const uint4 item = __ldg(ditems + it);
+        const uint32_t pos0 = item.x, cnt = item.y, g = item.z, mi = item.w;
+        const uint32_t tb = g / nt, tk = g - tb * nt;
+        const int4 kb = __ldg(T.tk3 + tb), kk = __ldg(T.tk3 + tk);
+        const uint4 sg = __ldg(T.sgrp3 + g);
+        const int sjb = kb.w & 255, sjk = kk.w & 255, mm = min(sjb, sjk);
+        const int imb = (int)mi + ((sjb - mm) >> 1), imk = (int)mi + ((sjk - mm) >> 1);
+        const uint16_t* msb = T.mstart3 + __ldg(T.mstoff3 + tb);
+        const uint16_t* msk = T.mstart3 + __ldg(T.mstoff3 + tk);
+        const uint32_t s0b = __ldg(msb + imb), nmb = __ldg(msb + imb + 1) - s0b;
+        const uint32_t s0k = __ldg(msk + imk), nmk = __ldg(msk + imk + 1) - s0k;
+        const int Jminb = (kb.w >> 16) & 255, Jmink = (kk.w >> 16) & 255;
+        const int Jlo = max(Jminb, Jmink), nblk = ((min((kb.w >> 24) & 255, (kk.w >> 24) & 255) - Jlo) >> 1) + 1;
+        const int q0 = max(0, (abs(2 * imb - sjb) - Jlo + 1) >> 1);   // first J block with J >= |M|
+        // flattened ket rows of the blocks q0 .. nblk-1
+        int2 jb = make_int2(0, 0), jk = make_int2(0, 0);
+        if (lane < nblk) {
+            jb = __ldg(T.jinfo3 + kb.z + ((Jlo - Jminb) >> 1) + lane);
+            jk = __ldg(T.jinfo3 + kk.z + ((Jlo - Jmink) >> 1) + lane);
+        }
+        const uint32_t vv = (uint32_t)(jb.y * row_pitch3(jk.y)), rk = lane >= q0 ? (uint32_t)jk.y : 0u;
+        uint32_t iv = vv, ir = rk;
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            uint32_t xv = __shfl_up_sync(0xFFFFFFFFu, iv, off), xr = __shfl_up_sync(0xFFFFFFFFu, ir, off);
+            if (lane >= off) { iv += xv; ir += xr; }
+        }
+        const uint32_t R = __shfl_sync(0xFFFFFFFFu, ir, 31);   // ket rows in play (<= DENSE_RMAX by the upload's feasibility test)
+        if (lane >= q0 && lane < nblk)
+            for (int k = 0; k < jk.y; k++)
+                W.rmap[ir - rk + k] = make_uint4((uint32_t)kb.x + (uint32_t)jb.x, (uint32_t)jb.y | ((uint32_t)jk.y << 8) | ((uint32_t)k << 16),
+                                                 iv - vv + (uint32_t)k, (uint32_t)kk.x + (uint32_t)jk.x);
+        // isospin bins present in the run
+        uint32_t bits = 0u;
+        for (uint32_t i = lane; i < cnt; i += 32) bits |= 1u << ((uint32_t)(__ldg(recs + pos0 + i) >> 24) & 31u);
+        bits = __reduce_or_sync(0xFFFFFFFFu, bits);
+        __syncwarp();
+        const uint32_t gsize = sg.y, S = vw_stride(gsize), ldv = (nmk + 7u) & ~7u;
+        const int nchunk = (int)((R + 3u) >> 2);
+        const uint32_t mrow = (uint32_t)lane >> 2, kcol = (uint32_t)lane & 3u;
+        for (uint32_t bin = 0; bin < (uint32_t)NBIN3; bin++) {
+            if (!((bits >> bin) & 1u)) continue;   // warp-uniform
+            const uint32_t* __restrict__ vwb = T.vw20 + (size_t)sg.z * 4 + (size_t)bin * S;
+            for (uint32_t mt = 0; mt * 8u < nmb; mt++) {
+                // A fragments: T[mu = 8 mt + lane/4][r = 4 c + lane%4] for every K chunk c
+                double a[DN_CHUNKS];
+                const uint32_t mu = mt * 8u + mrow;
+#pragma unroll
+                for (int c = 0; c < DN_CHUNKS; c++) {
+                    a[c] = 0.0;
+                    const uint32_t r = 4u * c + kcol;
+                    if (c < nchunk && r < R && mu < nmb) {
+                        const uint4 e = W.rmap[r];
+                        const uint32_t nb = e.y & 255u, P = (uint32_t)row_pitch3((e.y >> 8) & 255u);
+                        const double* __restrict__ cb = dtab + (e.x + (s0b + mu) * nb);
+                        double t = 0.0;
+                        for (uint32_t i = 0; i < nb; i++) {
+                            const uint32_t cell = e.z + i * P;
+                            t = fma(__ldg(cb + i), __hiloint2double((int)__ldg(vwb + gsize + cell), (int)__ldg(vwb + cell)), t);
+                        }
+                        a[c] = t;
+                    }
+                }
+                for (uint32_t nt8 = 0; nt8 * 8u < nmk; nt8++) {
+                    const uint32_t mup = nt8 * 8u + mrow;   // B fragment: Ck[mu' = 8 nt8 + lane/4][r = 4 c + lane%4]
+                    double c0 = 0.0, c1 = 0.0;
+#pragma unroll
+                    for (int c = 0; c < DN_CHUNKS; c++) {
+                        if (c < nchunk) {   // warp-uniform
+                            const uint32_t r = 4u * c + kcol;
+                            double b = 0.0;
+                            if (r < R && mup < nmk) {
+                                const uint4 e = W.rmap[r];
+                                b = __ldg(dtab + (e.w + (s0k + mup) * ((e.y >> 8) & 255u) + (e.y >> 16)));
+                            }
+                            asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                                         : "+d"(c0), "+d"(c1) : "d"(a[c]), "d"(b));
+                        }
+                    }
+                    *reinterpret_cast<double2*>(&W.vm[(mt * 8u + mrow) * ldv + nt8 * 8u + 2u * kcol]) = make_double2(c0, c1);
+                }
+            }
+            __syncwarp();
+            for (uint32_t i = lane; i < cnt; i += 32) {
+                const unsigned long long rec = __ldg(recs + pos0 + i);
+                const uint32_t lo = (uint32_t)rec;
+                if (((lo >> 24) & 31u) != bin) continue;
+                // a record of another tuple pair in a mis-ordered MFDN_PRESORTED stream must not index outside the buffer
+                const uint32_t rb = min((lo & 0xFFFu) - s0b, nmb - 1u), rkk = min(((lo >> 12) & 0xFFFu) - s0k, nmk - 1u);
+                const double v = W.vm[rb * ldv + rkk];
+                out[pos0 + i] = (((lo >> 29) & 1u) ? -v : v) + 0.0;
+            }
+            __syncwarp();
+        }
+    }
+}
+
 __global__ void __launch_bounds__(128) k_transform2(Tables T, long long n, const unsigned long long* __restrict__ recs,
                                                    double* __restrict__ out)
 {
@@ -1069,6 +1207,8 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
 {
     if (!c || !work_bytes || n < 0 || n >= (int64_t)0xFFFFFFF0ll) return c ? fail(c, MFDN_ERR_ARG, "bad n / work_bytes") : MFDN_ERR_ARG;
     if (BODY == 3 ? !c->has3 : !c->has2) return fail(c, MFDN_ERR_STATE, "mscheme before coupled upload");
+    if ((flags & MFDN_FORCE_DENSE) && (BODY != 3 || (flags & MFDN_FORCE_NAIVE)))
+        return fail(c, MFDN_ERR_ARG, "MFDN_FORCE_DENSE: 3-body only, not together with MFDN_FORCE_NAIVE");
     const long long nt = BODY == 3 ? c->t.n_tup3 : c->t.n_tup2;
     if (nt * nt >= (long long)REC_INVALID) return fail(c, MFDN_ERR_ARG, "too many tuples for 27-bit group keys");
     // sort buckets: 2-body one per group, 3-body one per (group, M); last bucket: requests failing S1-S6
@@ -1082,7 +1222,9 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
     // or per SMALL_ITEM3 records of an oversized one
     const long long max_items = 5 * (n / ITEM3 + n / (SMALL_ITEM3 + 1) + 1) + n / SMALL_ITEM3 + std::min<long long>(n, nt * nt + 1) + 1;
     size_t need = 256;
-    size_t o_recs = 0, o_sorted = 0, o_order = 0, o_hist = 0, o_sums = 0, o_items = 0, o_count = 0;
+    const bool dense = items && (flags & MFDN_FORCE_DENSE);
+    const long long max_ditems = dense ? std::min<long long>(n, n_buckets) + 1 : 0;
+    size_t o_recs = 0, o_sorted = 0, o_order = 0, o_hist = 0, o_sums = 0, o_items = 0, o_count = 0, o_ditems = 0;
     if (!naive) {
         need = o_recs + align256((size_t)n * 8);
         if (sort) {
@@ -1098,7 +1240,8 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
         if (items) {
             o_items = need;
             o_count = o_items + align256((size_t)max_items * 16);
-            need = o_count + 256;
+            o_ditems = o_count + 256;
+            need = o_ditems + align256((size_t)max_ditems * 16);
         }
     }
     if (!d_work) { *work_bytes = need; return MFDN_OK; }
@@ -1158,10 +1301,11 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
         if (items) {
             uint4* itm = (uint4*)(w + o_items);
             uint32_t* cnt = (uint32_t*)(w + o_count);
-            MFDN_CUDA(c, cudaMemsetAsync(cnt, 0, 8, st));
+            MFDN_CUDA(c, cudaMemsetAsync(cnt, 0, 16, st));
+            uint4* ditm = (uint4*)(w + o_ditems);
             const uint32_t last_slot = (uint32_t)(max_items - 1);
             k_items3<<<(unsigned)((nt * nt + 1 + 255) / 256), 256, 0, st>>>(hist, c->t.gbase3, (uint32_t)(nt * nt), (uint32_t)n_buckets, sort ? 1 : 0,
-                                                                             (uint32_t)n, c->t.sgrp3, itm, last_slot, cnt);
+                                                                             (uint32_t)n, c->t.sgrp3, itm, last_slot, cnt, dense ? 0.f : -1.f, ditm);
             if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.b, st));
             if (c->tr_blocks_per_sm == 0) {
                 int per_sm = 0;
@@ -1173,6 +1317,11 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
             const unsigned grid_s = (unsigned)std::min<long long>((std::min<long long>(n, nt * nt + 1) + 3) / 4, (long long)c->num_sms * 16);
             k_transform3_small<<<grid_s, 128, 0, st>>>(c->t, itm, last_slot, cnt, trecs, tout);
             c->launches += 3;
+            if (dense) {
+                const unsigned grid_d = (unsigned)std::min<long long>((max_ditems + DN_WARPS - 1) / DN_WARPS, (long long)c->num_sms * 8);
+                k_dense3<<<grid_d, DN_WARPS * 32, 0, st>>>(c->t, ditm, cnt, trecs, tout);
+                c->launches += 1;
+            }
         } else {
             if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.b, st));
             k_transform2<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(c->t, n, trecs, tout);

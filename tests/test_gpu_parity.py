@@ -104,17 +104,26 @@ def test_cg_tables_match_exact(torch, B, emax):
 
 
 # --------------------------------------------------------------------------------- whole small configs
-@pytest.mark.parametrize("mode", list(MODES) + ["presorted"])
+@pytest.mark.parametrize("mode", list(MODES) + ["presorted", "dense", "dense_presorted"])
 @pytest.mark.parametrize("idx", [0, 2])
 def test_all_pairs_configs(torch, B, oracle, idx, mode):
     cfg = get_cfg(idx)
     ctx = get_ctx(B, idx)
     req = cfg.requests()
+    if mode.startswith("dense") and cfg.body == 2:           # the dense-block path (H5') is 3-body only
+        with pytest.raises(B.MfdnError) as e:
+            run_gpu(torch, ctx, req[:100], B.MFDN_FORCE_DENSE)
+        assert e.value.code == B.MFDN_ERR_ARG
+        return
     want, wmask, _, _ = oracle.mscheme(cfg.basis, cfg.table, req)
-    if mode == "presorted":
+    if mode.endswith("presorted"):
+        flags = B.MFDN_PRESORTED | (B.MFDN_FORCE_DENSE if mode.startswith("dense") else 0)
         sreq, order = presort(torch, ctx, req)
-        got, gmask = run_gpu(torch, ctx, sreq, B.MFDN_PRESORTED)
+        got, gmask = run_gpu(torch, ctx, sreq, flags)
         check(cfg, got, gmask, want[order], wmask[order])
+    elif mode == "dense":
+        got, gmask = run_gpu(torch, ctx, req, B.MFDN_FORCE_DENSE)
+        check(cfg, got, gmask, want, wmask)
     else:
         got, gmask = run_gpu(torch, ctx, req, MODES[mode])
         check(cfg, got, gmask, want, wmask)
@@ -132,6 +141,9 @@ def test_sampled_configs_prefix(torch, B, oracle, idx, n):
     assert 0.85 < wmask.mean() < 1.0
     for mode, flags in MODES.items():
         got, gmask = run_gpu(torch, ctx, req, flags)
+        check(cfg, got, gmask, want, wmask)
+    if cfg.body == 3:      # dense-block path wherever a group's blocks fit (sparse requests: correct, not fast)
+        got, gmask = run_gpu(torch, ctx, req, B.MFDN_FORCE_DENSE)
         check(cfg, got, gmask, want, wmask)
     sreq, order = presort(torch, ctx, req)
     got, gmask = run_gpu(torch, ctx, sreq, B.MFDN_PRESORTED)
@@ -314,7 +326,7 @@ def _check_all_modes(torch, B, oracle, basis, table, req):
     ctx = B.Context(basis, 0).upload(table)
     want, wmask, _, _ = oracle.mscheme(basis, table, req)
     assert wmask.mean() > 0.5
-    for flags in (0, B.MFDN_FORCE_NAIVE):
+    for flags in (0, B.MFDN_FORCE_NAIVE, B.MFDN_FORCE_DENSE):
         got, gmask = run_gpu(torch, ctx, req, flags)
         check(cfg, got, gmask, want, wmask)
     sreq, order = presort(torch, ctx, req)
