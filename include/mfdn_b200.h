@@ -105,8 +105,10 @@ int mfdn_coupled_upload_3b(mfdn_ctx*, int32_t e3max, int32_t n_chan, const int32
  *         the size needed for n requests in *work_bytes (nothing is launched).  The call itself never
  *         allocates and never synchronises: it is asynchronous on `stream`.
  * Per-request problems never fail the call: an out-of-range SPS index gives value 0, mask 0 and is
- * counted (mfdn_bad_request_count).  Concurrent calls on different streams are allowed provided
- * each uses its own scratch (one stream per host thread). */
+ * counted (mfdn_bad_request_count).  Concurrent calls are allowed -- from one host thread or from several -- provided
+ * each call in flight has its own stream and its own scratch (one stream per host thread); the tables
+ * are read-only and the context's bookkeeping is locked.  The call makes the context's device the calling thread's
+ * current device. */
 int mfdn_mscheme_2b(mfdn_ctx*, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_mask, void* d_work,
                     size_t* work_bytes, uint32_t flags, void* stream);
 int mfdn_mscheme_3b(mfdn_ctx*, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_mask, void* d_work,
@@ -117,7 +119,8 @@ int mfdn_mscheme_3b(mfdn_ctx*, int64_t n, const int32_t* d_req, double* d_out, u
  * are cut into chunks of `chunk` (0 = library default) and H2D copy / transform / D2H copy of successive chunks
  * overlap on two internal streams.  body = 2 or 3; h_mask may be NULL; flags as above (MFDN_PRESORTED then means
  * the whole host array is group-ordered).  d_work/work_bytes: DEVICE scratch, queried with d_work == NULL.
- * BLOCKING: returns after the last result byte has landed in h_out. */
+ * BLOCKING: returns after the last result byte has landed in h_out (also on failure: no copy is left in flight on the
+ * caller's buffers).  Uses two streams owned by the context: one mfdn_mscheme_host call at a time per context. */
 int mfdn_mscheme_host(mfdn_ctx*, int body, int64_t n, const int32_t* h_req, double* h_out, uint8_t* h_mask,
                       void* d_work, size_t* work_bytes, uint32_t flags, int64_t chunk);
 
@@ -147,6 +150,7 @@ int64_t mfdn_info(mfdn_ctx*, int which);
  * fail S1-S6.  body = 2 or 3.  Asynchronous on `stream`. */
 int mfdn_group_keys(mfdn_ctx*, int body, int64_t n, const int32_t* d_req, uint32_t* d_key, void* stream);
 
+/* Message of the context's most recent failure; the pointer stays valid until the calling thread's next call of this function. */
 const char* mfdn_last_error(mfdn_ctx*);
 void mfdn_destroy(mfdn_ctx*);
 

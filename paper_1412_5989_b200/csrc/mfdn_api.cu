@@ -14,12 +14,18 @@ using namespace mfdn;
 namespace mfdn {
 int fail(mfdn_ctx* c, int code, const std::string& msg)
 {
-    if (c) c->err = msg;
+    if (c) {
+        std::lock_guard<std::mutex> lk(c->mu);
+        c->err = msg;
+    }
     return code;
 }
 int cuda_fail(mfdn_ctx* c, cudaError_t e, const char* what)
 {
-    if (c) c->err = std::string(what) + ": " + cudaGetErrorString(e);
+    if (c) {
+        std::lock_guard<std::mutex> lk(c->mu);
+        c->err = std::string(what) + ": " + cudaGetErrorString(e);
+    }
     return e == cudaErrorMemoryAllocation ? MFDN_ERR_OOM : MFDN_ERR_CUDA;
 }
 }  // namespace mfdn
@@ -1004,7 +1010,7 @@ extern "C" int64_t mfdn_info(mfdn_ctx* c, int which)
         case 3: return c->slab_bytes3;
         case 4: return c->n_cg1;
         case 5: return c->n_cg2;
-        case 6: return c->launches;
+        case 6: return c->launches.load();
         case 7: return c->dtab_bytes3;
         case 8: return c->vw_bytes3;
         case 9: return c->t.n_buckets3;
@@ -1012,7 +1018,14 @@ extern "C" int64_t mfdn_info(mfdn_ctx* c, int which)
     }
 }
 
-extern "C" const char* mfdn_last_error(mfdn_ctx* c) { return c ? c->err.c_str() : "null context"; }
+extern "C" const char* mfdn_last_error(mfdn_ctx* c)
+{
+    if (!c) return "null context";
+    static thread_local std::string copy;   // valid until the calling thread's next mfdn_last_error
+    std::lock_guard<std::mutex> lk(c->mu);
+    copy = c->err;
+    return copy.c_str();
+}
 
 extern "C" void mfdn_destroy(mfdn_ctx* c)
 {

@@ -3,6 +3,8 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <atomic>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -131,7 +133,8 @@ struct mfdn_ctx {
     int device = 0;
     int stage = 0;  // 1 orbitals, 2 cg built
     bool has2 = false, has3 = false;
-    std::string err;
+    std::string err;            // last error message; guarded by `mu` (mfdn_last_error hands out a per-thread copy)
+    std::mutex mu;              // guards err, ev_pending, ev_pool: mscheme_* may be called from several host threads
     mfdn::Tables t{};
     int tjmax = 0;
     // host copies
@@ -140,9 +143,9 @@ struct mfdn_ctx {
     std::vector<void*> owned;  // device allocations
     int64_t n_cg1 = 0, n_cg2 = 0;
     int64_t slab_bytes2 = 0, slab_bytes3 = 0, dtab_bytes3 = 0, vw_bytes3 = 0;
-    int64_t launches = 0;
+    std::atomic<int64_t> launches{0};
     int num_sms = 148;
-    int tr_blocks_per_sm = 0;   // resident k_transform3 blocks per SM (occupancy query at the first call)
+    std::atomic<int> tr_blocks_per_sm{0};   // resident k_transform3 blocks per SM (occupancy query at the first call)
     // measurement hooks
     bool profile = false;
     struct EvTriple { cudaEvent_t a, b, d, c; bool has_sort; };   // start | transform kernel start | its end | end of call

@@ -1250,11 +1250,15 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
     if (!d_req || !d_out) return fail(c, MFDN_ERR_ARG, "null request/output pointer");
     cudaStream_t st = (cudaStream_t)stream;
     mfdn_ctx::EvTriple ev{nullptr, nullptr, nullptr, nullptr, sort};
+    MFDN_CUDA(c, cudaSetDevice(c->device));   // the tables live on the context's device, whatever the caller's current one
     if (c->profile) {
         cudaEvent_t* e3[4] = {&ev.a, &ev.b, &ev.d, &ev.c};
         for (auto pe : e3) {
-            if (!c->ev_pool.empty()) { *pe = c->ev_pool.back(); c->ev_pool.pop_back(); }
-            else MFDN_CUDA(c, cudaEventCreate(pe));
+            {
+                std::lock_guard<std::mutex> lk(c->mu);
+                if (!c->ev_pool.empty()) { *pe = c->ev_pool.back(); c->ev_pool.pop_back(); continue; }
+            }
+            MFDN_CUDA(c, cudaEventCreate(pe));
         }
         MFDN_CUDA(c, cudaEventRecord(ev.a, st));
     }
@@ -1307,12 +1311,13 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
             k_items3<<<(unsigned)((nt * nt + 1 + 255) / 256), 256, 0, st>>>(hist, c->t.gbase3, (uint32_t)(nt * nt), (uint32_t)n_buckets, sort ? 1 : 0,
                                                                              (uint32_t)n, c->t.sgrp3, itm, last_slot, cnt, dense ? 0.f : -1.f, ditm);
             if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.b, st));
-            if (c->tr_blocks_per_sm == 0) {
-                int per_sm = 0;
+            int per_sm = c->tr_blocks_per_sm.load();
+            if (per_sm == 0) {   // benign if two threads do it at once: both store the same number
                 MFDN_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_transform3, TR_THREADS, 0));
-                c->tr_blocks_per_sm = std::max(per_sm, 1);
+                per_sm = std::max(per_sm, 1);
+                c->tr_blocks_per_sm.store(per_sm);
             }
-            const unsigned grid = (unsigned)std::min<long long>(max_items, (long long)c->num_sms * c->tr_blocks_per_sm);
+            const unsigned grid = (unsigned)std::min<long long>(max_items, (long long)c->num_sms * per_sm);
             k_transform3<<<grid, TR_THREADS, 0, st>>>(c->t, itm, cnt, trecs, tout);
             const unsigned grid_s = (unsigned)std::min<long long>((std::min<long long>(n, nt * nt + 1) + 3) / 4, (long long)c->num_sms * 16);
             k_transform3_small<<<grid_s, 128, 0, st>>>(c->t, itm, last_slot, cnt, trecs, tout);
@@ -1336,6 +1341,7 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
     MFDN_CUDA(c, cudaGetLastError());
     if (c->profile) {
         MFDN_CUDA(c, cudaEventRecord(ev.c, st));
+        std::lock_guard<std::mutex> lk(c->mu);
         c->ev_pending.push_back(ev);
     }
     return MFDN_OK;
@@ -1372,6 +1378,7 @@ extern "C" int mfdn_group_keys(mfdn_ctx* c, int body, int64_t n, const int32_t* 
     if (!c || (body != 2 && body != 3) || n < 0 || !d_key || (n > 0 && !d_req)) return c ? fail(c, MFDN_ERR_ARG, "bad argument") : MFDN_ERR_ARG;
     if (body == 3 ? !c->has3 : !c->has2) return fail(c, MFDN_ERR_STATE, "group_keys before coupled upload");
     if (n == 0) return MFDN_OK;
+    MFDN_CUDA(c, cudaSetDevice(c->device));
     cudaStream_t st = (cudaStream_t)stream;
     if (body == 3) k_keys<3, false, false><<<(unsigned)((n + KEYS_PER_BLOCK - 1) / KEYS_PER_BLOCK), 256, 0, st>>>(c->t, n, d_req, nullptr, nullptr, nullptr, 0u, d_key);
     else k_keys<2, false, false><<<(unsigned)((n + KEYS_PER_BLOCK - 1) / KEYS_PER_BLOCK), 256, 0, st>>>(c->t, n, d_req, nullptr, nullptr, nullptr, 0u, d_key);
@@ -1391,7 +1398,12 @@ extern "C" int mfdn_profile_read(mfdn_ctx* c, double* ms_sort, double* ms_transf
     if (!c || !ms_sort || !ms_transform || !ms_unpermute || !calls) return MFDN_ERR_ARG;
     *ms_sort = *ms_transform = *ms_unpermute = 0.0;
     *calls = 0;
-    for (auto& ev : c->ev_pending) {
+    std::vector<mfdn_ctx::EvTriple> pending;
+    {
+        std::lock_guard<std::mutex> lk(c->mu);
+        pending.swap(c->ev_pending);
+    }
+    for (auto& ev : pending) {
         MFDN_CUDA(c, cudaEventSynchronize(ev.c));
         float t1 = 0.f, t2 = 0.f, t3 = 0.f;
         MFDN_CUDA(c, cudaEventElapsedTime(&t1, ev.a, ev.b));
@@ -1401,9 +1413,9 @@ extern "C" int mfdn_profile_read(mfdn_ctx* c, double* ms_sort, double* ms_transf
         *ms_transform += t2;
         *ms_unpermute += t3;
         *calls += 1;
+        std::lock_guard<std::mutex> lk(c->mu);
         c->ev_pool.push_back(ev.a); c->ev_pool.push_back(ev.b); c->ev_pool.push_back(ev.d); c->ev_pool.push_back(ev.c);
     }
-    c->ev_pending.clear();
     return MFDN_OK;
 }
 
@@ -1463,13 +1475,18 @@ extern "C" int mfdn_mscheme_host(mfdn_ctx* c, int body, int64_t n, const int32_t
         uint8_t* dmask = (uint8_t*)(base + b_req + b_out);
         void* dw = base + b_req + b_out + b_mask;
         size_t wb = align256(inner);
-        MFDN_CUDA(c, cudaMemcpyAsync(dreq, h_req + lo * width, (size_t)m * width * 4, cudaMemcpyHostToDevice, st));
-        rc = body == 3 ? run<3>(c, m, dreq, dout, dmask, dw, &wb, flags, st) : run<2>(c, m, dreq, dout, dmask, dw, &wb, flags, st);
-        if (rc) return rc;
-        MFDN_CUDA(c, cudaMemcpyAsync(h_out + lo, dout, (size_t)m * 8, cudaMemcpyDeviceToHost, st));
-        if (h_mask) MFDN_CUDA(c, cudaMemcpyAsync(h_mask + lo, dmask, (size_t)m, cudaMemcpyDeviceToHost, st));
+        // on any failure: no copy may still be in flight on the caller's buffers when the call returns
+        cudaError_t e = cudaMemcpyAsync(dreq, h_req + lo * width, (size_t)m * width * 4, cudaMemcpyHostToDevice, st);
+        if (e == cudaSuccess) {
+            rc = body == 3 ? run<3>(c, m, dreq, dout, dmask, dw, &wb, flags, st) : run<2>(c, m, dreq, dout, dmask, dw, &wb, flags, st);
+            if (rc) { cudaStreamSynchronize(c->hs[0]); cudaStreamSynchronize(c->hs[1]); return rc; }
+            e = cudaMemcpyAsync(h_out + lo, dout, (size_t)m * 8, cudaMemcpyDeviceToHost, st);
+        }
+        if (e == cudaSuccess && h_mask) e = cudaMemcpyAsync(h_mask + lo, dmask, (size_t)m, cudaMemcpyDeviceToHost, st);
+        if (e != cudaSuccess) { cudaStreamSynchronize(c->hs[0]); cudaStreamSynchronize(c->hs[1]); return cuda_fail(c, e, "mfdn_mscheme_host copy"); }
     }
-    MFDN_CUDA(c, cudaStreamSynchronize(c->hs[0]));
-    MFDN_CUDA(c, cudaStreamSynchronize(c->hs[1]));
+    cudaError_t e0 = cudaStreamSynchronize(c->hs[0]), e1 = cudaStreamSynchronize(c->hs[1]);
+    if (e0 != cudaSuccess) return cuda_fail(c, e0, "cudaStreamSynchronize");
+    if (e1 != cudaSuccess) return cuda_fail(c, e1, "cudaStreamSynchronize");
     return MFDN_OK;
 }

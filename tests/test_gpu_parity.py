@@ -423,3 +423,48 @@ def test_full_size_config4_batches(torch, B, oracle):
         if pending[slot] is not None:
             verify(slot)
     assert len(mask_frac) == nb and all(0.98 < f <= 1.0 for f in mask_frac)   # ~99.4%
+
+
+def test_multi_client_threads(torch, B):
+    """Several host threads share one context, each with its own stream and scratch, shipping ~20 000-request chunks
+    (PAPER.md:93 buffer size, :103 'each OpenMP thread uses a separate stream'); profiling on, so the event
+    bookkeeping is exercised too.  Results are bitwise those of one big call."""
+    import threading
+    cfg = get_cfg(2)
+    ctx = get_ctx(B, 2)
+    req = cfg.requests()
+    rng = np.random.default_rng(14)
+    req = req[rng.choice(len(req), 400000, replace=False)]
+    base, bmask = run_gpu(torch, ctx, req, 0)
+    d_req = torch.from_numpy(req).cuda()
+    out = torch.empty(len(req), dtype=torch.float64, device="cuda")
+    mask = torch.empty(len(req), dtype=torch.uint8, device="cuda")
+    chunk, nthreads = 20000, 4
+    chunks = [(lo, min(lo + chunk, len(req))) for lo in range(0, len(req), chunk)]
+    errors = []
+    torch.cuda.synchronize()
+    B.mfdn_profile(ctx.ctx, 1)
+
+    def client(t):
+        try:
+            torch.cuda.set_device(0)
+            s = torch.cuda.Stream()
+            work = torch.empty(ctx.work_bytes(3, chunk), dtype=torch.uint8, device="cuda")
+            for k in range(t, len(chunks), nthreads):
+                lo, hi = chunks[k]
+                ctx.mscheme(d_req[lo:hi], out[lo:hi], mask[lo:hi], 0, work, s.cuda_stream)
+            s.synchronize()
+        except Exception as e:      # noqa: BLE001 - reported by the main thread
+            errors.append(e)
+
+    threads = [threading.Thread(target=client, args=(t,)) for t in range(nthreads)]
+    for th in threads:
+        th.start()
+    for th in threads:
+        th.join()
+    torch.cuda.synchronize()
+    B.mfdn_profile(ctx.ctx, 0)
+    _, _, _, calls = B.mfdn_profile_read(ctx.ctx)
+    assert not errors, errors
+    assert calls == len(chunks)
+    assert np.array_equal(out.cpu().numpy(), base) and np.array_equal(mask.cpu().numpy(), bmask)
