@@ -98,7 +98,7 @@ def host_requests(cfg, n, start):
         r = cfg.requests()
         reps = (n + len(r) - 1) // len(r)
         return np.ascontiguousarray(np.tile(r, (reps, 1))[:n])
-    return cfg.requests(n, start=start)
+    return cfg.requests(n, start=start, workers=os.cpu_count() or 1)
 
 
 def cpu_baseline(cfg, n_sample, threads=0):
@@ -156,6 +156,8 @@ def main():
                     help="log2 of the CPU-oracle sample (default: 25 for the cpu_baseline leg, 21 per step of --impl reference)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-configs", action="store_true", help="skip the per-config block (all five BASELINE.json workloads)")
+    ap.add_argument("--config-reps", type=int, default=10)
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -220,6 +222,17 @@ def main():
     ms, ms_sort, ms_tr, ms_un, launches, clocks = timed(0, d_req, args.steps, args.warmup, sampler)
     n_mask = int(d_mask.sum(dtype=torch.int64).item())
     frac_mask = n_mask / n
+    # 2^14 sampled outputs of the timed launch configuration against the CPU oracle (rank 0, N = 1)
+    headline_check = None
+    do_configs = world == 1 and not args.no_configs
+    if do_configs:
+        from oracle import mscheme_c
+        sample = np.sort(np.random.default_rng(1234 + args.config).choice(n, min(n, 1 << 14), replace=False))
+        want, wmask, _, _ = mscheme_c.mscheme(cfg.basis, cfg.table, h_req.numpy()[sample])
+        ds = torch.from_numpy(sample).cuda()
+        got, gmask = d_out[ds].cpu().numpy(), d_mask[ds].cpu().numpy()
+        headline_check = {"sampled": int(len(sample)), "max_abs_delta": float(np.max(np.abs(got - want))),
+                          "tolerance": 1e-12 * float(np.max(np.abs(cfg.table.values))), "mask_bit_exact": bool(np.array_equal(gmask, wmask))}
     # ---- the same multiset pre-ordered by the library's group key (MFDN_PRESORTED): transform proper
     keys = ctx.group_keys(d_req)
     order = torch.argsort(keys.to(torch.int64) & 0xFFFFFFFF)
@@ -239,6 +252,18 @@ def main():
     e2e_s = shard.max_over_ranks(e2e_s, "cuda")
     assert int(h_mask.sum(dtype=torch.int64).item()) == n_mask, "host-buffer path disagrees with device path"
     fp64_peak = B.mfdn_fp64_peak(ctx.ctx)
+    # ---- all five BASELINE.json workloads inside the same run (same clocks record): whole call, unsorted and MFDN_PRESORTED
+    configs = None
+    if do_configs:
+        from paper_1412_5989_b200 import report
+        ctx.close()
+        del d_req, d_out, d_mask, work, h_out, h_mask
+        torch.cuda.empty_cache()
+        configs = {}
+        for idx in (0, 1, 2, 4):
+            if idx != args.config:
+                configs[str(idx)] = report.measure(idx, reps=args.config_reps, check=14, oracle=mscheme_c, fp64_peak=fp64_peak,
+                                                   workers=os.cpu_count() or 1)
 
     if rank != 0:
         if world > 1:
@@ -290,6 +315,15 @@ def main():
         v, cores, dt = cpu_baseline(cfg, n_s)
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                                "sample": f"first 2^{args.ref_log2n} requests of the same stream, {dt:.1f} s"}
+    if configs is not None:
+        b_pre, b_uns, fl = alg["bytes_presorted"], alg["bytes_unsorted"], alg["flops"]
+        mine = {"workload": cfg.name, "requests": n, "calls": 1, "mask1_fraction": frac_mask, "oracle_check": headline_check}
+        for mode, t, byts in (("unsorted", ms, b_uns), ("presorted", ms_p, b_pre)):
+            t_h, t_a = byts * n / (hbm_peak * 1e9) * 1e3, fl * n / (fp64_peak * 1e12) * 1e3
+            mine[mode] = {"ms": t, "elements_per_s": n / t * 1e3, "alg_bytes_per_request": byts, "alg_flops_per_request": fl,
+                          "roof_ms": {"hbm": t_h, "alu": t_a}, "applicable": "hbm" if t_h >= t_a else "alu", "frac_of_roof": max(t_h, t_a) / t}
+        configs[str(args.config)] = mine
+        out["configs"] = {k: configs[k] for k in sorted(configs)}
     out["context"] = "paper (Titan, K20): 2.2-2.7x matrix-construction, 1.2-1.4x whole-run speedup; not a target"
     print(json.dumps(out))
     if world > 1:

@@ -317,7 +317,7 @@ _CHUNK = 1 << 20
 
 
 def sampled_pairs(ms: MStates, n: int, seed: int, start: int = 0, permute_frac: float = 0.0,
-                  ms_low: MStates | None = None, low_frac: float = 0.0) -> np.ndarray:
+                  ms_low: MStates | None = None, low_frac: float = 0.0, workers: int = 0) -> np.ndarray:
     """``n`` requests of the stream ``seed`` beginning at request index ``start``.
 
     The stream is defined chunk-wise (chunks of 2^20, chunk k drawn from
@@ -329,16 +329,28 @@ def sampled_pairs(ms: MStates, n: int, seed: int, start: int = 0, permute_frac: 
     permuted (exercises the sign path; parity runs only)."""
     A = ms.states.shape[1]
     out = np.empty((n, 2 * A), dtype=np.int32)
+    jobs = []   # (chunk, first row of the chunk wanted, one past the last, destination row)
     pos = 0
     k = start // _CHUNK
     while pos < n:
         c0 = k * _CHUNK
         lo = max(start, c0) - c0
         hi = min(start + n, c0 + _CHUNK) - c0
-        chunk = _sample_chunk(ms, seed, k, permute_frac, ms_low, low_frac)
-        out[pos:pos + hi - lo] = chunk[lo:hi]
+        jobs.append((k, lo, hi, pos))
         pos += hi - lo
         k += 1
+
+    def fill(job):
+        k, lo, hi, pos = job
+        out[pos:pos + hi - lo] = _sample_chunk(ms, seed, k, permute_frac, ms_low, low_frac)[lo:hi]
+
+    if workers > 1 and len(jobs) > 1:   # chunks are independent streams: the result does not depend on `workers`
+        from concurrent.futures import ThreadPoolExecutor
+        with ThreadPoolExecutor(workers) as ex:
+            list(ex.map(fill, jobs))
+    else:
+        for job in jobs:
+            fill(job)
     return out
 
 
@@ -389,12 +401,13 @@ class Config:
     n_batches: int = 1
     extra: dict = field(default_factory=dict)
 
-    def requests(self, n: int | None = None, start: int = 0, permute_frac: float = 0.0) -> np.ndarray:
+    def requests(self, n: int | None = None, start: int = 0, permute_frac: float = 0.0, workers: int = 0) -> np.ndarray:
+        """``workers`` > 1: chunks of the stream drawn by that many host threads (same result)."""
         if self.all_pairs:
             r = all_conserving_pairs(self.ms)
             return r if n is None else r[start:start + n]
         n = self.n_requests if n is None else n
-        return sampled_pairs(self.ms, n, self.seed_req, start, permute_frac, self.ms_low, self.low_frac)
+        return sampled_pairs(self.ms, n, self.seed_req, start, permute_frac, self.ms_low, self.low_frac, workers)
 
 
 def make_config(index: int, table_values: str = "normal") -> Config:
