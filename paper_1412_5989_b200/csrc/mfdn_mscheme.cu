@@ -565,10 +565,85 @@ __global__ void __launch_bounds__(256) k_items3(const uint32_t* __restrict__ bou
             items[slot++] = make_uint4(start + j * ITEM3, min((uint32_t)ITEM3, cnt - j * ITEM3), gz, (r * bpr) | (min(bpr, NBIN3 - r * bpr) << 8));
 }
 
-// H3-H6 for small groups: one warp per item, lane = record.  The group's loop bounds, table rows and slab addresses
-// are warp-uniform, the lanes differ in their projections (sigma) and isospin weights.  Same operations in the same
-// order as the staged path of k_transform3 (Vw first, then ck, then cb, then the sum over J), so a request's value
-// does not depend on which of the two kernels its group happened to go to.
+// H3-H6 for small groups: one warp per item.  The group's loop bounds, table rows and slab addresses are warp-uniform, the
+// lanes differ in their projections (sigma) and isospin bin.  Same operations in the same order as the staged path of
+// k_transform3 (Vw of the record's bin from the isospin-combined slabs, then ck, then cb, then the sum over J in ascending
+// order), so a request's value does not depend on which of the two kernels its group happened to go to.
+// A warp is PARTS sub-warps of 32 / PARTS lanes: lane = (record r, part p).  Part p evaluates the J blocks q = p, p + PARTS, ..
+// of its record; the PARTS blocks of a round run side by side under the largest bounds of the round (neighbouring J have
+// similar ranges), the block sums are then added in ascending J by every lane (shuffles), which keeps the summation
+// order of the one-lane-per-record form.  Groups of at most SMALL_SPLIT records (config 4: a 2^24-request batch leaves
+// about 6 records per group of its uniform part) take PARTS = 4, eight records per pass; larger ones PARTS = 1.
+constexpr uint32_t SMALL_SPLIT = 24;
+template <int PARTS>
+__device__ __forceinline__ void small_group3(const Tables& T, uint32_t pos0, uint32_t cnt, int nblk, int2 ib_l, int2 ik_l, uint32_t voff_l,
+                                             uint32_t tb_off, uint32_t tk_off, const uint32_t* __restrict__ vw, uint32_t gsize,
+                                             const unsigned long long* __restrict__ recs, double* __restrict__ out, int lane)
+{
+    constexpr int W = 32 / PARTS;
+    const int r = lane % W, p = lane / W;
+    const double* __restrict__ dtab = T.dtab3;
+    const uint32_t S = vw_stride(gsize);
+    for (uint32_t r0 = 0; r0 < cnt; r0 += W) {
+        const bool valid = r0 + r < cnt;
+        const uint32_t lo = (uint32_t)__ldg(recs + pos0 + (valid ? r0 + r : r0));
+        const uint32_t sb = lo & 0xFFFu, sk = (lo >> 12) & 0xFFFu;
+        const uint32_t* __restrict__ vwl = vw + (size_t)((lo >> 24) & 31u) * S;   // low words of the record's bin; high words gsize further
+        double total = 0.0;
+        for (int q0 = 0; q0 < nblk; q0 += PARTS) {
+            const int q = q0 + p;
+            const bool has = q < nblk;
+            const int src = has ? q : 0;
+            const uint32_t ibx = (uint32_t)__shfl_sync(0xFFFFFFFFu, ib_l.x, src), ikx = (uint32_t)__shfl_sync(0xFFFFFFFFu, ik_l.x, src);
+            int nb = __shfl_sync(0xFFFFFFFFu, ib_l.y, src), nk = __shfl_sync(0xFFFFFFFFu, ik_l.y, src);
+            uint32_t c = __shfl_sync(0xFFFFFFFFu, voff_l, src);
+            if (!has || nk <= 0) nb = 0;
+            int nbmax = nb, nkmax = nb > 0 ? nk : 0;
+            if (PARTS > 1) {
+#pragma unroll
+                for (int off = W; off < 32; off <<= 1) {
+                    nbmax = max(nbmax, __shfl_xor_sync(0xFFFFFFFFu, nbmax, off));
+                    nkmax = max(nkmax, __shfl_xor_sync(0xFFFFFFFFu, nkmax, off));
+                }
+            }
+            const uint32_t P = (uint32_t)row_pitch3(nk);
+            const double* __restrict__ cbp = dtab + (tb_off + ibx + sb * (uint32_t)nb);
+            const double* __restrict__ ckp = dtab + (tk_off + ikx + sk * (uint32_t)nk);
+            double t = 0.0;
+            for (int i = 0; i < nbmax; i++) {
+                const bool row = i < nb;
+                const double cb = row ? __ldg(cbp + i) : 0.0;
+                double acc = 0.0;
+                for (int k0 = 0; k0 < nkmax; k0 += 4) {   // four cells' loads (12) in flight before the first multiply
+                    double ck[4], v[4];
+#pragma unroll
+                    for (int u = 0; u < 4; u++) {
+                        const bool on = row && k0 + u < nk;
+                        const uint32_t cell = on ? c + (uint32_t)(k0 + u) : 0u;
+                        ck[u] = on ? __ldg(ckp + k0 + u) : 0.0;
+                        const uint32_t lw = on ? __ldg(vwl + cell) : 0u, hw = on ? __ldg(vwl + gsize + cell) : 0u;
+                        v[u] = __hiloint2double((int)hw, (int)lw);
+                    }
+#pragma unroll
+                    for (int u = 0; u < 4; u++)
+                        if (row && k0 + u < nk) acc = (k0 + u) ? fma(ck[u], v[u], acc) : ck[u] * v[u];
+                }
+                if (row) { t = fma(cb, acc, t); c += P; }
+            }
+            if (PARTS > 1) {
+#pragma unroll
+                for (int pp = 0; pp < PARTS; pp++) {
+                    const double tt = __shfl_sync(0xFFFFFFFFu, t, pp * W + r);
+                    if (q0 + pp < nblk) total += tt;
+                }
+            } else {
+                total += t;
+            }
+        }
+        if (valid && p == 0) out[pos0 + r0 + r] = (((lo >> 29) & 1u) ? -total : total) + 0.0;   // + 0.0: never store -0
+    }
+}
+
 __global__ void __launch_bounds__(128) k_transform3_small(Tables T, const uint4* __restrict__ items, uint32_t last_slot,
                                                           const uint32_t* __restrict__ n_items_p,
                                                           const unsigned long long* __restrict__ recs, double* __restrict__ out)
@@ -577,7 +652,6 @@ __global__ void __launch_bounds__(128) k_transform3_small(Tables T, const uint4*
     const uint32_t gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
     const uint32_t n_small = __ldg(n_items_p + 1);
     const uint32_t nt = (uint32_t)T.n_tup3;
-    const double* __restrict__ dtab = T.dtab3;
     for (uint32_t it = gw; it < n_small; it += nw) {
         const uint4 item = __ldg(items + (last_slot - it));
         const uint32_t pos0 = item.x, cnt = item.y, g = item.z;
@@ -591,45 +665,22 @@ __global__ void __launch_bounds__(128) k_transform3_small(Tables T, const uint4*
         const int Jminb = (kb.w >> 16) & 255, Jmink = (kk.w >> 16) & 255;
         const int Jlo = max(Jminb, Jmink), Jhi = min((kb.w >> 24) & 255, (kk.w >> 24) & 255);
         const int nblk = ((Jhi - Jlo) >> 1) + 1;
-        const int2* __restrict__ jib = T.jinfo3 + kb.z + ((Jlo - Jminb) >> 1);
-        const int2* __restrict__ jik = T.jinfo3 + kk.z + ((Jlo - Jmink) >> 1);
-        const uint32_t gsize = sg.y;
-        for (uint32_t r0 = 0; r0 < cnt; r0 += 32) {   // 32 records per pass
-            const bool valid = r0 + lane < cnt;
-            const unsigned long long rec = __ldg(recs + pos0 + (valid ? r0 + lane : r0));
-            const uint32_t lo = (uint32_t)rec;
-            const double* wp = T.wbin3 + ((lo >> 24) & 31u) * NISO3;
-            const double w0 = __ldg(wp), w1 = __ldg(wp + 1), w2 = __ldg(wp + 2), w3 = __ldg(wp + 3), w4 = __ldg(wp + 4);
-            const uint32_t sb = lo & 0xFFFu, sk = (lo >> 12) & 0xFFFu;
-            const double* __restrict__ row = T.slab3 + (size_t)sg.x * 2;
-            double total = 0.0;
-            for (int q = 0; q < nblk; q++) {
-                const int2 ib = __ldg(jib + q), ik = __ldg(jik + q);
-                const int nb = ib.y, nk = ik.y;
-                const int P = row_pitch3(nk);
-                const double* __restrict__ cbp = dtab + (uint32_t)kb.x + (uint32_t)ib.x + sb * (uint32_t)nb;
-                const double* __restrict__ ckp = dtab + (uint32_t)kk.x + (uint32_t)ik.x + sk * (uint32_t)nk;
-                double t = 0.0;
-                for (int i = 0; i < nb; i++) {
-                    const double cb = __ldg(cbp + i);
-                    double acc = 0.0;
-                    for (int k = 0; k < nk; k++) {
-                        const double ck = __ldg(ckp + k);
-                        const double* cell = row + k;
-                        double v = w0 * __ldg(cell);
-                        v = fma(w1, __ldg(cell + gsize), v);
-                        v = fma(w2, __ldg(cell + 2 * gsize), v);
-                        v = fma(w3, __ldg(cell + 3 * gsize), v);
-                        v = fma(w4, __ldg(cell + 4 * gsize), v);
-                        acc = k ? fma(ck, v, acc) : ck * v;
-                    }
-                    t = fma(cb, acc, t);
-                    if (nk > 0) row += P;
-                }
-                total += t;
-            }
-            if (valid) out[pos0 + r0 + lane] = (((lo >> 29) & 1u) ? -total : total) + 0.0;   // + 0.0: never store -0
+        // lane q holds the J block q: {offset in the tuple's coefficient table, rows} of either side, first Vw cell
+        int2 ib = make_int2(0, 0), ik = make_int2(0, 0);
+        if (lane < nblk) {
+            ib = __ldg(T.jinfo3 + kb.z + ((Jlo - Jminb) >> 1) + lane);
+            ik = __ldg(T.jinfo3 + kk.z + ((Jlo - Jmink) >> 1) + lane);
         }
+        const uint32_t vv = (uint32_t)(ib.y * row_pitch3(ik.y));
+        uint32_t iv = vv;
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            const uint32_t x = __shfl_up_sync(0xFFFFFFFFu, iv, off);
+            if (lane >= off) iv += x;
+        }
+        const uint32_t* __restrict__ vw = T.vw20 + (size_t)sg.z * 4;
+        if (cnt <= SMALL_SPLIT) small_group3<4>(T, pos0, cnt, nblk, ib, ik, iv - vv, (uint32_t)kb.x, (uint32_t)kk.x, vw, sg.y, recs, out, lane);
+        else small_group3<1>(T, pos0, cnt, nblk, ib, ik, iv - vv, (uint32_t)kb.x, (uint32_t)kk.x, vw, sg.y, recs, out, lane);
     }
 }
 
@@ -675,6 +726,9 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 #endif
 #ifndef MFDN_TR_RING
 #define MFDN_TR_RING 6656
+#endif
+#ifndef MFDN_TR_PF
+#define MFDN_TR_PF 0
 #endif
 constexpr int TR_CW = MFDN_TR_CW;               // consumer warps per block
 constexpr int TR_THREADS = (TR_CW + 1) * 32;    // + one producer warp
@@ -864,30 +918,57 @@ __global__ void __launch_bounds__(TR_THREADS, MFDN_TR_MINB) k_transform3(Tables 
     if (warp == TR_CW) {
         // ------------------------------------------------------------------ producer (all lanes run the same control flow)
         uint32_t k = 0, rel = 0, head = 0;       // items issued, items released (FIFO), next free ring word
-        for (uint32_t it = blockIdx.x; it < n_items; it += gridDim.x, k++) {
-            const uint32_t s = k % TR_SLOTS;
-            const uint4 item = __ldg(items + it);
-            const uint32_t pos0 = item.x, cnt = item.y, g = item.z;
-            const bool zero = g == ZERO_ITEM;
-            // descriptor loads first: they do not need the slot
-            int4 kb = make_int4(0, 0, 0, 0), kk = kb;
-            uint4 sg = make_uint4(0u, 0u, 0u, 0u);
-            int2 jb = make_int2(0, 0), jk = make_int2(0, 0);
-            int gJlo = 0, gnblk = 0;
-            if (!zero) {
-                const uint32_t tb = g / nt, tk = g - tb * nt;
-                kb = __ldg(T.tk3 + tb);
-                kk = __ldg(T.tk3 + tk);
-                sg = __ldg(T.sgrp3 + g);
-                const int Jminb = (kb.w >> 16) & 255, Jmink = (kk.w >> 16) & 255;
-                gJlo = max(Jminb, Jmink);
-                gnblk = ((min((kb.w >> 24) & 255, (kk.w >> 24) & 255) - gJlo) >> 1) + 1;
-                if (lane < gnblk) {
-                    jb = __ldg(T.jinfo3 + kb.z + ((gJlo - Jminb) >> 1) + lane);
-                    jk = __ldg(T.jinfo3 + kk.z + ((gJlo - Jmink) >> 1) + lane);
+        // The descriptor loads of an item form a chain of three dependent global loads (list entry -> tuple and group
+        // descriptors -> J-block rows).  They are software-pipelined over the item loop: every load is issued one full
+        // iteration before its result is used, so the producer's time per item is one slot hand-over, not three L2 latencies
+        // (ncu: consumers spent 11 % of their samples waiting on `full` behind short items).
+        struct D1 { int4 kb, kk; uint4 sg; };
+        struct D2 { int2 jb, jk; int gJlo, gnblk; };
+        auto ld_item = [&](uint32_t it) { return it < n_items ? __ldg(items + it) : make_uint4(0u, 0u, ZERO_ITEM, 0u); };
+        auto ld_d1 = [&](const uint4& item) {
+            D1 d{make_int4(0, 0, 0, 0), make_int4(0, 0, 0, 0), make_uint4(0u, 0u, 0u, 0u)};
+            if (item.z != ZERO_ITEM) {
+                const uint32_t tb = item.z / nt, tk = item.z - tb * nt;
+                d.kb = __ldg(T.tk3 + tb);
+                d.kk = __ldg(T.tk3 + tk);
+                d.sg = __ldg(T.sgrp3 + item.z);
+            }
+            return d;
+        };
+        auto ld_d2 = [&](const uint4& item, const D1& d) {
+            D2 e{make_int2(0, 0), make_int2(0, 0), 0, 0};
+            if (item.z != ZERO_ITEM) {
+                const int Jminb = (d.kb.w >> 16) & 255, Jmink = (d.kk.w >> 16) & 255;
+                e.gJlo = max(Jminb, Jmink);
+                e.gnblk = ((min((d.kb.w >> 24) & 255, (d.kk.w >> 24) & 255) - e.gJlo) >> 1) + 1;
+                if (lane < e.gnblk) {
+                    e.jb = __ldg(T.jinfo3 + d.kb.z + ((e.gJlo - Jminb) >> 1) + lane);
+                    e.jk = __ldg(T.jinfo3 + d.kk.z + ((e.gJlo - Jmink) >> 1) + lane);
                 }
             }
-            const uint32_t gsize = sg.y, S = vw_stride(gsize), bin_lo = item.w & 255u, bins = item.w >> 8;
+            return e;
+        };
+        const uint32_t G = gridDim.x;
+        uint4 item = ld_item(blockIdx.x), item1 = ld_item(blockIdx.x + G), item2 = ld_item(blockIdx.x + 2u * G);
+        D1 d0 = ld_d1(item), d1 = ld_d1(item1);
+        D2 e0 = ld_d2(item, d0);
+        for (uint32_t it = blockIdx.x; it < n_items; it += G, k++) {
+            const uint32_t s = k % TR_SLOTS;
+            // loads for the items behind this one
+            const uint4 item3 = ld_item(it + 3u * G);
+            const D1 d2 = ld_d1(item2);
+            const D2 e1 = ld_d2(item1, d1);
+            const uint4 cur = item;
+            const int4 kb = d0.kb, kk = d0.kk;
+            const uint4 sg = d0.sg;
+            const int2 jb = e0.jb, jk = e0.jk;
+            const int gnblk = e0.gnblk, gJlo = e0.gJlo;
+            item = item1; item1 = item2; item2 = item3;
+            d0 = d1; d1 = d2;
+            e0 = e1;
+            const uint32_t pos0 = cur.x, cnt = cur.y, g = cur.z;
+            const bool zero = g == ZERO_ITEM;
+            const uint32_t gsize = sg.y, S = vw_stride(gsize), bin_lo = cur.w & 255u, bins = cur.w >> 8;
             const uint32_t vw_words = zero ? 0u : (bins * S + 3u) & ~3u;
             const uint32_t rec_words = zero ? 0u : (((pos0 & 1u) + cnt + 1u) & ~1u) * 2u;
             const uint32_t need = vw_words + rec_words + (uint32_t)gnblk * 4u;
@@ -940,7 +1021,7 @@ __global__ void __launch_bounds__(TR_THREADS, MFDN_TR_MINB) k_transform3(Tables 
                 sc[SC_POS0] = pos0; sc[SC_CNT] = cnt; sc[SC_GROUP] = g;
                 sc[SC_SB] = 0u; sc[SC_SK] = 0u; sc[SC_PB0] = 0u; sc[SC_PK0] = 0u;
                 sc[SC_JINFO] = ((uint32_t)kb.w & 0xFFu) | ((uint32_t)gJlo << 8) | ((uint32_t)gnblk << 16);
-                sc[SC_GSIZE] = gsize; sc[SC_STRIDE] = S; sc[SC_BINS] = item.w; sc[SC_ROFF] = pos0 & 1u;
+                sc[SC_GSIZE] = gsize; sc[SC_STRIDE] = S; sc[SC_BINS] = cur.w; sc[SC_ROFF] = pos0 & 1u;
                 sc[SC_VW] = o_vw; sc[SC_REC] = o_rec; sc[SC_DESC] = o_desc; sc[SC_NEXT] = 0u;
             }
             __syncwarp();
@@ -999,6 +1080,16 @@ __global__ void __launch_bounds__(TR_THREADS, MFDN_TR_MINB) k_transform3(Tables 
                 for (int q = q0; q < nblk; q++) {
                     const uint4 d = desc[q];
                     const int nb = d.x & 255, nk = (d.x >> 8) & 255;
+#if MFDN_TR_PF > 0
+                    if (q + MFDN_TR_PF < nblk) {   // coefficient lines of a later J block on their way to L1 while this one is summed
+                        const uint4 dn = desc[q + MFDN_TR_PF];
+                        const uint32_t nbn = dn.x & 255u, nkn = (dn.x >> 8) & 255u;
+                        asm volatile("prefetch.global.L1 [%0];" ::"l"(dtab + (dn.y + sbA * nbn)));
+                        asm volatile("prefetch.global.L1 [%0];" ::"l"(dtab + (dn.z + skA * nkn)));
+                        asm volatile("prefetch.global.L1 [%0];" ::"l"(dtab + (dn.y + sbB * nbn)));
+                        asm volatile("prefetch.global.L1 [%0];" ::"l"(dtab + (dn.z + skB * nkn)));
+                    }
+#endif
                     const uint32_t vlA = wA + d.w * 4u, vlB = wB + d.w * 4u, vhA = vlA + G4, vhB = vlB + G4;
 #define MFDN_BLK(NB, NK) case ((NB) - 1) * 4 + ((NK) - 1): j_block3x2<NB, NK>(dtab, d.y, d.z, sbA, skA, sbB, skB, vlA, vhA, vlB, vhB, totA, totB); break;
 #define MFDN_ROWS(NK) case 16 + (NK): j_block3x2_rows<NK>(dtab, d.y, d.z, sbA, skA, sbB, skB, nb, vlA, vhA, vlB, vhB, totA, totB); break;
