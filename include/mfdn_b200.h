@@ -46,12 +46,16 @@ enum {
                              ordered gives undefined VALUES (never a fault); the mask stays correct */
     MFDN_FORCE_NAIVE = 2, /* one thread per request in request order, no sort, no staging: the paper's own
                              kernel design; kept as on-device reference */
-    MFDN_FORCE_DENSE = 4  /* 3-body: every group whose blocks fit takes the dense-block path (step H5'): per (group, M,
+    MFDN_FORCE_DENSE = 4, /* 3-body: every group whose blocks fit takes the dense-block path (step H5'): per (group, M,
                              isospin pattern) the whole block C_bra * V * C_ket^T of m-scheme elements (PAPER.md:55
                              A' = D^T A D, Fig. 1) is formed with fp64 tensor-core products (mma.sync m8n8k4) and the
                              requested entries are picked from it; the other groups take the default path.  Values
                              agree with the default path to rounding (another summation order), the mask bit for bit.
                              MFDN_ERR_ARG for 2-body calls and together with MFDN_FORCE_NAIVE */
+    MFDN_ONE_PASS_SORT = 8 /* steps H2 / H6 by the one-pass scatter and gather instead of the two-pass partition through
+                             shared memory.  The library takes this path by itself for tables with more than 2048 x 4096
+                             sort buckets (2-body: orbital-tuple pairs; 3-body: (pair, M) combinations); the flag forces
+                             it for any table (test hook and the measured baseline of DESIGN.md).  Same values bit for bit */
 };
 
 /* A0. Single-particle basis (quantum numbers flattened into one linear SPS index).

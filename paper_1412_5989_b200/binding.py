@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmfdn_b200.so")
 
 MFDN_OK, MFDN_ERR_ARG, MFDN_ERR_STATE, MFDN_ERR_CUDA, MFDN_ERR_OOM, MFDN_ERR_TABLE = 0, -1, -2, -3, -4, -5
-MFDN_PRESORTED, MFDN_FORCE_NAIVE, MFDN_FORCE_DENSE = 1, 2, 4
+MFDN_PRESORTED, MFDN_FORCE_NAIVE, MFDN_FORCE_DENSE, MFDN_ONE_PASS_SORT = 1, 2, 4, 8
 
 # every symbol include/mfdn_b200.h declares
 SYMBOLS = ["mfdn_orbitals_init", "mfdn_cg_build", "mfdn_cg_download", "mfdn_coupled_upload_2b",

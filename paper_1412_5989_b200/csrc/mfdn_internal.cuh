@@ -145,6 +145,7 @@ struct mfdn_ctx {
     int64_t slab_bytes2 = 0, slab_bytes3 = 0, dtab_bytes3 = 0, vw_bytes3 = 0;
     std::atomic<int64_t> launches{0};
     int num_sms = 148;
+    std::atomic<bool> part_attr_set{false};  // dynamic shared-memory limit of the partition kernels raised (first sort-path call)
     std::atomic<int> tr_blocks_per_sm{0};   // resident k_transform3 blocks per SM (occupancy query at the first call)
     // measurement hooks
     bool profile = false;

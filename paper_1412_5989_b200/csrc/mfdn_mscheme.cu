@@ -13,12 +13,14 @@
 // Pipeline of one call:
 //   k_keys        H1  decode, selection S1-S7 -> mask, canonicalise -> 64-bit record; histogram of the group keys
 //   k_scan_*      H2  exclusive scan of the histogram -> bucket bounds
-//   k_scatter     H2  records -> group order, posof[request] = position        (skipped if MFDN_PRESORTED)
+//   k_tscan_*, k_tiles2, k_part<1>, k_part<2>   H2  records -> bucket order by a two-pass partition through shared
+//                 memory (skipped if MFDN_PRESORTED)
 //   k_items3      H3  one-group work items from the bucket bounds (3-body); groups of <= 64 records on a second list
 //   k_transform3  H3-H5  block per item: staged isospin-combined slab, records ordered by M, paired channel sums
 //   k_transform3_small   warp per small group, direct sums in the same operation order
 //   k_transform2  H3-H5  2-body: warp per 32 records of the group-ordered stream
-//   k_unpermute   H6  values from group order back to request order            (skipped if MFDN_PRESORTED)
+//   k_back<2>, k_back<1>   H6  values from bucket order back to request order, the same two passes in reverse
+//                 (skipped if MFDN_PRESORTED)
 //   k_mscheme_naive      MFDN_FORCE_NAIVE: the paper's design, thread per request in request order
 #include <algorithm>
 #include <cstdio>
@@ -295,16 +297,24 @@ __global__ void __launch_bounds__(128) k_mscheme_naive(Tables T, long long n, co
 // records, the (a,b) -> tuple map) are copied to shared memory once per block: a random 4..16-byte
 // look-up there costs a few bank-conflict wavefronts instead of up to 32 L1 tag look-ups (ncu: k_keys was bound by
 // the L1 data pipe, 81 % of peak).
+// Sort path: a block also counts its tile's records per COARSE bin (bucket >> csh, at most PART_NC bins) in shared memory
+// and leaves the counts in tcnt[tile][bin] for the two-pass partition below (no global atomics for it).
 constexpr int KEYS_SPS_SMEM = 2048, KEYS_AB_SMEM = 2048, KEYS_PER_BLOCK = 256 * 32;
+constexpr int PART_NC = 2048;
 
 template <int BODY, bool AGG, bool SMEM>
 __global__ void __launch_bounds__(256) k_keys(Tables T, long long n, const int32_t* __restrict__ req,
                                               unsigned long long* __restrict__ recs, uint8_t* __restrict__ maskout,
                                               uint32_t* __restrict__ hist, uint32_t invalid_bucket,
-                                              uint32_t* __restrict__ keys32)
+                                              uint32_t* __restrict__ keys32, uint32_t* __restrict__ tcnt, int csh, int nc)
 {
     __shared__ uint32_t s_sps[SMEM ? KEYS_SPS_SMEM : 1];
     __shared__ int2 s_ab[SMEM && BODY == 3 ? KEYS_AB_SMEM : 1];
+    __shared__ uint32_t s_ch[AGG ? 1 : PART_NC];
+    if (!AGG && tcnt) {
+        for (int k = threadIdx.x; k < nc; k += blockDim.x) s_ch[k] = 0u;
+        if (!SMEM) __syncthreads();
+    }
     if (SMEM) {
         for (int k = threadIdx.x; k < T.n_sps; k += blockDim.x) s_sps[k] = __ldg(T.sps_rec + k);
         if (BODY == 3) {
@@ -365,9 +375,14 @@ __global__ void __launch_bounds__(256) k_keys(Tables T, long long n, const int32
                 if ((threadIdx.x & 31) == __ffs(same) - 1) atomicAdd(hist + bucket, (uint32_t)__popc(same));
             } else {
                 atomicAdd(hist + bucket, 1u);
+                if (tcnt) atomicAdd(&s_ch[bucket >> csh], 1u);
             }
         }
         if (keys32) keys32[i] = key == REC_INVALID ? 0xFFFFFFFFu : key;
+    }
+    if (!AGG && tcnt) {
+        __syncthreads();
+        for (int k = threadIdx.x; k < nc; k += blockDim.x) tcnt[(size_t)blockIdx.x * nc + k] = s_ch[k];
     }
 }
 
@@ -431,12 +446,262 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_add(uint32_t* __restrict__ data
         if (base + k < m) data[base + k] += add;
 }
 
-// H2 scatter: records -> group order; the cursor array (scanned histogram) ends up holding the END of every bucket.
-// posof[i] = position of request i in the group-ordered stream (coalesced write); the results are computed in group
-// order and gathered back by k_unpermute.  Measured alternatives: ranks from a returning histogram atomic in k_keys
-// (scatter without atomics) made k_keys 1.3 ms slower and the scatter no faster -- it is bound by the scattered
-// 8-byte writes, not by the atomics.
+// H2 group sort and H6 gather back = a two-pass partition of the 8-byte records and its mirror image for the values.
+// What decides the speed of a permutation of 2^26 8-byte elements on this machine is the number of sectors a memory
+// instruction touches, not DRAM locality: a store (or load) whose 32 lanes hit 32 different sectors costs 32 L1
+// wavefronts and 32 L2 requests, and the one-pass forms ran at 50-75 G elements/s whatever the window they wrote into
+// (measured at n = 2^26: one-pass scatter 1.71 ms, gather 1.06 ms; a two-pass partition with direct 8-byte stores 1.06 +
+// 1.38 ms; the same first pass staged in shared memory 0.33 ms).  So every pass below permutes a TILE in shared memory
+// first and then moves runs of consecutive elements with consecutive lanes:
+//   pass 1 (k_part1)  tile of KEYS_PER_BLOCK requests -> coarse bins (bucket >> csh).  The tile's first position in
+//           every bin comes from tcnt (k_keys' per-tile counts, exclusive-scanned over the tiles by k_tscan_*): no
+//           global atomics, the (tile, bin) runs are contiguous.  Leaves map1[tile slot] = coarse-order position and
+//           slot1[request] = tile slot for the way back.
+//   pass 2 (k_part2)  tiles of the coarse-ordered stream that do not straddle a coarse bin (k_tiles2) -> buckets: local
+//           counting in shared memory, one global atomic per (tile, non-empty bucket) on the scanned histogram, runs
+//           written to their final place.  Leaves map2 / slot2 likewise.  The cursor array ends up holding bucket ENDS.
+//   transform          reads the bucket-ordered records, writes the values in the same order (coalesced).
+//   H6a (k_back<2>)    per pass-2 tile: values of its runs -> shared memory -> coarse order.
+//   H6b (k_back<1>)    per pass-1 tile: values of its runs -> shared memory -> request order.
+// Capacity: PART_NC coarse bins x PART_NF buckets per bin; tables with more (group, M) buckets than that take the
+// one-pass scatter / gather (k_scatter, k_unpermute) instead.
 constexpr int SC_PER_THREAD = 4;
+constexpr int TS_CHUNK = 64;      // tiles per chunk of the two-level scan over the tiles
+constexpr int PART_NF = 4096;     // buckets per coarse bin, at most
+constexpr int P_THREADS = 512;
+constexpr int PART_SMEM = KEYS_PER_BLOCK * 8 + 2 * PART_NF * 4;   // staged tile + two tables of max(PART_NC, PART_NF) words
+static_assert(PART_NC <= PART_NF && KEYS_PER_BLOCK <= 65536, "table sizes / 16-bit tile slots");
+
+// part[chunk][bin] = sum of tcnt over the chunk's tiles
+__global__ void __launch_bounds__(128) k_tscan_sum(const uint32_t* __restrict__ tcnt, int n_tiles, int nc, uint32_t* __restrict__ part)
+{
+    const int c = blockIdx.x * 128 + threadIdx.x, k = blockIdx.y;
+    if (c >= nc) return;
+    const int t0 = k * TS_CHUNK, t1 = min(n_tiles, t0 + TS_CHUNK);
+    uint32_t sum = 0;
+#pragma unroll 8
+    for (int t = t0; t < t1; t++) sum += __ldg(tcnt + (size_t)t * nc + c);
+    part[(size_t)k * nc + c] = sum;
+}
+
+// exclusive scan of v over the threads of a block of NT threads (NT a multiple of 32, at most 1024); `total` = sum
+template <int NT>
+__device__ __forceinline__ uint32_t block_excl_scan(uint32_t v, uint32_t* s_warp /* [NT / 32 + 1] */, uint32_t& total)
+{
+    const int tid = threadIdx.x;
+    uint32_t inc = v;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+        const uint32_t x = __shfl_up_sync(0xFFFFFFFFu, inc, off);
+        if ((tid & 31) >= off) inc += x;
+    }
+    __syncthreads();   // s_warp may still be read from a previous call
+    if ((tid & 31) == 31) s_warp[tid >> 5] = inc;
+    __syncthreads();
+    if (tid < 32) {
+        const uint32_t w = tid < NT / 32 ? s_warp[tid] : 0u;
+        uint32_t wi = w;
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            const uint32_t x = __shfl_up_sync(0xFFFFFFFFu, wi, off);
+            if (tid >= off) wi += x;
+        }
+        if (tid < NT / 32) s_warp[tid] = wi - w;
+        if (tid == 31) s_warp[NT / 32] = wi;
+    }
+    __syncthreads();
+    total = s_warp[NT / 32];
+    return s_warp[tid >> 5] + inc - v;
+}
+
+// part[chunk][bin] -> first position of the chunk in the bin (exclusive scan over chunks, plus the start of the bin);
+// cstart[bin] = start of the bin in the coarse-ordered stream, cstart[nc] = n; tiles2[0] (the pass-2 tile counter) = 0
+__global__ void __launch_bounds__(1024) k_tscan_mid(uint32_t* __restrict__ part, int n_chunks, int nc, uint32_t* __restrict__ cstart)
+{
+    __shared__ uint32_t s_warp[33];
+    uint32_t carry = 0;
+    for (int c0 = 0; c0 < nc; c0 += 1024) {
+        const int c = c0 + threadIdx.x;
+        uint32_t total = 0;
+        if (c < nc) {
+            for (int k0 = 0; k0 < n_chunks; k0 += 16) {
+                uint32_t v[16];
+#pragma unroll
+                for (int u = 0; u < 16; u++) v[u] = k0 + u < n_chunks ? part[(size_t)(k0 + u) * nc + c] : 0u;
+#pragma unroll
+                for (int u = 0; u < 16; u++) {
+                    if (k0 + u < n_chunks) part[(size_t)(k0 + u) * nc + c] = total;
+                    total += v[u];
+                }
+            }
+        }
+        uint32_t all;
+        const uint32_t start = carry + block_excl_scan<1024>(total, s_warp, all);
+        carry += all;
+        if (c < nc) {
+            cstart[c] = start;
+            for (int k = 0; k < n_chunks; k++) part[(size_t)k * nc + c] += start;
+        }
+    }
+    if (threadIdx.x == 0) cstart[nc] = carry;
+}
+// tcnt[tile][bin] -> first position of the tile in the bin
+__global__ void __launch_bounds__(128) k_tscan_fill(uint32_t* __restrict__ tcnt, int n_tiles, int nc, const uint32_t* __restrict__ part)
+{
+    const int c = blockIdx.x * 128 + threadIdx.x, k = blockIdx.y;
+    if (c >= nc) return;
+    const int t0 = k * TS_CHUNK, t1 = min(n_tiles, t0 + TS_CHUNK);
+    uint32_t run = part[(size_t)k * nc + c];
+    for (int ta = t0; ta < t1; ta += 8) {
+        uint32_t v[8];
+#pragma unroll
+        for (int u = 0; u < 8; u++) v[u] = ta + u < t1 ? tcnt[(size_t)(ta + u) * nc + c] : 0u;
+#pragma unroll
+        for (int u = 0; u < 8; u++) {
+            if (ta + u < t1) tcnt[(size_t)(ta + u) * nc + c] = run;
+            run += v[u];
+        }
+    }
+}
+// pass-2 tiles: every coarse bin is cut into tiles of at most KEYS_PER_BLOCK records: tiles2[1 + k] = {first position,
+// records, bin, 0}; tiles2[0].x = number of tiles
+__global__ void __launch_bounds__(1024) k_tiles2(const uint32_t* __restrict__ cstart, int nc, uint4* __restrict__ tiles2)
+{
+    __shared__ uint32_t s_warp[33];
+    uint32_t carry = 0;
+    for (int c0 = 0; c0 < nc; c0 += 1024) {
+        const int c = c0 + threadIdx.x;
+        uint32_t s = 0, e = 0;
+        if (c < nc) { s = cstart[c]; e = cstart[c + 1]; }
+        const uint32_t k = (e - s + KEYS_PER_BLOCK - 1) / KEYS_PER_BLOCK;
+        uint32_t all;
+        const uint32_t first = carry + block_excl_scan<1024>(k, s_warp, all);
+        carry += all;
+        for (uint32_t j = 0; j < k; j++)
+            tiles2[1 + first + j] = make_uint4(s + j * KEYS_PER_BLOCK, min((uint32_t)KEYS_PER_BLOCK, e - s - j * KEYS_PER_BLOCK), (uint32_t)c, 0u);
+    }
+    if (threadIdx.x == 0) tiles2[0] = make_uint4(carry, 0u, 0u, 0u);
+}
+
+__device__ __forceinline__ uint32_t rec_bucket(unsigned long long r, uint32_t invalid_bucket)
+{
+    const uint32_t key = (uint32_t)(r >> REC_KEY_SHIFT);
+    return key == REC_INVALID ? invalid_bucket : key;
+}
+
+// One partition pass over one tile.  PASS 1: tile = k_keys tile blockIdx.x, digit = bucket >> csh, first positions from
+// toff[tile][digit].  PASS 2: tile = tiles2[1 + blockIdx.x] (inside coarse bin c), digit = bucket - (c << csh), first
+// positions reserved on cursor[bucket].  map[tile start + slot] = destination of the tile's slot-th record in digit order,
+// slot_of[source position] = slot.
+template <int PASS>
+__global__ void __launch_bounds__(P_THREADS) k_part(long long n, const unsigned long long* __restrict__ src, const uint32_t* __restrict__ toff,
+                                                   const uint4* __restrict__ tiles2, uint32_t* __restrict__ cursor, int csh, int nd,
+                                                   unsigned long long* __restrict__ dst, uint32_t* __restrict__ map, uint16_t* __restrict__ slot_of,
+                                                   uint32_t invalid_bucket)
+{
+    extern __shared__ __align__(16) unsigned char part_smem[];
+    unsigned long long* stage = reinterpret_cast<unsigned long long*>(part_smem);   // [KEYS_PER_BLOCK]
+    uint32_t* s_cnt = reinterpret_cast<uint32_t*>(stage + KEYS_PER_BLOCK);           // [nd] counts, then first slot of the digit
+    uint32_t* s_g = s_cnt + PART_NF;                                                 // [nd] destination - slot
+    __shared__ uint32_t s_warp[P_THREADS / 32 + 1];
+    constexpr int PER = KEYS_PER_BLOCK / P_THREADS;
+    const int tid = threadIdx.x;
+    long long i0;
+    int m;
+    uint32_t d0;   // digit = (bucket >> dsh) - d0
+    int dsh;
+    if (PASS == 1) {
+        i0 = (long long)blockIdx.x * KEYS_PER_BLOCK;
+        m = (int)min((long long)KEYS_PER_BLOCK, n - i0);
+        d0 = 0u; dsh = csh;
+    } else {
+        if (blockIdx.x >= __ldg(&tiles2[0].x)) return;
+        const uint4 t = __ldg(tiles2 + 1 + blockIdx.x);
+        i0 = t.x; m = (int)t.y;
+        d0 = t.z << csh; dsh = 0;
+        nd = min(nd, (int)(invalid_bucket + 1u - d0));   // the last coarse bin may be short
+    }
+    for (int k = tid; k < nd; k += P_THREADS) s_cnt[k] = 0u;
+    __syncthreads();
+    unsigned long long r[PER];
+    uint32_t rank[PER];
+#pragma unroll
+    for (int u = 0; u < PER; u++) r[u] = tid + u * P_THREADS < m ? __ldcs(src + i0 + tid + u * P_THREADS) : 0ull;
+#pragma unroll
+    for (int u = 0; u < PER; u++)
+        rank[u] = tid + u * P_THREADS < m ? atomicAdd(&s_cnt[(rec_bucket(r[u], invalid_bucket) >> dsh) - d0], 1u) : 0u;
+    __syncthreads();
+    // exclusive scan of the counts: thread t owns the digits [t * per, (t + 1) * per)
+    {
+        const int per = (nd + P_THREADS - 1) / P_THREADS, a = tid * per, b = min(nd, a + per);
+        uint32_t sum = 0;
+        for (int k = a; k < b; k++) sum += s_cnt[k];
+        uint32_t all;
+        uint32_t run = block_excl_scan<P_THREADS>(sum, s_warp, all);
+        for (int k = a; k < b; k++) {
+            const uint32_t v = s_cnt[k];
+            s_cnt[k] = run;
+            uint32_t g = 0u;
+            if (PASS == 1) g = __ldg(toff + (size_t)blockIdx.x * nd + k);
+            else if (v) g = atomicAdd(cursor + d0 + k, v);
+            s_g[k] = g - run;
+            run += v;
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int u = 0; u < PER; u++) {
+        const int l = tid + u * P_THREADS;
+        if (l < m) {
+            const uint32_t slot = s_cnt[(rec_bucket(r[u], invalid_bucket) >> dsh) - d0] + rank[u];
+            stage[slot] = r[u];
+            slot_of[i0 + l] = (uint16_t)slot;
+        }
+    }
+    __syncthreads();
+    for (int j = tid; j < m; j += P_THREADS) {
+        const unsigned long long rc = stage[j];
+        const uint32_t to = s_g[(rec_bucket(rc, invalid_bucket) >> dsh) - d0] + (uint32_t)j;
+        dst[to] = rc;
+        __stcs(map + i0 + j, to);
+    }
+}
+
+// The way back, one tile of pass PASS per block: vals[map[tile start + slot]] -> shared memory -> out[tile start + l] =
+// staged[slot_of[tile start + l]].
+template <int PASS>
+__global__ void __launch_bounds__(P_THREADS) k_back(long long n, const double* __restrict__ vals, const uint4* __restrict__ tiles2,
+                                                   const uint32_t* __restrict__ map, const uint16_t* __restrict__ slot_of, double* __restrict__ out)
+{
+    extern __shared__ __align__(16) unsigned char part_smem[];
+    double* stage = reinterpret_cast<double*>(part_smem);
+    const int tid = threadIdx.x;
+    long long i0;
+    int m;
+    if (PASS == 1) {
+        i0 = (long long)blockIdx.x * KEYS_PER_BLOCK;
+        m = (int)min((long long)KEYS_PER_BLOCK, n - i0);
+    } else {
+        if (blockIdx.x >= __ldg(&tiles2[0].x)) return;
+        const uint4 t = __ldg(tiles2 + 1 + blockIdx.x);
+        i0 = t.x; m = (int)t.y;
+    }
+    constexpr int PER = KEYS_PER_BLOCK / P_THREADS;
+    uint32_t from[PER];
+#pragma unroll
+    for (int u = 0; u < PER; u++) from[u] = tid + u * P_THREADS < m ? __ldcs(map + i0 + tid + u * P_THREADS) : 0u;
+#pragma unroll
+    for (int u = 0; u < PER; u++)
+        if (tid + u * P_THREADS < m) stage[tid + u * P_THREADS] = __ldcs(vals + from[u]);
+    __syncthreads();
+    for (int l = tid; l < m; l += P_THREADS) {
+        const double v = stage[__ldcs(slot_of + i0 + l)];
+        if (PASS == 1) __stcs(out + i0 + l, v); else out[i0 + l] = v;
+    }
+}
+
+// One-pass forms (tables with more buckets than PART_NC x PART_NF): records -> bucket order with one returning atomic
+// and one scattered store per request, posof[i] = position of request i; the cursor array ends up holding bucket ENDS.
 __global__ void __launch_bounds__(256) k_scatter(long long n, const unsigned long long* __restrict__ recs,
                                                  uint32_t* __restrict__ cursor, unsigned long long* __restrict__ sorted,
                                                  uint32_t* __restrict__ posof, uint32_t invalid_bucket)
@@ -447,13 +712,12 @@ __global__ void __launch_bounds__(256) k_scatter(long long n, const unsigned lon
 #pragma unroll
     for (int u = 0; u < SC_PER_THREAD; u++) {
         const long long i = base + u * 256;
-        r[u] = i < n ? __ldcs(recs + i) : 0ull;   // streamed once: evict first, keep the write frontier of `sorted` in L2
+        r[u] = i < n ? __ldcs(recs + i) : 0ull;
     }
 #pragma unroll
     for (int u = 0; u < SC_PER_THREAD; u++) {   // SC_PER_THREAD independent atomics in flight per thread
         const long long i = base + u * 256;
-        const uint32_t key = (uint32_t)(r[u] >> REC_KEY_SHIFT);
-        pos[u] = i < n ? atomicAdd(cursor + (key == REC_INVALID ? invalid_bucket : key), 1u) : 0u;
+        pos[u] = i < n ? atomicAdd(cursor + rec_bucket(r[u], invalid_bucket), 1u) : 0u;
     }
 #pragma unroll
     for (int u = 0; u < SC_PER_THREAD; u++) {
@@ -465,7 +729,7 @@ __global__ void __launch_bounds__(256) k_scatter(long long n, const unsigned lon
     }
 }
 
-// H6 (sort path): results from group order back to request order
+// H6, one-pass form: results from bucket order back to request order
 __global__ void __launch_bounds__(256) k_unpermute(long long n, const double* __restrict__ vals, const uint32_t* __restrict__ posof,
                                                    double* __restrict__ out)
 {
@@ -1315,13 +1579,33 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
     size_t need = 256;
     const bool dense = items && (flags & MFDN_FORCE_DENSE);
     const long long max_ditems = dense ? std::min<long long>(n, n_buckets) + 1 : 0;
-    size_t o_recs = 0, o_sorted = 0, o_order = 0, o_hist = 0, o_sums = 0, o_items = 0, o_count = 0, o_ditems = 0;
+    // sort path: coarse bins of the two-pass partition = bucket >> csh with about as many bins as buckets per bin
+    int csh = 0;
+    while ((1ll << (2 * csh)) < n_buckets) csh++;
+    csh = std::min(csh, 12);   // PART_NF = 4096 buckets per bin at most
+    while (((n_buckets + (1ll << csh) - 1) >> csh) > PART_NC) csh++;
+    const bool two_pass = sort && csh <= 12 && !(flags & MFDN_ONE_PASS_SORT);
+    const int nc = (int)((n_buckets + (1ll << csh) - 1) >> csh);
+    const long long n_ktiles = (n + KEYS_PER_BLOCK - 1) / KEYS_PER_BLOCK, n_chunks = (n_ktiles + TS_CHUNK - 1) / TS_CHUNK;
+    const long long max_tiles2 = n_ktiles + nc;
+    size_t o_recs = 0, o_p1rec = 0, o_map1 = 0, o_map2 = 0, o_slot1 = 0, o_slot2 = 0, o_tcnt = 0, o_part = 0, o_cstart = 0, o_tiles2 = 0,
+           o_hist = 0, o_sums = 0, o_items = 0, o_count = 0, o_ditems = 0;
     if (!naive) {
         need = o_recs + align256((size_t)n * 8);
         if (sort) {
-            o_sorted = need;
-            o_order = o_sorted + align256((size_t)n * 8);
-            need = o_order + align256((size_t)n * 4);
+            o_p1rec = need;
+            o_map1 = o_p1rec + align256((size_t)n * 8);
+            need = o_map1 + align256((size_t)n * 4);
+        }
+        if (two_pass) {
+            o_map2 = need;
+            o_slot1 = o_map2 + align256((size_t)n * 4);
+            o_slot2 = o_slot1 + align256((size_t)n * 2);
+            o_tcnt = o_slot2 + align256((size_t)n * 2);
+            o_part = o_tcnt + align256((size_t)n_ktiles * nc * 4);
+            o_cstart = o_part + align256((size_t)n_chunks * nc * 4);
+            o_tiles2 = o_cstart + align256((size_t)(nc + 1) * 4);
+            need = o_tiles2 + align256((size_t)(max_tiles2 + 1) * 16);
         }
         if (hist_needed) {
             o_hist = need;
@@ -1369,11 +1653,12 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
         const bool sm = c->t.n_sps <= KEYS_SPS_SMEM && (BODY == 2 || (c->t.ab3 && c->t.n_orb * c->t.n_orb <= KEYS_AB_SMEM));
         const unsigned gkb = (unsigned)((n + KEYS_PER_BLOCK - 1) / KEYS_PER_BLOCK);
         if (sort) {
-            if (sm) k_keys<BODY, false, true><<<gkb, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr);
-            else k_keys<BODY, false, false><<<gkb, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr);
+            uint32_t* tcnt = two_pass ? (uint32_t*)(w + o_tcnt) : nullptr;
+            if (sm) k_keys<BODY, false, true><<<gkb, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr, tcnt, csh, nc);
+            else k_keys<BODY, false, false><<<gkb, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr, tcnt, csh, nc);
         } else {
-            if (sm) k_keys<BODY, true, true><<<gkb, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr);
-            else k_keys<BODY, true, false><<<gkb, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr);
+            if (sm) k_keys<BODY, true, true><<<gkb, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr, nullptr, 0, 0);
+            else k_keys<BODY, true, false><<<gkb, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr, nullptr, 0, 0);
         }
         c->launches += 1;
         if (hist_needed) {
@@ -1382,15 +1667,36 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
             k_scan_add<<<(unsigned)n_tiles, SCAN_T, 0, st>>>(hist, n_buckets, sums);
             c->launches += 3;
         }
-        double* tout = d_out;   // where the transform writes: request order if pre-sorted, else group order (scratch)
-        const uint32_t* posof = nullptr;
-        if (sort) {
-            unsigned long long* sorted = (unsigned long long*)(w + o_sorted);
-            uint32_t* po = (uint32_t*)(w + o_order);
-            k_scatter<<<(unsigned)((n + 256 * SC_PER_THREAD - 1) / (256 * SC_PER_THREAD)), 256, 0, st>>>(n, recs, hist, sorted, po, invalid_bucket);
+        double* tout = d_out;   // where the transform writes: request order if pre-sorted, else bucket order (scratch)
+        unsigned long long* p1rec = (unsigned long long*)(w + o_p1rec);
+        uint32_t *map1 = (uint32_t*)(w + o_map1), *map2 = (uint32_t*)(w + o_map2);
+        uint16_t *slot1 = (uint16_t*)(w + o_slot1), *slot2 = (uint16_t*)(w + o_slot2);
+        uint4* tiles2 = (uint4*)(w + o_tiles2);
+        if (two_pass) {
+            uint32_t* tcnt = (uint32_t*)(w + o_tcnt);
+            uint32_t* part = (uint32_t*)(w + o_part);
+            uint32_t* cstart = (uint32_t*)(w + o_cstart);
+            if (!c->part_attr_set.load()) {   // benign if two threads do it at once
+                MFDN_CUDA(c, cudaFuncSetAttribute(k_part<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, PART_SMEM));
+                MFDN_CUDA(c, cudaFuncSetAttribute(k_part<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, PART_SMEM));
+                MFDN_CUDA(c, cudaFuncSetAttribute(k_back<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, KEYS_PER_BLOCK * 8));
+                MFDN_CUDA(c, cudaFuncSetAttribute(k_back<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, KEYS_PER_BLOCK * 8));
+                c->part_attr_set.store(true);
+            }
+            const dim3 gts((unsigned)((nc + 127) / 128), (unsigned)n_chunks);
+            k_tscan_sum<<<gts, 128, 0, st>>>(tcnt, (int)n_ktiles, nc, part);
+            k_tscan_mid<<<1, 1024, 0, st>>>(part, (int)n_chunks, nc, cstart);
+            k_tscan_fill<<<gts, 128, 0, st>>>(tcnt, (int)n_ktiles, nc, part);
+            k_tiles2<<<1, 1024, 0, st>>>(cstart, nc, tiles2);
+            k_part<1><<<gkb, P_THREADS, PART_SMEM, st>>>(n, recs, tcnt, nullptr, nullptr, csh, nc, p1rec, map1, slot1, invalid_bucket);
+            // the request-order records are dead after pass 1: the bucket-ordered records take their place
+            k_part<2><<<(unsigned)max_tiles2, P_THREADS, PART_SMEM, st>>>(n, p1rec, nullptr, tiles2, hist, csh, 1 << csh, recs, map2, slot2, invalid_bucket);
+            c->launches += 6;
+            tout = (double*)p1rec;   // ... and the coarse-ordered records are dead after pass 2: the values take theirs
+        } else if (sort) {
+            k_scatter<<<(unsigned)((n + 256 * SC_PER_THREAD - 1) / (256 * SC_PER_THREAD)), 256, 0, st>>>(n, recs, hist, p1rec, map1, invalid_bucket);
             c->launches += 1;
-            trecs = sorted;
-            posof = po;
+            trecs = p1rec;
             tout = (double*)recs;   // the request-order records are dead after the scatter: reuse them for the values
         }
         if (items) {
@@ -1424,8 +1730,13 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
             c->launches += 1;
         }
         if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.d, st));
-        if (sort) {
-            k_unpermute<<<(unsigned)((n + 256 * SC_PER_THREAD - 1) / (256 * SC_PER_THREAD)), 256, 0, st>>>(n, tout, posof, d_out);
+        if (two_pass) {
+            double* tmp = (double*)recs;   // the bucket-ordered records are dead after the transform
+            k_back<2><<<(unsigned)max_tiles2, P_THREADS, KEYS_PER_BLOCK * 8, st>>>(n, tout, tiles2, map2, slot2, tmp);
+            k_back<1><<<gkb, P_THREADS, KEYS_PER_BLOCK * 8, st>>>(n, tmp, nullptr, map1, slot1, d_out);
+            c->launches += 2;
+        } else if (sort) {
+            k_unpermute<<<(unsigned)((n + 256 * SC_PER_THREAD - 1) / (256 * SC_PER_THREAD)), 256, 0, st>>>(n, tout, map1, d_out);
             c->launches += 1;
         }
     }
@@ -1471,8 +1782,8 @@ extern "C" int mfdn_group_keys(mfdn_ctx* c, int body, int64_t n, const int32_t* 
     if (n == 0) return MFDN_OK;
     MFDN_CUDA(c, cudaSetDevice(c->device));
     cudaStream_t st = (cudaStream_t)stream;
-    if (body == 3) k_keys<3, false, false><<<(unsigned)((n + KEYS_PER_BLOCK - 1) / KEYS_PER_BLOCK), 256, 0, st>>>(c->t, n, d_req, nullptr, nullptr, nullptr, 0u, d_key);
-    else k_keys<2, false, false><<<(unsigned)((n + KEYS_PER_BLOCK - 1) / KEYS_PER_BLOCK), 256, 0, st>>>(c->t, n, d_req, nullptr, nullptr, nullptr, 0u, d_key);
+    if (body == 3) k_keys<3, false, false><<<(unsigned)((n + KEYS_PER_BLOCK - 1) / KEYS_PER_BLOCK), 256, 0, st>>>(c->t, n, d_req, nullptr, nullptr, nullptr, 0u, d_key, nullptr, 0, 0);
+    else k_keys<2, false, false><<<(unsigned)((n + KEYS_PER_BLOCK - 1) / KEYS_PER_BLOCK), 256, 0, st>>>(c->t, n, d_req, nullptr, nullptr, nullptr, 0u, d_key, nullptr, 0, 0);
     MFDN_CUDA(c, cudaGetLastError());
     return MFDN_OK;
 }

@@ -9,7 +9,7 @@ from paper_1412_5989_b200 import workloads as W
 pytestmark = pytest.mark.gpu
 
 TOL = 1e-12
-MODES = {"sorted_internally": 0, "naive": 2}
+MODES = {"sorted_internally": 0, "naive": 2, "one_pass_sort": 8}
 
 
 @pytest.fixture(scope="module")
@@ -157,10 +157,11 @@ def test_edge_sizes_and_bad_indices(torch, B, oracle, idx):
     ctx = get_ctx(B, idx)
     allreq = cfg.requests()
     rng = np.random.default_rng(9)
-    for n in (0, 1, 31, 32, 33, 127, 128, 129, 4097):
+    # ragged sizes around the warp, the block and the sort tile (8192 requests: last tile of 1, full, full + 1)
+    for n in (0, 1, 31, 32, 33, 127, 128, 129, 4097, 8191, 8192, 8193, 16385):
         req = allreq[rng.choice(len(allreq), n, replace=False)] if n else allreq[:0]
         want, wmask, _, _ = oracle.mscheme(cfg.basis, cfg.table, req)
-        for flags in (0, 2):
+        for flags in (0, 2, 8):
             got, gmask = run_gpu(torch, ctx, req, flags)
             check(cfg, got, gmask, want, wmask)
     # random (mostly forbidden) requests, duplicates inside bra/ket, and out-of-range SPS indices
@@ -174,8 +175,16 @@ def test_edge_sizes_and_bad_indices(torch, B, oracle, idx):
     got, gmask = run_gpu(torch, ctx, req, 2)
     check(cfg, got, gmask, want, wmask)
     assert ctx.bad_request_count() - before == nbad == 400
-    got, gmask = run_gpu(torch, ctx, req, 0)
-    check(cfg, got, gmask, want, wmask)
+    for flags in (0, 8):
+        got, gmask = run_gpu(torch, ctx, req, flags)
+        check(cfg, got, gmask, want, wmask)
+    # one hot bucket: the same request many times over (every copy lands in one run of the partition), plus a few others
+    req = np.concatenate([np.repeat(allreq[len(allreq) // 2][None, :], 30000, axis=0), allreq[rng.choice(len(allreq), 3000, replace=False)]])
+    req = req[rng.permutation(len(req))]
+    want, wmask, _, _ = oracle.mscheme(cfg.basis, cfg.table, req)
+    for flags in (0, 8):
+        got, gmask = run_gpu(torch, ctx, req, flags)
+        check(cfg, got, gmask, want, wmask)
     # mask pointer may be NULL
     d_req = torch.from_numpy(allreq[:1000].copy()).cuda()
     out = torch.empty(1000, dtype=torch.float64, device="cuda")
