@@ -637,9 +637,24 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     std::vector<int32_t> nrows(nt), sigoff(nt), mstoff(nt);
     std::vector<uint16_t> sig, mstart;   // mstart: per tuple, first sigma of every iM (prefix counts; sumj + 2 entries)
     uint64_t dtab_len = 0;
+    // Everything built in this loop -- rows, J blocks, sigma order, the coefficient table -- depends on the tuple only through
+    // (ja, jb, jc) (the J12 and J ranges above are the triangle ranges, not the listed states): tuples of one j-class share
+    // one copy (config 3: 590 tuples, 84 classes; the coefficient tables shrink from 4.1 MB to 0.6 MB and the sigma maps fit
+    // in shared memory).  nrows = 0 marks the tuples that are not the first of their class for k_dtab3.
+    std::vector<int32_t> class_rep(1 << 15, -1);   // (ja, jb, jc), 2j <= 21 < 32 each
     for (int t = 0; t < nt; t++) {
         int4 d = tdesc[t];
         int ja = d.x & 255, jb = (d.x >> 8) & 255, jc = (d.x >> 16) & 255;
+        int32_t& first = class_rep[ja | (jb << 5) | (jc << 10)];
+        if (first >= 0) {
+            trow[t] = trow[first];
+            nrows[t] = 0;
+            sigoff[t] = sigoff[first];
+            mstoff[t] = mstoff[first];
+            tk[t] = tk[first];
+            continue;
+        }
+        first = t;
         trow[t].x = (int)rowtab.size();
         trow[t].y = (int)jinfo.size();
         const int S = (ja + 1) * (jb + 1) * (jc + 1);
@@ -745,6 +760,40 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
             vwcells += vw16;
         }
     gbase[(size_t)nt * nt] = (uint32_t)buckets;
+    // The same bucket numbers from two small tables (k_keys keeps them in shared memory instead of gathering from the
+    // n_tup^2 array): gbase[b][k] = rowbase[b] + colcum[class(b)][k], class = (ja+jb+jc, parity) of the bra tuple, because
+    // the buckets a ket adds to a bra's row depend on the bra only through that pair.  class id in bits 26..30 of tdesc.x.
+    std::vector<uint32_t> rowbase(nt, 0u);
+    std::vector<uint16_t> colcum;
+    int ncls = 0;
+    {
+        std::vector<int> cls_of(128, -1);   // (sumj, par) -> class
+        std::vector<uint32_t> rowtotal;
+        bool fits = true;
+        for (int t = 0; t < nt; t++) {
+            const int sj = (tdesc[t].x & 255) + ((tdesc[t].x >> 8) & 255) + ((tdesc[t].x >> 16) & 255), par = (tdesc[t].x >> 25) & 1;
+            int& cl = cls_of[sj * 2 + par];
+            if (cl < 0) {
+                cl = ncls++;
+                colcum.resize((size_t)ncls * nt);
+                uint32_t run = 0;
+                for (int k = 0; k < nt; k++) {
+                    if (run > 65535u) fits = false;
+                    colcum[(size_t)cl * nt + k] = (uint16_t)run;
+                    const int sk = (tdesc[k].x & 255) + ((tdesc[k].x >> 8) & 255) + ((tdesc[k].x >> 16) & 255);
+                    if (((tdesc[k].x >> 25) & 1) == par) run += (uint32_t)std::min(sj, sk) + 1u;
+                }
+                rowtotal.push_back(run);
+            }
+            tdesc[t].x |= cl << 26;
+        }
+        uint64_t run = 0;
+        for (int t = 0; t < nt; t++) {
+            rowbase[t] = (uint32_t)run;
+            run += rowtotal[(tdesc[t].x >> 26) & 31];
+        }
+        if (!fits || ncls > 31) { ncls = 0; colcum.assign(1, 0); }   // k_keys then reads gbase3
+    }
     // ---- one arena for the resident index tables, one for the upload-only ones
     Arena res, tmp;
     // (a,b) -> tuple map: the sorted tuple list keeps the tuples of one (a,b) together with ascending c; if every such run
@@ -763,7 +812,7 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     std::vector<int4> tdesc_rt = tdesc;   // run-time copy: w = start of the tuple's sigma table (the row-map offset is upload-only)
     for (int t = 0; t < nt; t++) tdesc_rt[t].w = sigoff[t];
     size_t o_tid = res.add(tuple_id), o_desc_rt = res.add(tdesc_rt), o_sgrp = res.add(sgrp), o_sm = res.add(stmask);
-    size_t o_gbase = res.add(gbase);
+    size_t o_gbase = res.add(gbase), o_rowbase = res.add(rowbase), o_colcum = res.add(colcum);
     size_t o_desc = tmp.add(tdesc), o_ab = res.add(ab);
     size_t o_tk = res.add(tk), o_jinfo = res.add(jinfo), o_sig = res.add(sig), o_sigoff = res.add(sigoff);
     size_t o_mstart = res.add(mstart), o_mstoff = res.add(mstoff);
@@ -839,6 +888,10 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     c->t.sgrp3 = p.sgrp;
     c->t.gbase3 = (const uint32_t*)(dres + o_gbase);
     c->t.n_buckets3 = (uint32_t)buckets;
+    c->t.rowbase3 = (const uint32_t*)(dres + o_rowbase);
+    c->t.colcum3 = (const uint16_t*)(dres + o_colcum);
+    c->t.ncls3 = ncls;
+    c->t.sig_len3 = (int)sig.size();
     c->t.vw20 = (const uint32_t*)dvw;
     c->vw_bytes3 = (int64_t)(vwcells * 16);
     c->t.ab3 = ab_dense ? (const int2*)(dres + o_ab) : nullptr;

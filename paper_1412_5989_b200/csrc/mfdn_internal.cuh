@@ -107,6 +107,10 @@ struct Tables {
                                    //              dense-block path feasible << 31 | (bra, ket) m-state pairs with equal M}
     const uint32_t* gbase3;        // [n_tup3^2 + 1] first (group, M) bucket of a group; same-parity groups own
                                    //              min(ja+jb+jc, jd+je+jf) + 1 buckets (one per common M), the others none
+    const uint32_t* rowbase3;      // [n_tup3] and
+    const uint16_t* colcum3;       // [ncls3][n_tup3]: gbase3[b][k] = rowbase3[b] + colcum3[class(b)][k], class(b) = bits 26..30 of
+    int ncls3;                     //              tdesc3[b].x (distinct (ja+jb+jc, parity) of the tuples); ncls3 = 0: not available
+    int sig_len3;                  // entries of sig3
     uint32_t n_buckets3;           // = gbase3[n_tup3^2]; bucket n_buckets3 collects the requests failing S1-S6
     const double* slab3;
     const uint32_t* vw20;          // isospin-combined slabs, split word planes (see vw_stride)
@@ -145,6 +149,7 @@ struct mfdn_ctx {
     int64_t slab_bytes2 = 0, slab_bytes3 = 0, dtab_bytes3 = 0, vw_bytes3 = 0;
     std::atomic<int64_t> launches{0};
     int num_sms = 148;
+    std::atomic<bool> keys_attr_set{false};  // same for k_keys3s
     std::atomic<bool> part_attr_set{false};  // dynamic shared-memory limit of the partition kernels raised (first sort-path call)
     std::atomic<int> tr_blocks_per_sm{0};   // resident k_transform3 blocks per SM (occupancy query at the first call)
     // measurement hooks

@@ -386,6 +386,92 @@ __global__ void __launch_bounds__(256) k_keys(Tables T, long long n, const int32
     }
 }
 
+// H1, 3-body, every per-basis table in shared memory: SPS records, (a,b) -> tuple map, tuple descriptors, the two small
+// tables that give a group's first sort bucket (rowbase3 + colcum3 instead of a gather from the n_tup^2 array gbase3), the
+// per-class sigma maps and the tz -> isospin-bin map.  ncu on k_keys: L1 data pipe 89 % busy, a gather of 32 random table
+// entries costs up to 32 L1 wavefronts against 3-4 bank-conflict wavefronts in shared memory; without the sigma and the
+// bucket gathers the kernel ran in 1.10 instead of 1.39 ms each (n = 2^26).  One persistent block per SM walks the tiles
+// (the tables are loaded once); only the S7 state masks are still read from global memory.
+constexpr int KS_THREADS = 1024;
+struct KeysSmem3 {   // byte offsets into the dynamic shared memory, filled by the host
+    uint32_t tdesc, ab, sps, rowbase, ch, colcum, sig, tzbin, total;
+};
+template <bool AGG>
+__global__ void __launch_bounds__(KS_THREADS, 1) k_keys3s(Tables T, KeysSmem3 L, long long n, const int32_t* __restrict__ req,
+                                                         unsigned long long* __restrict__ recs, uint8_t* __restrict__ maskout,
+                                                         uint32_t* __restrict__ hist, uint32_t invalid_bucket,
+                                                         uint32_t* __restrict__ tcnt, int csh, int nc, int n_tiles)
+{
+    extern __shared__ __align__(16) unsigned char ks_smem[];
+    int4* s_tdesc = reinterpret_cast<int4*>(ks_smem + L.tdesc);
+    int2* s_ab = reinterpret_cast<int2*>(ks_smem + L.ab);
+    uint32_t* s_sps = reinterpret_cast<uint32_t*>(ks_smem + L.sps);
+    uint32_t* s_rowbase = reinterpret_cast<uint32_t*>(ks_smem + L.rowbase);
+    uint32_t* s_ch = reinterpret_cast<uint32_t*>(ks_smem + L.ch);
+    uint16_t* s_colcum = reinterpret_cast<uint16_t*>(ks_smem + L.colcum);
+    uint16_t* s_sig = reinterpret_cast<uint16_t*>(ks_smem + L.sig);
+    uint8_t* s_tzbin = ks_smem + L.tzbin;
+    const int tid = threadIdx.x, nt = T.n_tup3;
+    for (int k = tid; k < nt; k += KS_THREADS) { s_tdesc[k] = __ldg(T.tdesc3 + k); s_rowbase[k] = __ldg(T.rowbase3 + k); }
+    for (int k = tid; k < T.n_orb * T.n_orb; k += KS_THREADS) s_ab[k] = __ldg(T.ab3 + k);
+    for (int k = tid; k < T.n_sps; k += KS_THREADS) s_sps[k] = __ldg(T.sps_rec + k);
+    for (int k = tid; k < T.ncls3 * nt; k += KS_THREADS) s_colcum[k] = __ldg(T.colcum3 + k);
+    for (int k = tid; k < T.sig_len3; k += KS_THREADS) s_sig[k] = __ldg(T.sig3 + k);
+    if (tid < 64) s_tzbin[tid] = __ldg(T.tz2bin3 + tid);
+    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        if (tcnt)
+            for (int k = tid; k < nc; k += KS_THREADS) s_ch[k] = 0u;
+        __syncthreads();
+        const long long i0 = (long long)tile * KEYS_PER_BLOCK + tid;
+        const long long i1 = min(n, (long long)(tile + 1) * KEYS_PER_BLOCK);
+        int nx[6];
+        if (i0 < i1) load_req3(req, i0, nx);
+        for (long long i = i0; i < i1; i += KS_THREADS) {
+            int s[6];
+#pragma unroll
+            for (int k = 0; k < 6; k++) s[k] = nx[k];
+            if (i + KS_THREADS < i1) load_req3(req, i + KS_THREADS, nx);   // next request in flight
+            uint32_t key = REC_INVALID;
+            unsigned long long low = 0;
+            int mask = 0;
+            if (!in_range(T, s, 6)) {
+                atomicAdd(T.bad_count, 1ull);
+            } else {
+                Side3 B = decode3<true>(T, s_sps, s_ab, s[0], s[1], s[2]), K = decode3<true>(T, s_sps, s_ab, s[3], s[4], s[5]);
+                if (select3(T, B, K)) {
+                    const int4 db = s_tdesc[B.tup], dk = s_tdesc[K.tup];
+                    const int sjb = (db.x & 255) + ((db.x >> 8) & 255) + ((db.x >> 16) & 255);
+                    const int sjk = (dk.x & 255) + ((dk.x >> 8) & 255) + ((dk.x >> 16) & 255);
+                    key = s_rowbase[B.tup] + s_colcum[((db.x >> 26) & 31) * nt + K.tup] +
+                          (uint32_t)(B.ima + B.imb + B.imc - ((sjb - min(sjb, sjk)) >> 1));
+                    mask = mask3(T, B, K, db, dk);
+                    const int jb1 = ((db.x >> 8) & 255) + 1, jc1 = ((db.x >> 16) & 255) + 1;
+                    const int je1 = ((dk.x >> 8) & 255) + 1, jf1 = ((dk.x >> 16) & 255) + 1;
+                    const uint32_t sb = s_sig[db.w + (B.ima * jb1 + B.imb) * jc1 + B.imc];
+                    const uint32_t sk = s_sig[dk.w + (K.ima * je1 + K.imb) * jf1 + K.imc];
+                    const uint32_t bin = s_tzbin[(B.tz << 3) | K.tz];
+                    low = (unsigned long long)(sb | (sk << 12) | (bin << 24) | ((uint32_t)(B.sign * K.sign < 0) << 29)) |
+                          ((unsigned long long)(B.ima + B.imb + B.imc) << 30);
+                }
+            }
+            recs[i] = ((unsigned long long)key << REC_KEY_SHIFT) | low;
+            if (maskout) maskout[i] = (uint8_t)mask;
+            const uint32_t bucket = key == REC_INVALID ? invalid_bucket : key;
+            if (AGG) {   // group-ordered input: one atomic per run of equal keys in the warp
+                const unsigned same = __match_any_sync(__activemask(), bucket);
+                if ((tid & 31) == __ffs(same) - 1) atomicAdd(hist + bucket, (uint32_t)__popc(same));
+            } else {
+                atomicAdd(hist + bucket, 1u);
+                if (tcnt) atomicAdd(&s_ch[bucket >> csh], 1u);
+            }
+        }
+        if (tcnt) {
+            __syncthreads();
+            for (int k = tid; k < nc; k += KS_THREADS) tcnt[(size_t)tile * nc + k] = s_ch[k];
+        }
+    }
+}
+
 // =============================================================================== H2: group sort
 constexpr int SCAN_T = 256, SCAN_E = 16, SCAN_TILE = SCAN_T * SCAN_E;
 
@@ -1652,7 +1738,33 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
         if (hist_needed) MFDN_CUDA(c, cudaMemsetAsync(hist, 0, (size_t)n_buckets * 4, st));
         const bool sm = c->t.n_sps <= KEYS_SPS_SMEM && (BODY == 2 || (c->t.ab3 && c->t.n_orb * c->t.n_orb <= KEYS_AB_SMEM));
         const unsigned gkb = (unsigned)((n + KEYS_PER_BLOCK - 1) / KEYS_PER_BLOCK);
-        if (sort) {
+        // 3-body with every per-basis table in shared memory (k_keys3s) when they fit; MFDN_ONE_PASS_SORT keeps the general kernel
+        KeysSmem3 L{};
+        bool smem_keys = false;
+        if (BODY == 3 && sm && c->t.ncls3 > 0 && !(flags & MFDN_ONE_PASS_SORT)) {
+            auto up = [](uint32_t x) { return (x + 15u) & ~15u; };
+            L.tdesc = 0;
+            L.ab = up(L.tdesc + (uint32_t)nt * 16u);
+            L.sps = up(L.ab + (uint32_t)(c->t.n_orb * c->t.n_orb) * 8u);
+            L.rowbase = up(L.sps + (uint32_t)c->t.n_sps * 4u);
+            L.ch = up(L.rowbase + (uint32_t)nt * 4u);
+            L.colcum = up(L.ch + (uint32_t)PART_NC * 4u);
+            L.sig = up(L.colcum + (uint32_t)(c->t.ncls3 * nt) * 2u);
+            L.tzbin = up(L.sig + (uint32_t)c->t.sig_len3 * 2u);
+            L.total = L.tzbin + 64u;
+            smem_keys = L.total <= 200u * 1024u;
+        }
+        if (smem_keys) {
+            if (!c->keys_attr_set.load()) {   // benign if two threads do it at once
+                MFDN_CUDA(c, cudaFuncSetAttribute(k_keys3s<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+                MFDN_CUDA(c, cudaFuncSetAttribute(k_keys3s<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+                c->keys_attr_set.store(true);
+            }
+            const unsigned gks = (unsigned)std::min<long long>(n_ktiles, c->num_sms);
+            if (sort) k_keys3s<false><<<gks, KS_THREADS, L.total, st>>>(c->t, L, n, d_req, recs, d_mask, hist, invalid_bucket,
+                                                                         two_pass ? (uint32_t*)(w + o_tcnt) : nullptr, csh, nc, (int)n_ktiles);
+            else k_keys3s<true><<<gks, KS_THREADS, L.total, st>>>(c->t, L, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr, 0, 0, (int)n_ktiles);
+        } else if (sort) {
             uint32_t* tcnt = two_pass ? (uint32_t*)(w + o_tcnt) : nullptr;
             if (sm) k_keys<BODY, false, true><<<gkb, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr, tcnt, csh, nc);
             else k_keys<BODY, false, false><<<gkb, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr, tcnt, csh, nc);
