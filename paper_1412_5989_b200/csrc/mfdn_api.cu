@@ -620,6 +620,22 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     for (int t = 0; t < nt; t++)
         for (int i = nJ12v[t] - 2; i >= 0; i--)
             for (int T12 = 0; T12 < 2; T12++) stmask[tdesc[t].z + i * 2 + T12] |= stmask[tdesc[t].z + (i + 1) * 2 + T12];
+    // tuples with identical mask rows share one copy (a complete table has one per (ja, jb, jc, a == b) class): k_keys3s keeps
+    // the deduplicated array in shared memory
+    {
+        std::map<std::vector<unsigned long long>, int> seen;
+        std::vector<unsigned long long> packed;
+        for (int t = 0; t < nt; t++) {
+            std::vector<unsigned long long> rows(stmask.begin() + tdesc[t].z, stmask.begin() + tdesc[t].z + (size_t)nJ12v[t] * 2);
+            auto it = seen.find(rows);
+            if (it == seen.end()) {
+                it = seen.emplace(rows, (int)packed.size()).first;
+                packed.insert(packed.end(), rows.begin(), rows.end());
+            }
+            tdesc[t].z = it->second;
+        }
+        stmask.swap(packed);
+    }
     auto range = [&](int4 d, int twoJ, int& lo, int& hi) {
         int jc = (d.x >> 16) & 255;
         lo = std::max(d.y & 255, std::abs(twoJ - jc) >> 1);
@@ -892,6 +908,7 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     c->t.colcum3 = (const uint16_t*)(dres + o_colcum);
     c->t.ncls3 = ncls;
     c->t.sig_len3 = (int)sig.size();
+    c->t.stmask_len3 = (int)stmask.size();
     c->t.vw20 = (const uint32_t*)dvw;
     c->vw_bytes3 = (int64_t)(vwcells * 16);
     c->t.ab3 = ab_dense ? (const int2*)(dres + o_ab) : nullptr;

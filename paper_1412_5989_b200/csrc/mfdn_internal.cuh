@@ -110,7 +110,7 @@ struct Tables {
     const uint32_t* rowbase3;      // [n_tup3] and
     const uint16_t* colcum3;       // [ncls3][n_tup3]: gbase3[b][k] = rowbase3[b] + colcum3[class(b)][k], class(b) = bits 26..30 of
     int ncls3;                     //              tdesc3[b].x (distinct (ja+jb+jc, parity) of the tuples); ncls3 = 0: not available
-    int sig_len3;                  // entries of sig3
+    int sig_len3, stmask_len3;     // entries of sig3 and of stmask3
     uint32_t n_buckets3;           // = gbase3[n_tup3^2]; bucket n_buckets3 collects the requests failing S1-S6
     const double* slab3;
     const uint32_t* vw20;          // isospin-combined slabs, split word planes (see vw_stride)

@@ -125,24 +125,27 @@ __device__ __forceinline__ bool select2(const Side2& B, const Side2& K)
 }
 
 // S7 helper: set of (J,T) channels in which this side has an admissible listed state
-__device__ __forceinline__ unsigned long long chanmask3(const Tables& T, int4 d, int twoM12, int twoMT12)
+template <bool SMEM = false>
+__device__ __forceinline__ unsigned long long chanmask3(const unsigned long long* stm, int4 d, int twoM12, int twoMT12)
 {
     const int J12min = d.y & 255, J12max = (d.y >> 8) & 255;
     const int lo = max(J12min, (abs(twoM12) + 1) >> 1);   // 2*J12 >= |2*M12|
     if (lo > J12max) return 0ull;
     // stmask3 holds suffix ORs over J12: one 16-byte entry {T12 = 0, T12 = 1} covers all J12 >= lo
-    const ulonglong2 m = __ldg(reinterpret_cast<const ulonglong2*>(T.stmask3 + d.z + (lo - J12min) * 2));
+    const ulonglong2* p = reinterpret_cast<const ulonglong2*>(stm + d.z + (lo - J12min) * 2);
+    const ulonglong2 m = SMEM ? *p : __ldg(p);
     return (twoMT12 == 0 ? m.x : 0ull) | m.y;
 }
 
 // S7 for a decoded 3-body request that passed S1-S6: at least one admissible channel term
-__device__ __forceinline__ bool mask3(const Tables& T, const Side3& B, const Side3& K, int4 db, int4 dk)
+template <bool SMEM = false>
+__device__ __forceinline__ bool mask3(const unsigned long long* stm, const Side3& B, const Side3& K, int4 db, int4 dk)
 {
     if (max((db.y >> 16) & 255, (dk.y >> 16) & 255) > min((db.y >> 24) & 255, (dk.y >> 24) & 255)) return false;   // no common J: no slab
     const int ja = db.x & 255, jb = (db.x >> 8) & 255, jd = dk.x & 255, je = (dk.x >> 8) & 255;
     const int twoM12b = 2 * (B.ima + B.imb) - ja - jb, twoM12k = 2 * (K.ima + K.imb) - jd - je;
     const int tzb12 = (B.tz >> 2) + ((B.tz >> 1) & 1) - 1, tzk12 = (K.tz >> 2) + ((K.tz >> 1) & 1) - 1;  // MT12
-    unsigned long long mm = chanmask3(T, db, twoM12b, 2 * tzb12) & chanmask3(T, dk, twoM12k, 2 * tzk12);
+    unsigned long long mm = chanmask3<SMEM>(stm, db, twoM12b, 2 * tzb12) & chanmask3<SMEM>(stm, dk, twoM12k, 2 * tzk12);
     mm &= ~0ull << (2 * (abs(B.twoM) >> 1));                   // J >= |M|
     if (abs(B.twoMT) == 3) mm &= 0xAAAAAAAAAAAAAAAAull;        // T = 3/2 only
     return mm != 0;
@@ -179,7 +182,7 @@ __device__ __forceinline__ double eval3_naive(const Tables& T, const Side3& B, c
     const uint4 sg = __ldg(T.sgrp3 + (size_t)B.tup * T.n_tup3 + K.tup);
     if (sg.x == NO_SLAB) return 0.0;
     const int4 db = __ldg(T.tdesc3 + B.tup), dk = __ldg(T.tdesc3 + K.tup);
-    if (!mask3(T, B, K, db, dk)) return 0.0;
+    if (!mask3(T.stmask3, B, K, db, dk)) return 0.0;
     mask = 1;
     const int ja = db.x & 255, jb = (db.x >> 8) & 255, jc = (db.x >> 16) & 255;
     const int jd = dk.x & 255, je = (dk.x >> 8) & 255, jf = (dk.x >> 16) & 255;
@@ -347,7 +350,7 @@ __global__ void __launch_bounds__(256) k_keys(Tables T, long long n, const int32
                     const int sjk = (dk.x & 255) + ((dk.x >> 8) & 255) + ((dk.x >> 16) & 255);
                     key = __ldg(T.gbase3 + (size_t)B.tup * T.n_tup3 + K.tup) + (uint32_t)(B.ima + B.imb + B.imc - ((sjb - min(sjb, sjk)) >> 1));
                 }
-                mask = mask3(T, B, K, db, dk);
+                mask = mask3(T.stmask3, B, K, db, dk);
                 const int jb1 = ((db.x >> 8) & 255) + 1, jc1 = ((db.x >> 16) & 255) + 1;
                 const int je1 = ((dk.x >> 8) & 255) + 1, jf1 = ((dk.x >> 16) & 255) + 1;
                 const uint32_t sb = __ldg(T.sig3 + db.w + (B.ima * jb1 + B.imb) * jc1 + B.imc);
@@ -391,10 +394,10 @@ __global__ void __launch_bounds__(256) k_keys(Tables T, long long n, const int32
 // per-class sigma maps and the tz -> isospin-bin map.  ncu on k_keys: L1 data pipe 89 % busy, a gather of 32 random table
 // entries costs up to 32 L1 wavefronts against 3-4 bank-conflict wavefronts in shared memory; without the sigma and the
 // bucket gathers the kernel ran in 1.10 instead of 1.39 ms each (n = 2^26).  One persistent block per SM walks the tiles
-// (the tables are loaded once); only the S7 state masks are still read from global memory.
+// (the tables are loaded once).  The S7 state masks, deduplicated at upload, are there too (0.21 ms of gathers otherwise).
 constexpr int KS_THREADS = 1024;
 struct KeysSmem3 {   // byte offsets into the dynamic shared memory, filled by the host
-    uint32_t tdesc, ab, sps, rowbase, ch, colcum, sig, tzbin, total;
+    uint32_t tdesc, stm, ab, sps, rowbase, ch, colcum, sig, tzbin, total;
 };
 template <bool AGG>
 __global__ void __launch_bounds__(KS_THREADS, 1) k_keys3s(Tables T, KeysSmem3 L, long long n, const int32_t* __restrict__ req,
@@ -404,6 +407,7 @@ __global__ void __launch_bounds__(KS_THREADS, 1) k_keys3s(Tables T, KeysSmem3 L,
 {
     extern __shared__ __align__(16) unsigned char ks_smem[];
     int4* s_tdesc = reinterpret_cast<int4*>(ks_smem + L.tdesc);
+    unsigned long long* s_stm = reinterpret_cast<unsigned long long*>(ks_smem + L.stm);
     int2* s_ab = reinterpret_cast<int2*>(ks_smem + L.ab);
     uint32_t* s_sps = reinterpret_cast<uint32_t*>(ks_smem + L.sps);
     uint32_t* s_rowbase = reinterpret_cast<uint32_t*>(ks_smem + L.rowbase);
@@ -413,6 +417,7 @@ __global__ void __launch_bounds__(KS_THREADS, 1) k_keys3s(Tables T, KeysSmem3 L,
     uint8_t* s_tzbin = ks_smem + L.tzbin;
     const int tid = threadIdx.x, nt = T.n_tup3;
     for (int k = tid; k < nt; k += KS_THREADS) { s_tdesc[k] = __ldg(T.tdesc3 + k); s_rowbase[k] = __ldg(T.rowbase3 + k); }
+    for (int k = tid; k < T.stmask_len3; k += KS_THREADS) s_stm[k] = __ldg(T.stmask3 + k);
     for (int k = tid; k < T.n_orb * T.n_orb; k += KS_THREADS) s_ab[k] = __ldg(T.ab3 + k);
     for (int k = tid; k < T.n_sps; k += KS_THREADS) s_sps[k] = __ldg(T.sps_rec + k);
     for (int k = tid; k < T.ncls3 * nt; k += KS_THREADS) s_colcum[k] = __ldg(T.colcum3 + k);
@@ -444,7 +449,7 @@ __global__ void __launch_bounds__(KS_THREADS, 1) k_keys3s(Tables T, KeysSmem3 L,
                     const int sjk = (dk.x & 255) + ((dk.x >> 8) & 255) + ((dk.x >> 16) & 255);
                     key = s_rowbase[B.tup] + s_colcum[((db.x >> 26) & 31) * nt + K.tup] +
                           (uint32_t)(B.ima + B.imb + B.imc - ((sjb - min(sjb, sjk)) >> 1));
-                    mask = mask3(T, B, K, db, dk);
+                    mask = mask3<true>(s_stm, B, K, db, dk);
                     const int jb1 = ((db.x >> 8) & 255) + 1, jc1 = ((db.x >> 16) & 255) + 1;
                     const int je1 = ((dk.x >> 8) & 255) + 1, jf1 = ((dk.x >> 16) & 255) + 1;
                     const uint32_t sb = s_sig[db.w + (B.ima * jb1 + B.imb) * jc1 + B.imc];
@@ -1744,7 +1749,8 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
         if (BODY == 3 && sm && c->t.ncls3 > 0 && !(flags & MFDN_ONE_PASS_SORT)) {
             auto up = [](uint32_t x) { return (x + 15u) & ~15u; };
             L.tdesc = 0;
-            L.ab = up(L.tdesc + (uint32_t)nt * 16u);
+            L.stm = up(L.tdesc + (uint32_t)nt * 16u);
+            L.ab = up(L.stm + (uint32_t)c->t.stmask_len3 * 8u);
             L.sps = up(L.ab + (uint32_t)(c->t.n_orb * c->t.n_orb) * 8u);
             L.rowbase = up(L.sps + (uint32_t)c->t.n_sps * 4u);
             L.ch = up(L.rowbase + (uint32_t)nt * 4u);
