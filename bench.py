@@ -277,13 +277,17 @@ def main():
     gbs_tr = alg["bytes_presorted"] * n / t_tr / 1e9
     roof_hbm_ms = alg["bytes_presorted"] * n / (hbm_peak * 1e9) * 1e3
     roof_alu_ms = alg["flops"] * n / (fp64_peak * 1e12) * 1e3
-    traffic = None
+    # figures taken from the ncu --set full capture of the dominant kernel (profiles/dram_traffic.txt names the capture, its
+    # command and the commit it was made at; a capture cannot run inside a timed bench)
+    prof = {}
     tp = os.path.join(ROOT, "profiles", "dram_traffic.txt")
     if os.path.exists(tp):
         for line in open(tp):
-            f = line.split()
-            if len(f) >= 2 and f[0] == f"k_mscheme_body{body}_bytes_per_launch":
-                traffic = float(f[1])
+            f = line.split("#")[0].split()
+            if len(f) >= 2:
+                prof[f[0]] = f[1]
+    traffic = float(prof[f"k_transform{body}_dram_bytes_per_launch"]) if f"k_transform{body}_dram_bytes_per_launch" in prof else None
+    exec_flops = float(prof.get(f"k_transform{body}_executed_flops_per_request", "nan"))
     out = {
         "metric": METRIC, "value": world * n / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -301,7 +305,15 @@ def main():
                       "note": "same multiset pre-ordered by mfdn_group_keys, flag MFDN_PRESORTED"},
         "roofline": {"kernel": f"k_transform{body}" + (" + k_transform3_small (groups of <= 64 records; 3 % of the time)" if body == 3 else "") + ": dominant kernel of the unsorted step; CUDA events on the launch stream", "bound": "alu",
                      "achieved": flops_rate, "peak": fp64_peak, "unit": "TFLOP/s", "frac": flops_rate / fp64_peak,
-                     "traffic": traffic, "flops_per_request": alg["flops"],
+                     "traffic": traffic, "traffic_source": {"file": "profiles/dram_traffic.txt", "capture": prof.get("capture"),
+                                                            "commit": prof.get("commit")},
+                     "flops_per_request": alg["flops"],
+                     "note": "frac = ALGORITHMIC flops of the direct channel sum (SURVEY.md 8(d)) / kernel time / measured DFMA peak; "
+                             "the kernel executes fewer (isospin-combined slabs are built at upload), see `as_built`",
+                     "as_built": {"executed_flops_per_request": exec_flops,
+                                  "frac_alu_executed": (exec_flops * n / t_tr / 1e12 / fp64_peak) if exec_flops == exec_flops else None,
+                                  "applicable_bound": "hbm", "frac_hbm": gbs_tr / hbm_peak,
+                                  "limiter_measured": prof.get(f"k_transform{body}_limiter")},
                      "peak_source": "measured DFMA micro-benchmark (mfdn_fp64_peak); nominal %.1f" % FP64_NOMINAL_TFLOPS,
                      "hbm": {"achieved": gbs_tr, "peak": hbm_peak, "unit": "GB/s", "frac": gbs_tr / hbm_peak,
                              "bytes_per_request": alg["bytes_presorted"], "peak_source": peak_src},
@@ -314,6 +326,7 @@ def main():
         n_s = 1 << args.ref_log2n
         v, cores, dt = cpu_baseline(cfg, n_s)
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                               "note": "definition-order checker (oracle/mscheme_oracle.c), never tuned: a reported baseline, not a CPU implementation",
                                "sample": f"first 2^{args.ref_log2n} requests of the same stream, {dt:.1f} s"}
     if configs is not None:
         b_pre, b_uns, fl = alg["bytes_presorted"], alg["bytes_unsorted"], alg["flops"]

@@ -570,7 +570,7 @@ __global__ void __launch_bounds__(128) k_tscan_sum(const uint32_t* __restrict__ 
     if (c >= nc) return;
     const int t0 = k * TS_CHUNK, t1 = min(n_tiles, t0 + TS_CHUNK);
     uint32_t sum = 0;
-#pragma unroll 8
+#pragma unroll 16
     for (int t = t0; t < t1; t++) sum += __ldg(tcnt + (size_t)t * nc + c);
     part[(size_t)k * nc + c] = sum;
 }
@@ -605,8 +605,8 @@ __device__ __forceinline__ uint32_t block_excl_scan(uint32_t v, uint32_t* s_warp
     return s_warp[tid >> 5] + inc - v;
 }
 
-// part[chunk][bin] -> first position of the chunk in the bin (exclusive scan over chunks, plus the start of the bin);
-// cstart[bin] = start of the bin in the coarse-ordered stream, cstart[nc] = n; tiles2[0] (the pass-2 tile counter) = 0
+// part[chunk][bin] -> records of the bin in the chunks before (exclusive scan over chunks); cstart[bin] = start of the bin
+// in the coarse-ordered stream, cstart[nc] = n
 __global__ void __launch_bounds__(1024) k_tscan_mid(uint32_t* __restrict__ part, int n_chunks, int nc, uint32_t* __restrict__ cstart)
 {
     __shared__ uint32_t s_warp[33];
@@ -629,26 +629,24 @@ __global__ void __launch_bounds__(1024) k_tscan_mid(uint32_t* __restrict__ part,
         uint32_t all;
         const uint32_t start = carry + block_excl_scan<1024>(total, s_warp, all);
         carry += all;
-        if (c < nc) {
-            cstart[c] = start;
-            for (int k = 0; k < n_chunks; k++) part[(size_t)k * nc + c] += start;
-        }
+        if (c < nc) cstart[c] = start;
     }
     if (threadIdx.x == 0) cstart[nc] = carry;
 }
 // tcnt[tile][bin] -> first position of the tile in the bin
-__global__ void __launch_bounds__(128) k_tscan_fill(uint32_t* __restrict__ tcnt, int n_tiles, int nc, const uint32_t* __restrict__ part)
+__global__ void __launch_bounds__(128) k_tscan_fill(uint32_t* __restrict__ tcnt, int n_tiles, int nc, const uint32_t* __restrict__ part,
+                                                    const uint32_t* __restrict__ cstart)
 {
     const int c = blockIdx.x * 128 + threadIdx.x, k = blockIdx.y;
     if (c >= nc) return;
     const int t0 = k * TS_CHUNK, t1 = min(n_tiles, t0 + TS_CHUNK);
-    uint32_t run = part[(size_t)k * nc + c];
-    for (int ta = t0; ta < t1; ta += 8) {
-        uint32_t v[8];
+    uint32_t run = part[(size_t)k * nc + c] + cstart[c];
+    for (int ta = t0; ta < t1; ta += 16) {
+        uint32_t v[16];
 #pragma unroll
-        for (int u = 0; u < 8; u++) v[u] = ta + u < t1 ? tcnt[(size_t)(ta + u) * nc + c] : 0u;
+        for (int u = 0; u < 16; u++) v[u] = ta + u < t1 ? tcnt[(size_t)(ta + u) * nc + c] : 0u;
 #pragma unroll
-        for (int u = 0; u < 8; u++) {
+        for (int u = 0; u < 16; u++) {
             if (ta + u < t1) tcnt[(size_t)(ta + u) * nc + c] = run;
             run += v[u];
         }
@@ -1804,7 +1802,7 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
             const dim3 gts((unsigned)((nc + 127) / 128), (unsigned)n_chunks);
             k_tscan_sum<<<gts, 128, 0, st>>>(tcnt, (int)n_ktiles, nc, part);
             k_tscan_mid<<<1, 1024, 0, st>>>(part, (int)n_chunks, nc, cstart);
-            k_tscan_fill<<<gts, 128, 0, st>>>(tcnt, (int)n_ktiles, nc, part);
+            k_tscan_fill<<<gts, 128, 0, st>>>(tcnt, (int)n_ktiles, nc, part, cstart);
             k_tiles2<<<1, 1024, 0, st>>>(cstart, nc, tiles2);
             k_part<1><<<gkb, P_THREADS, PART_SMEM, st>>>(n, recs, tcnt, nullptr, nullptr, csh, nc, p1rec, map1, slot1, invalid_bucket);
             // the request-order records are dead after pass 1: the bucket-ordered records take their place
