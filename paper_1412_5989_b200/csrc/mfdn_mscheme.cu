@@ -559,7 +559,10 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_add(uint32_t* __restrict__ data
 constexpr int SC_PER_THREAD = 4;
 constexpr int TS_CHUNK = 64;      // tiles per chunk of the two-level scan over the tiles
 constexpr int PART_NF = 4096;     // buckets per coarse bin, at most
-constexpr int P_THREADS = 512;
+#ifndef MFDN_P_THREADS
+#define MFDN_P_THREADS 512
+#endif
+constexpr int P_THREADS = MFDN_P_THREADS;
 constexpr int PART_SMEM = KEYS_PER_BLOCK * 8 + 2 * PART_NF * 4;   // staged tile + two tables of max(PART_NC, PART_NF) words
 static_assert(PART_NC <= PART_NF && KEYS_PER_BLOCK <= 65536, "table sizes / 16-bit tile slots");
 

@@ -431,3 +431,21 @@ def make_config(index: int, table_values: str = "normal") -> Config:
         return Config(4, "3b_E3max10_e6_16x2^24", 3, b, coupled_3b(b, 10, 4, table_values), ms, 1 << 28, False, 1004,
                       ms_low=low, low_frac=0.7, n_batches=16)
     raise ValueError(f"no config {index}")
+
+
+def many_body_targets(n: int, h_len: int, seed: int, mean_run: float = 4.0):
+    """Where MFDn would add the n results (every buffered request carries the many-body element it
+    pertains to and a phase): consecutive requests belong to one many-body element in runs of geometric length (mean
+    `mean_run`; the recursive loop of PAPER.md:91 asks for the 3-body elements of one many-body element one after the
+    other), the element of a run is uniform in [0, h_len), the phase of a request is +1 or -1.  Seeded, no arithmetic of
+    the method.  Returns (loc int64 [n], phase float64 [n])."""
+    rng = np.random.default_rng([777, seed])
+    heads = rng.random(n) < 1.0 / mean_run
+    if n:
+        heads[0] = True
+    run_id = np.cumsum(heads) - 1
+    targets = rng.integers(0, h_len, size=int(run_id[-1]) + 1 if n else 0, dtype=np.int64)
+    loc = targets[run_id] if n else np.zeros(0, np.int64)
+    phase = np.where(rng.random(n) < 0.5, 1.0, -1.0)
+    return np.ascontiguousarray(loc, np.int64), np.ascontiguousarray(phase, np.float64)
+

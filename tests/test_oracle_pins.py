@@ -478,3 +478,37 @@ def test_structure_counts_large_configs():
         assert ms.sec_size.max() == g[f"cfg{i}.largest_sector"]
         if i == 3:
             assert ms.n_conserving_pairs == g["cfg3.conserving_pairs"]
+
+
+# --------------------------------------------------------------------------------- NEXT-1: the accumulate step
+def test_accumulate_definition_pins():
+    """oracle/accumulate_ref.py against what the definition fixes without re-typing it: one request per location gives
+    phase * v; one location for all requests gives the exactly rounded sum (math.fsum) within n ulp; the total is
+    conserved; out-of-range locations are dropped; numpy's unbuffered add.at (a library routine) agrees."""
+    import math
+    from oracle.accumulate_ref import accumulate
+    from paper_1412_5989_b200 import workloads as Wl
+    rng = np.random.default_rng(3)
+    n = 5000
+    v = rng.standard_normal(n)
+    ph = np.where(rng.random(n) < 0.5, 1.0, -1.0)
+    H = accumulate(v, np.arange(n), ph, n)
+    assert np.array_equal(H, ph * v)
+    H = accumulate(v, np.arange(n)[::-1], None, n)
+    assert np.array_equal(H, v[::-1])
+    H = accumulate(v, np.zeros(n, np.int64), ph, 3)
+    assert H[1] == 0.0 and H[2] == 0.0
+    assert abs(H[0] - math.fsum(ph * v)) <= n * np.finfo(float).eps * float(np.sum(np.abs(v)))
+    loc, phase = Wl.many_body_targets(n, 700, seed=1)
+    assert loc.min() >= 0 and loc.max() < 700 and set(np.unique(phase)) == {-1.0, 1.0}
+    assert 2.5 < n / (1 + np.count_nonzero(np.diff(loc))) < 6.0          # runs of mean length about 4
+    H = accumulate(v, loc, phase, 700)
+    assert abs(math.fsum(H) - math.fsum(phase * v)) <= 1e-12
+    ref = np.zeros(700)
+    np.add.at(ref, loc, phase * v)
+    assert np.array_equal(H, ref)
+    bad = loc.copy()
+    bad[::7] = -1
+    bad[3::11] = 700
+    keep = (bad >= 0) & (bad < 700)
+    assert np.array_equal(accumulate(v, bad, phase, 700), accumulate(v[keep], bad[keep], phase[keep], 700))
