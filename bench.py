@@ -233,6 +233,30 @@ def main():
         got, gmask = d_out[ds].cpu().numpy(), d_mask[ds].cpu().numpy()
         headline_check = {"sampled": int(len(sample)), "max_abs_delta": float(np.max(np.abs(got - want))),
                           "tolerance": 1e-12 * float(np.max(np.abs(cfg.table.values))), "mask_bit_exact": bool(np.array_equal(gmask, wmask))}
+    # ---- NEXT-1: the same step with the results accumulated into a many-body array instead of returned
+    accum = None
+    if world == 1:
+        h_len = 1 << 24
+        loc, phase = W.many_body_targets(n, h_len, seed=args.config)
+        d_loc, d_phase = torch.from_numpy(loc).cuda(), torch.from_numpy(phase).cuda()
+        d_H = torch.zeros(h_len, dtype=torch.float64, device="cuda")
+        awork = torch.empty(B.mfdn_mscheme_accumulate(ctx.ctx, body, n, 0, 0, 0, 0, 0, 0, 0, 0, 0), dtype=torch.uint8, device="cuda")
+        for _ in range(args.warmup):
+            ctx.accumulate(d_req, d_loc, d_phase, d_H, d_mask, 0, awork)
+        d_H.zero_()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        ctx.accumulate(d_req, d_loc, d_phase, d_H, d_mask, 0, awork)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        # property that holds at any size: the accumulated array equals a library index_add of the returned values
+        ref = torch.zeros(h_len, dtype=torch.float64, device="cuda").index_add_(0, d_loc, d_phase * d_out)
+        accum = {"ms_per_step": e0.elapsed_time(e1), "value": n / (e0.elapsed_time(e1) * 1e-3), "unit": UNIT, "h_len": h_len,
+                 "targets": "runs of geometric length (mean 4) on uniform elements, phases +-1 (workloads.many_body_targets)",
+                 "max_abs_delta_vs_index_add_of_returned_values": float((d_H - ref).abs().max().item()),
+                 "api": "mfdn_mscheme_accumulate_3b" if body == 3 else "mfdn_mscheme_accumulate_2b"}
+        del d_loc, d_phase, d_H, awork, ref, loc, phase
     # ---- the same multiset pre-ordered by the library's group key (MFDN_PRESORTED): transform proper
     keys = ctx.group_keys(d_req)
     order = torch.argsort(keys.to(torch.int64) & 0xFFFFFFFF)
@@ -328,6 +352,8 @@ def main():
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                                "note": "definition-order checker (oracle/mscheme_oracle.c), never tuned: a reported baseline, not a CPU implementation",
                                "sample": f"first 2^{args.ref_log2n} requests of the same stream, {dt:.1f} s"}
+    if accum is not None:
+        out["accumulate_epilogue"] = accum
     if configs is not None:
         b_pre, b_uns, fl = alg["bytes_presorted"], alg["bytes_unsorted"], alg["flops"]
         mine = {"workload": cfg.name, "requests": n, "calls": 1, "mask1_fraction": frac_mask, "oracle_check": headline_check}

@@ -118,6 +118,25 @@ int mfdn_mscheme_2b(mfdn_ctx*, int64_t n, const int32_t* d_req, double* d_out, u
 int mfdn_mscheme_3b(mfdn_ctx*, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_mask, void* d_work,
                     size_t* work_bytes, uint32_t flags, void* stream);
 
+/* The step that follows the transformation in MFDn, fused into the call.  PAPER.md:93: every
+ * buffered request carries "which many-body element the request pertains to" and "a specific phase"; the host
+ * "iterates through the returned three-body elements in the chunk, multiplies them by the stored phases, and adds them to
+ * the array of many-body elements at the stored locations".  Here the results are not returned:
+ *     d_H[d_loc[i]] += d_phase[i] * v_i      for every request i with 0 <= d_loc[i] < h_len,
+ * v_i being what mfdn_mscheme_2b/3b would have written to d_out[i].
+ * d_loc  : DEVICE int64 [n], index into d_H; an entry outside [0, h_len) is skipped (its mask is still written).
+ * d_phase: DEVICE double [n] or NULL (= +1 everywhere).   d_H: DEVICE double [h_len], caller-owned and caller-initialised;
+ *          it is updated with fp64 atomic adds, so concurrent calls may target the same array; the order of the additions
+ *          to one element is not fixed (results agree to rounding from run to run, not bit for bit).
+ * Everything else (d_req, d_mask, scratch query with d_work == NULL, flags, stream, error behaviour) as for mfdn_mscheme_2b/3b;
+ * the scratch size differs from theirs. */
+int mfdn_mscheme_accumulate_2b(mfdn_ctx*, int64_t n, const int32_t* d_req, const int64_t* d_loc, const double* d_phase,
+                               double* d_H, int64_t h_len, uint8_t* d_mask, void* d_work, size_t* work_bytes, uint32_t flags,
+                               void* stream);
+int mfdn_mscheme_accumulate_3b(mfdn_ctx*, int64_t n, const int32_t* d_req, const int64_t* d_loc, const double* d_phase,
+                               double* d_H, int64_t h_len, uint8_t* d_mask, void* d_work, size_t* work_bytes, uint32_t flags,
+                               void* stream);
+
 /* The paper's wrapper ("transfer a chunk of 3-body element requests to the GPU, invoke the kernel,
  * and transfer the results back"), for HOST request/result buffers (pinned memory recommended).  The n requests
  * are cut into chunks of `chunk` (0 = library default) and H2D copy / transform / D2H copy of successive chunks

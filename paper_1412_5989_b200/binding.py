@@ -22,7 +22,7 @@ MFDN_PRESORTED, MFDN_FORCE_NAIVE, MFDN_FORCE_DENSE, MFDN_ONE_PASS_SORT = 1, 2, 4
 SYMBOLS = ["mfdn_orbitals_init", "mfdn_cg_build", "mfdn_cg_download", "mfdn_coupled_upload_2b",
            "mfdn_coupled_upload_3b", "mfdn_mscheme_2b", "mfdn_mscheme_3b", "mfdn_bad_request_count",
            "mfdn_info", "mfdn_group_keys", "mfdn_last_error", "mfdn_destroy", "mfdn_mscheme_host", "mfdn_profile",
-           "mfdn_profile_read", "mfdn_fp64_peak"]
+           "mfdn_profile_read", "mfdn_fp64_peak", "mfdn_mscheme_accumulate_2b", "mfdn_mscheme_accumulate_3b"]
 
 _lib = None
 
@@ -49,6 +49,8 @@ def lib():
         L.mfdn_coupled_upload_3b.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, C.c_int, vp]
         for f in (L.mfdn_mscheme_2b, L.mfdn_mscheme_3b):
             f.argtypes = [vp, i64, vp, vp, vp, vp, C.POINTER(C.c_size_t), u32, vp]
+        for f in (L.mfdn_mscheme_accumulate_2b, L.mfdn_mscheme_accumulate_3b):
+            f.argtypes = [vp, i64, vp, vp, vp, vp, i64, vp, vp, C.POINTER(C.c_size_t), u32, vp]
         L.mfdn_mscheme_host.argtypes = [vp, C.c_int, i64, vp, vp, vp, vp, C.POINTER(C.c_size_t), u32, i64]
         L.mfdn_profile.argtypes = [vp, C.c_int]
         L.mfdn_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(i64)]
@@ -154,6 +156,15 @@ def mfdn_mscheme_3b(ctx, n, d_req, d_out, d_mask, d_work, work_bytes, flags=0, s
     return _mscheme(lib().mfdn_mscheme_3b, ctx, n, d_req, d_out, d_mask, d_work, work_bytes, flags, stream)
 
 
+def mfdn_mscheme_accumulate(ctx, body, n, d_req, d_loc, d_phase, d_H, h_len, d_mask, d_work, work_bytes, flags=0, stream=None):
+    """Raw call of mfdn_mscheme_accumulate_2b/3b: device pointers as ints (0 = NULL).  Returns work_bytes."""
+    fn = lib().mfdn_mscheme_accumulate_3b if body == 3 else lib().mfdn_mscheme_accumulate_2b
+    wb = C.c_size_t(int(work_bytes))
+    _check(ctx, fn(ctx, int(n), C.c_void_p(d_req), C.c_void_p(d_loc), C.c_void_p(d_phase), C.c_void_p(d_H), int(h_len),
+                   C.c_void_p(d_mask), C.c_void_p(d_work), C.byref(wb), int(flags), _stream(stream) if d_work else C.c_void_p(0)))
+    return wb.value
+
+
 def mfdn_mscheme_host(ctx, body, n, h_req, h_out, h_mask, d_work, work_bytes, flags=0, chunk=0):
     """Host-buffer wrapper: h_* are host addresses (ints, 0 = NULL).  Returns work_bytes."""
     wb = C.c_size_t(int(work_bytes))
@@ -243,6 +254,28 @@ class Context:
         fn(self.ctx, n, d_req.data_ptr(), d_out.data_ptr(), d_mask.data_ptr(), work.data_ptr(), work.numel(), flags,
            stream)
         return d_out, d_mask
+
+    def accumulate(self, d_req, d_loc, d_phase, d_H, d_mask=None, flags=0, work=None, stream=None):
+        """d_H[d_loc[i]] += d_phase[i] * v_i (PAPER.md:93, 97).  d_loc: CUDA int64 [n]; d_phase: CUDA float64 [n] or None;
+        d_H: CUDA float64, updated in place.  Returns d_mask."""
+        torch = self.torch
+        assert d_req.is_cuda and d_req.dtype == torch.int32 and d_req.is_contiguous()
+        assert d_loc.is_cuda and d_loc.dtype == torch.int64 and d_loc.is_contiguous() and d_loc.numel() == d_req.shape[0]
+        assert d_phase is None or (d_phase.is_cuda and d_phase.dtype == torch.float64 and d_phase.is_contiguous())
+        assert d_H.is_cuda and d_H.dtype == torch.float64 and d_H.is_contiguous()
+        n, width = d_req.shape
+        body = width // 2
+        if d_mask is None:
+            d_mask = torch.empty(n, dtype=torch.uint8, device=d_req.device)
+        need = mfdn_mscheme_accumulate(self.ctx, body, n, 0, 0, 0, 0, 0, 0, 0, 0, flags)
+        if work is None:
+            if self._work is None or self._work.numel() < need:
+                self._work = torch.empty(max(need, 256), dtype=torch.uint8, device=d_req.device)
+            work = self._work
+        assert work.numel() >= need
+        mfdn_mscheme_accumulate(self.ctx, body, n, d_req.data_ptr(), d_loc.data_ptr(), d_phase.data_ptr() if d_phase is not None else 0,
+                                d_H.data_ptr(), d_H.numel(), d_mask.data_ptr(), work.data_ptr(), work.numel(), flags, stream)
+        return d_mask
 
     def mscheme_host(self, h_req, h_out=None, h_mask=None, flags=0, chunk=0):
         """h_req: CPU int32 tensor [n][4|6] (pinned recommended).  Returns (h_out, h_mask) CPU tensors."""

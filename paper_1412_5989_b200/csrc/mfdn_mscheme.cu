@@ -759,11 +759,56 @@ __global__ void __launch_bounds__(P_THREADS) k_part(long long n, const unsigned 
     }
 }
 
+// NEXT-1 epilogue: instead of being returned, result i is multiplied by its stored phase and added to
+// the many-body element it pertains to, H[loc[i]] += phase[i] * v[i].  MFDn asks for the 3-body elements of one many-body
+// element one after the other, so neighbouring requests often share loc: the lanes of a warp first sum runs of equal
+// loc among themselves (segmented scan with shuffles), then the last lane of every run issues ONE fp64 atomic.  Entries
+// with loc outside [0, h_len) and exact zeros (mask = 0) are skipped.  All 32 lanes must call this.
+struct Accum {
+    const long long* loc;
+    const double* phase;   // NULL: +1
+    double* H;
+    long long h_len;
+};
+__device__ __forceinline__ void accumulate_warp(const Accum& A, long long i, bool valid, double v)
+{
+    const int lane = threadIdx.x & 31;
+    long long l = -1 - lane;   // distinct negative values: lanes without a target never form a run
+    double x = 0.0;
+    if (valid) {
+        const long long t = __ldcs(A.loc + i);
+        if (t >= 0 && t < A.h_len) {
+            l = t;
+            x = A.phase ? __ldcs(A.phase + i) * v : v;
+        }
+    }
+    const long long up = __shfl_up_sync(0xFFFFFFFFu, l, 1);
+    const unsigned heads = __ballot_sync(0xFFFFFFFFu, lane == 0 || up != l);
+    const int start = 31 - __clz((int)(heads & (0xFFFFFFFFu >> (31 - lane))));   // first lane of this lane's run
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+        const double y = __shfl_up_sync(0xFFFFFFFFu, x, off);
+        if (lane - off >= start) x += y;
+    }
+    const bool tail = lane == 31 || ((heads >> (lane + 1)) & 1u);
+    if (tail && l >= 0 && x != 0.0) atomicAdd(A.H + l, x);
+}
+
+// the same for values already in request order (every path but the default one)
+__global__ void __launch_bounds__(256) k_accumulate(long long n, const double* __restrict__ vals, Accum A)
+{
+    const long long i = (long long)blockIdx.x * 256 + threadIdx.x;
+    const bool valid = i < n;
+    accumulate_warp(A, i, valid, valid ? __ldcs(vals + i) : 0.0);
+}
+
 // The way back, one tile of pass PASS per block: vals[map[tile start + slot]] -> shared memory -> out[tile start + l] =
 // staged[slot_of[tile start + l]].
-template <int PASS>
+// ACC (pass 1 only): the request-order values are not stored but accumulated (NEXT-1), out is unused.
+template <int PASS, bool ACC = false>
 __global__ void __launch_bounds__(P_THREADS) k_back(long long n, const double* __restrict__ vals, const uint4* __restrict__ tiles2,
-                                                   const uint32_t* __restrict__ map, const uint16_t* __restrict__ slot_of, double* __restrict__ out)
+                                                   const uint32_t* __restrict__ map, const uint16_t* __restrict__ slot_of, double* __restrict__ out,
+                                                   Accum A)
 {
     extern __shared__ __align__(16) unsigned char part_smem[];
     double* stage = reinterpret_cast<double*>(part_smem);
@@ -786,9 +831,17 @@ __global__ void __launch_bounds__(P_THREADS) k_back(long long n, const double* _
     for (int u = 0; u < PER; u++)
         if (tid + u * P_THREADS < m) stage[tid + u * P_THREADS] = __ldcs(vals + from[u]);
     __syncthreads();
-    for (int l = tid; l < m; l += P_THREADS) {
-        const double v = stage[__ldcs(slot_of + i0 + l)];
-        if (PASS == 1) __stcs(out + i0 + l, v); else out[i0 + l] = v;
+    if constexpr (ACC) {
+        for (int l0 = 0; l0 < m; l0 += P_THREADS) {   // warp-uniform trip count: every lane takes part in the shuffles
+            const int l = l0 + tid;
+            const bool valid = l < m;
+            accumulate_warp(A, i0 + l, valid, valid ? stage[__ldcs(slot_of + i0 + l)] : 0.0);
+        }
+    } else {
+        for (int l = tid; l < m; l += P_THREADS) {
+            const double v = stage[__ldcs(slot_of + i0 + l)];
+            if (PASS == 1) __stcs(out + i0 + l, v); else out[i0 + l] = v;
+        }
     }
 }
 
@@ -1653,7 +1706,7 @@ size_t align256(size_t x) { return (x + 255) & ~size_t(255); }
 
 template <int BODY>
 int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_mask, void* d_work, size_t* work_bytes,
-        uint32_t flags, void* stream)
+        uint32_t flags, void* stream, const Accum* acc = nullptr)
 {
     if (!c || !work_bytes || n < 0 || n >= (int64_t)0xFFFFFFF0ll) return c ? fail(c, MFDN_ERR_ARG, "bad n / work_bytes") : MFDN_ERR_ARG;
     if (BODY == 3 ? !c->has3 : !c->has2) return fail(c, MFDN_ERR_STATE, "mscheme before coupled upload");
@@ -1714,10 +1767,21 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
             need = o_ditems + align256((size_t)max_ditems * 16);
         }
     }
+    // NEXT-1: on every path but the default one the values go to scratch in request order and are accumulated from there
+    const bool acc_fused = acc && two_pass;
+    size_t o_accvals = 0;
+    if (acc && !acc_fused) {
+        o_accvals = align256(need);
+        need = o_accvals + align256((size_t)n * 8);
+    }
     if (!d_work) { *work_bytes = need; return MFDN_OK; }
     if (*work_bytes < need) return fail(c, MFDN_ERR_OOM, "scratch too small");
     if (n == 0) return MFDN_OK;
-    if (!d_req || !d_out) return fail(c, MFDN_ERR_ARG, "null request/output pointer");
+    if (acc) {
+        if (!acc->loc || !acc->H || acc->h_len < 0) return fail(c, MFDN_ERR_ARG, "null location / target pointer");
+        d_out = acc_fused ? nullptr : (double*)((char*)d_work + o_accvals);
+    }
+    if (!d_req || (!d_out && !acc)) return fail(c, MFDN_ERR_ARG, "null request/output pointer");
     cudaStream_t st = (cudaStream_t)stream;
     mfdn_ctx::EvTriple ev{nullptr, nullptr, nullptr, nullptr, sort};
     MFDN_CUDA(c, cudaSetDevice(c->device));   // the tables live on the context's device, whatever the caller's current one
@@ -1803,6 +1867,7 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
                 MFDN_CUDA(c, cudaFuncSetAttribute(k_part<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, PART_SMEM));
                 MFDN_CUDA(c, cudaFuncSetAttribute(k_back<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, KEYS_PER_BLOCK * 8));
                 MFDN_CUDA(c, cudaFuncSetAttribute(k_back<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, KEYS_PER_BLOCK * 8));
+                MFDN_CUDA(c, (cudaFuncSetAttribute(k_back<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, KEYS_PER_BLOCK * 8)));
                 c->part_attr_set.store(true);
             }
             const dim3 gts((unsigned)((nc + 127) / 128), (unsigned)n_chunks);
@@ -1854,13 +1919,18 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
         if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.d, st));
         if (two_pass) {
             double* tmp = (double*)recs;   // the bucket-ordered records are dead after the transform
-            k_back<2><<<(unsigned)max_tiles2, P_THREADS, KEYS_PER_BLOCK * 8, st>>>(n, tout, tiles2, map2, slot2, tmp);
-            k_back<1><<<gkb, P_THREADS, KEYS_PER_BLOCK * 8, st>>>(n, tmp, nullptr, map1, slot1, d_out);
+            k_back<2><<<(unsigned)max_tiles2, P_THREADS, KEYS_PER_BLOCK * 8, st>>>(n, tout, tiles2, map2, slot2, tmp, Accum{});
+            if (acc) k_back<1, true><<<gkb, P_THREADS, KEYS_PER_BLOCK * 8, st>>>(n, tmp, nullptr, map1, slot1, nullptr, *acc);
+            else k_back<1><<<gkb, P_THREADS, KEYS_PER_BLOCK * 8, st>>>(n, tmp, nullptr, map1, slot1, d_out, Accum{});
             c->launches += 2;
         } else if (sort) {
             k_unpermute<<<(unsigned)((n + 256 * SC_PER_THREAD - 1) / (256 * SC_PER_THREAD)), 256, 0, st>>>(n, tout, map1, d_out);
             c->launches += 1;
         }
+    }
+    if (acc && !acc_fused) {
+        k_accumulate<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, d_out, *acc);
+        c->launches += 1;
     }
     MFDN_CUDA(c, cudaGetLastError());
     if (c->profile) {
@@ -1895,6 +1965,22 @@ extern "C" int mfdn_mscheme_3b(mfdn_ctx* c, int64_t n, const int32_t* d_req, dou
                                size_t* work_bytes, uint32_t flags, void* stream)
 {
     return run<3>(c, n, d_req, d_out, d_mask, d_work, work_bytes, flags, stream);
+}
+
+extern "C" int mfdn_mscheme_accumulate_2b(mfdn_ctx* c, int64_t n, const int32_t* d_req, const int64_t* d_loc, const double* d_phase,
+                                          double* d_H, int64_t h_len, uint8_t* d_mask, void* d_work, size_t* work_bytes, uint32_t flags,
+                                          void* stream)
+{
+    const Accum a{(const long long*)d_loc, d_phase, d_H, (long long)h_len};
+    return run<2>(c, n, d_req, nullptr, d_mask, d_work, work_bytes, flags, stream, &a);
+}
+
+extern "C" int mfdn_mscheme_accumulate_3b(mfdn_ctx* c, int64_t n, const int32_t* d_req, const int64_t* d_loc, const double* d_phase,
+                                          double* d_H, int64_t h_len, uint8_t* d_mask, void* d_work, size_t* work_bytes, uint32_t flags,
+                                          void* stream)
+{
+    const Accum a{(const long long*)d_loc, d_phase, d_H, (long long)h_len};
+    return run<3>(c, n, d_req, nullptr, d_mask, d_work, work_bytes, flags, stream, &a);
 }
 
 extern "C" int mfdn_group_keys(mfdn_ctx* c, int body, int64_t n, const int32_t* d_req, uint32_t* d_key, void* stream)

@@ -477,3 +477,44 @@ def test_multi_client_threads(torch, B):
     assert not errors, errors
     assert calls == len(chunks)
     assert np.array_equal(out.cpu().numpy(), base) and np.array_equal(mask.cpu().numpy(), bmask)
+
+
+# --------------------------------------------------------------------------------- NEXT-1: fused accumulate epilogue
+@pytest.mark.gpu
+@pytest.mark.parametrize("idx", [0, 2])
+def test_accumulate_epilogue(torch, B, oracle, idx):
+    """H[loc[i]] += phase[i] * v[i] against oracle/accumulate_ref.py applied to the ORACLE's values, on every
+    path: default (fused into the last gather pass), one-pass sort, pre-sorted, naive.  Tolerance: each value is within
+    1e-12 max|V| of the oracle's and an element sums at most m of them in an order that is not fixed, so
+    |dH| <= 1e-12 * max|V| * m (m = largest number of requests on one element)."""
+    from oracle.accumulate_ref import accumulate
+    cfg = get_cfg(idx)
+    ctx = get_ctx(B, idx)
+    rng = np.random.default_rng(21)
+    allreq = cfg.requests()
+    for n, h_len in ((0, 5), (1, 1), (33, 7), (8193, 1500), (min(len(allreq), 60000), 9000)):
+        req = allreq[rng.choice(len(allreq), n, replace=False)] if n else allreq[:0]
+        loc, phase = W.many_body_targets(n, h_len, seed=n)
+        if n > 100:
+            loc[::13] = -1                      # skipped entries
+            loc[5::17] = h_len
+        want, wmask, _, _ = oracle.mscheme(cfg.basis, cfg.table, req)
+        m = max(1, int(np.bincount(loc[(loc >= 0) & (loc < h_len)], minlength=1).max())) if n else 1
+        tol = TOL * float(np.max(np.abs(cfg.table.values))) * m
+        d_req = torch.from_numpy(np.ascontiguousarray(req, np.int32)).cuda()
+        d_loc, d_phase = torch.from_numpy(loc).cuda(), torch.from_numpy(phase).cuda()
+        for flags, ph in ((0, True), (0, False), (B.MFDN_ONE_PASS_SORT, True), (B.MFDN_FORCE_NAIVE, True)):
+            H0 = rng.standard_normal(h_len)     # the target is updated, not overwritten
+            d_H = torch.from_numpy(H0.copy()).cuda()
+            mask = ctx.accumulate(d_req, d_loc, d_phase if ph else None, d_H, flags=flags)
+            torch.cuda.synchronize()
+            ref = H0 + accumulate(want, loc, phase if ph else None, h_len)
+            assert np.array_equal(mask.cpu().numpy(), wmask)
+            assert float(np.max(np.abs(d_H.cpu().numpy() - ref))) <= tol + 1e-15 * np.max(np.abs(H0))
+        if n > 100:                             # pre-sorted input: the targets travel with their requests
+            sreq, order = presort(torch, ctx, req)
+            d_H = torch.zeros(h_len, dtype=torch.float64, device="cuda")
+            ctx.accumulate(torch.from_numpy(sreq).cuda(), torch.from_numpy(loc[order].copy()).cuda(),
+                           torch.from_numpy(phase[order].copy()).cuda(), d_H, flags=B.MFDN_PRESORTED)
+            torch.cuda.synchronize()
+            assert float(np.max(np.abs(d_H.cpu().numpy() - accumulate(want, loc, phase, h_len)))) <= tol
