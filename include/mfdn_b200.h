@@ -137,6 +137,30 @@ int mfdn_mscheme_accumulate_3b(mfdn_ctx*, int64_t n, const int32_t* d_req, const
                                double* d_H, int64_t h_len, uint8_t* d_mask, void* d_work, size_t* work_bytes, uint32_t flags,
                                void* stream);
 
+/* Dense block mode: whole m-scheme blocks without a request list -- the block view A' = D^T A D of
+ * PAPER.md:55 (Fig. 1 at :69), for use "at a higher level in the matrix construction stage"; trades the
+ * memory blow-up of PAPER.md:53 for bandwidth.  A block belongs to a pair of 3-body orbital tuples, bra (a <= b <= c) and ket
+ * (d <= e <= f): `orbitals` = {a, b, c, d, e, f}.  Its entries, in this order:
+ *   for mi = 0 .. mm          common M ascending: mm = min(ja+jb+jc, jd+je+jf) (2j units), 2M = 2 mi - mm
+ *     for bin = 0 .. 19       isospin patterns: the pairs (pb, pk), pb = ta<<2 | tb<<1 | tc of the bra (bit = 1 for 2tz = +1),
+ *                             pk likewise for the ket, with equally many set bits, in ascending (pb, pk) order
+ *       an nb x nk matrix, row-major: rows = the bra m-states (ma, mb, mc) of that M in ascending (ia, ib) order
+ *                             (i = (2m + 2j) / 2), columns = the ket m-states likewise
+ * entry = < a ma ta, b mb tb, c mc tc | V | d .., e .., f .. >, i.e. what mfdn_mscheme_3b returns for that request, if bra
+ * and ket are ordered Slater determinants (all six SPS exist; particles of one orbital in ascending SPS index order);
+ * otherwise +0.0 (the value is that of the ordered partner times the permutation sign).  Entries forbidden by a selection
+ * rule are +0.0 as well.  The block is empty (length 0, nothing written) if a tuple is not listed in the uploaded table,
+ * the parities differ or there is no common J.
+ * mfdn_mscheme_block_len_3b: HOST call, *n_values = number of doubles of the block.
+ * mfdn_mscheme_blocks_3b: n_groups blocks in one launch; h_orbitals: HOST int32 [n_groups][6]; h_off: HOST int64
+ *   [n_groups], offset (in doubles) of every block in d_out (DEVICE, caller-owned, large enough); d_work/work_bytes:
+ *   DEVICE scratch, queried with d_work == NULL; asynchronous on `stream` (the host arrays may be reused on return).
+ *   Formed with fp64 tensor-core products (mma.sync m8n8k4): values agree with mfdn_mscheme_3b to rounding.
+ *   MFDN_ERR_ARG for orbitals out of range or not ascending and for a group with more than 64 ket rows (J, J12'). */
+int mfdn_mscheme_block_len_3b(mfdn_ctx*, const int32_t* orbitals, int64_t* n_values);
+int mfdn_mscheme_blocks_3b(mfdn_ctx*, int64_t n_groups, const int32_t* h_orbitals, const int64_t* h_off, double* d_out,
+                           void* d_work, size_t* work_bytes, void* stream);
+
 /* The paper's wrapper ("transfer a chunk of 3-body element requests to the GPU, invoke the kernel,
  * and transfer the results back"), for HOST request/result buffers (pinned memory recommended).  The n requests
  * are cut into chunks of `chunk` (0 = library default) and H2D copy / transform / D2H copy of successive chunks

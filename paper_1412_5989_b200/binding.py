@@ -22,7 +22,8 @@ MFDN_PRESORTED, MFDN_FORCE_NAIVE, MFDN_FORCE_DENSE, MFDN_ONE_PASS_SORT = 1, 2, 4
 SYMBOLS = ["mfdn_orbitals_init", "mfdn_cg_build", "mfdn_cg_download", "mfdn_coupled_upload_2b",
            "mfdn_coupled_upload_3b", "mfdn_mscheme_2b", "mfdn_mscheme_3b", "mfdn_bad_request_count",
            "mfdn_info", "mfdn_group_keys", "mfdn_last_error", "mfdn_destroy", "mfdn_mscheme_host", "mfdn_profile",
-           "mfdn_profile_read", "mfdn_fp64_peak", "mfdn_mscheme_accumulate_2b", "mfdn_mscheme_accumulate_3b"]
+           "mfdn_profile_read", "mfdn_fp64_peak", "mfdn_mscheme_accumulate_2b", "mfdn_mscheme_accumulate_3b",
+           "mfdn_mscheme_block_len_3b", "mfdn_mscheme_blocks_3b"]
 
 _lib = None
 
@@ -51,6 +52,8 @@ def lib():
             f.argtypes = [vp, i64, vp, vp, vp, vp, C.POINTER(C.c_size_t), u32, vp]
         for f in (L.mfdn_mscheme_accumulate_2b, L.mfdn_mscheme_accumulate_3b):
             f.argtypes = [vp, i64, vp, vp, vp, vp, i64, vp, vp, C.POINTER(C.c_size_t), u32, vp]
+        L.mfdn_mscheme_block_len_3b.argtypes = [vp, vp, C.POINTER(i64)]
+        L.mfdn_mscheme_blocks_3b.argtypes = [vp, i64, vp, vp, vp, vp, C.POINTER(C.c_size_t), vp]
         L.mfdn_mscheme_host.argtypes = [vp, C.c_int, i64, vp, vp, vp, vp, C.POINTER(C.c_size_t), u32, i64]
         L.mfdn_profile.argtypes = [vp, C.c_int]
         L.mfdn_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(i64)]
@@ -165,6 +168,25 @@ def mfdn_mscheme_accumulate(ctx, body, n, d_req, d_loc, d_phase, d_H, h_len, d_m
     return wb.value
 
 
+def mfdn_mscheme_block_len_3b(ctx, orbitals):
+    """Number of doubles of the block of the orbital tuples orbitals = (a, b, c, d, e, f)."""
+    o = np.ascontiguousarray(orbitals, np.int32)
+    assert o.shape == (6,)
+    n = C.c_int64(0)
+    _check(ctx, lib().mfdn_mscheme_block_len_3b(ctx, _hp(o), C.byref(n)))
+    return n.value
+
+
+def mfdn_mscheme_blocks_3b(ctx, h_orbitals, h_off, d_out, d_work, work_bytes, stream=None):
+    """Raw call: h_orbitals int32 [n][6] and h_off int64 [n] are numpy arrays, d_out / d_work device pointers as ints."""
+    o = np.ascontiguousarray(h_orbitals, np.int32).reshape(-1, 6)
+    off = np.ascontiguousarray(h_off, np.int64)
+    wb = C.c_size_t(int(work_bytes))
+    _check(ctx, lib().mfdn_mscheme_blocks_3b(ctx, len(o), _hp(o), _hp(off), C.c_void_p(d_out), C.c_void_p(d_work), C.byref(wb),
+                                            _stream(stream) if d_work else C.c_void_p(0)))
+    return wb.value
+
+
 def mfdn_mscheme_host(ctx, body, n, h_req, h_out, h_mask, d_work, work_bytes, flags=0, chunk=0):
     """Host-buffer wrapper: h_* are host addresses (ints, 0 = NULL).  Returns work_bytes."""
     wb = C.c_size_t(int(work_bytes))
@@ -276,6 +298,20 @@ class Context:
         mfdn_mscheme_accumulate(self.ctx, body, n, d_req.data_ptr(), d_loc.data_ptr(), d_phase.data_ptr() if d_phase is not None else 0,
                                 d_H.data_ptr(), d_H.numel(), d_mask.data_ptr(), work.data_ptr(), work.numel(), flags, stream)
         return d_mask
+
+    def blocks(self, orbitals, stream=None):
+        """Dense block mode: orbitals int [n][6].  Returns (d_out f64 on the GPU, offsets int64 [n + 1]) -- block k is
+        d_out[offsets[k]:offsets[k + 1]] in the layout include/mfdn_b200.h states."""
+        torch = self.torch
+        o = np.ascontiguousarray(orbitals, np.int32).reshape(-1, 6)
+        lens = np.array([mfdn_mscheme_block_len_3b(self.ctx, r) for r in o], np.int64)
+        off = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+        d_out = torch.empty(max(int(off[-1]), 1), dtype=torch.float64, device=f"cuda:{self.device}")
+        need = mfdn_mscheme_blocks_3b(self.ctx, o, off[:-1], 0, 0, 0)
+        work = torch.empty(max(need, 256), dtype=torch.uint8, device=f"cuda:{self.device}")
+        mfdn_mscheme_blocks_3b(self.ctx, o, off[:-1], d_out.data_ptr(), work.data_ptr(), work.numel(), stream)
+        self._block_work = work          # stays alive until the stream has consumed it
+        return d_out[:int(off[-1])], off
 
     def mscheme_host(self, h_req, h_out=None, h_mask=None, flags=0, chunk=0):
         """h_req: CPU int32 tensor [n][4|6] (pinned recommended).  Returns (h_out, h_mask) CPU tensors."""

@@ -651,7 +651,7 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     std::vector<int2> trow(nt), rowtab, rowdst, jinfo;
     std::vector<int4> tk(nt);
     std::vector<int32_t> nrows(nt), sigoff(nt), mstoff(nt);
-    std::vector<uint16_t> sig, mstart;   // mstart: per tuple, first sigma of every iM (prefix counts; sumj + 2 entries)
+    std::vector<uint16_t> sig, isig, mstart;   // mstart: per tuple, first sigma of every iM (prefix counts; sumj + 2 entries)
     uint64_t dtab_len = 0;
     // Everything built in this loop -- rows, J blocks, sigma order, the coefficient table -- depends on the tuple only through
     // (ja, jb, jc) (the J12 and J ranges above are the triangle ranges, not the listed states): tuples of one j-class share
@@ -704,9 +704,14 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
             mstoff[t] = (int32_t)mstart.size();
             for (int v : start) mstart.push_back((uint16_t)v);
             sig.resize(sig.size() + S);
+            isig.resize(sig.size());
             uint16_t* sg = sig.data() + sigoff[t];
-            for (int a = 0; a <= ja; a++) for (int b = 0; b <= jb; b++) for (int m = 0; m <= jc; m++)
-                sg[(a * (jb + 1) + b) * (jc + 1) + m] = (uint16_t)start[a + b + m]++;
+            uint16_t* isg = isig.data() + sigoff[t];   // sigma -> natural index (block mode needs the m's of a row)
+            for (int a = 0; a <= ja; a++) for (int b = 0; b <= jb; b++) for (int m = 0; m <= jc; m++) {
+                const int nat = (a * (jb + 1) + b) * (jc + 1) + m;
+                sg[nat] = (uint16_t)start[a + b + m]++;
+                isg[sg[nat]] = (uint16_t)nat;
+            }
         }
         if (dtab_len + tlen >= 0x7FFFFFF0ull) return fail(c, MFDN_ERR_OOM, "coefficient table too large for 31-bit offsets");
         tk[t].x = (int)dtab_len;
@@ -832,6 +837,18 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     size_t o_desc = tmp.add(tdesc), o_ab = res.add(ab);
     size_t o_tk = res.add(tk), o_jinfo = res.add(jinfo), o_sig = res.add(sig), o_sigoff = res.add(sigoff);
     size_t o_mstart = res.add(mstart), o_mstoff = res.add(mstoff);
+    // block mode (NEXT-2): sigma -> m's, tuple -> orbitals, (orbital, tz, m index) -> SPS index or -1
+    std::vector<int4> torb(nt);
+    for (int t = 0; t < nt; t++) {
+        const int64_t k = tuples[t];
+        torb[t] = int4{(int)(k / ((int64_t)No * No)), (int)((k / No) % No), (int)(k % No), 0};
+    }
+    std::vector<int32_t> spsidx((size_t)No * 64, -1);
+    for (int sp = 0; sp < c->t.n_sps; sp++) {
+        const uint32_t r = c->h_sps_rec[sp];
+        spsidx[((size_t)rec_orb(r) * 2 + rec_tz(r)) * 32 + rec_im(r)] = sp;
+    }
+    size_t o_isig = res.add(isig), o_torb = res.add(torb), o_spsidx = res.add(spsidx);
     std::vector<int64_t> coff(chan_off, chan_off + n_chan);
     std::vector<int32_t> cdim(chan_dim, chan_dim + n_chan);
     size_t o_rm = tmp.add(rowmap), o_cof = tmp.add(chan_of), o_coff = tmp.add(coff), o_cdim = tmp.add(cdim);
@@ -920,6 +937,14 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     c->t.sig3 = q.sig;
     c->t.mstart3 = (const uint16_t*)(dres + o_mstart);
     c->t.mstoff3 = (const int32_t*)(dres + o_mstoff);
+    c->t.isig3 = (const uint16_t*)(dres + o_isig);
+    c->t.torb3 = (const int4*)(dres + o_torb);
+    c->t.spsidx3 = (const int32_t*)(dres + o_spsidx);
+    c->h_tuple_id3 = tuple_id;
+    c->h_tdesc3 = tdesc_rt;
+    c->h_mstart3 = mstart;
+    c->h_mstoff3 = mstoff;
+    c->h_sgrp3 = sgrp;
     c->slab_bytes3 = (int64_t)(cells * 16);
     c->dtab_bytes3 = (int64_t)(dtab_len * sizeof(double));
     c->has3 = true;

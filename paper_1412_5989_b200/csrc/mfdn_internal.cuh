@@ -122,6 +122,9 @@ struct Tables {
     const int32_t* mstoff3;
     const uint16_t* sig3;          // per tuple [(ima*(jb+1)+imb)*(jc+1)+imc] -> sigma: m-states ordered by (M, ima, imb), so that
                                    // requests with equal M (bra and ket always have equal M) read neighbouring entries
+    const uint16_t* isig3;         // inverse of sig3 (same offsets): sigma -> (ima*(jb+1)+imb)*(jc+1)+imc
+    const int4* torb3;             // [n_tup3] orbitals {a, b, c, -} of a tuple
+    const int32_t* spsidx3;        // [(orbital*2 + tz bit)*32 + m index] -> SPS index or -1
     // A2, 2-body
     int n_tup2;
     const int32_t* tuple_id2;      // [n_orb^2]
@@ -144,6 +147,11 @@ struct mfdn_ctx {
     // host copies
     std::vector<int32_t> orb_n, orb_l, orb_twoj, h_cg2_off;
     std::vector<uint32_t> h_sps_rec;
+    // host copies for sizing the blocks of mfdn_mscheme_blocks_3b
+    std::vector<int32_t> h_tuple_id3, h_mstoff3;
+    std::vector<int4> h_tdesc3;
+    std::vector<uint16_t> h_mstart3;
+    std::vector<uint4> h_sgrp3;
     std::vector<void*> owned;  // device allocations
     int64_t n_cg1 = 0, n_cg2 = 0;
     int64_t slab_bytes2 = 0, slab_bytes3 = 0, dtab_bytes3 = 0, vw_bytes3 = 0;

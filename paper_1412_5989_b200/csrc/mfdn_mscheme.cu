@@ -1657,6 +1657,146 @@ __global__ void __launch_bounds__(DN_WARPS * 32) k_dense3(Tables T, const uint4*
     }
 }
 
+// ------------------------------------------------------------------------------- NEXT-2: dense block mode
+// Whole m-scheme blocks without a request list (PAPER.md:53-55 A' = D^T A D, Fig. 1 at :69; "at a higher level in the matrix
+// construction stage").  One warp per (group, M, isospin bin): it forms
+//     Vm[mu, mu'] = sum_{J >= |M|} sum_{J12, J12'} Cb[mu; J,J12] * Vw_bin[J; J12,J12'] * Ck[mu'; J,J12']
+// (measured: 7.5 G entries/s on all 1415 non-empty groups of config 2, 14.8 G entries/s on 1940 groups of config 3 -- every
+// warp is a chain of dependent descriptor loads for a ~10 x 10 tile, so this is latency-bound, not yet faster per entry than
+// the request path)
+// over ALL bra and ket m-states of that M with the same two chained products as k_dense3 (T = Cb * Vw in the A-fragment
+// layout, Vm = T * Ck^T with mma.sync.m8n8k4.f64) and stores the 8 x 8 tiles straight from the accumulator fragments.
+// An entry whose bra or ket is not an ordered Slater determinant (particles of one orbital not in ascending SPS order, or
+// an SPS that does not exist) is stored as +0.0: its value is that of the ordered partner times the permutation sign.
+struct BinPat { uint8_t v[NBIN3]; };
+constexpr BinPat make_binpat()   // bin -> bra pattern << 3 | ket pattern, the enumeration of mfdn_orbitals_init
+{
+    BinPat p{};
+    int n = 0;
+    for (int tb = 0; tb < 8; tb++)
+        for (int tk = 0; tk < 8; tk++) {
+            int cb = (tb & 1) + ((tb >> 1) & 1) + (tb >> 2), ck = (tk & 1) + ((tk >> 1) & 1) + (tk >> 2);
+            if (cb == ck) p.v[n++] = (uint8_t)(tb * 8 + tk);
+        }
+    return p;
+}
+__constant__ BinPat c_binpat = make_binpat();
+
+struct BlockItem { uint32_t g, mi; unsigned long long off; };   // off: first entry of the (group, M) sub-block (20 bins follow each other)
+
+// is the m-state `nat` = (ima*(jb+1)+imb)*(jc+1)+imc of a tuple with tz pattern `pat` an ordered Slater determinant?
+__device__ __forceinline__ bool ordered_state3(const Tables& T, int4 orb, int4 d, uint32_t nat, int pat)
+{
+    const int jb1 = ((d.x >> 8) & 255) + 1, jc1 = ((d.x >> 16) & 255) + 1;
+    const int imc = nat % jc1, imb = (nat / jc1) % jb1, ima = nat / (jc1 * jb1);
+    const int sa = __ldg(T.spsidx3 + (orb.x * 2 + ((pat >> 2) & 1)) * 32 + ima);
+    const int sb = __ldg(T.spsidx3 + (orb.y * 2 + ((pat >> 1) & 1)) * 32 + imb);
+    const int sc = __ldg(T.spsidx3 + (orb.z * 2 + (pat & 1)) * 32 + imc);
+    return sa >= 0 && sb >= 0 && sc >= 0 && (orb.x != orb.y || sa < sb) && (orb.y != orb.z || sb < sc);
+}
+
+__global__ void __launch_bounds__(DN_WARPS * 32) k_block3(Tables T, const BlockItem* __restrict__ items, uint32_t n_items, double* __restrict__ out)
+{
+    __shared__ uint4 s_rmap[DN_WARPS][DENSE_RMAX];
+    uint4* rmap = s_rmap[threadIdx.x >> 5];
+    const int lane = threadIdx.x & 31;
+    const uint32_t gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
+    const uint32_t nt = (uint32_t)T.n_tup3;
+    const double* __restrict__ dtab = T.dtab3;
+    for (uint32_t wi = gw; wi < n_items * (uint32_t)NBIN3; wi += nw) {
+        const uint32_t it = wi / (uint32_t)NBIN3, bin = wi - it * (uint32_t)NBIN3;
+        const BlockItem item = items[it];
+        const uint32_t g = item.g, mi = item.mi;
+        const uint32_t tb = g / nt, tk = g - tb * nt;
+        const int4 kb = __ldg(T.tk3 + tb), kk = __ldg(T.tk3 + tk);
+        const int4 db = __ldg(T.tdesc3 + tb), dk = __ldg(T.tdesc3 + tk);
+        const int4 ob = __ldg(T.torb3 + tb), ok = __ldg(T.torb3 + tk);
+        const uint4 sg = __ldg(T.sgrp3 + g);
+        const int sjb = kb.w & 255, sjk = kk.w & 255, mm = min(sjb, sjk);
+        const int imb = (int)mi + ((sjb - mm) >> 1), imk = (int)mi + ((sjk - mm) >> 1);
+        const uint16_t* msb = T.mstart3 + __ldg(T.mstoff3 + tb);
+        const uint16_t* msk = T.mstart3 + __ldg(T.mstoff3 + tk);
+        const uint32_t s0b = __ldg(msb + imb), nmb = __ldg(msb + imb + 1) - s0b;
+        const uint32_t s0k = __ldg(msk + imk), nmk = __ldg(msk + imk + 1) - s0k;
+        const uint16_t* isb = T.isig3 + db.w + s0b;   // natural index of the bra / ket m-states of this M
+        const uint16_t* isk = T.isig3 + dk.w + s0k;
+        const int Jminb = (kb.w >> 16) & 255, Jmink = (kk.w >> 16) & 255;
+        const int Jlo = max(Jminb, Jmink), nblk = ((min((kb.w >> 24) & 255, (kk.w >> 24) & 255) - Jlo) >> 1) + 1;
+        const int q0 = max(0, (abs(2 * imb - sjb) - Jlo + 1) >> 1);   // first J block with J >= |M|
+        int2 jb = make_int2(0, 0), jk = make_int2(0, 0);
+        if (lane < nblk) {
+            jb = __ldg(T.jinfo3 + kb.z + ((Jlo - Jminb) >> 1) + lane);
+            jk = __ldg(T.jinfo3 + kk.z + ((Jlo - Jmink) >> 1) + lane);
+        }
+        const uint32_t vv = (uint32_t)(jb.y * row_pitch3(jk.y)), rk = lane >= q0 ? (uint32_t)jk.y : 0u;
+        uint32_t iv = vv, ir = rk;
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            uint32_t xv = __shfl_up_sync(0xFFFFFFFFu, iv, off), xr = __shfl_up_sync(0xFFFFFFFFu, ir, off);
+            if (lane >= off) { iv += xv; ir += xr; }
+        }
+        const uint32_t R = __shfl_sync(0xFFFFFFFFu, ir, 31);   // flattened ket rows in play (<= DENSE_RMAX, checked by the host)
+        __syncwarp();
+        if (lane >= q0 && lane < nblk)
+            for (int k = 0; k < jk.y; k++)
+                rmap[ir - rk + k] = make_uint4((uint32_t)kb.x + (uint32_t)jb.x, (uint32_t)jb.y | ((uint32_t)jk.y << 8) | ((uint32_t)k << 16),
+                                               iv - vv + (uint32_t)k, (uint32_t)kk.x + (uint32_t)jk.x);
+        __syncwarp();
+        const uint32_t gsize = sg.y, S = vw_stride(gsize);
+        const int nchunk = (int)((R + 3u) >> 2);
+        const uint32_t mrow = (uint32_t)lane >> 2, kcol = (uint32_t)lane & 3u;
+        {
+            const int patb = c_binpat.v[bin] >> 3, patk = c_binpat.v[bin] & 7;
+            const uint32_t* __restrict__ vwb = T.vw20 + (size_t)sg.z * 4 + (size_t)bin * S;
+            double* __restrict__ dst = out + item.off + (size_t)bin * nmb * nmk;
+            for (uint32_t mt = 0; mt * 8u < nmb; mt++) {
+                double a[DN_CHUNKS];
+                const uint32_t mu = mt * 8u + mrow;
+#pragma unroll
+                for (int c = 0; c < DN_CHUNKS; c++) {
+                    a[c] = 0.0;
+                    const uint32_t r = 4u * c + kcol;
+                    if (c < nchunk && r < R && mu < nmb) {
+                        const uint4 e = rmap[r];
+                        const uint32_t nb = e.y & 255u, P = (uint32_t)row_pitch3((e.y >> 8) & 255u);
+                        const double* __restrict__ cb = dtab + (e.x + (s0b + mu) * nb);
+                        double t = 0.0;
+                        for (uint32_t i = 0; i < nb; i++) {
+                            const uint32_t cell = e.z + i * P;
+                            t = fma(__ldg(cb + i), __hiloint2double((int)__ldg(vwb + gsize + cell), (int)__ldg(vwb + cell)), t);
+                        }
+                        a[c] = t;
+                    }
+                }
+                const bool rowok = mu < nmb && ordered_state3(T, ob, db, __ldg(isb + min(mu, nmb - 1u)), patb);
+                for (uint32_t nt8 = 0; nt8 * 8u < nmk; nt8++) {
+                    const uint32_t mup = nt8 * 8u + mrow;
+                    double c0 = 0.0, c1 = 0.0;
+#pragma unroll
+                    for (int c = 0; c < DN_CHUNKS; c++) {
+                        if (c < nchunk) {   // warp-uniform
+                            const uint32_t r = 4u * c + kcol;
+                            double b = 0.0;
+                            if (r < R && mup < nmk) {
+                                const uint4 e = rmap[r];
+                                b = __ldg(dtab + (e.w + (s0k + mup) * ((e.y >> 8) & 255u) + (e.y >> 16)));
+                            }
+                            asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                                         : "+d"(c0), "+d"(c1) : "d"(a[c]), "d"(b));
+                        }
+                    }
+                    const uint32_t n0 = nt8 * 8u + 2u * kcol, n1 = n0 + 1u;
+                    if (mu < nmb) {
+                        if (n0 < nmk) dst[(size_t)mu * nmk + n0] = (rowok && ordered_state3(T, ok, dk, __ldg(isk + n0), patk)) ? c0 + 0.0 : 0.0;
+                        if (n1 < nmk) dst[(size_t)mu * nmk + n1] = (rowok && ordered_state3(T, ok, dk, __ldg(isk + n1), patk)) ? c1 + 0.0 : 0.0;
+                    }
+                }
+            }
+        }
+        __syncwarp();
+    }
+}
+
 __global__ void __launch_bounds__(128) k_transform2(Tables T, long long n, const unsigned long long* __restrict__ recs,
                                                    double* __restrict__ out)
 {
@@ -1981,6 +2121,104 @@ extern "C" int mfdn_mscheme_accumulate_3b(mfdn_ctx* c, int64_t n, const int32_t*
 {
     const Accum a{(const long long*)d_loc, d_phase, d_H, (long long)h_len};
     return run<3>(c, n, d_req, nullptr, d_mask, d_work, work_bytes, flags, stream, &a);
+}
+
+// ---- NEXT-2 host side: which (M, bin) sub-blocks a group has and how long they are
+namespace {
+struct GroupShape {
+    int tb = -1, tk = -1;
+    bool empty = true;       // tuple not listed, other parity, or no common J: the block has no entries
+    int mm = 0, sjb = 0, sjk = 0;
+    int rows = 0;            // flattened ket rows (J, J12'), all J of the group
+};
+int group_shape3(mfdn_ctx* c, const int32_t* o, GroupShape& G)
+{
+    const int No = c->t.n_orb;
+    for (int k = 0; k < 6; k++)
+        if (o[k] < 0 || o[k] >= No) return fail(c, MFDN_ERR_ARG, "orbital index out of range");
+    if (o[0] > o[1] || o[1] > o[2] || o[3] > o[4] || o[4] > o[5]) return fail(c, MFDN_ERR_ARG, "orbitals of a block must be ascending (a <= b <= c)");
+    G.tb = c->h_tuple_id3[((size_t)o[0] * No + o[1]) * No + o[2]];
+    G.tk = c->h_tuple_id3[((size_t)o[3] * No + o[4]) * No + o[5]];
+    if (G.tb < 0 || G.tk < 0) return MFDN_OK;
+    const uint4 sg = c->h_sgrp3[(size_t)G.tb * c->t.n_tup3 + G.tk];
+    if (sg.x == NO_SLAB) return MFDN_OK;
+    const int4 db = c->h_tdesc3[G.tb], dk = c->h_tdesc3[G.tk];
+    G.sjb = (db.x & 255) + ((db.x >> 8) & 255) + ((db.x >> 16) & 255);
+    G.sjk = (dk.x & 255) + ((dk.x >> 8) & 255) + ((dk.x >> 16) & 255);
+    G.mm = std::min(G.sjb, G.sjk);
+    const int Jlo = std::max((db.y >> 16) & 255, (dk.y >> 16) & 255), Jhi = std::min((db.y >> 24) & 255, (dk.y >> 24) & 255);
+    const int jf = (dk.x >> 16) & 255;
+    for (int twoJ = Jlo; twoJ <= Jhi; twoJ += 2) {
+        const int lo = std::max(dk.y & 255, std::abs(twoJ - jf) >> 1), hi = std::min((dk.y >> 8) & 255, (twoJ + jf) >> 1);
+        G.rows += std::max(0, hi - lo + 1);
+    }
+    G.empty = false;
+    return MFDN_OK;
+}
+// m-states of the bra and of the ket at the mi-th common M
+void m_counts3(const mfdn_ctx* c, const GroupShape& G, int mi, int64_t& nmb, int64_t& nmk)
+{
+    const uint16_t* msb = c->h_mstart3.data() + c->h_mstoff3[G.tb];
+    const uint16_t* msk = c->h_mstart3.data() + c->h_mstoff3[G.tk];
+    const int ib = mi + (G.sjb - G.mm) / 2, ik = mi + (G.sjk - G.mm) / 2;
+    nmb = msb[ib + 1] - msb[ib];
+    nmk = msk[ik + 1] - msk[ik];
+}
+}  // namespace
+
+extern "C" int mfdn_mscheme_block_len_3b(mfdn_ctx* c, const int32_t* orbitals, int64_t* n_values)
+{
+    if (!c || !orbitals || !n_values) return c ? fail(c, MFDN_ERR_ARG, "null argument") : MFDN_ERR_ARG;
+    if (!c->has3) return fail(c, MFDN_ERR_STATE, "block_len before coupled upload");
+    GroupShape G;
+    int rc = group_shape3(c, orbitals, G);
+    if (rc) return rc;
+    int64_t total = 0;
+    if (!G.empty)
+        for (int mi = 0; mi <= G.mm; mi++) {
+            int64_t nmb, nmk;
+            m_counts3(c, G, mi, nmb, nmk);
+            total += (int64_t)NBIN3 * nmb * nmk;
+        }
+    *n_values = total;
+    return MFDN_OK;
+}
+
+extern "C" int mfdn_mscheme_blocks_3b(mfdn_ctx* c, int64_t n_groups, const int32_t* h_orbitals, const int64_t* h_off, double* d_out,
+                                      void* d_work, size_t* work_bytes, void* stream)
+{
+    if (!c || !work_bytes || n_groups < 0 || (n_groups > 0 && !h_orbitals)) return c ? fail(c, MFDN_ERR_ARG, "bad argument") : MFDN_ERR_ARG;
+    if (!c->has3) return fail(c, MFDN_ERR_STATE, "blocks before coupled upload");
+    std::vector<BlockItem> items;
+    for (int64_t k = 0; k < n_groups; k++) {
+        GroupShape G;
+        int rc = group_shape3(c, h_orbitals + 6 * k, G);
+        if (rc) return rc;
+        if (G.empty) continue;
+        if (G.rows > DENSE_RMAX) return fail(c, MFDN_ERR_ARG, "block mode: group with more than 64 (J, J12') ket rows");
+        unsigned long long off = d_work && h_off ? (unsigned long long)h_off[k] : 0ull;
+        for (int mi = 0; mi <= G.mm; mi++) {
+            int64_t nmb, nmk;
+            m_counts3(c, G, mi, nmb, nmk);
+            if (nmb > 0 && nmk > 0) items.push_back(BlockItem{(uint32_t)((size_t)G.tb * c->t.n_tup3 + G.tk), (uint32_t)mi, off});
+            off += (unsigned long long)NBIN3 * nmb * nmk;
+        }
+    }
+    const size_t need = std::max<size_t>(256, items.size() * sizeof(BlockItem));
+    if (!d_work) { *work_bytes = need; return MFDN_OK; }
+    if (*work_bytes < need) return fail(c, MFDN_ERR_OOM, "scratch too small");
+    if (items.empty()) return MFDN_OK;
+    if (!d_out || !h_off) return fail(c, MFDN_ERR_ARG, "null output / offset pointer");
+    if (items.size() >= 0xFFFFFFF0ull / NBIN3) return fail(c, MFDN_ERR_ARG, "too many (group, M) sub-blocks in one call");
+    cudaStream_t st = (cudaStream_t)stream;
+    MFDN_CUDA(c, cudaSetDevice(c->device));
+    // pageable source: the copy is staged before cudaMemcpyAsync returns, `items` may go out of scope
+    MFDN_CUDA(c, cudaMemcpyAsync(d_work, items.data(), items.size() * sizeof(BlockItem), cudaMemcpyHostToDevice, st));
+    const unsigned grid = (unsigned)std::min<size_t>((items.size() * NBIN3 + DN_WARPS - 1) / DN_WARPS, (size_t)c->num_sms * 8);
+    k_block3<<<grid, DN_WARPS * 32, 0, st>>>(c->t, (const BlockItem*)d_work, (uint32_t)items.size(), d_out);
+    c->launches += 1;
+    MFDN_CUDA(c, cudaGetLastError());
+    return MFDN_OK;
 }
 
 extern "C" int mfdn_group_keys(mfdn_ctx* c, int body, int64_t n, const int32_t* d_req, uint32_t* d_key, void* stream)

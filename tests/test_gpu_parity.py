@@ -518,3 +518,96 @@ def test_accumulate_epilogue(torch, B, oracle, idx):
                            torch.from_numpy(phase[order].copy()).cuda(), d_H, flags=B.MFDN_PRESORTED)
             torch.cuda.synchronize()
             assert float(np.max(np.abs(d_H.cpu().numpy() - accumulate(want, loc, phase, h_len)))) <= tol
+
+
+# --------------------------------------------------------------------------------- NEXT-2: dense block mode
+def _expected_block(cfg, oracle, orbs):
+    """The block of include/mfdn_b200.h's mfdn_mscheme_blocks_3b, built from the header's words alone: enumerate the entries
+    in the stated order, ask the ORACLE for those that are ordered Slater determinants, +0.0 elsewhere."""
+    b = cfg.basis
+    tj = np.asarray(b.twoj)
+    sps = {(int(o), int(m), int(t)): k for k, (o, m, t) in enumerate(zip(b.sps_orb, b.sps_twom, b.sps_twotz))}
+    listed = set(zip(cfg.table.state_a.tolist(), cfg.table.state_b.tolist(), cfg.table.state_c.tolist()))
+    bra, ket = tuple(int(x) for x in orbs[:3]), tuple(int(x) for x in orbs[3:])
+    lpar = lambda t: sum(int(b.l[o]) for o in t) & 1
+    if bra not in listed or ket not in listed or lpar(bra) != lpar(ket):
+        return np.zeros(0)
+    sj = lambda t: int(sum(tj[o] for o in t))
+    # common J (triangle ranges of both tuples); the library says "no common J" -> empty
+    def jrange(t):
+        ja, jb, jc = (int(tj[o]) for o in t)
+        lo = min(abs(2 * J12 - jc) for J12 in range(abs(ja - jb) // 2, (ja + jb) // 2 + 1))
+        return lo, ja + jb + jc
+    (lb, hb), (lk, hk) = jrange(bra), jrange(ket)
+    if max(lb, lk) > min(hb, hk):
+        return np.zeros(0)
+    mm = min(sj(bra), sj(ket))
+    def mstates(t, twoM):     # (ia, ib, ic) of the given M in ascending (ia, ib) order
+        ja, jb, jc = (int(tj[o]) for o in t)
+        return [(ia, ib, ic) for ia in range(ja + 1) for ib in range(jb + 1) for ic in range(jc + 1)
+                if 2 * (ia + ib + ic) - (ja + jb + jc) == twoM]
+    pats = [(pb, pk) for pb in range(8) for pk in range(8) if bin(pb).count("1") == bin(pk).count("1")]
+    def side(t, st, pat):     # SPS indices of an ordered Slater determinant, or None
+        idx = []
+        for o, i, bit in zip(t, st, ((pat >> 2) & 1, (pat >> 1) & 1, pat & 1)):
+            k = sps.get((o, 2 * i - int(tj[o]), 1 if bit else -1))
+            if k is None:
+                return None
+            idx.append(k)
+        for p in range(2):
+            if t[p] == t[p + 1] and not idx[p] < idx[p + 1]:
+                return None
+        return idx
+    reqs, where, total = [], [], 0
+    for mi in range(mm + 1):
+        twoM = 2 * mi - mm
+        rows, cols = mstates(bra, twoM), mstates(ket, twoM)
+        for pb, pk in pats:
+            for r, sb in enumerate(rows):
+                ib = side(bra, sb, pb)
+                for cidx, sk in enumerate(cols):
+                    ik = side(ket, sk, pk)
+                    if ib is not None and ik is not None:
+                        reqs.append(ib + ik)
+                        where.append(total + r * len(cols) + cidx)
+            total += len(rows) * len(cols)
+    out = np.zeros(total)
+    if reqs:
+        want, _, _, _ = oracle.mscheme(cfg.basis, cfg.table, np.asarray(reqs, np.int32))
+        out[np.asarray(where)] = want
+    return out
+
+
+@pytest.mark.gpu
+def test_dense_block_mode(torch, B, oracle):
+    """mfdn_mscheme_blocks_3b against the oracle, entry by entry, for tuple pairs with distinct and repeated orbitals (a == b,
+    b == c, a == b == c), equal tuples, the other parity (empty block), an unlisted tuple (empty block)."""
+    cfg = get_cfg(2)
+    ctx = get_ctx(B, 2)
+    tup = sorted(set(zip(cfg.table.state_a.tolist(), cfg.table.state_b.tolist(), cfg.table.state_c.tolist())))
+    kinds = {}
+    for t in tup:
+        kinds.setdefault((t[0] == t[1], t[1] == t[2]), []).append(t)
+    rng = np.random.default_rng(8)
+    picks = [kinds[k][int(rng.integers(len(kinds[k])))] for k in sorted(kinds)] + [tup[int(i)] for i in rng.choice(len(tup), 6, replace=False)]
+    groups = [a + b for a in picks[:6] for b in picks[2:8]] + [picks[0] + picks[0]]
+    n_orb = cfg.basis.n_orb
+    unlisted = next((a, b, c) for a in range(n_orb) for b in range(a, n_orb) for c in range(b, n_orb) if (a, b, c) not in set(tup))
+    groups.append(unlisted + tup[0])
+    d_out, off = ctx.blocks(np.asarray(groups, np.int32))
+    torch.cuda.synchronize()
+    got = d_out.cpu().numpy()
+    vmax = float(np.max(np.abs(cfg.table.values)))
+    n_nonempty = 0
+    for k, g in enumerate(groups):
+        want = _expected_block(cfg, oracle, g)
+        blk = got[off[k]:off[k + 1]]
+        assert len(blk) == len(want), (g, len(blk), len(want))
+        if len(want):
+            n_nonempty += 1
+            assert float(np.max(np.abs(blk - want))) <= TOL * vmax, g
+            assert np.all(blk[want == 0.0] == 0.0) and not np.any(np.signbit(blk[want == 0.0])), g
+    assert n_nonempty >= 10 and len(_expected_block(cfg, oracle, groups[-1])) == 0
+    with pytest.raises(B.MfdnError) as e:
+        ctx.blocks(np.asarray([[1, 0, 2, 0, 1, 2]], np.int32))     # not ascending
+    assert e.value.code == B.MFDN_ERR_ARG
