@@ -52,10 +52,13 @@ enum {
                              requested entries are picked from it; the other groups take the default path.  Values
                              agree with the default path to rounding (another summation order), the mask bit for bit.
                              MFDN_ERR_ARG for 2-body calls and together with MFDN_FORCE_NAIVE */
-    MFDN_ONE_PASS_SORT = 8 /* steps H2 / H6 by the one-pass scatter and gather instead of the two-pass partition through
+    MFDN_ONE_PASS_SORT = 8, /* steps H2 / H6 by the one-pass scatter and gather instead of the two-pass partition through
                              shared memory.  The library takes this path by itself for tables with more than 2048 x 4096
                              sort buckets (2-body: orbital-tuple pairs; 3-body: (pair, M) combinations); the flag forces
                              it for any table (test hook and the measured baseline of DESIGN.md).  Same values bit for bit */
+    MFDN_REQ_U16 = 16      /* compact requests: d_req / h_req point to uint16 SPS indices, [n][4] or [n][6] (8 / 12 bytes per request
+                             instead of 16 / 24: half the host-to-device bytes of mfdn_mscheme_host, whose time is the PCIe
+                             copy).  Needs n_sps <= 65536 (else MFDN_ERR_ARG); 4-byte aligned; same results bit for bit */
 };
 
 /* A0. Single-particle basis (quantum numbers flattened into one linear SPS index).
@@ -164,10 +167,10 @@ int mfdn_mscheme_blocks_3b(mfdn_ctx*, int64_t n_groups, const int32_t* h_orbital
 /* The paper's wrapper ("transfer a chunk of 3-body element requests to the GPU, invoke the kernel,
  * and transfer the results back"), for HOST request/result buffers (pinned memory recommended).  The n requests
  * are cut into chunks of `chunk` (0 = library default) and H2D copy / transform / D2H copy of successive chunks
- * overlap on two internal streams.  body = 2 or 3; h_mask may be NULL; flags as above (MFDN_PRESORTED then means
+ * overlap on four internal streams.  body = 2 or 3; h_mask may be NULL; flags as above (MFDN_PRESORTED then means
  * the whole host array is group-ordered).  d_work/work_bytes: DEVICE scratch, queried with d_work == NULL.
  * BLOCKING: returns after the last result byte has landed in h_out (also on failure: no copy is left in flight on the
- * caller's buffers).  Uses two streams owned by the context: one mfdn_mscheme_host call at a time per context. */
+ * caller's buffers).  Uses four streams owned by the context: one mfdn_mscheme_host call at a time per context. */
 int mfdn_mscheme_host(mfdn_ctx*, int body, int64_t n, const int32_t* h_req, double* h_out, uint8_t* h_mask,
                       void* d_work, size_t* work_bytes, uint32_t flags, int64_t chunk);
 

@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmfdn_b200.so")
 
 MFDN_OK, MFDN_ERR_ARG, MFDN_ERR_STATE, MFDN_ERR_CUDA, MFDN_ERR_OOM, MFDN_ERR_TABLE = 0, -1, -2, -3, -4, -5
-MFDN_PRESORTED, MFDN_FORCE_NAIVE, MFDN_FORCE_DENSE, MFDN_ONE_PASS_SORT = 1, 2, 4, 8
+MFDN_PRESORTED, MFDN_FORCE_NAIVE, MFDN_FORCE_DENSE, MFDN_ONE_PASS_SORT, MFDN_REQ_U16 = 1, 2, 4, 8, 16
 
 # every symbol include/mfdn_b200.h declares
 SYMBOLS = ["mfdn_orbitals_init", "mfdn_cg_build", "mfdn_cg_download", "mfdn_coupled_upload_2b",
@@ -259,7 +259,11 @@ class Context:
     def mscheme(self, d_req, d_out=None, d_mask=None, flags=0, work=None, stream=None):
         """d_req: CUDA int32 tensor [n][4] or [n][6].  Returns (d_out f64[n], d_mask u8[n])."""
         torch = self.torch
-        assert d_req.is_cuda and d_req.dtype == torch.int32 and d_req.is_contiguous()
+        assert d_req.is_cuda and d_req.is_contiguous()
+        if d_req.dtype in (torch.uint16, torch.int16):
+            flags |= MFDN_REQ_U16            # compact requests: 16-bit SPS indices
+        else:
+            assert d_req.dtype == torch.int32 and not flags & MFDN_REQ_U16
         n, width = d_req.shape
         body = width // 2
         if d_out is None:
@@ -281,7 +285,11 @@ class Context:
         """d_H[d_loc[i]] += d_phase[i] * v_i (PAPER.md:93, 97).  d_loc: CUDA int64 [n]; d_phase: CUDA float64 [n] or None;
         d_H: CUDA float64, updated in place.  Returns d_mask."""
         torch = self.torch
-        assert d_req.is_cuda and d_req.dtype == torch.int32 and d_req.is_contiguous()
+        assert d_req.is_cuda and d_req.is_contiguous()
+        if d_req.dtype in (torch.uint16, torch.int16):
+            flags |= MFDN_REQ_U16
+        else:
+            assert d_req.dtype == torch.int32 and not flags & MFDN_REQ_U16
         assert d_loc.is_cuda and d_loc.dtype == torch.int64 and d_loc.is_contiguous() and d_loc.numel() == d_req.shape[0]
         assert d_phase is None or (d_phase.is_cuda and d_phase.dtype == torch.float64 and d_phase.is_contiguous())
         assert d_H.is_cuda and d_H.dtype == torch.float64 and d_H.is_contiguous()
@@ -316,7 +324,11 @@ class Context:
     def mscheme_host(self, h_req, h_out=None, h_mask=None, flags=0, chunk=0):
         """h_req: CPU int32 tensor [n][4|6] (pinned recommended).  Returns (h_out, h_mask) CPU tensors."""
         torch = self.torch
-        assert (not h_req.is_cuda) and h_req.dtype == torch.int32 and h_req.is_contiguous()
+        assert (not h_req.is_cuda) and h_req.is_contiguous()
+        if h_req.dtype in (torch.uint16, torch.int16):
+            flags |= MFDN_REQ_U16
+        else:
+            assert h_req.dtype == torch.int32 and not flags & MFDN_REQ_U16
         n, width = h_req.shape
         if h_out is None:
             h_out = torch.empty(n, dtype=torch.float64).pin_memory()

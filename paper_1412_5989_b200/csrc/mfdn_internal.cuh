@@ -47,6 +47,7 @@ constexpr int CG_GUARD = 8192;     // zero doubles before and after the stage-2 
 // not listed.  The isospin-combined copy Vw = sum_s w[s] * plane[s] that the transform stages in shared memory has
 // the same indexing.
 __host__ __device__ inline int row_pitch3(int nk) { return (nk + 1) & ~1; }
+constexpr int HOST_STREAMS = 4;    // internal streams / chunk buffers of mfdn_mscheme_host
 constexpr int ITEM3 = 512;         // max records per work item of the 3-body transform (one group per item)
 // Isospin-combined slabs (A2): for every group and every isospin bin the weighted plane sum Vw[cell] =
 // sum_s w[bin][s] * plane_s[cell], precomputed at upload so that staging it is a pure bulk copy.  The two 32-bit
@@ -166,7 +167,7 @@ struct mfdn_ctx {
     std::vector<EvTriple> ev_pending;
     std::vector<cudaEvent_t> ev_pool;
     // host-buffer wrapper
-    cudaStream_t hs[2] = {nullptr, nullptr};
+    cudaStream_t hs[4] = {nullptr, nullptr, nullptr, nullptr};
 };
 
 namespace mfdn {

@@ -611,3 +611,30 @@ def test_dense_block_mode(torch, B, oracle):
     with pytest.raises(B.MfdnError) as e:
         ctx.blocks(np.asarray([[1, 0, 2, 0, 1, 2]], np.int32))     # not ascending
     assert e.value.code == B.MFDN_ERR_ARG
+
+
+# --------------------------------------------------------------------------------- compact requests
+@pytest.mark.gpu
+@pytest.mark.parametrize("idx", [0, 2])
+def test_compact_u16_requests(torch, B, oracle, idx):
+    """MFDN_REQ_U16: the same requests as 16-bit SPS indices give the same values and masks bit for bit, on the device paths
+    and through the host wrapper; out-of-range indices are still caught."""
+    cfg = get_cfg(idx)
+    ctx = get_ctx(B, idx)
+    rng = np.random.default_rng(31)
+    allreq = cfg.requests()
+    req = allreq[rng.choice(len(allreq), min(len(allreq), 30011), replace=False)].copy()
+    req[:50, 0] = cfg.basis.n_sps            # out of range
+    want, wmask, _, nbad = oracle.mscheme(cfg.basis, cfg.table, req)
+    r16 = np.ascontiguousarray(req.astype(np.uint16))
+    before = ctx.bad_request_count()
+    for flags in (0, B.MFDN_ONE_PASS_SORT, B.MFDN_FORCE_NAIVE):
+        got32, m32 = run_gpu(torch, ctx, req, flags)
+        out, mask = ctx.mscheme(torch.from_numpy(r16).cuda(), flags=flags)
+        torch.cuda.synchronize()
+        assert np.array_equal(out.cpu().numpy(), got32) and np.array_equal(mask.cpu().numpy(), m32)
+        check(cfg, out.cpu().numpy(), mask.cpu().numpy(), want, wmask)
+    assert ctx.bad_request_count() - before == 6 * nbad == 300
+    h_out, h_mask = ctx.mscheme_host(torch.from_numpy(r16).pin_memory(), chunk=7000)
+    check(cfg, h_out.numpy(), h_mask.numpy(), want, wmask)
+
