@@ -413,11 +413,11 @@ constexpr int KS_THREADS = 1024;
 struct KeysSmem3 {   // byte offsets into the dynamic shared memory, filled by the host
     uint32_t tdesc, stm, ab, sps, rowbase, ch, colcum, sig, tzbin, total;
 };
-template <bool AGG>
+template <bool AGG, bool U16>
 __global__ void __launch_bounds__(KS_THREADS, 1) k_keys3s(Tables T, KeysSmem3 L, long long n, const int32_t* __restrict__ req,
                                                          unsigned long long* __restrict__ recs, uint8_t* __restrict__ maskout,
                                                          uint32_t* __restrict__ hist, uint32_t invalid_bucket,
-                                                         uint32_t* __restrict__ tcnt, int csh, int nc, int n_tiles, int u16)
+                                                         uint32_t* __restrict__ tcnt, int csh, int nc, int n_tiles)
 {
     extern __shared__ __align__(16) unsigned char ks_smem[];
     int4* s_tdesc = reinterpret_cast<int4*>(ks_smem + L.tdesc);
@@ -444,12 +444,12 @@ __global__ void __launch_bounds__(KS_THREADS, 1) k_keys3s(Tables T, KeysSmem3 L,
         const long long i0 = (long long)tile * KEYS_PER_BLOCK + tid;
         const long long i1 = min(n, (long long)(tile + 1) * KEYS_PER_BLOCK);
         int nx[6];
-        if (i0 < i1) load_req3(req, i0, nx, u16);
+        if (i0 < i1) load_req3(req, i0, nx, U16);
         for (long long i = i0; i < i1; i += KS_THREADS) {
             int s[6];
 #pragma unroll
             for (int k = 0; k < 6; k++) s[k] = nx[k];
-            if (i + KS_THREADS < i1) load_req3(req, i + KS_THREADS, nx, u16);   // next request in flight
+            if (i + KS_THREADS < i1) load_req3(req, i + KS_THREADS, nx, U16);   // next request in flight
             uint32_t key = REC_INVALID;
             unsigned long long low = 0;
             int mask = 0;
@@ -1988,14 +1988,17 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
         }
         if (smem_keys) {
             if (!c->keys_attr_set.load()) {   // benign if two threads do it at once
-                MFDN_CUDA(c, cudaFuncSetAttribute(k_keys3s<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-                MFDN_CUDA(c, cudaFuncSetAttribute(k_keys3s<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+                MFDN_CUDA(c, (cudaFuncSetAttribute(k_keys3s<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)));
+                MFDN_CUDA(c, (cudaFuncSetAttribute(k_keys3s<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)));
+                MFDN_CUDA(c, (cudaFuncSetAttribute(k_keys3s<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)));
+                MFDN_CUDA(c, (cudaFuncSetAttribute(k_keys3s<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)));
                 c->keys_attr_set.store(true);
             }
             const unsigned gks = (unsigned)std::min<long long>(n_ktiles, c->num_sms);
-            if (sort) k_keys3s<false><<<gks, KS_THREADS, L.total, st>>>(c->t, L, n, d_req, recs, d_mask, hist, invalid_bucket,
-                                                                         two_pass ? (uint32_t*)(w + o_tcnt) : nullptr, csh, nc, (int)n_ktiles, u16);
-            else k_keys3s<true><<<gks, KS_THREADS, L.total, st>>>(c->t, L, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr, 0, 0, (int)n_ktiles, u16);
+            uint32_t* tc = sort && two_pass ? (uint32_t*)(w + o_tcnt) : nullptr;
+            const int tsh = sort ? csh : 0, tnc = sort ? nc : 0;
+            auto kern = sort ? (u16 ? k_keys3s<false, true> : k_keys3s<false, false>) : (u16 ? k_keys3s<true, true> : k_keys3s<true, false>);
+            kern<<<gks, KS_THREADS, L.total, st>>>(c->t, L, n, d_req, recs, d_mask, hist, invalid_bucket, tc, tsh, tnc, (int)n_ktiles);
         } else if (sort) {
             uint32_t* tcnt = two_pass ? (uint32_t*)(w + o_tcnt) : nullptr;
             if (sm) k_keys<BODY, false, true><<<gkb, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr, tcnt, csh, nc, u16);
