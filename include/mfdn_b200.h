@@ -41,7 +41,7 @@ typedef enum {
 enum {
     MFDN_PRESORTED = 1,   /* requests are already ordered by the library's sort key: NON-DECREASING mfdn_group_keys value
                              (2-body: orbital-tuple group; 3-body: group, then M; requests failing S1-S6, key
-                             0xFFFFFFFF, last).  Skips the scatter of step H2 and the gather of step H6; 3-body still
+                             0xFFFFFFFF, last).  Skips the partition passes of step H2 and of step H6; 3-body still
                              histograms the keys to cut the stream into one-group work items.  Input that is not so
                              ordered gives undefined VALUES (never a fault); the mask stays correct */
     MFDN_FORCE_NAIVE = 2, /* one thread per request in request order, no sort, no staging: the paper's own
@@ -175,7 +175,7 @@ int mfdn_mscheme_host(mfdn_ctx*, int body, int64_t n, const int32_t* h_req, doub
                       void* d_work, size_t* work_bytes, uint32_t flags, int64_t chunk);
 
 /* Measurement hooks.  mfdn_profile(ctx, 1) makes every later mfdn_mscheme_2b/3b call record CUDA events on the
- * call's stream around (1) its group-sort kernels (H1-H2: keys, scans, scatter, work-item list), (2) its transform
+ * call's stream around (1) its group-sort kernels (H1-H2: keys, scans, partition passes, work-item list), (2) its transform
  * kernel (H3-H6) and (3) the gather of the results back into request order (sort path only; 0 for MFDN_PRESORTED
  * and MFDN_FORCE_NAIVE).  mfdn_profile_read synchronises those events, returns the accumulated milliseconds of the
  * three parts and the call count since the last read, and resets them.  mfdn_fp64_peak runs a register-resident
