@@ -69,6 +69,16 @@ int mfdn_orbitals_init(mfdn_ctx** out, int device, int32_t n_orb, const int32_t*
                        const int32_t* twoj, int32_t n_sps, const int32_t* sps_orb, const int32_t* sps_twom,
                        const int32_t* sps_twotz);
 
+/* Options, set between mfdn_orbitals_init and the upload they concern (MFDN_ERR_STATE afterwards).
+ * MFDN_OPT_SLAB_FP32 (value != 0): footprint variant of the 3-body tables (the memory
+ *   footprint is the reason for coupled storage, the paper is silent on precision): the isospin-combined slabs -- the
+ *   largest resident array, 4/5 of the 3-body table memory -- are STORED in fp32, every sum is still accumulated in fp64.
+ *   Halves that array and the shared-memory traffic of the transform.  Values then carry the rounding of the stored
+ *   numbers: |delta| <= 2^-24 * 5 max|V| per coupled cell summed, i.e. about 1e-6 max|V| instead of 1e-12 max|V|; the mask
+ *   is unchanged.  MFDN_FORCE_NAIVE keeps reading the fp64 planes. */
+enum { MFDN_OPT_SLAB_FP32 = 1 };
+int mfdn_option(mfdn_ctx*, int option, int64_t value);
+
 /* A1. Device-resident fp64 Clebsch-Gordan tables ("D is developed from a series of angular momentum and
  * isospin coupling coefficients"; Q1/Q2/Q10), built by one kernel from Racah's
  * formula with a double-double log-factorial table.  Asynchronous on `stream` (cudaStream_t). */

@@ -17,13 +17,14 @@ LIB_PATH = os.path.join(_HERE, "libmfdn_b200.so")
 
 MFDN_OK, MFDN_ERR_ARG, MFDN_ERR_STATE, MFDN_ERR_CUDA, MFDN_ERR_OOM, MFDN_ERR_TABLE = 0, -1, -2, -3, -4, -5
 MFDN_PRESORTED, MFDN_FORCE_NAIVE, MFDN_FORCE_DENSE, MFDN_ONE_PASS_SORT, MFDN_REQ_U16 = 1, 2, 4, 8, 16
+MFDN_OPT_SLAB_FP32 = 1
 
 # every symbol include/mfdn_b200.h declares
 SYMBOLS = ["mfdn_orbitals_init", "mfdn_cg_build", "mfdn_cg_download", "mfdn_coupled_upload_2b",
            "mfdn_coupled_upload_3b", "mfdn_mscheme_2b", "mfdn_mscheme_3b", "mfdn_bad_request_count",
            "mfdn_info", "mfdn_group_keys", "mfdn_last_error", "mfdn_destroy", "mfdn_mscheme_host", "mfdn_profile",
            "mfdn_profile_read", "mfdn_fp64_peak", "mfdn_mscheme_accumulate_2b", "mfdn_mscheme_accumulate_3b",
-           "mfdn_mscheme_block_len_3b", "mfdn_mscheme_blocks_3b"]
+           "mfdn_mscheme_block_len_3b", "mfdn_mscheme_blocks_3b", "mfdn_option"]
 
 _lib = None
 
@@ -52,6 +53,7 @@ def lib():
             f.argtypes = [vp, i64, vp, vp, vp, vp, C.POINTER(C.c_size_t), u32, vp]
         for f in (L.mfdn_mscheme_accumulate_2b, L.mfdn_mscheme_accumulate_3b):
             f.argtypes = [vp, i64, vp, vp, vp, vp, i64, vp, vp, C.POINTER(C.c_size_t), u32, vp]
+        L.mfdn_option.argtypes = [vp, C.c_int, i64]
         L.mfdn_mscheme_block_len_3b.argtypes = [vp, vp, C.POINTER(i64)]
         L.mfdn_mscheme_blocks_3b.argtypes = [vp, i64, vp, vp, vp, vp, C.POINTER(C.c_size_t), vp]
         L.mfdn_mscheme_host.argtypes = [vp, C.c_int, i64, vp, vp, vp, vp, C.POINTER(C.c_size_t), u32, i64]
@@ -240,6 +242,11 @@ class Context:
         with torch.cuda.device(device):
             mfdn_cg_build(self.ctx)
         self._work = None
+
+    def option(self, option, value=1):
+        """mfdn_option (e.g. MFDN_OPT_SLAB_FP32), before upload()."""
+        _check(self.ctx, lib().mfdn_option(self.ctx, int(option), int(value)))
+        return self
 
     def upload(self, table):
         with self.torch.cuda.device(self.device):

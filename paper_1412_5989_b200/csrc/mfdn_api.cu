@@ -334,6 +334,17 @@ extern "C" int mfdn_cg_build(mfdn_ctx* c, void* stream)
     return MFDN_OK;
 }
 
+extern "C" int mfdn_option(mfdn_ctx* c, int option, int64_t value)
+{
+    if (!c) return MFDN_ERR_ARG;
+    if (option == MFDN_OPT_SLAB_FP32) {
+        if (c->has3) return fail(c, MFDN_ERR_STATE, "MFDN_OPT_SLAB_FP32 must be set before mfdn_coupled_upload_3b");
+        c->opt_slab_fp32 = value != 0;
+        return MFDN_OK;
+    }
+    return fail(c, MFDN_ERR_ARG, "unknown option");
+}
+
 extern "C" int mfdn_cg_download(mfdn_ctx* c, int stage, double* host_out, int64_t cap, int64_t* n)
 {
     if (!c || !n || (stage != 1 && stage != 2)) return MFDN_ERR_ARG;
@@ -414,12 +425,12 @@ __global__ void k_retile3(Retile3 p)
 // request.  Same operation order as the kernels that sum the five planes themselves (k_transform3_small,
 // k_mscheme_naive use w0*p0, then fma over s = 1..4), so a value does not depend on the path its group takes.
 __global__ void k_vw20(long long n_groups, const uint4* __restrict__ sgrp, const double* __restrict__ slab,
-                       const double* __restrict__ wbin, uint32_t* __restrict__ vw20)
+                       const double* __restrict__ wbin, uint32_t* __restrict__ vw20, int f32)
 {
     for (long long g = blockIdx.x; g < n_groups; g += gridDim.x) {
         const uint4 sg = sgrp[g];
         if (sg.x == NO_SLAB) continue;
-        const uint32_t gsize = sg.y, S = vw_stride(gsize);
+        const uint32_t gsize = sg.y, S = vw_stride(gsize, f32);
         const double* src = slab + (size_t)sg.x * 2;
         uint32_t* dst = vw20 + (size_t)sg.z * 4;
         for (uint32_t idx = threadIdx.x; idx < NBIN3 * gsize; idx += blockDim.x) {
@@ -430,10 +441,15 @@ __global__ void k_vw20(long long n_groups, const uint4* __restrict__ sgrp, const
             v = fma(w[2], src[2 * (size_t)gsize + cell], v);
             v = fma(w[3], src[3 * (size_t)gsize + cell], v);
             v = fma(w[4], src[4 * (size_t)gsize + cell], v);
-            dst[(size_t)b * S + cell] = (uint32_t)__double2loint(v);
-            dst[(size_t)b * S + gsize + cell] = (uint32_t)__double2hiint(v);
+            if (f32) {   // footprint variant: the combined value rounded to fp32 (arithmetic stays fp64)
+                dst[(size_t)b * S + cell] = __float_as_uint((float)v);
+            } else {
+                dst[(size_t)b * S + cell] = (uint32_t)__double2loint(v);
+                dst[(size_t)b * S + gsize + cell] = (uint32_t)__double2hiint(v);
+            }
         }
-        for (uint32_t b = threadIdx.x; b < NBIN3; b += blockDim.x) dst[(size_t)b * S + 2 * gsize] = 0u;
+        for (uint32_t b = threadIdx.x; b < NBIN3; b += blockDim.x)
+            if (!f32 || !(gsize & 1u)) dst[(size_t)b * S + (f32 ? gsize : 2 * gsize)] = 0u;   // the pad word, if there is one
     }
 }
 
@@ -722,6 +738,7 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     }
     // ---- group descriptors: slab offset (16-byte units) and plane size, rows in loop order J, J12
     //      and the (group, M) buckets of the request sort: every same-parity group owns one bucket per common M
+    const int f32 = c->opt_slab_fp32 ? 1 : 0;
     std::vector<uint4> sgrp((size_t)nt * nt, uint4{NO_SLAB, 0u, 0u, 0u});
     std::vector<uint32_t> gbase((size_t)nt * nt + 1, 0u);
     uint64_t cells = 0;   // in 16-byte units
@@ -747,7 +764,7 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
                 if (hb >= lb && hk >= lk) gsize += (uint64_t)(hb - lb + 1) * row_pitch3(hk - lk + 1);
             }
             if (gsize == 0) continue;
-            const uint64_t vw16 = ((uint64_t)NBIN3 * vw_stride((uint32_t)gsize) + 3) / 4;   // 16-byte units, rounded up
+            const uint64_t vw16 = ((uint64_t)NBIN3 * vw_stride((uint32_t)gsize, f32) + 3) / 4;   // 16-byte units, rounded up
             if (cells + gsize * NISO3 / 2 >= 0xFFFFFFF0ull || vwcells + vw16 >= 0xFFFFFFF0ull)
                 return fail(c, MFDN_ERR_OOM, "table too large for 32-bit slab offsets");
             // dense-block path (H5'): feasible if every (M) block of m-states fits one warp's tile buffer and the
@@ -893,7 +910,7 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     p.slab = (double*)dslab;
     long long groups = (long long)nt * nt;
     k_retile3<<<(unsigned)std::min<long long>(groups, 1 << 20), 64, 0, st>>>(p);
-    k_vw20<<<(unsigned)std::min<long long>(groups, 1 << 20), 128, 0, st>>>(groups, p.sgrp, (const double*)dslab, c->t.wbin3, (uint32_t*)dvw);
+    k_vw20<<<(unsigned)std::min<long long>(groups, 1 << 20), 128, 0, st>>>(groups, p.sgrp, (const double*)dslab, c->t.wbin3, (uint32_t*)dvw, f32);
     Dtab3 q;
     q.tdesc = p.tdesc;
     q.tk = (const int4*)(dres + o_tk);
@@ -927,6 +944,7 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     c->t.sig_len3 = (int)sig.size();
     c->t.stmask_len3 = (int)stmask.size();
     c->t.vw20 = (const uint32_t*)dvw;
+    c->t.vw_f32 = f32;
     c->vw_bytes3 = (int64_t)(vwcells * 16);
     c->t.ab3 = ab_dense ? (const int2*)(dres + o_ab) : nullptr;
     c->t.slab3 = (const double*)dslab;

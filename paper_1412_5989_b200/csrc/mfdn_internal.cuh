@@ -55,7 +55,8 @@ constexpr int ITEM3 = 512;         // max records per work item of the 3-body tr
 // [0, gsize), high words at [gsize, 2*gsize), one pad word.  The stride is ODD, so the 20 bins of one cell fall
 // into 20 different shared-memory banks: a warp whose lanes sit in any mixture of bins reads a cell with two
 // conflict-free 32-bit loads (measured: 2.0 cycles per cell against 3.7 for 64-bit loads over 20 random bins).
-__host__ __device__ inline uint32_t vw_stride(uint32_t gsize) { return 2u * gsize + 1u; }
+// With MFDN_OPT_SLAB_FP32 a value is ONE fp32 word (footprint variant, NEXT-4): bin b occupies gsize | 1 words (odd again).
+__host__ __device__ inline uint32_t vw_stride(uint32_t gsize, int f32 = 0) { return f32 ? (gsize | 1u) : 2u * gsize + 1u; }
 constexpr int DENSE_CAP = 1024;    // doubles of one (group, M, bin) block of the dense path, both dimensions padded to 8 (one warp's tile buffer)
 constexpr int DENSE_RMAX = 64;     // flattened ket rows (J, J12') of a group on the dense path
 constexpr int VW_WORDS = 5120;     // 32-bit words of one staged slab (20 KB): all 20 bins of a group with gsize <= 127
@@ -115,6 +116,7 @@ struct Tables {
     uint32_t n_buckets3;           // = gbase3[n_tup3^2]; bucket n_buckets3 collects the requests failing S1-S6
     const double* slab3;
     const uint32_t* vw20;          // isospin-combined slabs, split word planes (see vw_stride)
+    int vw_f32;                    // 1: the slabs hold fp32 values, one word each (MFDN_OPT_SLAB_FP32)
     const unsigned long long* stmask3;
     const int4* tk3;               // [n_tup3] see above
     const int2* jinfo3;            // per (tuple, J): {offset of the J block in the tuple's coefficient table (doubles, even), rows nb(J)}
@@ -141,6 +143,7 @@ struct mfdn_ctx {
     int device = 0;
     int stage = 0;  // 1 orbitals, 2 cg built
     bool has2 = false, has3 = false;
+    bool opt_slab_fp32 = false;   // mfdn_option(MFDN_OPT_SLAB_FP32), read by mfdn_coupled_upload_3b
     std::string err;            // last error message; guarded by `mu` (mfdn_last_error hands out a per-thread copy)
     std::mutex mu;              // guards err, ev_pending, ev_pool: mscheme_* may be called from several host threads
     mfdn::Tables t{};

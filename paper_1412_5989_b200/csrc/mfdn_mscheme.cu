@@ -919,9 +919,9 @@ __global__ void __launch_bounds__(256) k_unpermute(long long n, const double* __
 // of three j = 15/2 orbitals have one) go to the same list in chunks of SMALL_ITEM3 records: that path has no
 // capacity limit.
 constexpr uint32_t SMALL_ITEM3 = 64;
-__device__ __forceinline__ uint32_t bins_per_round3(uint32_t gsize)
+__device__ __forceinline__ uint32_t bins_per_round3(uint32_t gsize, int f32)
 {
-    const uint32_t b = ((uint32_t)VW_WORDS / vw_stride(gsize)) & ~3u;   // multiple of 4: every round starts 16-byte aligned
+    const uint32_t b = ((uint32_t)VW_WORDS / vw_stride(gsize, f32)) & ~3u;   // multiple of 4: every round starts 16-byte aligned
     return min(b, (uint32_t)NBIN3);
 }
 // dense_tau < 0: no group takes the dense-block path (H5'); otherwise a feasible group does if its records number at
@@ -930,7 +930,7 @@ __device__ __forceinline__ uint32_t bins_per_round3(uint32_t gsize)
 __global__ void __launch_bounds__(256) k_items3(const uint32_t* __restrict__ bounds, const uint32_t* __restrict__ gbase,
                                                uint32_t n_groups, uint32_t n_buckets, int ends, uint32_t n,
                                                const uint4* __restrict__ sgrp, uint4* __restrict__ items, uint32_t last_slot,
-                                               uint32_t* __restrict__ n_items, float dense_tau, uint4* __restrict__ ditems)
+                                               uint32_t* __restrict__ n_items, float dense_tau, uint4* __restrict__ ditems, int vw_f32)
 {
     const uint32_t g = blockIdx.x * 256u + threadIdx.x;   // g == n_groups: the bucket of the invalid requests
     uint32_t start = 0, end = 0, gsize = 0, b0 = 0, b1 = 0;
@@ -958,7 +958,7 @@ __global__ void __launch_bounds__(256) k_items3(const uint32_t* __restrict__ bou
         start = end = 0;
     }
     const uint32_t cnt = end - start;
-    const uint32_t bpr = zero ? (uint32_t)NBIN3 : bins_per_round3(gsize);
+    const uint32_t bpr = zero ? (uint32_t)NBIN3 : bins_per_round3(gsize, vw_f32);
     const bool small = cnt <= SMALL_ITEM3 || bpr == 0u;
     const uint32_t rounds = small ? 0u : (NBIN3 + bpr - 1u) / bpr;
     const uint32_t k = small ? 0u : ((cnt + ITEM3 - 1) / ITEM3) * rounds, ks = small ? (cnt + SMALL_ITEM3 - 1) / SMALL_ITEM3 : 0u;
@@ -998,7 +998,7 @@ __global__ void __launch_bounds__(256) k_items3(const uint32_t* __restrict__ bou
 // order of the one-lane-per-record form.  Groups of at most SMALL_SPLIT records (config 4: a 2^24-request batch leaves
 // about 6 records per group of its uniform part) take PARTS = 4, eight records per pass; larger ones PARTS = 1.
 constexpr uint32_t SMALL_SPLIT = 24;
-template <int PARTS>
+template <int PARTS, bool F32>
 __device__ __forceinline__ void small_group3(const Tables& T, uint32_t pos0, uint32_t cnt, int nblk, int2 ib_l, int2 ik_l, uint32_t voff_l,
                                              uint32_t tb_off, uint32_t tk_off, const uint32_t* __restrict__ vw, uint32_t gsize,
                                              const unsigned long long* __restrict__ recs, double* __restrict__ out, int lane)
@@ -1006,7 +1006,7 @@ __device__ __forceinline__ void small_group3(const Tables& T, uint32_t pos0, uin
     constexpr int W = 32 / PARTS;
     const int r = lane % W, p = lane / W;
     const double* __restrict__ dtab = T.dtab3;
-    const uint32_t S = vw_stride(gsize);
+    const uint32_t S = vw_stride(gsize, F32);
     for (uint32_t r0 = 0; r0 < cnt; r0 += W) {
         const bool valid = r0 + r < cnt;
         const uint32_t lo = (uint32_t)__ldg(recs + pos0 + (valid ? r0 + r : r0));
@@ -1044,8 +1044,8 @@ __device__ __forceinline__ void small_group3(const Tables& T, uint32_t pos0, uin
                         const bool on = row && k0 + u < nk;
                         const uint32_t cell = on ? c + (uint32_t)(k0 + u) : 0u;
                         ck[u] = on ? __ldg(ckp + k0 + u) : 0.0;
-                        const uint32_t lw = on ? __ldg(vwl + cell) : 0u, hw = on ? __ldg(vwl + gsize + cell) : 0u;
-                        v[u] = __hiloint2double((int)hw, (int)lw);
+                        const uint32_t lw = on ? __ldg(vwl + cell) : 0u, hw = (on && !F32) ? __ldg(vwl + gsize + cell) : 0u;
+                        v[u] = F32 ? (double)__uint_as_float(lw) : __hiloint2double((int)hw, (int)lw);
                     }
 #pragma unroll
                     for (int u = 0; u < 4; u++)
@@ -1067,6 +1067,7 @@ __device__ __forceinline__ void small_group3(const Tables& T, uint32_t pos0, uin
     }
 }
 
+template <bool F32>
 __global__ void __launch_bounds__(128) k_transform3_small(Tables T, const uint4* __restrict__ items, uint32_t last_slot,
                                                           const uint32_t* __restrict__ n_items_p,
                                                           const unsigned long long* __restrict__ recs, double* __restrict__ out)
@@ -1102,8 +1103,8 @@ __global__ void __launch_bounds__(128) k_transform3_small(Tables T, const uint4*
             if (lane >= off) iv += x;
         }
         const uint32_t* __restrict__ vw = T.vw20 + (size_t)sg.z * 4;
-        if (cnt <= SMALL_SPLIT) small_group3<4>(T, pos0, cnt, nblk, ib, ik, iv - vv, (uint32_t)kb.x, (uint32_t)kk.x, vw, sg.y, recs, out, lane);
-        else small_group3<1>(T, pos0, cnt, nblk, ib, ik, iv - vv, (uint32_t)kb.x, (uint32_t)kk.x, vw, sg.y, recs, out, lane);
+        if (cnt <= SMALL_SPLIT) small_group3<4, F32>(T, pos0, cnt, nblk, ib, ik, iv - vv, (uint32_t)kb.x, (uint32_t)kk.x, vw, sg.y, recs, out, lane);
+        else small_group3<1, F32>(T, pos0, cnt, nblk, ib, ik, iv - vv, (uint32_t)kb.x, (uint32_t)kk.x, vw, sg.y, recs, out, lane);
     }
 }
 
@@ -1176,9 +1177,15 @@ struct __align__(16) Pipe3 {
 
 // one Vw value from its two staged 32-bit words: `lo` / `hi` are shared-space byte addresses of word 0 of the low / high plane
 // of the record's bin, OFF the compile-time word offset of the cell
-template <int OFF>
+// F32 (fp32-stored slabs, MFDN_OPT_SLAB_FP32): one word per value at `lo`, widened to fp64; `hi` is unused
+template <int OFF, bool F32>
 __device__ __forceinline__ double ldvw(uint32_t lo, uint32_t hi)
 {
+    if constexpr (F32) {
+        float f;
+        asm("ld.shared.f32 %0, [%1+%2];" : "=f"(f) : "r"(lo), "n"(OFF * 4));
+        return (double)f;
+    }
     uint32_t a, b;
     asm("ld.shared.u32 %0, [%1+%2];" : "=r"(a) : "r"(lo), "n"(OFF * 4));
     asm("ld.shared.u32 %0, [%1+%2];" : "=r"(b) : "r"(hi), "n"(OFF * 4));
@@ -1207,27 +1214,27 @@ __device__ __forceinline__ void ldcoef(const double* __restrict__ p, double (&c)
 // (bq, kq: the J block of the bra / ket tuple's coefficient table), Vw rows (padded to even length) read from the staged
 // word planes at vi + i * P + k.  Bra and ket range sizes known at compile time: every load of the block is issued before
 // the first multiply, the loop control is shared by the two records.
-template <int NB, int NK, int I>
+template <int NB, int NK, int I, bool F32>
 __device__ __forceinline__ void vw_row(uint32_t lo, uint32_t hi, double (&v)[NK])
 {
     constexpr int P = (NK + 1) & ~1;
-    if constexpr (NK >= 1) v[0] = ldvw<I * P + 0>(lo, hi);
-    if constexpr (NK >= 2) v[1] = ldvw<I * P + 1>(lo, hi);
-    if constexpr (NK >= 3) v[2] = ldvw<I * P + 2>(lo, hi);
-    if constexpr (NK >= 4) v[3] = ldvw<I * P + 3>(lo, hi);
-    if constexpr (NK >= 5) v[4] = ldvw<I * P + 4>(lo, hi);
-    if constexpr (NK >= 6) v[5] = ldvw<I * P + 5>(lo, hi);
-    if constexpr (NK >= 7) v[6] = ldvw<I * P + 6>(lo, hi);
-    if constexpr (NK >= 8) v[7] = ldvw<I * P + 7>(lo, hi);
+    if constexpr (NK >= 1) v[0] = ldvw<I * P + 0, F32>(lo, hi);
+    if constexpr (NK >= 2) v[1] = ldvw<I * P + 1, F32>(lo, hi);
+    if constexpr (NK >= 3) v[2] = ldvw<I * P + 2, F32>(lo, hi);
+    if constexpr (NK >= 4) v[3] = ldvw<I * P + 3, F32>(lo, hi);
+    if constexpr (NK >= 5) v[4] = ldvw<I * P + 4, F32>(lo, hi);
+    if constexpr (NK >= 6) v[5] = ldvw<I * P + 5, F32>(lo, hi);
+    if constexpr (NK >= 7) v[6] = ldvw<I * P + 6, F32>(lo, hi);
+    if constexpr (NK >= 8) v[7] = ldvw<I * P + 7, F32>(lo, hi);
 }
-template <int NB, int NK, int I>
+template <int NB, int NK, int I, bool F32>
 __device__ __forceinline__ void j_rows(const double (&ckA)[NK], const double (&ckB)[NK], const double (&cbA)[NB], const double (&cbB)[NB],
                                        uint32_t loA, uint32_t hiA, uint32_t loB, uint32_t hiB, double& tA, double& tB)
 {
     if constexpr (I < NB) {
         double vA[NK], vB[NK];
-        vw_row<NB, NK, I>(loA, hiA, vA);
-        vw_row<NB, NK, I>(loB, hiB, vB);
+        vw_row<NB, NK, I, F32>(loA, hiA, vA);
+        vw_row<NB, NK, I, F32>(loB, hiB, vB);
         double accA = ckA[0] * vA[0], accB = ckB[0] * vB[0];
 #pragma unroll
         for (int k = 1; k < NK; k++) {
@@ -1236,12 +1243,12 @@ __device__ __forceinline__ void j_rows(const double (&ckA)[NK], const double (&c
         }
         tA = fma(cbA[I], accA, tA);
         tB = fma(cbB[I], accB, tB);
-        j_rows<NB, NK, I + 1>(ckA, ckB, cbA, cbB, loA, hiA, loB, hiB, tA, tB);
+        j_rows<NB, NK, I + 1, F32>(ckA, ckB, cbA, cbB, loA, hiA, loB, hiB, tA, tB);
     }
 }
 // boff / koff: offsets (doubles) of the J block in the bra / ket tuple's coefficient table; loA.. : shared-space byte addresses
 // of the block's first Vw cell in the low / high word plane of record A's / B's bin
-template <int NB, int NK>
+template <int NB, int NK, bool F32>
 __device__ __forceinline__ void j_block3x2(const double* __restrict__ dtab, uint32_t boff, uint32_t koff, uint32_t sbA,
                                            uint32_t skA, uint32_t sbB, uint32_t skB, uint32_t loA, uint32_t hiA, uint32_t loB, uint32_t hiB,
                                            double& totA, double& totB)
@@ -1252,12 +1259,12 @@ __device__ __forceinline__ void j_block3x2(const double* __restrict__ dtab, uint
     ldcoef<NB>(dtab + (boff + sbA * NB), cbA);
     ldcoef<NB>(dtab + (boff + sbB * NB), cbB);
     double tA = 0.0, tB = 0.0;
-    j_rows<NB, NK, 0>(ckA, ckB, cbA, cbB, loA, hiA, loB, hiB, tA, tB);
+    j_rows<NB, NK, 0, F32>(ckA, ckB, cbA, cbB, loA, hiA, loB, hiB, tA, tB);
     totA += tA;
     totB += tB;
 }
 // The same with a run-time loop over the bra rows (blocks with more than 4 rows or columns, NK <= 8)
-template <int NK>
+template <int NK, bool F32>
 __device__ __forceinline__ void j_block3x2_rows(const double* __restrict__ dtab, uint32_t boff, uint32_t koff, uint32_t sbA,
                                                 uint32_t skA, uint32_t sbB, uint32_t skB, int nb, uint32_t loA, uint32_t hiA, uint32_t loB,
                                                 uint32_t hiB, double& totA, double& totB)
@@ -1273,8 +1280,8 @@ __device__ __forceinline__ void j_block3x2_rows(const double* __restrict__ dtab,
     for (int i = 0; i < nb; i++) {
         const double cbA = __ldg(bA + i), cbB = __ldg(bB + i);
         double vA[NK], vB[NK];
-        vw_row<1, NK, 0>(loA, hiA, vA);
-        vw_row<1, NK, 0>(loB, hiB, vB);
+        vw_row<1, NK, 0, F32>(loA, hiA, vA);
+        vw_row<1, NK, 0, F32>(loB, hiB, vB);
         loA += P * 4; hiA += P * 4; loB += P * 4; hiB += P * 4;
         double accA = ckA[0] * vA[0], accB = ckB[0] * vB[0];
 #pragma unroll
@@ -1291,7 +1298,7 @@ __device__ __forceinline__ void j_block3x2_rows(const double* __restrict__ dtab,
 
 // any ket range size (nk > 8): ket coefficient re-read per cell
 __device__ __noinline__ double j_block3_generic(const double* __restrict__ bp, const double* __restrict__ kp, int nb, int nk, uint32_t lo,
-                                                uint32_t hi)
+                                                uint32_t hi, bool f32)
 {
     const int P = row_pitch3(nk);
     double total = 0.0;
@@ -1299,10 +1306,10 @@ __device__ __noinline__ double j_block3_generic(const double* __restrict__ bp, c
         const double cb = __ldg(bp + i);
         double acc = 0.0;
         for (int k = 0; k < nk; k++) {
-            uint32_t a, b;
+            uint32_t a, b = 0u;
             asm("ld.shared.u32 %0, [%1];" : "=r"(a) : "r"(lo + 4u * k));
-            asm("ld.shared.u32 %0, [%1];" : "=r"(b) : "r"(hi + 4u * k));
-            const double ck = __ldg(kp + k), v = __hiloint2double((int)b, (int)a);
+            if (!f32) asm("ld.shared.u32 %0, [%1];" : "=r"(b) : "r"(hi + 4u * k));
+            const double ck = __ldg(kp + k), v = f32 ? (double)__uint_as_float(a) : __hiloint2double((int)b, (int)a);
             acc = k ? fma(ck, v, acc) : ck * v;
         }
         total = fma(cb, acc, total);
@@ -1326,6 +1333,7 @@ __device__ __noinline__ double j_block3_generic(const double* __restrict__ bp, c
 //    for its records with warp-uniform loop bounds (first J block = the smallest |M| in the warp; coefficients are 0
 //    for J < |M|), and stores the signed value at the record's stream position (coalesced).
 // No block-wide barrier after the prologue.
+template <bool F32>
 __global__ void __launch_bounds__(TR_THREADS, MFDN_TR_MINB) k_transform3(Tables T, const uint4* __restrict__ items, const uint32_t* __restrict__ n_items_p,
                                                                      const unsigned long long* __restrict__ recs, double* __restrict__ out)
 {
@@ -1391,7 +1399,7 @@ __global__ void __launch_bounds__(TR_THREADS, MFDN_TR_MINB) k_transform3(Tables 
             e0 = e1;
             const uint32_t pos0 = cur.x, cnt = cur.y, g = cur.z;
             const bool zero = g == ZERO_ITEM;
-            const uint32_t gsize = sg.y, S = vw_stride(gsize), bin_lo = cur.w & 255u, bins = cur.w >> 8;
+            const uint32_t gsize = sg.y, S = vw_stride(gsize, F32), bin_lo = cur.w & 255u, bins = cur.w >> 8;
             const uint32_t vw_words = zero ? 0u : (bins * S + 3u) & ~3u;
             const uint32_t rec_words = zero ? 0u : (((pos0 & 1u) + cnt + 1u) & ~1u) * 2u;
             const uint32_t need = vw_words + rec_words + (uint32_t)gnblk * 4u;
@@ -1517,8 +1525,8 @@ __global__ void __launch_bounds__(TR_THREADS, MFDN_TR_MINB) k_transform3(Tables 
                     }
 #endif
                     const uint32_t vlA = wA + d.w * 4u, vlB = wB + d.w * 4u, vhA = vlA + G4, vhB = vlB + G4;
-#define MFDN_BLK(NB, NK) case ((NB) - 1) * 4 + ((NK) - 1): j_block3x2<NB, NK>(dtab, d.y, d.z, sbA, skA, sbB, skB, vlA, vhA, vlB, vhB, totA, totB); break;
-#define MFDN_ROWS(NK) case 16 + (NK): j_block3x2_rows<NK>(dtab, d.y, d.z, sbA, skA, sbB, skB, nb, vlA, vhA, vlB, vhB, totA, totB); break;
+#define MFDN_BLK(NB, NK) case ((NB) - 1) * 4 + ((NK) - 1): j_block3x2<NB, NK, F32>(dtab, d.y, d.z, sbA, skA, sbB, skB, vlA, vhA, vlB, vhB, totA, totB); break;
+#define MFDN_ROWS(NK) case 16 + (NK): j_block3x2_rows<NK, F32>(dtab, d.y, d.z, sbA, skA, sbB, skB, nb, vlA, vhA, vlB, vhB, totA, totB); break;
                     switch (d.x >> 16) {
                         MFDN_BLK(1, 1) MFDN_BLK(1, 2) MFDN_BLK(1, 3) MFDN_BLK(1, 4)
                         MFDN_BLK(2, 1) MFDN_BLK(2, 2) MFDN_BLK(2, 3) MFDN_BLK(2, 4)
@@ -1527,8 +1535,8 @@ __global__ void __launch_bounds__(TR_THREADS, MFDN_TR_MINB) k_transform3(Tables 
                         MFDN_ROWS(1) MFDN_ROWS(2) MFDN_ROWS(3) MFDN_ROWS(4) MFDN_ROWS(5) MFDN_ROWS(6) MFDN_ROWS(7) MFDN_ROWS(8)
                         default: {
                             if (nk > 0 && nb > 0) {
-                                totA += j_block3_generic(dtab + (d.y + sbA * (uint32_t)nb), dtab + (d.z + skA * (uint32_t)nk), nb, nk, vlA, vhA);
-                                totB += j_block3_generic(dtab + (d.y + sbB * (uint32_t)nb), dtab + (d.z + skB * (uint32_t)nk), nb, nk, vlB, vhB);
+                                totA += j_block3_generic(dtab + (d.y + sbA * (uint32_t)nb), dtab + (d.z + skA * (uint32_t)nk), nb, nk, vlA, vhA, F32);
+                                totB += j_block3_generic(dtab + (d.y + sbB * (uint32_t)nb), dtab + (d.z + skB * (uint32_t)nk), nb, nk, vlB, vhB, F32);
                             }
                             break;
                         }
@@ -1558,6 +1566,12 @@ __global__ void __launch_bounds__(TR_THREADS, MFDN_TR_MINB) k_transform3(Tables 
 // mu' tiles.  Pays only where most pairs of a block are requested (config 2, "ALL pairs"); see DESIGN.md for the
 // measured break-even.  Summation order differs from the direct kernels: values agree to rounding, not bitwise.
 constexpr int DN_WARPS = 4;
+// one value of an isospin-combined slab from global memory (bin base vwb), either storage width
+__device__ __forceinline__ double ldvw_global(const uint32_t* __restrict__ vwb, uint32_t gsize, uint32_t cell, int f32)
+{
+    if (f32) return (double)__uint_as_float(__ldg(vwb + cell));
+    return __hiloint2double((int)__ldg(vwb + gsize + cell), (int)__ldg(vwb + cell));
+}
 constexpr int DN_CHUNKS = DENSE_RMAX / 4;
 struct DenseWarp3 {
     double vm[DENSE_CAP];
@@ -1611,7 +1625,7 @@ __global__ void __launch_bounds__(DN_WARPS * 32) k_dense3(Tables T, const uint4*
         for (uint32_t i = lane; i < cnt; i += 32) bits |= 1u << ((uint32_t)(__ldg(recs + pos0 + i) >> 24) & 31u);
         bits = __reduce_or_sync(0xFFFFFFFFu, bits);
         __syncwarp();
-        const uint32_t gsize = sg.y, S = vw_stride(gsize), ldv = (nmk + 7u) & ~7u;
+        const uint32_t gsize = sg.y, S = vw_stride(gsize, T.vw_f32), ldv = (nmk + 7u) & ~7u;
         const int nchunk = (int)((R + 3u) >> 2);
         const uint32_t mrow = (uint32_t)lane >> 2, kcol = (uint32_t)lane & 3u;
         for (uint32_t bin = 0; bin < (uint32_t)NBIN3; bin++) {
@@ -1632,7 +1646,7 @@ __global__ void __launch_bounds__(DN_WARPS * 32) k_dense3(Tables T, const uint4*
                         double t = 0.0;
                         for (uint32_t i = 0; i < nb; i++) {
                             const uint32_t cell = e.z + i * P;
-                            t = fma(__ldg(cb + i), __hiloint2double((int)__ldg(vwb + gsize + cell), (int)__ldg(vwb + cell)), t);
+                            t = fma(__ldg(cb + i), ldvw_global(vwb, gsize, cell, T.vw_f32), t);
                         }
                         a[c] = t;
                     }
@@ -1756,7 +1770,7 @@ __global__ void __launch_bounds__(DN_WARPS * 32) k_block3(Tables T, const BlockI
                 rmap[ir - rk + k] = make_uint4((uint32_t)kb.x + (uint32_t)jb.x, (uint32_t)jb.y | ((uint32_t)jk.y << 8) | ((uint32_t)k << 16),
                                                iv - vv + (uint32_t)k, (uint32_t)kk.x + (uint32_t)jk.x);
         __syncwarp();
-        const uint32_t gsize = sg.y, S = vw_stride(gsize);
+        const uint32_t gsize = sg.y, S = vw_stride(gsize, T.vw_f32);
         const int nchunk = (int)((R + 3u) >> 2);
         const uint32_t mrow = (uint32_t)lane >> 2, kcol = (uint32_t)lane & 3u;
         {
@@ -1777,7 +1791,7 @@ __global__ void __launch_bounds__(DN_WARPS * 32) k_block3(Tables T, const BlockI
                         double t = 0.0;
                         for (uint32_t i = 0; i < nb; i++) {
                             const uint32_t cell = e.z + i * P;
-                            t = fma(__ldg(cb + i), __hiloint2double((int)__ldg(vwb + gsize + cell), (int)__ldg(vwb + cell)), t);
+                            t = fma(__ldg(cb + i), ldvw_global(vwb, gsize, cell, T.vw_f32), t);
                         }
                         a[c] = t;
                     }
@@ -2054,18 +2068,20 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
             uint4* ditm = (uint4*)(w + o_ditems);
             const uint32_t last_slot = (uint32_t)(max_items - 1);
             k_items3<<<(unsigned)((nt * nt + 1 + 255) / 256), 256, 0, st>>>(hist, c->t.gbase3, (uint32_t)(nt * nt), (uint32_t)n_buckets, sort ? 1 : 0,
-                                                                             (uint32_t)n, c->t.sgrp3, itm, last_slot, cnt, dense ? 0.f : -1.f, ditm);
+                                                                             (uint32_t)n, c->t.sgrp3, itm, last_slot, cnt, dense ? 0.f : -1.f, ditm, c->t.vw_f32);
             if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.b, st));
             int per_sm = c->tr_blocks_per_sm.load();
             if (per_sm == 0) {   // benign if two threads do it at once: both store the same number
-                MFDN_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_transform3, TR_THREADS, 0));
+                MFDN_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_transform3<false>, TR_THREADS, 0));
                 per_sm = std::max(per_sm, 1);
                 c->tr_blocks_per_sm.store(per_sm);
             }
             const unsigned grid = (unsigned)std::min<long long>(max_items, (long long)c->num_sms * per_sm);
-            k_transform3<<<grid, TR_THREADS, 0, st>>>(c->t, itm, cnt, trecs, tout);
+            if (c->t.vw_f32) k_transform3<true><<<grid, TR_THREADS, 0, st>>>(c->t, itm, cnt, trecs, tout);
+            else k_transform3<false><<<grid, TR_THREADS, 0, st>>>(c->t, itm, cnt, trecs, tout);
             const unsigned grid_s = (unsigned)std::min<long long>((std::min<long long>(n, nt * nt + 1) + 3) / 4, (long long)c->num_sms * 16);
-            k_transform3_small<<<grid_s, 128, 0, st>>>(c->t, itm, last_slot, cnt, trecs, tout);
+            if (c->t.vw_f32) k_transform3_small<true><<<grid_s, 128, 0, st>>>(c->t, itm, last_slot, cnt, trecs, tout);
+            else k_transform3_small<false><<<grid_s, 128, 0, st>>>(c->t, itm, last_slot, cnt, trecs, tout);
             c->launches += 3;
             if (dense) {
                 const unsigned grid_d = (unsigned)std::min<long long>((max_ditems + DN_WARPS - 1) / DN_WARPS, (long long)c->num_sms * 8);

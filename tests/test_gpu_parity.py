@@ -638,3 +638,45 @@ def test_compact_u16_requests(torch, B, oracle, idx):
     h_out, h_mask = ctx.mscheme_host(torch.from_numpy(r16).pin_memory(), chunk=7000)
     check(cfg, h_out.numpy(), h_mask.numpy(), want, wmask)
 
+
+# --------------------------------------------------------------------------------- NEXT-4: fp32-stored slabs
+@pytest.mark.gpu
+@pytest.mark.parametrize("idx", [2, 3])
+def test_fp32_stored_slabs(torch, B, oracle, idx):
+    """MFDN_OPT_SLAB_FP32: the isospin-combined slabs are stored in fp32, sums stay fp64.  Mask bit-exact; values within the
+    bound the header states: a stored value is within 2^-24 * 5 max|V| of the fp64 one (five isospin terms, weights <= 1) and
+    a request sums at most `cells` of them with coefficient products <= 1.  Every path that reads the slabs is checked
+    (work-item kernel, small groups, dense blocks, block mode); the table memory shrinks as stated."""
+    cfg = get_cfg(idx)
+    ctx64 = get_ctx(B, idx)
+    ctx = B.Context(cfg.basis, 0).option(B.MFDN_OPT_SLAB_FP32).upload(cfg.table)
+    assert B.mfdn_info(ctx.ctx, 8) <= 0.6 * B.mfdn_info(ctx64.ctx, 8)      # half, up to the 16-byte rounding per group
+    with pytest.raises(B.MfdnError) as e:
+        ctx.option(B.MFDN_OPT_SLAB_FP32, 0)             # too late
+    assert e.value.code == B.MFDN_ERR_STATE
+    req = cfg.requests() if cfg.all_pairs else cfg.requests(1 << 18, permute_frac=0.01)
+    if len(req) > 300000:
+        req = req[np.random.default_rng(2).choice(len(req), 300000, replace=False)]
+    want, wmask, nt, _ = oracle.mscheme(cfg.basis, cfg.table, req)
+    vmax = float(np.max(np.abs(cfg.table.values)))
+    cells = max(1, int(np.max(nt)))                      # coupled terms of a request: upper bound for its cells
+    tol = 2.0 ** -24 * 5 * vmax * cells
+    worst = 0.0
+    for flags in (0, B.MFDN_ONE_PASS_SORT, B.MFDN_FORCE_DENSE):
+        got, gmask = run_gpu(torch, ctx, req, flags)
+        assert np.array_equal(gmask, wmask)
+        err = float(np.max(np.abs(got - want)))
+        assert err <= tol, (flags, err, tol)
+        assert np.all(got[gmask == 0] == 0.0)
+        worst = max(worst, err)
+    assert worst > 1e-11 * vmax                          # it really is the fp32-stored table
+    got, gmask = run_gpu(torch, ctx, req, B.MFDN_FORCE_NAIVE)    # reads the fp64 planes
+    check(cfg, got, gmask, want, wmask)
+    tup = sorted(set(zip(cfg.table.state_a.tolist(), cfg.table.state_b.tolist(), cfg.table.state_c.tolist())))
+    g = np.asarray([tup[3] + tup[5], tup[0] + tup[0]], np.int32)
+    a, off = ctx.blocks(g)
+    b, off64 = ctx64.blocks(g)
+    torch.cuda.synchronize()
+    assert np.array_equal(off, off64) and float((a - b).abs().max()) <= tol
+    ctx.close()
+
