@@ -56,9 +56,14 @@ enum {
                              shared memory.  The library takes this path by itself for tables with more than 2048 x 4096
                              sort buckets (2-body: orbital-tuple pairs; 3-body: (pair, M) combinations); the flag forces
                              it for any table (test hook and the measured baseline of DESIGN.md).  Same values bit for bit */
-    MFDN_REQ_U16 = 16      /* compact requests: d_req / h_req point to uint16 SPS indices, [n][4] or [n][6] (8 / 12 bytes per request
+    MFDN_REQ_U16 = 16,     /* compact requests: d_req / h_req point to uint16 SPS indices, [n][4] or [n][6] (8 / 12 bytes per request
                              instead of 16 / 24: half the host-to-device bytes of mfdn_mscheme_host, whose time is the PCIe
                              copy).  Needs n_sps <= 65536 (else MFDN_ERR_ARG); 4-byte aligned; same results bit for bit */
+    MFDN_FORCE_SORT = 32   /* take the group-sort path with the two-pass partition whatever the batch size.  Without a flag
+                             that names a path the library chooses by n (all paths give the same values bit for bit):
+                             2-body and small 3-body batches (the ~20 000-request chunks of PAPER.md:93) are evaluated
+                             thread-per-request like MFDN_FORCE_NAIVE, larger 3-body batches by the group sort, one-pass
+                             below 2^23 requests and two-pass above */
 };
 
 /* A0. Single-particle basis (quantum numbers flattened into one linear SPS index).

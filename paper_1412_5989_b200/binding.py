@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libmfdn_b200.so")
 
 MFDN_OK, MFDN_ERR_ARG, MFDN_ERR_STATE, MFDN_ERR_CUDA, MFDN_ERR_OOM, MFDN_ERR_TABLE = 0, -1, -2, -3, -4, -5
 MFDN_PRESORTED, MFDN_FORCE_NAIVE, MFDN_FORCE_DENSE, MFDN_ONE_PASS_SORT, MFDN_REQ_U16 = 1, 2, 4, 8, 16
+MFDN_FORCE_SORT = 32
 MFDN_OPT_SLAB_FP32 = 1
 
 # every symbol include/mfdn_b200.h declares

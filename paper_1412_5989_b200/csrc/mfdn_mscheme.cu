@@ -317,6 +317,9 @@ __global__ void __launch_bounds__(128) k_mscheme_naive(Tables T, long long n, co
 // and leaves the counts in tcnt[tile][bin] for the two-pass partition below (no global atomics for it).
 constexpr int KEYS_SPS_SMEM = 2048, KEYS_AB_SMEM = 2048, KEYS_PER_BLOCK = 256 * 32;
 constexpr int PART_NC = 2048;
+#ifndef MFDN_TWO_PASS_MIN
+#define MFDN_TWO_PASS_MIN (1ll << 23)   // requests from which the two-pass partition beats the one-pass scatter / gather
+#endif
 
 template <int BODY, bool AGG, bool SMEM>
 __global__ void __launch_bounds__(256) k_keys(Tables T, long long n, const int32_t* __restrict__ req,
@@ -1889,7 +1892,15 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
     // sort buckets: 2-body one per group, 3-body one per (group, M); last bucket: requests failing S1-S6
     const long long n_buckets = (BODY == 3 ? (long long)c->t.n_buckets3 : nt * nt) + 1;
     const long long n_tiles = (n_buckets + SCAN_TILE - 1) / SCAN_TILE;
-    const bool naive = flags & MFDN_FORCE_NAIVE;
+    // Path choice by batch size.  The paths give the same values bit for bit (same operations in the same order), so the choice
+    // is invisible in the results.  Thread-per-request (the paper's kernel) needs no sort and no per-table scans, whose cost
+    // is fixed per call (config 3: 150 us at any n); measured cross-overs on B200: 2-body: direct wins at every n up to 2^26
+    // (~6 terms per request: sorting costs more than it saves; 2.95 against 3.12 ms at 2^26); 3-body: direct below ~2^17
+    // requests, below ~2^20 if the 5-plane slabs fit L2 comfortably (config 2); then the one-pass scatter/gather up to
+    // 2^23 requests, the two-pass partition above.  Any flag that names a path overrides the choice.
+    const bool named = flags & (MFDN_PRESORTED | MFDN_FORCE_DENSE | MFDN_ONE_PASS_SORT | MFDN_FORCE_SORT);
+    const bool auto_direct = !named && (BODY == 2 || (!c->t.vw_f32 && n < ((c->slab_bytes3 <= (32ll << 20)) ? (1ll << 20) : (1ll << 17))));
+    const bool naive = (flags & MFDN_FORCE_NAIVE) || auto_direct;
     const bool sort = !naive && !(flags & MFDN_PRESORTED);
     const bool items = !naive && BODY == 3;    // the 3-body transform walks a list of one-group work items
     const bool hist_needed = sort || items;
@@ -1904,7 +1915,7 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
     while ((1ll << (2 * csh)) < n_buckets) csh++;
     csh = std::min(csh, 12);   // PART_NF = 4096 buckets per bin at most
     while (((n_buckets + (1ll << csh) - 1) >> csh) > PART_NC) csh++;
-    const bool two_pass = sort && csh <= 12 && !(flags & MFDN_ONE_PASS_SORT);
+    const bool two_pass = sort && csh <= 12 && !(flags & MFDN_ONE_PASS_SORT) && ((flags & MFDN_FORCE_SORT) || n >= MFDN_TWO_PASS_MIN);
     const int nc = (int)((n_buckets + (1ll << csh) - 1) >> csh);
     const long long n_ktiles = (n + KEYS_PER_BLOCK - 1) / KEYS_PER_BLOCK, n_chunks = (n_ktiles + TS_CHUNK - 1) / TS_CHUNK;
     const long long max_tiles2 = n_ktiles + nc;

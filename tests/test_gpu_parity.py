@@ -9,7 +9,8 @@ from paper_1412_5989_b200 import workloads as W
 pytestmark = pytest.mark.gpu
 
 TOL = 1e-12
-MODES = {"sorted_internally": 0, "naive": 2, "one_pass_sort": 8}
+# 0 = the library's own choice by batch size (thread-per-request for 2-body and small 3-body batches, group sort above)
+MODES = {"auto": 0, "naive": 2, "one_pass_sort": 8, "two_pass_sort": 32}
 
 
 @pytest.fixture(scope="module")
@@ -161,7 +162,7 @@ def test_edge_sizes_and_bad_indices(torch, B, oracle, idx):
     for n in (0, 1, 31, 32, 33, 127, 128, 129, 4097, 8191, 8192, 8193, 16385):
         req = allreq[rng.choice(len(allreq), n, replace=False)] if n else allreq[:0]
         want, wmask, _, _ = oracle.mscheme(cfg.basis, cfg.table, req)
-        for flags in (0, 2, 8):
+        for flags in (0, 2, 8, 32):
             got, gmask = run_gpu(torch, ctx, req, flags)
             check(cfg, got, gmask, want, wmask)
     # random (mostly forbidden) requests, duplicates inside bra/ket, and out-of-range SPS indices
@@ -175,14 +176,14 @@ def test_edge_sizes_and_bad_indices(torch, B, oracle, idx):
     got, gmask = run_gpu(torch, ctx, req, 2)
     check(cfg, got, gmask, want, wmask)
     assert ctx.bad_request_count() - before == nbad == 400
-    for flags in (0, 8):
+    for flags in (0, 8, 32):
         got, gmask = run_gpu(torch, ctx, req, flags)
         check(cfg, got, gmask, want, wmask)
     # one hot bucket: the same request many times over (every copy lands in one run of the partition), plus a few others
     req = np.concatenate([np.repeat(allreq[len(allreq) // 2][None, :], 30000, axis=0), allreq[rng.choice(len(allreq), 3000, replace=False)]])
     req = req[rng.permutation(len(req))]
     want, wmask, _, _ = oracle.mscheme(cfg.basis, cfg.table, req)
-    for flags in (0, 8):
+    for flags in (0, 8, 32):
         got, gmask = run_gpu(torch, ctx, req, flags)
         check(cfg, got, gmask, want, wmask)
     # mask pointer may be NULL
@@ -206,27 +207,30 @@ def test_order_chunk_and_stream_invariance(torch, B):
     req = cfg.requests()
     rng = np.random.default_rng(4)
     req = req[rng.choice(len(req), 200000, replace=False)]
-    base, bmask = run_gpu(torch, ctx, req, 0)
+    base, bmask = run_gpu(torch, ctx, req, B.MFDN_FORCE_SORT)
     perm = rng.permutation(len(req))
-    got, gmask = run_gpu(torch, ctx, req[perm], 0)
+    got, gmask = run_gpu(torch, ctx, req[perm], B.MFDN_FORCE_SORT)
     assert np.array_equal(got, base[perm]) and np.array_equal(gmask, bmask[perm])
-    naive, nmask = run_gpu(torch, ctx, req, 2)          # different kernel, different summation tree
-    assert np.max(np.abs(naive - base)) < 1e-13 and np.array_equal(nmask, bmask)
-    # chunks of ~20 000 (the paper's buffer size) on two streams
+    # every path does the same operations in the same order: the library's choice of path by batch size is invisible
+    for flags in (0, B.MFDN_FORCE_NAIVE, B.MFDN_ONE_PASS_SORT):
+        other, omask = run_gpu(torch, ctx, req, flags)
+        assert np.array_equal(other, base) and np.array_equal(omask, bmask), flags
+    # chunks of ~20 000 (the paper's buffer size) on two streams, by the library's choice and by the sort path
     d_req = torch.from_numpy(req).cuda()
-    out = torch.empty(len(req), dtype=torch.float64, device="cuda")
-    mask = torch.empty(len(req), dtype=torch.uint8, device="cuda")
-    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
-    need = ctx.work_bytes(3, 20000)
-    works = [torch.empty(need, dtype=torch.uint8, device="cuda") for _ in streams]
-    torch.cuda.synchronize()
-    for k, lo in enumerate(range(0, len(req), 20000)):
-        hi = min(lo + 20000, len(req))
-        s = streams[k % 2]
-        with torch.cuda.stream(s):
-            ctx.mscheme(d_req[lo:hi], out[lo:hi], mask[lo:hi], 0, works[k % 2], s.cuda_stream)
-    torch.cuda.synchronize()
-    assert np.array_equal(out.cpu().numpy(), base) and np.array_equal(mask.cpu().numpy(), bmask)
+    for flags in (0, B.MFDN_FORCE_SORT):
+        out = torch.empty(len(req), dtype=torch.float64, device="cuda")
+        mask = torch.empty(len(req), dtype=torch.uint8, device="cuda")
+        streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+        need = ctx.work_bytes(3, 20000, flags)
+        works = [torch.empty(need, dtype=torch.uint8, device="cuda") for _ in streams]
+        torch.cuda.synchronize()
+        for k, lo in enumerate(range(0, len(req), 20000)):
+            hi = min(lo + 20000, len(req))
+            s = streams[k % 2]
+            with torch.cuda.stream(s):
+                ctx.mscheme(d_req[lo:hi], out[lo:hi], mask[lo:hi], flags, works[k % 2], s.cuda_stream)
+        torch.cuda.synchronize()
+        assert np.array_equal(out.cpu().numpy(), base) and np.array_equal(mask.cpu().numpy(), bmask)
 
 
 def test_call_order_and_table_validation(torch, B):
@@ -335,7 +339,7 @@ def _check_all_modes(torch, B, oracle, basis, table, req):
     ctx = B.Context(basis, 0).upload(table)
     want, wmask, _, _ = oracle.mscheme(basis, table, req)
     assert wmask.mean() > 0.5
-    for flags in (0, B.MFDN_FORCE_NAIVE, B.MFDN_FORCE_DENSE):
+    for flags in (0, B.MFDN_FORCE_SORT, B.MFDN_ONE_PASS_SORT, B.MFDN_FORCE_NAIVE, B.MFDN_FORCE_DENSE):
         got, gmask = run_gpu(torch, ctx, req, flags)
         check(cfg, got, gmask, want, wmask)
     sreq, order = presort(torch, ctx, req)
@@ -376,12 +380,16 @@ def test_full_size_config1_sampled(torch, B, oracle):
     n = 1 << 26
     req = cfg.requests(n)
     d_req = torch.from_numpy(req).cuda()
-    out, mask = ctx.mscheme(d_req, flags=0)
+    out, mask = ctx.mscheme(d_req, flags=0)                      # the library's choice: thread-per-request for 2-body
     torch.cuda.synchronize()
     sample = np.sort(np.random.default_rng(78).choice(n, 1 << 16, replace=False))
     want, wmask, _, _ = oracle.mscheme(cfg.basis, cfg.table, req[sample])
     ds = torch.from_numpy(sample).cuda()
     check(cfg, out[ds].cpu().numpy(), mask[ds].cpu().numpy(), want, wmask)
+    out_s, mask_s = ctx.mscheme(d_req, flags=B.MFDN_FORCE_SORT)   # group sort, two-pass partition
+    torch.cuda.synchronize()
+    assert bool((out_s == out).all()) and bool((mask_s == mask).all())
+    del out_s, mask_s
     assert 0.93 < float(mask.float().mean()) < 0.955       # ~94.3% of sampled pairs have mask 1
     assert bool((out[mask == 0] == 0).all())
     keys = ctx.group_keys(d_req)
@@ -444,11 +452,12 @@ def test_multi_client_threads(torch, B):
     req = cfg.requests()
     rng = np.random.default_rng(14)
     req = req[rng.choice(len(req), 400000, replace=False)]
-    base, bmask = run_gpu(torch, ctx, req, 0)
+    base, bmask = run_gpu(torch, ctx, req, B.MFDN_FORCE_SORT)
     d_req = torch.from_numpy(req).cuda()
     out = torch.empty(len(req), dtype=torch.float64, device="cuda")
     mask = torch.empty(len(req), dtype=torch.uint8, device="cuda")
     chunk, nthreads = 20000, 4
+    call_flags = [0, B.MFDN_FORCE_SORT]      # thread t uses call_flags[t % 2]: the library's choice and the sort path side by side
     chunks = [(lo, min(lo + chunk, len(req))) for lo in range(0, len(req), chunk)]
     errors = []
     torch.cuda.synchronize()
@@ -458,10 +467,10 @@ def test_multi_client_threads(torch, B):
         try:
             torch.cuda.set_device(0)
             s = torch.cuda.Stream()
-            work = torch.empty(ctx.work_bytes(3, chunk), dtype=torch.uint8, device="cuda")
+            work = torch.empty(ctx.work_bytes(3, chunk, call_flags[t % 2]), dtype=torch.uint8, device="cuda")
             for k in range(t, len(chunks), nthreads):
                 lo, hi = chunks[k]
-                ctx.mscheme(d_req[lo:hi], out[lo:hi], mask[lo:hi], 0, work, s.cuda_stream)
+                ctx.mscheme(d_req[lo:hi], out[lo:hi], mask[lo:hi], call_flags[t % 2], work, s.cuda_stream)
             s.synchronize()
         except Exception as e:      # noqa: BLE001 - reported by the main thread
             errors.append(e)
@@ -503,7 +512,7 @@ def test_accumulate_epilogue(torch, B, oracle, idx):
         tol = TOL * float(np.max(np.abs(cfg.table.values))) * m
         d_req = torch.from_numpy(np.ascontiguousarray(req, np.int32)).cuda()
         d_loc, d_phase = torch.from_numpy(loc).cuda(), torch.from_numpy(phase).cuda()
-        for flags, ph in ((0, True), (0, False), (B.MFDN_ONE_PASS_SORT, True), (B.MFDN_FORCE_NAIVE, True)):
+        for flags, ph in ((0, True), (B.MFDN_FORCE_SORT, True), (B.MFDN_FORCE_SORT, False), (B.MFDN_ONE_PASS_SORT, True), (B.MFDN_FORCE_NAIVE, True)):
             H0 = rng.standard_normal(h_len)     # the target is updated, not overwritten
             d_H = torch.from_numpy(H0.copy()).cuda()
             mask = ctx.accumulate(d_req, d_loc, d_phase if ph else None, d_H, flags=flags)
@@ -628,13 +637,13 @@ def test_compact_u16_requests(torch, B, oracle, idx):
     want, wmask, _, nbad = oracle.mscheme(cfg.basis, cfg.table, req)
     r16 = np.ascontiguousarray(req.astype(np.uint16))
     before = ctx.bad_request_count()
-    for flags in (0, B.MFDN_ONE_PASS_SORT, B.MFDN_FORCE_NAIVE):
+    for flags in (0, B.MFDN_FORCE_SORT, B.MFDN_ONE_PASS_SORT, B.MFDN_FORCE_NAIVE):
         got32, m32 = run_gpu(torch, ctx, req, flags)
         out, mask = ctx.mscheme(torch.from_numpy(r16).cuda(), flags=flags)
         torch.cuda.synchronize()
         assert np.array_equal(out.cpu().numpy(), got32) and np.array_equal(mask.cpu().numpy(), m32)
         check(cfg, out.cpu().numpy(), mask.cpu().numpy(), want, wmask)
-    assert ctx.bad_request_count() - before == 6 * nbad == 300
+    assert ctx.bad_request_count() - before == 8 * nbad == 400
     h_out, h_mask = ctx.mscheme_host(torch.from_numpy(r16).pin_memory(), chunk=7000)
     check(cfg, h_out.numpy(), h_mask.numpy(), want, wmask)
 
@@ -662,7 +671,7 @@ def test_fp32_stored_slabs(torch, B, oracle, idx):
     cells = max(1, int(np.max(nt)))                      # coupled terms of a request: upper bound for its cells
     tol = 2.0 ** -24 * 5 * vmax * cells
     worst = 0.0
-    for flags in (0, B.MFDN_ONE_PASS_SORT, B.MFDN_FORCE_DENSE):
+    for flags in (0, B.MFDN_FORCE_SORT, B.MFDN_ONE_PASS_SORT, B.MFDN_FORCE_DENSE):
         got, gmask = run_gpu(torch, ctx, req, flags)
         assert np.array_equal(gmask, wmask)
         err = float(np.max(np.abs(got - want)))
