@@ -85,7 +85,7 @@ struct Side2 {
 };
 
 template <bool SMEM>
-__device__ __forceinline__ Side2 decode2(const Tables& T, const uint32_t* sps, int s0, int s1)
+__device__ __forceinline__ Side2 decode2(const Tables& T, const uint32_t* sps, int s0, int s1, const int32_t* s_tid = nullptr)
 {
     Side2 S;
     uint32_t r0 = SMEM ? sps[s0] : __ldg(sps + s0), r1 = SMEM ? sps[s1] : __ldg(sps + s1);
@@ -93,7 +93,7 @@ __device__ __forceinline__ Side2 decode2(const Tables& T, const uint32_t* sps, i
     S.distinct = s0 != s1;
     S.sign = 1;
     cswap(k0, k1, r0, r1, S.sign);
-    S.tup = __ldg(T.tuple_id2 + rec_orb(r0) * T.n_orb + rec_orb(r1));
+    S.tup = s_tid ? s_tid[rec_orb(r0) * T.n_orb + rec_orb(r1)] : __ldg(T.tuple_id2 + rec_orb(r0) * T.n_orb + rec_orb(r1));
     S.ima = rec_im(r0); S.imb = rec_im(r1);
     S.tz = (rec_tz(r0) << 1) | rec_tz(r1);
     const uint32_t sum = (r0 >> 10) + (r1 >> 10);
@@ -255,21 +255,24 @@ __device__ __forceinline__ double eval3_naive(const Tables& T, const Side3& B, c
     return (B.sign * K.sign) * total;
 }
 
-__device__ __forceinline__ double eval2_naive(const Tables& T, const Side2& B, const Side2& K, int& mask)
+// s_desc / s_c1off: the tuple descriptors and the stage-1 block offsets in shared memory, or NULL (a variant of the kernel
+// below with these tables, the SPS records and the tuple map in shared memory ran no faster: 2.69 ms either way at 2^26)
+__device__ __forceinline__ double eval2_naive(const Tables& T, const Side2& B, const Side2& K, int& mask, const int4* s_desc = nullptr,
+                                              const int32_t* s_c1off = nullptr)
 {
     mask = 0;
     if (!select2(B, K)) return 0.0;
+    const int4 db = s_desc ? s_desc[B.tup] : __ldg(T.tdesc2 + B.tup), dk = s_desc ? s_desc[K.tup] : __ldg(T.tdesc2 + K.tup);
+    if (!mask2(B, db, dk)) return 0.0;   // implies a common J, i.e. a slab
     const uint32_t so = __ldg(T.slab_off2 + (size_t)B.tup * T.n_tup2 + K.tup);
-    if (so == NO_SLAB) return 0.0;
-    const int4 db = __ldg(T.tdesc2 + B.tup), dk = __ldg(T.tdesc2 + K.tup);
-    if (!mask2(B, db, dk)) return 0.0;
     mask = 1;
     const int ja = db.x & 255, jb = (db.x >> 8) & 255, jc = dk.x & 255, jd = (dk.x >> 8) & 255;
     const double w0 = T.iso2[B.tz][0] * T.iso2[K.tz][0], w1 = T.iso2[B.tz][1] * T.iso2[K.tz][1];
     const int nj = T.nj;
     const int Jminb = db.y & 255, Jmink = dk.y & 255;
-    const double* cb = T.cg1 + __ldg(T.cg1_off + (ja >> 1) * nj + (jb >> 1)) + B.ima * (jb + 1) + B.imb;
-    const double* ck = T.cg1 + __ldg(T.cg1_off + (jc >> 1) * nj + (jd >> 1)) + K.ima * (jd + 1) + K.imb;
+    const int ob = (ja >> 1) * nj + (jb >> 1), ok = (jc >> 1) * nj + (jd >> 1);
+    const double* cb = T.cg1 + (s_c1off ? s_c1off[ob] : __ldg(T.cg1_off + ob)) + B.ima * (jb + 1) + B.imb;
+    const double* ck = T.cg1 + (s_c1off ? s_c1off[ok] : __ldg(T.cg1_off + ok)) + K.ima * (jd + 1) + K.imb;
     const int Sb = (ja + 1) * (jb + 1), Sk = (jc + 1) * (jd + 1);
     const int Jlo = max(Jminb, Jmink), Jhi = min((db.y >> 8) & 255, (dk.y >> 8) & 255);
     const double2* cell = (const double2*)(T.slab2 + (size_t)so * CELL2);
