@@ -61,9 +61,9 @@ enum {
                              copy).  Needs n_sps <= 65536 (else MFDN_ERR_ARG); 4-byte aligned; same results bit for bit */
     MFDN_FORCE_SORT = 32   /* take the group-sort path with the two-pass partition whatever the batch size.  Without a flag
                              that names a path the library chooses by n (all paths give the same values bit for bit):
-                             2-body and small 3-body batches (the ~20 000-request chunks of PAPER.md:93) are evaluated
-                             thread-per-request like MFDN_FORCE_NAIVE, larger 3-body batches by the group sort, one-pass
-                             below 2^23 requests and two-pass above */
+                             2-body batches and 3-body batches of up to 2^20 requests (the ~20 000-request chunks of
+                             PAPER.md:93) are evaluated thread-per-request on the library's tables, larger 3-body batches
+                             by the group sort, one-pass below 2^23 requests and two-pass above */
 };
 
 /* A0. Single-particle basis (quantum numbers flattened into one linear SPS index).

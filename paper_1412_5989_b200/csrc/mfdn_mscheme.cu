@@ -185,6 +185,13 @@ __device__ __forceinline__ void load_req2(const int32_t* req, long long r, int s
     s[0] = a.x; s[1] = a.y; s[2] = a.z; s[3] = a.w;
 }
 
+// one value of an isospin-combined slab from global memory (bin base vwb), either storage width
+__device__ __forceinline__ double ldvw_global(const uint32_t* __restrict__ vwb, uint32_t gsize, uint32_t cell, int f32)
+{
+    if (f32) return (double)__uint_as_float(__ldg(vwb + cell));
+    return __hiloint2double((int)__ldg(vwb + gsize + cell), (int)__ldg(vwb + cell));
+}
+
 // =============================================================================== naive kernel
 // MFDN_FORCE_NAIVE: the paper's design -- one thread per request, in request order, the
 // loop nest inside the kernel, every index recomputed per thread.  Kept as the on-device reference.
@@ -310,6 +317,74 @@ __global__ void __launch_bounds__(128) k_mscheme_naive(Tables T, long long n, co
     if (maskout) maskout[i] = (uint8_t)mask;
 }
 
+// 3-body, thread per request on the library's own tables: the coefficient products dtab3 and the isospin-combined slabs vw20
+// instead of two CG factors and five planes per term (3 loads per cell instead of 7).  This is what the library takes by
+// itself for small 3-body batches (chunks of ~20 000 requests), where the group sort's per-call cost (memset and
+// scan of all sort buckets, the pass over all n_tup^2 groups) exceeds the work.  Same operations in the same order as
+// small_group3 / k_transform3 (and hence as k_mscheme_naive): bit-identical values.
+__global__ void __launch_bounds__(128) k_direct3(Tables T, long long n, const int32_t* __restrict__ req, double* __restrict__ out,
+                                                uint8_t* __restrict__ maskout, int u16)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int s[6];
+    load_req3(req, i, s, u16);
+    double v = 0.0;
+    int mask = 0;
+    if (!in_range(T, s, 6)) {
+        atomicAdd(T.bad_count, 1ull);
+    } else {
+        const Side3 B = decode3<false>(T, T.sps_rec, nullptr, s[0], s[1], s[2]), K = decode3<false>(T, T.sps_rec, nullptr, s[3], s[4], s[5]);
+        if (select3(T, B, K)) {
+            const uint4 sg = __ldg(T.sgrp3 + (size_t)B.tup * T.n_tup3 + K.tup);
+            const int4 db = __ldg(T.tdesc3 + B.tup), dk = __ldg(T.tdesc3 + K.tup);
+            if (sg.x != NO_SLAB && mask3(T.stmask3, B, K, db, dk)) {
+                mask = 1;
+                const int4 kb = __ldg(T.tk3 + B.tup), kk = __ldg(T.tk3 + K.tup);
+                const int jb1 = ((db.x >> 8) & 255) + 1, jc1 = ((db.x >> 16) & 255) + 1;
+                const int je1 = ((dk.x >> 8) & 255) + 1, jf1 = ((dk.x >> 16) & 255) + 1;
+                const uint32_t sb = __ldg(T.sig3 + db.w + (B.ima * jb1 + B.imb) * jc1 + B.imc);
+                const uint32_t sk = __ldg(T.sig3 + dk.w + (K.ima * je1 + K.imb) * jf1 + K.imc);
+                const uint32_t bin = __ldg(T.tz2bin3 + ((B.tz << 3) | K.tz));
+                const uint32_t gsize = sg.y;
+                const uint32_t* __restrict__ vwb = T.vw20 + (size_t)sg.z * 4 + (size_t)bin * vw_stride(gsize, T.vw_f32);
+                const int Jminb = (kb.w >> 16) & 255, Jmink = (kk.w >> 16) & 255;
+                const int Jlo = max(Jminb, Jmink), Jhi = min((kb.w >> 24) & 255, (kk.w >> 24) & 255);
+                const int2* __restrict__ jib = T.jinfo3 + kb.z + ((Jlo - Jminb) >> 1);
+                const int2* __restrict__ jik = T.jinfo3 + kk.z + ((Jlo - Jmink) >> 1);
+                const double* __restrict__ dtab = T.dtab3;
+                const int aM = abs(B.twoM);
+                uint32_t c = 0;   // first Vw cell of the J block
+                double total = 0.0;
+                for (int twoJ = Jlo, q = 0; twoJ <= Jhi; twoJ += 2, q++) {
+                    const int2 ib = __ldg(jib + q), ik = __ldg(jik + q);
+                    const int nb = ib.y, nk = ik.y;
+                    if (nb <= 0 || nk <= 0) continue;
+                    const uint32_t P = (uint32_t)row_pitch3(nk);
+                    if (twoJ >= aM) {   // below |M| every coefficient of the block is zero
+                        const double* __restrict__ bp = dtab + ((uint32_t)kb.x + (uint32_t)ib.x + sb * (uint32_t)nb);
+                        const double* __restrict__ kp = dtab + ((uint32_t)kk.x + (uint32_t)ik.x + sk * (uint32_t)nk);
+                        double t = 0.0;
+                        for (int r = 0; r < nb; r++) {
+                            double acc = 0.0;
+                            for (int k = 0; k < nk; k++) {
+                                const double ck = __ldg(kp + k), x = ldvw_global(vwb, gsize, c + (uint32_t)r * P + (uint32_t)k, T.vw_f32);
+                                acc = k ? fma(ck, x, acc) : ck * x;
+                            }
+                            t = fma(__ldg(bp + r), acc, t);
+                        }
+                        total += t;
+                    }
+                    c += (uint32_t)nb * P;
+                }
+                v = (B.sign * K.sign < 0 ? -total : total) + 0.0;
+            }
+        }
+    }
+    out[i] = mask ? v : 0.0;
+    if (maskout) maskout[i] = (uint8_t)mask;
+}
+
 // =============================================================================== H1: records
 // One thread per request: decode, S1-S7 -> mask (request order, coalesced), canonical packed record.
 // Blocks walk KEYS_PER_BLOCK consecutive requests.  With SMEM the small per-basis tables every request needs (SPS
@@ -320,6 +395,9 @@ __global__ void __launch_bounds__(128) k_mscheme_naive(Tables T, long long n, co
 // and leaves the counts in tcnt[tile][bin] for the two-pass partition below (no global atomics for it).
 constexpr int KEYS_SPS_SMEM = 2048, KEYS_AB_SMEM = 2048, KEYS_PER_BLOCK = 256 * 32;
 constexpr int PART_NC = 2048;
+#ifndef MFDN_DIRECT3_MAX
+#define MFDN_DIRECT3_MAX (1ll << 20)    // 3-body batches up to this size are evaluated thread-per-request (k_direct3)
+#endif
 #ifndef MFDN_TWO_PASS_MIN
 #define MFDN_TWO_PASS_MIN (1ll << 23)   // requests from which the two-pass partition beats the one-pass scatter / gather
 #endif
@@ -1572,12 +1650,6 @@ __global__ void __launch_bounds__(TR_THREADS, MFDN_TR_MINB) k_transform3(Tables 
 // mu' tiles.  Pays only where most pairs of a block are requested (config 2, "ALL pairs"); see DESIGN.md for the
 // measured break-even.  Summation order differs from the direct kernels: values agree to rounding, not bitwise.
 constexpr int DN_WARPS = 4;
-// one value of an isospin-combined slab from global memory (bin base vwb), either storage width
-__device__ __forceinline__ double ldvw_global(const uint32_t* __restrict__ vwb, uint32_t gsize, uint32_t cell, int f32)
-{
-    if (f32) return (double)__uint_as_float(__ldg(vwb + cell));
-    return __hiloint2double((int)__ldg(vwb + gsize + cell), (int)__ldg(vwb + cell));
-}
 constexpr int DN_CHUNKS = DENSE_RMAX / 4;
 struct DenseWarp3 {
     double vm[DENSE_CAP];
@@ -1896,13 +1968,13 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
     const long long n_buckets = (BODY == 3 ? (long long)c->t.n_buckets3 : nt * nt) + 1;
     const long long n_tiles = (n_buckets + SCAN_TILE - 1) / SCAN_TILE;
     // Path choice by batch size.  The paths give the same values bit for bit (same operations in the same order), so the choice
-    // is invisible in the results.  Thread-per-request (the paper's kernel) needs no sort and no per-table scans, whose cost
-    // is fixed per call (config 3: 150 us at any n); measured cross-overs on B200: 2-body: direct wins at every n up to 2^26
-    // (~6 terms per request: sorting costs more than it saves; 2.95 against 3.12 ms at 2^26); 3-body: direct below ~2^17
-    // requests, below ~2^20 if the 5-plane slabs fit L2 comfortably (config 2); then the one-pass scatter/gather up to
+    // is invisible in the results.  Thread-per-request needs no sort and no per-table scans, whose cost is fixed per call
+    // (config 3: ~150 us at any n).  Measured cross-overs on B200: 2-body: thread per request at every n up
+    // to 2^26 (~6 terms per request: sorting costs more than it saves; 2.69 against 3.08 ms at 2^26); 3-body: k_direct3 up to
+    // 2^20 requests (config 3: 45 against 124 us at 2^14, 304 against 379 us at 2^20), then the one-pass scatter / gather up to
     // 2^23 requests, the two-pass partition above.  Any flag that names a path overrides the choice.
     const bool named = flags & (MFDN_PRESORTED | MFDN_FORCE_DENSE | MFDN_ONE_PASS_SORT | MFDN_FORCE_SORT);
-    const bool auto_direct = !named && (BODY == 2 || (!c->t.vw_f32 && n < ((c->slab_bytes3 <= (32ll << 20)) ? (1ll << 20) : (1ll << 17))));
+    const bool auto_direct = !named && (BODY == 2 || n <= MFDN_DIRECT3_MAX);
     const bool naive = (flags & MFDN_FORCE_NAIVE) || auto_direct;
     const bool sort = !naive && !(flags & MFDN_PRESORTED);
     const bool items = !naive && BODY == 3;    // the 3-body transform walks a list of one-group work items
@@ -1984,7 +2056,8 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
     }
     if (naive) {
         if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.b, st));
-        k_mscheme_naive<BODY><<<(unsigned)((n + 127) / 128), 128, 0, st>>>(c->t, n, d_req, d_out, d_mask, u16);
+        if (BODY == 3 && !(flags & MFDN_FORCE_NAIVE)) k_direct3<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(c->t, n, d_req, d_out, d_mask, u16);
+        else k_mscheme_naive<BODY><<<(unsigned)((n + 127) / 128), 128, 0, st>>>(c->t, n, d_req, d_out, d_mask, u16);
         c->launches += 1;
         if (c->profile) MFDN_CUDA(c, cudaEventRecord(ev.d, st));
     } else {
