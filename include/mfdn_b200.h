@@ -196,6 +196,13 @@ int mfdn_mscheme_host(mfdn_ctx*, int body, int64_t n, const int32_t* h_req, doub
  * three parts and the call count since the last read, and resets them.  mfdn_fp64_peak runs a register-resident
  * DFMA micro-benchmark on all SMs (the fp64 roofline denominator; MEASURED_PEAKS.json has no fp64 entry) and
  * returns TFLOP/s (2 flops per FMA); synchronises. */
+/* mfdn_multi_client (SURVEY.md 8(f) NEXT-3; PAPER.md:93 request buffers of ~20 000 entries, :103 "each OpenMP thread is given
+ * its own stream"): n_threads host threads (<= 64) created by the call, each with its own stream and its own scratch, push
+ * the n DEVICE-resident requests through the context in chunks of `chunk` (thread t takes chunks t, t + n_threads, ...);
+ * d_out / d_mask receive the results as from one big call.  *seconds = wall clock of the whole job.  BLOCKING; allocates
+ * and frees its streams and scratch. */
+int mfdn_multi_client(mfdn_ctx*, int body, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_mask, int64_t chunk,
+                      int n_threads, uint32_t flags, double* seconds);
 int mfdn_profile(mfdn_ctx*, int enable);
 int mfdn_profile_read(mfdn_ctx*, double* ms_sort, double* ms_transform, double* ms_unpermute, int64_t* calls);
 int mfdn_fp64_peak(mfdn_ctx*, double* tflops);

@@ -25,7 +25,7 @@ SYMBOLS = ["mfdn_orbitals_init", "mfdn_cg_build", "mfdn_cg_download", "mfdn_coup
            "mfdn_coupled_upload_3b", "mfdn_mscheme_2b", "mfdn_mscheme_3b", "mfdn_bad_request_count",
            "mfdn_info", "mfdn_group_keys", "mfdn_last_error", "mfdn_destroy", "mfdn_mscheme_host", "mfdn_profile",
            "mfdn_profile_read", "mfdn_fp64_peak", "mfdn_mscheme_accumulate_2b", "mfdn_mscheme_accumulate_3b",
-           "mfdn_mscheme_block_len_3b", "mfdn_mscheme_blocks_3b", "mfdn_option"]
+           "mfdn_mscheme_block_len_3b", "mfdn_mscheme_blocks_3b", "mfdn_option", "mfdn_multi_client"]
 
 _lib = None
 
@@ -55,6 +55,7 @@ def lib():
         for f in (L.mfdn_mscheme_accumulate_2b, L.mfdn_mscheme_accumulate_3b):
             f.argtypes = [vp, i64, vp, vp, vp, vp, i64, vp, vp, C.POINTER(C.c_size_t), u32, vp]
         L.mfdn_option.argtypes = [vp, C.c_int, i64]
+        L.mfdn_multi_client.argtypes = [vp, C.c_int, i64, vp, vp, vp, i64, C.c_int, u32, C.POINTER(C.c_double)]
         L.mfdn_mscheme_block_len_3b.argtypes = [vp, vp, C.POINTER(i64)]
         L.mfdn_mscheme_blocks_3b.argtypes = [vp, i64, vp, vp, vp, vp, C.POINTER(C.c_size_t), vp]
         L.mfdn_mscheme_host.argtypes = [vp, C.c_int, i64, vp, vp, vp, vp, C.POINTER(C.c_size_t), u32, i64]
@@ -188,6 +189,14 @@ def mfdn_mscheme_blocks_3b(ctx, h_orbitals, h_off, d_out, d_work, work_bytes, st
     _check(ctx, lib().mfdn_mscheme_blocks_3b(ctx, len(o), _hp(o), _hp(off), C.c_void_p(d_out), C.c_void_p(d_work), C.byref(wb),
                                             _stream(stream) if d_work else C.c_void_p(0)))
     return wb.value
+
+
+def mfdn_multi_client(ctx, body, n, d_req, d_out, d_mask, chunk, n_threads, flags=0):
+    """Measurement hook: n_threads native host threads with own streams push chunks through the context.  Returns seconds."""
+    sec = C.c_double(0.0)
+    _check(ctx, lib().mfdn_multi_client(ctx, int(body), int(n), C.c_void_p(d_req), C.c_void_p(d_out), C.c_void_p(d_mask),
+                                        int(chunk), int(n_threads), int(flags), C.byref(sec)))
+    return sec.value
 
 
 def mfdn_mscheme_host(ctx, body, n, h_req, h_out, h_mask, d_work, work_bytes, flags=0, chunk=0):

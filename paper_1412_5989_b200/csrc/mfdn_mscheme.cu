@@ -23,7 +23,9 @@
 //                 (skipped if MFDN_PRESORTED)
 //   k_mscheme_naive      MFDN_FORCE_NAIVE: the paper's design, thread per request in request order
 #include <algorithm>
+#include <chrono>
 #include <cstdio>
+#include <thread>
 
 #include "mfdn_internal.cuh"
 
@@ -2413,6 +2415,60 @@ extern "C" int mfdn_fp64_peak(mfdn_ctx* c, double* tflops)
     cudaEventDestroy(a);
     cudaEventDestroy(b);
     *tflops = best;
+    return MFDN_OK;
+}
+
+// Measurement hook for multi-client operation: n_threads host threads, each with its own stream and its own
+// scratch, push the device-resident requests through the context in chunks (thread t takes chunks t, t + n_threads, ...);
+// *seconds = wall clock from the first launch to the last result.  What a many-threaded MFDn rank would do, without the
+// interpreter in the way.
+extern "C" int mfdn_multi_client(mfdn_ctx* c, int body, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_mask, int64_t chunk,
+                                 int n_threads, uint32_t flags, double* seconds)
+{
+    if (!c || (body != 2 && body != 3) || n < 0 || chunk <= 0 || n_threads <= 0 || n_threads > 64 || !seconds || !d_req || !d_out)
+        return c ? fail(c, MFDN_ERR_ARG, "bad argument") : MFDN_ERR_ARG;
+    size_t wb = 0;
+    int rc = body == 3 ? run<3>(c, chunk, nullptr, nullptr, nullptr, nullptr, &wb, flags, nullptr)
+                       : run<2>(c, chunk, nullptr, nullptr, nullptr, nullptr, &wb, flags, nullptr);
+    if (rc) return rc;
+    MFDN_CUDA(c, cudaSetDevice(c->device));
+    std::vector<cudaStream_t> st(n_threads, nullptr);
+    std::vector<void*> work(n_threads, nullptr);
+    std::vector<int> status(n_threads, MFDN_OK);
+    cudaError_t e = cudaSuccess;
+    for (int t = 0; t < n_threads && e == cudaSuccess; t++) {
+        e = cudaStreamCreateWithFlags(&st[t], cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaMalloc(&work[t], std::max<size_t>(wb, 256));
+    }
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    const int width = 2 * body;
+    const size_t isz = (flags & MFDN_REQ_U16) ? 2 : 4;
+    const auto t0 = std::chrono::steady_clock::now();
+    if (e == cudaSuccess) {
+        std::vector<std::thread> th;
+        for (int t = 0; t < n_threads; t++)
+            th.emplace_back([&, t]() {
+                cudaSetDevice(c->device);
+                for (int64_t lo = (int64_t)t * chunk; lo < n; lo += (int64_t)n_threads * chunk) {
+                    const int64_t m = std::min<int64_t>(chunk, n - lo);
+                    size_t w = wb;
+                    const int32_t* rq = (const int32_t*)((const char*)d_req + (size_t)lo * width * isz);
+                    const int r = body == 3 ? run<3>(c, m, rq, d_out + lo, d_mask ? d_mask + lo : nullptr, work[t], &w, flags, st[t])
+                                            : run<2>(c, m, rq, d_out + lo, d_mask ? d_mask + lo : nullptr, work[t], &w, flags, st[t]);
+                    if (r) { status[t] = r; break; }
+                }
+                if (cudaStreamSynchronize(st[t]) != cudaSuccess && status[t] == MFDN_OK) status[t] = MFDN_ERR_CUDA;
+            });
+        for (auto& x : th) x.join();
+    }
+    *seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+    for (int t = 0; t < n_threads; t++) {
+        if (work[t]) cudaFree(work[t]);
+        if (st[t]) cudaStreamDestroy(st[t]);
+    }
+    if (e != cudaSuccess) return cuda_fail(c, e, "mfdn_multi_client setup");
+    for (int t = 0; t < n_threads; t++)
+        if (status[t]) return status[t] == MFDN_ERR_CUDA ? fail(c, MFDN_ERR_CUDA, "mfdn_multi_client: stream failed") : status[t];
     return MFDN_OK;
 }
 

@@ -3,6 +3,7 @@
 one GPU, device-resident requests, whole call (selection + group sort + transform + store) timed with CUDA events.
 
     python -m paper_1412_5989_b200.report [--configs 0,1,2,3,4] [--reps 20] [--check 14] > report.md
+    python -m paper_1412_5989_b200.report --chunks           # multi-client operation: chunk size x host threads (NEXT-3)
     python -m paper_1412_5989_b200.report --dense            # dense-block path (H5') against the default path, by request density
 
 Configs 0 and 2 are small ("ALL conserving pairs"): they are latency measurements, an L2 flush (a 256 MiB memset)
@@ -183,16 +184,50 @@ def dense_table(reps=10):
         ctx.close()
 
 
+def chunk_table(idx=3, total_log2=22):
+    """Multi-client operation (SURVEY.md 8(f) NEXT-3; PAPER.md:93 buffers of ~20 000 requests, :103 one stream per OpenMP
+    thread): T native host threads (mfdn_multi_client), each with its own stream and scratch, push chunks of a fixed size through
+    one context until 2^total_log2 requests are done; wall-clock throughput of the whole job, device-resident requests; the
+    result is checked bitwise against one big call."""
+    import torch
+    from paper_1412_5989_b200 import binding as B, workloads as W
+    cfg = W.make_config(idx)
+    ctx = B.Context(cfg.basis, 0).upload(cfg.table)
+    n = 1 << total_log2
+    d_req = torch.from_numpy(cfg.requests(n, workers=os.cpu_count() or 1)).cuda()
+    out = torch.empty(n, dtype=torch.float64, device="cuda")
+    mask = torch.empty(n, dtype=torch.uint8, device="cuda")
+    base, bmask = ctx.mscheme(d_req, flags=B.MFDN_FORCE_SORT)
+    base, bmask = base.clone(), bmask.clone()
+    print("| chunk (requests) | " + " | ".join(f"{t} thread{'s' if t > 1 else ''}: elements/s" for t in (1, 2, 4, 8, 16)) + " |")
+    print("|---|---|---|---|---|---|")
+    for lg in (10, 12, 14, 15, 16, 18, 20, 22):
+        cells = []
+        for nthreads in (1, 2, 4, 8, 16):
+            best = 0.0
+            for _ in range(3):
+                out.zero_()
+                sec = B.mfdn_multi_client(ctx.ctx, cfg.body, n, d_req.data_ptr(), out.data_ptr(), mask.data_ptr(), 1 << lg, nthreads)
+                best = max(best, n / sec)
+            assert torch.equal(out, base) and torch.equal(mask, bmask), "chunked result differs from the single call"
+            cells.append(f"{best:.3e}")
+        print(f"| 2^{lg} = {1 << lg} | " + " | ".join(cells) + " |")
+    ctx.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--configs", default="0,1,2,3,4")
     ap.add_argument("--reps", type=int, default=20)
     ap.add_argument("--dense", action="store_true")
+    ap.add_argument("--chunks", action="store_true", help="multi-client table: chunk size x host threads (config 3)")
     args = ap.parse_args()
     import torch
     from paper_1412_5989_b200 import binding as B, workloads as W
     if args.dense:
         return dense_table()
+    if args.chunks:
+        return chunk_table()
     hbm, hbm_src = hbm_peak()
     ctx = B.Context(W.make_config(0).basis, 0)
     fp64 = B.mfdn_fp64_peak(ctx.ctx)

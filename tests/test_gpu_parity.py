@@ -486,6 +486,13 @@ def test_multi_client_threads(torch, B):
     assert not errors, errors
     assert calls == len(chunks)
     assert np.array_equal(out.cpu().numpy(), base) and np.array_equal(mask.cpu().numpy(), bmask)
+    # the same with native host threads (mfdn_multi_client, the measurement hook of report.py --chunks)
+    for flags in (0, B.MFDN_FORCE_SORT):
+        out.zero_()
+        mask.zero_()
+        sec = B.mfdn_multi_client(ctx.ctx, 3, len(req), d_req.data_ptr(), out.data_ptr(), mask.data_ptr(), 20000, 6, flags)
+        assert sec > 0.0
+        assert np.array_equal(out.cpu().numpy(), base) and np.array_equal(mask.cpu().numpy(), bmask)
 
 
 # --------------------------------------------------------------------------------- NEXT-1: fused accumulate epilogue
