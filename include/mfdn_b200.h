@@ -124,7 +124,7 @@ int mfdn_coupled_upload_3b(mfdn_ctx*, int32_t e3max, int32_t n_chan, const int32
  *         mask[i] = 1 iff the request passes the integer selection rules S1-S7; where
  *         mask[i] = 0 the value is exactly +0.0.
  * d_work/work_bytes: caller-provided DEVICE scratch, 256-byte aligned.  Call with d_work == NULL to get
- *         the size needed for n requests in *work_bytes (nothing is launched).  The call itself never
+ *         the size needed for n requests WITH THESE FLAGS in *work_bytes (nothing is launched; the size depends on both).  The call itself never
  *         allocates and never synchronises: it is asynchronous on `stream`.
  * Per-request problems never fail the call: an out-of-range SPS index gives value 0, mask 0 and is
  * counted (mfdn_bad_request_count).  Concurrent calls are allowed -- from one host thread or from several -- provided
