@@ -398,7 +398,8 @@ __global__ void __launch_bounds__(128) k_direct3(Tables T, long long n, const in
 constexpr int KEYS_SPS_SMEM = 2048, KEYS_AB_SMEM = 2048, KEYS_PER_BLOCK = 256 * 32;
 constexpr int PART_NC = 2048;
 #ifndef MFDN_DIRECT3_MAX
-#define MFDN_DIRECT3_MAX (1ll << 20)    // 3-body batches up to this size are evaluated thread-per-request (k_direct3)
+#define MFDN_DIRECT3_MAX (1ll << 20)    // 3-body batches up to this size are evaluated thread-per-request (k_direct3); twice that
+                                        // if the isospin-combined slabs are under 64 MB (cache-resident: config 2, 1.44 M requests)
 #endif
 #ifndef MFDN_TWO_PASS_MIN
 #define MFDN_TWO_PASS_MIN (1ll << 23)   // requests from which the two-pass partition beats the one-pass scatter / gather
@@ -1976,7 +1977,7 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
     // 2^20 requests (config 3: 45 against 124 us at 2^14, 304 against 379 us at 2^20), then the one-pass scatter / gather up to
     // 2^23 requests, the two-pass partition above.  Any flag that names a path overrides the choice.
     const bool named = flags & (MFDN_PRESORTED | MFDN_FORCE_DENSE | MFDN_ONE_PASS_SORT | MFDN_FORCE_SORT);
-    const bool auto_direct = !named && (BODY == 2 || n <= MFDN_DIRECT3_MAX);
+    const bool auto_direct = !named && (BODY == 2 || n <= (c->vw_bytes3 <= (64ll << 20) ? 2 * MFDN_DIRECT3_MAX : MFDN_DIRECT3_MAX));
     const bool naive = (flags & MFDN_FORCE_NAIVE) || auto_direct;
     const bool sort = !naive && !(flags & MFDN_PRESORTED);
     const bool items = !naive && BODY == 3;    // the 3-body transform walks a list of one-group work items
