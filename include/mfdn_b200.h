@@ -41,9 +41,10 @@ typedef enum {
 enum {
     MFDN_PRESORTED = 1,   /* requests are already ordered by the library's sort key: NON-DECREASING mfdn_group_keys value
                              (2-body: orbital-tuple group; 3-body: group, then M; requests failing S1-S6, key
-                             0xFFFFFFFF, last).  Skips the partition passes of step H2 and of step H6; 3-body still
-                             histograms the keys to cut the stream into one-group work items.  Input that is not so
-                             ordered gives undefined VALUES (never a fault); the mask stays correct */
+                             0xFFFFFFFF, last).  Where the library takes the group-sort path (large 3-body batches, or with
+                             MFDN_FORCE_SORT) it skips the partition passes of steps H2 and H6; 3-body still histograms
+                             the keys to cut the stream into one-group work items.  Input that is not so ordered gives
+                             undefined VALUES on that path (never a fault); the mask stays correct */
     MFDN_FORCE_NAIVE = 2, /* one thread per request in request order, no sort, no staging: the paper's own
                              kernel design; kept as on-device reference */
     MFDN_FORCE_DENSE = 4, /* 3-body: every group whose blocks fit takes the dense-block path (step H5'): per (group, M,

@@ -1976,7 +1976,9 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
     // to 2^26 (~6 terms per request: sorting costs more than it saves; 2.69 against 3.08 ms at 2^26); 3-body: k_direct3 up to
     // 2^20 requests (config 3: 45 against 124 us at 2^14, 304 against 379 us at 2^20), then the one-pass scatter / gather up to
     // 2^23 requests, the two-pass partition above.  Any flag that names a path overrides the choice.
-    const bool named = flags & (MFDN_PRESORTED | MFDN_FORCE_DENSE | MFDN_ONE_PASS_SORT | MFDN_FORCE_SORT);
+    // MFDN_PRESORTED is a property of the input, not a path: a pre-sorted 2-body batch is still fastest thread-per-request
+    // (1.03 against 1.30 ms at 2^26), and so is a small pre-sorted 3-body batch.
+    const bool named = flags & (MFDN_FORCE_DENSE | MFDN_ONE_PASS_SORT | MFDN_FORCE_SORT);
     const bool auto_direct = !named && (BODY == 2 || n <= (c->vw_bytes3 <= (64ll << 20) ? 2 * MFDN_DIRECT3_MAX : MFDN_DIRECT3_MAX));
     const bool naive = (flags & MFDN_FORCE_NAIVE) || auto_direct;
     const bool sort = !naive && !(flags & MFDN_PRESORTED);

@@ -178,7 +178,7 @@ def dense_table(reps=10):
             d = torch.from_numpy(req).cuda()
             keys = ctx.group_keys(d)
             ds = d[torch.argsort(keys.to(torch.int64) & 0xFFFFFFFF)].contiguous()
-            a = timed(ctx, ds, B.MFDN_PRESORTED)
+            a = timed(ctx, ds, B.MFDN_PRESORTED | B.MFDN_FORCE_SORT)     # the work-item kernels of the group-sort path
             b = timed(ctx, ds, B.MFDN_PRESORTED | B.MFDN_FORCE_DENSE)
             print(f"| {name} | {f:.2f} | {len(req)} | {a[0]:.3f} | {a[1]:.3f} | {b[0]:.3f} | {b[1]:.3f} | {float((a[2] - b[2]).abs().max()):.1e} |")
         ctx.close()

@@ -105,7 +105,7 @@ def test_cg_tables_match_exact(torch, B, emax):
 
 
 # --------------------------------------------------------------------------------- whole small configs
-@pytest.mark.parametrize("mode", list(MODES) + ["presorted", "dense", "dense_presorted"])
+@pytest.mark.parametrize("mode", list(MODES) + ["presorted", "sort_presorted", "dense", "dense_presorted"])
 @pytest.mark.parametrize("idx", [0, 2])
 def test_all_pairs_configs(torch, B, oracle, idx, mode):
     cfg = get_cfg(idx)
@@ -118,7 +118,7 @@ def test_all_pairs_configs(torch, B, oracle, idx, mode):
         return
     want, wmask, _, _ = oracle.mscheme(cfg.basis, cfg.table, req)
     if mode.endswith("presorted"):
-        flags = B.MFDN_PRESORTED | (B.MFDN_FORCE_DENSE if mode.startswith("dense") else 0)
+        flags = B.MFDN_PRESORTED | (B.MFDN_FORCE_DENSE if mode.startswith("dense") else 0) | (B.MFDN_FORCE_SORT if mode.startswith("sort") else 0)
         sreq, order = presort(torch, ctx, req)
         got, gmask = run_gpu(torch, ctx, sreq, flags)
         check(cfg, got, gmask, want[order], wmask[order])
@@ -147,8 +147,9 @@ def test_sampled_configs_prefix(torch, B, oracle, idx, n):
         got, gmask = run_gpu(torch, ctx, req, B.MFDN_FORCE_DENSE)
         check(cfg, got, gmask, want, wmask)
     sreq, order = presort(torch, ctx, req)
-    got, gmask = run_gpu(torch, ctx, sreq, B.MFDN_PRESORTED)
-    check(cfg, got, gmask, want[order], wmask[order])
+    for flags in (B.MFDN_PRESORTED, B.MFDN_PRESORTED | B.MFDN_FORCE_SORT):     # the library's choice / the group-sort path
+        got, gmask = run_gpu(torch, ctx, sreq, flags)
+        check(cfg, got, gmask, want[order], wmask[order])
 
 
 # --------------------------------------------------------------------------------- edge cases
@@ -343,8 +344,9 @@ def _check_all_modes(torch, B, oracle, basis, table, req):
         got, gmask = run_gpu(torch, ctx, req, flags)
         check(cfg, got, gmask, want, wmask)
     sreq, order = presort(torch, ctx, req)
-    got, gmask = run_gpu(torch, ctx, sreq, B.MFDN_PRESORTED)
-    check(cfg, got, gmask, want[order], wmask[order])
+    for flags in (B.MFDN_PRESORTED, B.MFDN_PRESORTED | B.MFDN_FORCE_SORT):
+        got, gmask = run_gpu(torch, ctx, sreq, flags)
+        check(cfg, got, gmask, want[order], wmask[order])
     ctx.close()
 
 
@@ -397,9 +399,10 @@ def test_full_size_config1_sampled(torch, B, oracle):
     del keys
     d_sorted = d_req[order].contiguous()
     del d_req
-    out3, mask3 = ctx.mscheme(d_sorted, flags=B.MFDN_PRESORTED)
-    torch.cuda.synchronize()
-    assert bool((out3 == out[order]).all()) and bool((mask3 == mask[order]).all())
+    for flags in (B.MFDN_PRESORTED, B.MFDN_PRESORTED | B.MFDN_FORCE_SORT):   # thread per request / group-sort kernels
+        out3, mask3 = ctx.mscheme(d_sorted, flags=flags)
+        torch.cuda.synchronize()
+        assert bool((out3 == out[order]).all()) and bool((mask3 == mask[order]).all())
 
 
 def test_full_size_config4_batches(torch, B, oracle):
