@@ -346,7 +346,7 @@ def main():
                          "presorted": {"keys_items_H1_H3": ms_sort_p, "transform_H3_H6": ms_tr_p}},
         "presorted": {"value": world * n / (ms_p * 1e-3), "unit": UNIT, "ms_per_step": ms_p,
                       "note": "same multiset pre-ordered by mfdn_group_keys, flag MFDN_PRESORTED"},
-        "roofline": {"kernel": f"k_transform{body}" + (" + k_transform3_small (groups of <= 64 records; 3 % of the time)" if body == 3 else "") + ": dominant kernel of the unsorted step; CUDA events on the launch stream", "bound": "alu",
+        "roofline": {"kernel": f"k_transform{body}" + (" + k_transform3_small (groups of <= 16 records)" if body == 3 else "") + ": dominant kernel of the unsorted step; CUDA events on the launch stream", "bound": "alu",
                      "achieved": flops_rate, "peak": fp64_peak, "unit": "TFLOP/s", "frac": flops_rate / fp64_peak,
                      "traffic": traffic, "traffic_source": {"file": "profiles/dram_traffic.txt", "capture": prof.get("capture"),
                                                             "commit": prof.get("commit")},

@@ -15,7 +15,7 @@
 //   k_scan_*      H2  exclusive scan of the histogram -> bucket bounds
 //   k_tscan_*, k_tiles2, k_part<1>, k_part<2>   H2  records -> bucket order by a two-pass partition through shared
 //                 memory (skipped if MFDN_PRESORTED)
-//   k_items3      H3  one-group work items from the bucket bounds (3-body); groups of <= 64 records on a second list
+//   k_items3      H3  one-group work items from the bucket bounds (3-body); groups of <= 16 records on a second list
 //   k_transform3  H3-H5  block per item: staged isospin-combined slab, records ordered by M, paired channel sums
 //   k_transform3_small   warp per small group, direct sums in the same operation order
 //   k_transform2  H3-H5  2-body: warp per 32 records of the group-ordered stream
@@ -1005,7 +1005,9 @@ __global__ void __launch_bounds__(256) k_unpermute(long long n, const double* __
 // slab does not fit a stage even four bins at a time (gsize > 639: no such group in the five workloads, but tuples
 // of three j = 15/2 orbitals have one) go to the same list in chunks of SMALL_ITEM3 records: that path has no
 // capacity limit.
-constexpr uint32_t SMALL_ITEM3 = 64;
+// 16: measured optimum (64 -> 16: config 3 at 2^22 requests 619 -> 551 us, config 4 batch of 2^24 2.64 -> 2.49 ms, config 3 at
+// 2^26 unchanged; 8: same; 4: worse) -- the staged kernel amortises its slab copy from about 16 records on
+constexpr uint32_t SMALL_ITEM3 = 16;
 __device__ __forceinline__ uint32_t bins_per_round3(uint32_t gsize, int f32)
 {
     const uint32_t b = ((uint32_t)VW_WORDS / vw_stride(gsize, f32)) & ~3u;   // multiple of 4: every round starts 16-byte aligned
