@@ -220,7 +220,7 @@ int64_t mfdn_info(mfdn_ctx*, int which);
  * n_tuples + ket_tuple; 3-body the (group, M) bucket = first bucket of the group bra_tuple * n_tuples + ket_tuple + index
  * of the request's M in the group's common M range (requests of one group are contiguous, ordered by M: the
  * coefficient tables are M-major, so neighbouring requests read neighbouring entries).  0xFFFFFFFF for requests that
- * fail S1-S6.  body = 2 or 3.  Asynchronous on `stream`. */
+ * fail S1-S6.  body = 2 or 3; d_req holds int32 indices (no MFDN_REQ_U16 form).  Asynchronous on `stream`. */
 int mfdn_group_keys(mfdn_ctx*, int body, int64_t n, const int32_t* d_req, uint32_t* d_key, void* stream);
 
 /* Message of the context's most recent failure; the pointer stays valid until the calling thread's next call of this function. */
