@@ -524,10 +524,13 @@ __global__ void __launch_bounds__(KS_THREADS, 1) k_keys3s(Tables T, KeysSmem3 L,
     for (int k = tid; k < T.ncls3 * nt; k += KS_THREADS) s_colcum[k] = __ldg(T.colcum3 + k);
     for (int k = tid; k < T.sig_len3; k += KS_THREADS) s_sig[k] = __ldg(T.sig3 + k);
     if (tid < 64) s_tzbin[tid] = __ldg(T.tz2bin3 + tid);
+    // the coarse counts are double-buffered: ONE block barrier per tile (the counts of tile t are flushed and zeroed while tile
+    // t + 1 is counted into the other half; the barrier was 14 % of the stall samples on the skewed config-4 stream)
+    if (tcnt)
+        for (int k = tid; k < 2 * nc; k += KS_THREADS) s_ch[k] = 0u;
+    __syncthreads();   // also: the tables are loaded
+    uint32_t* s_cur = s_ch;
     for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-        if (tcnt)
-            for (int k = tid; k < nc; k += KS_THREADS) s_ch[k] = 0u;
-        __syncthreads();
         const long long i0 = (long long)tile * KEYS_PER_BLOCK + tid;
         const long long i1 = min(n, (long long)(tile + 1) * KEYS_PER_BLOCK);
         int nx[6];
@@ -568,12 +571,16 @@ __global__ void __launch_bounds__(KS_THREADS, 1) k_keys3s(Tables T, KeysSmem3 L,
                 if ((tid & 31) == __ffs(same) - 1) atomicAdd(hist + bucket, (uint32_t)__popc(same));
             } else {
                 atomicAdd(hist + bucket, 1u);
-                if (tcnt) atomicAdd(&s_ch[bucket >> csh], 1u);
+                if (tcnt) atomicAdd(&s_cur[bucket >> csh], 1u);
             }
         }
         if (tcnt) {
             __syncthreads();
-            for (int k = tid; k < nc; k += KS_THREADS) tcnt[(size_t)tile * nc + k] = s_ch[k];
+            for (int k = tid; k < nc; k += KS_THREADS) {
+                tcnt[(size_t)tile * nc + k] = s_cur[k];
+                s_cur[k] = 0u;   // used again two tiles from now, after the next barrier
+            }
+            s_cur = s_cur == s_ch ? s_ch + nc : s_ch;
         }
     }
 }
@@ -2088,7 +2095,7 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
             L.sps = up(L.ab + (uint32_t)(c->t.n_orb * c->t.n_orb) * 8u);
             L.rowbase = up(L.sps + (uint32_t)c->t.n_sps * 4u);
             L.ch = up(L.rowbase + (uint32_t)nt * 4u);
-            L.colcum = up(L.ch + (uint32_t)PART_NC * 4u);
+            L.colcum = up(L.ch + 2u * (uint32_t)PART_NC * 4u);
             L.sig = up(L.colcum + (uint32_t)(c->t.ncls3 * nt) * 2u);
             L.tzbin = up(L.sig + (uint32_t)c->t.sig_len3 * 2u);
             L.total = L.tzbin + 64u;
