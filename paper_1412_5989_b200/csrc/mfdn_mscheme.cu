@@ -570,7 +570,7 @@ __global__ void __launch_bounds__(KS_THREADS, 1) k_keys3s(Tables T, KeysSmem3 L,
                 const unsigned same = __match_any_sync(__activemask(), bucket);
                 if ((tid & 31) == __ffs(same) - 1) atomicAdd(hist + bucket, (uint32_t)__popc(same));
             } else {
-                atomicAdd(hist + bucket, 1u);
+                if (hist) atomicAdd(hist + bucket, 1u);   // NULL: the buckets are counted per pass-2 tile (k_count2) instead
                 if (tcnt) atomicAdd(&s_cur[bucket >> csh], 1u);
             }
         }
@@ -787,6 +787,28 @@ __device__ __forceinline__ uint32_t rec_bucket(unsigned long long r, uint32_t in
 {
     const uint32_t key = (uint32_t)(r >> REC_KEY_SHIFT);
     return key == REC_INVALID ? invalid_bucket : key;
+}
+
+// Histogram of the sort buckets from the coarse-ordered stream, one block per pass-2 tile: counted in shared memory, then ONE
+// global atomic per (tile, non-empty bucket).  Replaces the per-request histogram atomic of H1 on the two-pass path: on a
+// skewed stream those atomics pile up on a few L2 lines (config 4: H1 0.57 ms per 2^24 requests against 0.26 ms on a uniform
+// stream over the same tables); here a hot bucket costs one atomic per tile.  Price: the records are read once more.
+__global__ void __launch_bounds__(P_THREADS) k_count2(const unsigned long long* __restrict__ p1rec, const uint4* __restrict__ tiles2,
+                                                     uint32_t* __restrict__ hist, int csh, uint32_t invalid_bucket)
+{
+    __shared__ uint32_t s_cnt[PART_NF];
+    if (blockIdx.x >= __ldg(&tiles2[0].x)) return;
+    const uint4 t = __ldg(tiles2 + 1 + blockIdx.x);
+    const uint32_t d0 = t.z << csh;
+    const int nd = min(1 << csh, (int)(invalid_bucket + 1u - d0)), m = (int)t.y, tid = threadIdx.x;
+    for (int k = tid; k < nd; k += P_THREADS) s_cnt[k] = 0u;
+    __syncthreads();
+    for (int l = tid; l < m; l += P_THREADS) atomicAdd(&s_cnt[rec_bucket(__ldg(p1rec + t.x + l), invalid_bucket) - d0], 1u);
+    __syncthreads();
+    for (int k = tid; k < nd; k += P_THREADS) {
+        const uint32_t v = s_cnt[k];
+        if (v) atomicAdd(hist + d0 + k, v);
+    }
 }
 
 // One partition pass over one tile.  PASS 1: tile = k_keys tile blockIdx.x, digit = bucket >> csh, first positions from
@@ -2086,7 +2108,7 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
         const unsigned gkb = (unsigned)((n + KEYS_PER_BLOCK - 1) / KEYS_PER_BLOCK);
         // 3-body with every per-basis table in shared memory (k_keys3s) when they fit; MFDN_ONE_PASS_SORT keeps the general kernel
         KeysSmem3 L{};
-        bool smem_keys = false;
+        bool smem_keys = false, late_hist = false;
         if (BODY == 3 && sm && c->t.ncls3 > 0 && !(flags & MFDN_ONE_PASS_SORT)) {
             auto up = [](uint32_t x) { return (x + 15u) & ~15u; };
             L.tdesc = 0;
@@ -2111,9 +2133,10 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
             }
             const unsigned gks = (unsigned)std::min<long long>(n_ktiles, c->num_sms);
             uint32_t* tc = sort && two_pass ? (uint32_t*)(w + o_tcnt) : nullptr;
+            late_hist = sort && two_pass;   // the buckets are then counted by k_count2 after pass 1
             const int tsh = sort ? csh : 0, tnc = sort ? nc : 0;
             auto kern = sort ? (u16 ? k_keys3s<false, true> : k_keys3s<false, false>) : (u16 ? k_keys3s<true, true> : k_keys3s<true, false>);
-            kern<<<gks, KS_THREADS, L.total, st>>>(c->t, L, n, d_req, recs, d_mask, hist, invalid_bucket, tc, tsh, tnc, (int)n_ktiles);
+            kern<<<gks, KS_THREADS, L.total, st>>>(c->t, L, n, d_req, recs, d_mask, late_hist ? nullptr : hist, invalid_bucket, tc, tsh, tnc, (int)n_ktiles);
         } else if (sort) {
             uint32_t* tcnt = two_pass ? (uint32_t*)(w + o_tcnt) : nullptr;
             if (sm) k_keys<BODY, false, true><<<gkb, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr, tcnt, csh, nc, u16);
@@ -2123,7 +2146,7 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
             else k_keys<BODY, true, false><<<gkb, 256, 0, st>>>(c->t, n, d_req, recs, d_mask, hist, invalid_bucket, nullptr, nullptr, 0, 0, u16);
         }
         c->launches += 1;
-        if (hist_needed) {
+        if (hist_needed && !late_hist) {
             k_scan_tiles<<<(unsigned)n_tiles, SCAN_T, 0, st>>>(hist, n_buckets, sums);
             k_scan_sums<<<1, 1024, 0, st>>>(sums, (int)n_tiles);
             k_scan_add<<<(unsigned)n_tiles, SCAN_T, 0, st>>>(hist, n_buckets, sums);
@@ -2152,6 +2175,13 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
             k_tscan_fill<<<gts, 128, 0, st>>>(tcnt, (int)n_ktiles, nc, part, cstart);
             k_tiles2<<<1, 1024, 0, st>>>(cstart, nc, tiles2);
             k_part<1><<<gkb, P_THREADS, PART_SMEM, st>>>(n, recs, tcnt, nullptr, nullptr, csh, nc, p1rec, map1, slot1, invalid_bucket);
+            if (late_hist) {
+                k_count2<<<(unsigned)max_tiles2, P_THREADS, 0, st>>>(p1rec, tiles2, hist, csh, invalid_bucket);
+                k_scan_tiles<<<(unsigned)n_tiles, SCAN_T, 0, st>>>(hist, n_buckets, sums);
+                k_scan_sums<<<1, 1024, 0, st>>>(sums, (int)n_tiles);
+                k_scan_add<<<(unsigned)n_tiles, SCAN_T, 0, st>>>(hist, n_buckets, sums);
+                c->launches += 4;
+            }
             // the request-order records are dead after pass 1: the bucket-ordered records take their place
             k_part<2><<<(unsigned)max_tiles2, P_THREADS, PART_SMEM, st>>>(n, p1rec, nullptr, tiles2, hist, csh, 1 << csh, recs, map2, slot2, invalid_bucket);
             c->launches += 6;
