@@ -81,6 +81,35 @@ __device__ __forceinline__ Side3 decode3(const Tables& T, const uint32_t* sps, c
     return S;
 }
 
+// The same from the SPS records as k_keys3s keeps them in shared memory (at most 64 orbitals, 2048 SPS):
+//   [26,32) orbital  [15,26) SPS index  [14] l & 1  [12,14) tz bit  [6,12) 2j  [0,6) im
+// Sorted as unsigned words they are in (orbital, SPS) order, so the canonical order is min / middle / max (no compare-and-swap
+// network with payloads), the sign is the parity of the three pairwise inversions, and the low 15 bits of p0 + p1 + p2 are the
+// packed sums of im, 2j, tz and l over the three particles (every sum fits its field: 3 * 21 <= 63).
+__host__ __device__ inline uint32_t sps_pack_sorted(uint32_t r, int s)
+{
+    return ((uint32_t)rec_orb(r) << 26) | ((uint32_t)s << 15) | ((uint32_t)rec_lpar(r) << 14) | ((uint32_t)rec_tz(r) << 12) |
+           ((uint32_t)rec_twoj(r) << 6) | (uint32_t)rec_im(r);
+}
+__device__ __forceinline__ Side3 decode3s(const Tables& T, const uint32_t* sps, const int2* ab, int s0, int s1, int s2)
+{
+    Side3 S;
+    const uint32_t p0 = sps[s0], p1 = sps[s1], p2 = sps[s2], tot = p0 + p1 + p2;
+    const uint32_t lo = min(p0, min(p1, p2)), hi = max(p0, max(p1, p2)), mid = tot - lo - hi;
+    S.distinct = lo != mid && mid != hi;
+    S.sign = ((p0 > p1) != (p1 > p2)) != (p0 > p2) ? -1 : 1;
+    const int a = (int)(lo >> 26), b = (int)(mid >> 26), c = (int)(hi >> 26);
+    const int2 e = ab[a * T.n_orb + b];
+    const int d = c - (e.y & 0xFFFF);
+    S.tup = (e.x >= 0 && (unsigned)d < (unsigned)(e.y >> 16)) ? e.x + d : -1;
+    S.ima = (int)(lo & 63u); S.imb = (int)(mid & 63u); S.imc = (int)(hi & 63u);
+    S.tz = (int)(((lo >> 10) & 4u) | ((mid >> 11) & 2u) | ((hi >> 12) & 1u));
+    S.twoM = 2 * (int)(tot & 63u) - (int)((tot >> 6) & 63u);
+    S.twoMT = 2 * (int)((tot >> 12) & 3u) - 3;
+    S.par = (int)((tot >> 14) & 1u);
+    return S;
+}
+
 struct Side2 {
     int tup, ima, imb, tz, twoM, twoMT, par, sign;
     bool distinct;
@@ -397,6 +426,7 @@ __global__ void __launch_bounds__(128) k_direct3(Tables T, long long n, const in
 // and leaves the counts in tcnt[tile][bin] for the two-pass partition below (no global atomics for it).
 constexpr int KEYS_SPS_SMEM = 2048, KEYS_AB_SMEM = 2048, KEYS_PER_BLOCK = 256 * 32;
 constexpr int PART_NC = 2048;
+static_assert(KEYS_SPS_SMEM <= 2048 && KEYS_AB_SMEM <= 64 * 64 && 3 * MAX_TWOJ <= 63, "field widths of sps_pack_sorted");
 #ifndef MFDN_DIRECT3_MAX
 #define MFDN_DIRECT3_MAX (1ll << 20)    // 3-body batches up to this size are evaluated thread-per-request (k_direct3); twice that
                                         // if the isospin-combined slabs are under 64 MB (cache-resident: config 2, 1.44 M requests)
@@ -520,7 +550,7 @@ __global__ void __launch_bounds__(KS_THREADS, 1) k_keys3s(Tables T, KeysSmem3 L,
     for (int k = tid; k < nt; k += KS_THREADS) { s_tdesc[k] = __ldg(T.tdesc3 + k); s_rowbase[k] = __ldg(T.rowbase3 + k); }
     for (int k = tid; k < T.stmask_len3; k += KS_THREADS) s_stm[k] = __ldg(T.stmask3 + k);
     for (int k = tid; k < T.n_orb * T.n_orb; k += KS_THREADS) s_ab[k] = __ldg(T.ab3 + k);
-    for (int k = tid; k < T.n_sps; k += KS_THREADS) s_sps[k] = __ldg(T.sps_rec + k);
+    for (int k = tid; k < T.n_sps; k += KS_THREADS) s_sps[k] = sps_pack_sorted(__ldg(T.sps_rec + k), k);
     for (int k = tid; k < T.ncls3 * nt; k += KS_THREADS) s_colcum[k] = __ldg(T.colcum3 + k);
     for (int k = tid; k < T.sig_len3; k += KS_THREADS) s_sig[k] = __ldg(T.sig3 + k);
     if (tid < 64) s_tzbin[tid] = __ldg(T.tz2bin3 + tid);
@@ -543,10 +573,10 @@ __global__ void __launch_bounds__(KS_THREADS, 1) k_keys3s(Tables T, KeysSmem3 L,
             uint32_t key = REC_INVALID;
             unsigned long long low = 0;
             int mask = 0;
-            if (!in_range(T, s, 6)) {
+            if (max(max((unsigned)s[0], (unsigned)s[1]), max(max((unsigned)s[2], (unsigned)s[3]), max((unsigned)s[4], (unsigned)s[5]))) >= (unsigned)T.n_sps) {
                 atomicAdd(T.bad_count, 1ull);
             } else {
-                Side3 B = decode3<true>(T, s_sps, s_ab, s[0], s[1], s[2]), K = decode3<true>(T, s_sps, s_ab, s[3], s[4], s[5]);
+                Side3 B = decode3s(T, s_sps, s_ab, s[0], s[1], s[2]), K = decode3s(T, s_sps, s_ab, s[3], s[4], s[5]);
                 if (select3(T, B, K)) {
                     const int4 db = s_tdesc[B.tup], dk = s_tdesc[K.tup];
                     const int sjb = (db.x & 255) + ((db.x >> 8) & 255) + ((db.x >> 16) & 255);
