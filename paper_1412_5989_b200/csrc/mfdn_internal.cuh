@@ -61,6 +61,7 @@ constexpr int DENSE_CAP = 1024;    // doubles of one (group, M, bin) block of th
 constexpr int DENSE_RMAX = 64;     // flattened ket rows (J, J12') of a group on the dense path
 constexpr int VW_WORDS = 5120;     // 32-bit words of one staged slab (20 KB): all 20 bins of a group with gsize <= 127
 constexpr uint32_t ZERO_ITEM = 0xFFFFFFFFu;   // work item whose records all have value 0 (no slab / failed S1-S6)
+constexpr uint32_t STOP_ITEM = 0xFFFFFFFEu;   // posted by the producer warp of k_transform3 after its last item
 
 // ---- packed canonical request record (H1 output), 64 bit --------------------------------------------
 // 2-body: [0,30) im of the canonical particles (5 bits each: bra at 0,5; ket at 15,20)   [30,36) tz bits (bra then ket)
