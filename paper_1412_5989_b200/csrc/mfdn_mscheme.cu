@@ -1297,7 +1297,7 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 #define MFDN_TR_MINB 4
 #endif
 #ifndef MFDN_TR_RING
-#define MFDN_TR_RING 6656
+#define MFDN_TR_RING 9216
 #endif
 #ifndef MFDN_TR_PF
 #define MFDN_TR_PF 0
@@ -1309,10 +1309,11 @@ constexpr int MAX_JBLK = 32;                    // common J values of a group (2
 constexpr int BATCH3 = 64;                      // records per consumer-warp batch (two per lane)
 constexpr int REC_WORDS_MAX = (ITEM3 + 2) * 2;  // records are copied from an even position: one record of slack at either end
 // Ring of 32-bit words holding, per work item in flight, everything its consumer warps read: the isospin-combined slabs
-// and the records (both landed by bulk copies) and the J-block descriptors (written by the producer warp).  Sized for
-// one item of maximal size; typical items (4 KB of slabs, 3 KB of records) leave room for three to four in flight.  A
-// small ring keeps most of the SM's 228 KB as L1 for the coefficient tables (ncu: with two fixed 25 KB stages per
-// block the L1 hit rate of the coefficient gathers was 60 %).
+// and the records (both landed by bulk copies) and the J-block descriptors (written by the producer warp).  At least
+// one item of maximal size; typical items (4 KB of slabs, 3 KB of records) leave room for five in flight.  A small ring
+// keeps more of the SM's 228 KB as L1 for the coefficient tables (ncu: with two fixed 25 KB stages per block the L1 hit
+// rate of the coefficient gathers was 60 %).  Swept with the items handed out dynamically (pre-sorted call of config 3 /
+// one batch of config 4, ms): 6656 words 2.053 / 2.142, 7424 2.033, 8192 2.034 / 2.095, 9216 2.025, 10240 2.043 / 2.067.
 constexpr int RING_WORDS = MFDN_TR_RING;
 static_assert(RING_WORDS >= VW_WORDS + REC_WORDS_MAX + MAX_JBLK * 4, "ring must hold one maximal work item");
 enum { SC_POS0, SC_CNT, SC_GROUP, SC_SB, SC_SK, SC_PB0, SC_PK0, SC_JINFO, SC_GSIZE, SC_STRIDE, SC_BINS, SC_ROFF, SC_VW, SC_REC, SC_DESC, SC_NEXT };
