@@ -190,6 +190,28 @@ int mfdn_mscheme_blocks_3b(mfdn_ctx*, int64_t n_groups, const int32_t* h_orbital
 int mfdn_mscheme_host(mfdn_ctx*, int body, int64_t n, const int32_t* h_req, double* h_out, uint8_t* h_mask,
                       void* d_work, size_t* work_bytes, uint32_t flags, int64_t chunk);
 
+/* The allocation-free call, for callers that cannot allocate device memory (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): mfdn_mscheme_2b/3b (the same steps H1-H6, the same kernels, the
+ * same values bit for bit) with the scratch the group-sort path needs taken from an array that is PART OF THE LIBRARY
+ * instead of from the caller: MFDN_STATIC_SCRATCH_BYTES of device memory, which every GPU that loads the library holds until
+ * the process exits.  body = 2 or 3; d_req, d_out, d_mask (may be NULL), flags and stream as for mfdn_mscheme_2b/3b;
+ * asynchronous on `stream`.  It calls no cudaMalloc, cudaFree or other allocating routine.
+ *  - The first call on a device looks up the array's device address once (cudaGetSymbolAddress, with that device
+ *    current); a call with n = 0 does just that and is the set-up call to make before a capture or a timed loop.
+ *  - A batch that needs more scratch than the array holds is rejected with MFDN_ERR_OOM (mfdn_last_error names both
+ *    sizes): the need is what mfdn_mscheme_2b/3b report for the same (n, flags) with d_work == NULL, about 45 bytes per
+ *    3-body request on the group-sort path plus 4 bytes per sort bucket of the table (config 3: 6.4 MB + n * 45 B, i.e. up
+ *    to ~5 * 10^5 requests per call; the paper's request buffers hold ~20 000).  2-body batches and 3-body
+ *    batches of up to 2^20 requests are evaluated thread per request unless a flag names the sort path, and need none.
+ *  - MFDN_ERR_STATE while mfdn_profile is on (profiling creates events).
+ *  - EVERY call in the process, from any context on the same device, uses the SAME array, and the array keeps the
+ *    last call's contents: the call clears what must start at zero (histogram, work-item counters) itself, on `stream`;
+ *    two calls that overlap on the GPU (different streams, or different host threads) race on it and give undefined
+ *    values.  Calls on one stream are ordered and safe. */
+#define MFDN_STATIC_SCRATCH_BYTES (32u << 20)
+int mfdn_mscheme_static(mfdn_ctx*, int body, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_mask, uint32_t flags,
+                        void* stream);
+
 /* Measurement hooks.  mfdn_profile(ctx, 1) makes every later mfdn_mscheme_2b/3b call record CUDA events on the
  * call's stream around (1) its group-sort kernels (H1-H2: keys, scans, partition passes, work-item list), (2) its transform
  * kernel (H3-H6) and (3) the gather of the results back into request order (sort path only; 0 for MFDN_PRESORTED

@@ -25,7 +25,8 @@ SYMBOLS = ["mfdn_orbitals_init", "mfdn_cg_build", "mfdn_cg_download", "mfdn_coup
            "mfdn_coupled_upload_3b", "mfdn_mscheme_2b", "mfdn_mscheme_3b", "mfdn_bad_request_count",
            "mfdn_info", "mfdn_group_keys", "mfdn_last_error", "mfdn_destroy", "mfdn_mscheme_host", "mfdn_profile",
            "mfdn_profile_read", "mfdn_fp64_peak", "mfdn_mscheme_accumulate_2b", "mfdn_mscheme_accumulate_3b",
-           "mfdn_mscheme_block_len_3b", "mfdn_mscheme_blocks_3b", "mfdn_option", "mfdn_multi_client"]
+           "mfdn_mscheme_block_len_3b", "mfdn_mscheme_blocks_3b", "mfdn_option", "mfdn_multi_client", "mfdn_mscheme_static"]
+MFDN_STATIC_SCRATCH_BYTES = 32 << 20
 
 _lib = None
 
@@ -59,6 +60,7 @@ def lib():
         L.mfdn_mscheme_block_len_3b.argtypes = [vp, vp, C.POINTER(i64)]
         L.mfdn_mscheme_blocks_3b.argtypes = [vp, i64, vp, vp, vp, vp, C.POINTER(C.c_size_t), vp]
         L.mfdn_mscheme_host.argtypes = [vp, C.c_int, i64, vp, vp, vp, vp, C.POINTER(C.c_size_t), u32, i64]
+        L.mfdn_mscheme_static.argtypes = [vp, C.c_int, i64, vp, vp, vp, u32, vp]
         L.mfdn_profile.argtypes = [vp, C.c_int]
         L.mfdn_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(i64)]
         L.mfdn_fp64_peak.argtypes = [vp, C.POINTER(C.c_double)]
@@ -207,6 +209,12 @@ def mfdn_mscheme_host(ctx, body, n, h_req, h_out, h_mask, d_work, work_bytes, fl
     return wb.value
 
 
+def mfdn_mscheme_static(ctx, body, n, d_req, d_out, d_mask, flags=0, stream=None):
+    """The allocation-free call: scratch from the library's own static device array (MFDN_STATIC_SCRATCH_BYTES)."""
+    _check(ctx, lib().mfdn_mscheme_static(ctx, int(body), int(n), C.c_void_p(d_req), C.c_void_p(d_out), C.c_void_p(d_mask),
+                                          int(flags), _stream(stream) if n else C.c_void_p(0)))
+
+
 def mfdn_profile(ctx, enable):
     _check(ctx, lib().mfdn_profile(ctx, int(bool(enable))))
 
@@ -296,6 +304,17 @@ class Context:
         fn = mfdn_mscheme_3b if body == 3 else mfdn_mscheme_2b
         fn(self.ctx, n, d_req.data_ptr(), d_out.data_ptr(), d_mask.data_ptr(), work.data_ptr(), work.numel(), flags,
            stream)
+        return d_out, d_mask
+
+    def mscheme_static(self, d_req, d_out, d_mask, flags=0, stream=None):
+        """mfdn_mscheme_static: the caller passes inputs and outputs, the scratch is the library's static array."""
+        torch = self.torch
+        assert d_req.is_cuda and d_req.is_contiguous() and d_out.is_cuda and d_mask.is_cuda
+        if d_req.dtype in (torch.uint16, torch.int16):
+            flags |= MFDN_REQ_U16
+        n, width = d_req.shape
+        with torch.cuda.device(self.device):
+            mfdn_mscheme_static(self.ctx, width // 2, n, d_req.data_ptr(), d_out.data_ptr(), d_mask.data_ptr(), flags, stream)
         return d_out, d_mask
 
     def accumulate(self, d_req, d_loc, d_phase, d_H, d_mask=None, flags=0, work=None, stream=None):

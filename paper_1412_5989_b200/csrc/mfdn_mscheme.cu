@@ -2319,6 +2319,53 @@ extern "C" int mfdn_mscheme_3b(mfdn_ctx* c, int64_t n, const int32_t* d_req, dou
     return run<3>(c, n, d_req, d_out, d_mask, d_work, work_bytes, flags, stream);
 }
 
+// ------------------------------------------------------------------------------- allocation-free call
+// mfdn_mscheme_static: run<BODY>() with its scratch in an array that is part of the library image (include/mfdn_b200.h).
+// In host code `g_static_scratch` is the host-side stand-in of the symbol, NOT a device address: the kernels are given the
+// address cudaGetSymbolAddress returns, looked up once per device with that device current and kept in g_static_ptr.
+// Every call on a device shares the array and finds the previous call's contents in it; run() never assumes zeroed
+// scratch (it clears the histogram and the work-item counters on the call's stream), so nothing else needs clearing.
+static __device__ __align__(256) unsigned char g_static_scratch[MFDN_STATIC_SCRATCH_BYTES];
+static std::mutex g_static_mu;
+constexpr int STATIC_MAX_DEVICES = 64;
+static void* g_static_ptr[STATIC_MAX_DEVICES] = {};
+
+extern "C" int mfdn_mscheme_static(mfdn_ctx* c, int body, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_mask, uint32_t flags,
+                                   void* stream)
+{
+    if (!c) return MFDN_ERR_ARG;
+    if (body != 2 && body != 3) return fail(c, MFDN_ERR_ARG, "body must be 2 or 3");
+    if (n < 0) return fail(c, MFDN_ERR_ARG, "negative request count");
+    if (c->profile) return fail(c, MFDN_ERR_STATE, "mfdn_mscheme_static: not while mfdn_profile is on (profiling creates events)");
+    if (c->device < 0 || c->device >= STATIC_MAX_DEVICES) return fail(c, MFDN_ERR_ARG, "mfdn_mscheme_static: device ordinal above 63");
+    void* scratch = nullptr;
+    {
+        std::lock_guard<std::mutex> lk(g_static_mu);
+        scratch = g_static_ptr[c->device];
+        if (!scratch) {   // set-up, once per device
+            MFDN_CUDA(c, cudaSetDevice(c->device));
+            MFDN_CUDA(c, cudaGetSymbolAddress(&scratch, g_static_scratch));
+            if (!scratch) return fail(c, MFDN_ERR_CUDA, "cudaGetSymbolAddress returned a null address");
+            g_static_ptr[c->device] = scratch;
+        }
+    }
+    // what this (n, flags) needs: the query form of the ordinary call (host arithmetic only)
+    size_t need = 0;
+    int rc = body == 3 ? run<3>(c, n, nullptr, nullptr, nullptr, nullptr, &need, flags, nullptr)
+                       : run<2>(c, n, nullptr, nullptr, nullptr, nullptr, &need, flags, nullptr);
+    if (rc != MFDN_OK) return rc;
+    if (need > (size_t)MFDN_STATIC_SCRATCH_BYTES) {
+        char msg[192];
+        snprintf(msg, sizeof msg, "mfdn_mscheme_static: %lld requests need %zu bytes of scratch, the static array holds %zu: split the batch or use mfdn_mscheme_%db",
+                 (long long)n, need, (size_t)MFDN_STATIC_SCRATCH_BYTES, body);
+        return fail(c, MFDN_ERR_OOM, msg);
+    }
+    if (n == 0) return MFDN_OK;
+    size_t have = (size_t)MFDN_STATIC_SCRATCH_BYTES;
+    return body == 3 ? run<3>(c, n, d_req, d_out, d_mask, scratch, &have, flags, stream)
+                     : run<2>(c, n, d_req, d_out, d_mask, scratch, &have, flags, stream);
+}
+
 extern "C" int mfdn_mscheme_accumulate_2b(mfdn_ctx* c, int64_t n, const int32_t* d_req, const int64_t* d_loc, const double* d_phase,
                                           double* d_H, int64_t h_len, uint8_t* d_mask, void* d_work, size_t* work_bytes, uint32_t flags,
                                           void* stream)
