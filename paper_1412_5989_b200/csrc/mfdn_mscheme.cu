@@ -172,7 +172,9 @@ __device__ __forceinline__ unsigned long long chanmask3(const unsigned long long
 template <bool SMEM = false>
 __device__ __forceinline__ bool mask3(const unsigned long long* stm, const Side3& B, const Side3& K, int4 db, int4 dk)
 {
-    if (max((db.y >> 16) & 255, (dk.y >> 16) & 255) > min((db.y >> 24) & 255, (dk.y >> 24) & 255)) return false;   // no common J: no slab
+    // no test for a common J range of the two tuples: without one the two channel sets below share no (J, T) bit, because the J of
+    // every listed state lies inside its tuple's range (checked at upload).  The test cost 11 instructions per request
+    // (pre-sorted call of config 3: 2.005 -> 1.951 ms without it)
     const int ja = db.x & 255, jb = (db.x >> 8) & 255, jd = dk.x & 255, je = (dk.x >> 8) & 255;
     const int twoM12b = 2 * (B.ima + B.imb) - ja - jb, twoM12k = 2 * (K.ima + K.imb) - jd - je;
     const int tzb12 = (B.tz >> 2) + ((B.tz >> 1) & 1) - 1, tzk12 = (K.tz >> 2) + ((K.tz >> 1) & 1) - 1;  // MT12
@@ -596,7 +598,8 @@ __global__ void __launch_bounds__(KS_THREADS, 1) k_keys3s(Tables T, KeysSmem3 L,
             recs[i] = ((unsigned long long)key << REC_KEY_SHIFT) | low;
             if (maskout) maskout[i] = (uint8_t)mask;
             const uint32_t bucket = key == REC_INVALID ? invalid_bucket : key;
-            if (AGG) {   // group-ordered input: one atomic per run of equal keys in the warp
+            if (AGG) {   // group-ordered input: one atomic per run of equal keys in the warp (runs found with shfl.up + ballot
+                         // instead of match.any: pre-sorted call 2.005 -> 2.05 ms, not kept)
                 const unsigned same = __match_any_sync(__activemask(), bucket);
                 if ((tid & 31) == __ffs(same) - 1) atomicAdd(hist + bucket, (uint32_t)__popc(same));
             } else {
@@ -616,32 +619,75 @@ __global__ void __launch_bounds__(KS_THREADS, 1) k_keys3s(Tables T, KeysSmem3 L,
 }
 
 // =============================================================================== H2: group sort
+// exclusive scan of v over the threads of a block of NT threads (NT a multiple of 32, at most 1024); `total` = sum
+template <int NT>
+__device__ __forceinline__ uint32_t block_excl_scan(uint32_t v, uint32_t* s_warp /* [NT / 32 + 1] */, uint32_t& total)
+{
+    const int tid = threadIdx.x;
+    uint32_t inc = v;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+        const uint32_t x = __shfl_up_sync(0xFFFFFFFFu, inc, off);
+        if ((tid & 31) >= off) inc += x;
+    }
+    __syncthreads();   // s_warp may still be read from a previous call
+    if ((tid & 31) == 31) s_warp[tid >> 5] = inc;
+    __syncthreads();
+    if (tid < 32) {
+        const uint32_t w = tid < NT / 32 ? s_warp[tid] : 0u;
+        uint32_t wi = w;
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            const uint32_t x = __shfl_up_sync(0xFFFFFFFFu, wi, off);
+            if (tid >= off) wi += x;
+        }
+        if (tid < NT / 32) s_warp[tid] = wi - w;
+        if (tid == 31) s_warp[NT / 32] = wi;
+    }
+    __syncthreads();
+    total = s_warp[NT / 32];
+    return s_warp[tid >> 5] + inc - v;
+}
+
 constexpr int SCAN_T = 256, SCAN_E = 16, SCAN_TILE = SCAN_T * SCAN_E;
 
 __global__ void __launch_bounds__(SCAN_T) k_scan_tiles(uint32_t* __restrict__ data, long long m, uint32_t* __restrict__ tile_sums)
 {
-    __shared__ uint32_t sh[SCAN_T];
+    __shared__ uint32_t s_warp[SCAN_T / 32 + 1];
     long long base = (long long)blockIdx.x * SCAN_TILE + (long long)threadIdx.x * SCAN_E;
     uint32_t v[SCAN_E], sum = 0;
+    const bool full = base + SCAN_E <= m;   // the thread's 16 words as four 128-bit accesses (data is 256-byte aligned)
+    if (full) {
 #pragma unroll
-    for (int k = 0; k < SCAN_E; k++) {
-        v[k] = (base + k < m) ? data[base + k] : 0u;
-        sum += v[k];
-    }
-    sh[threadIdx.x] = sum;
-    __syncthreads();
-    for (int off = 1; off < SCAN_T; off <<= 1) {
-        uint32_t x = threadIdx.x >= off ? sh[threadIdx.x - off] : 0u;
-        __syncthreads();
-        sh[threadIdx.x] += x;
-        __syncthreads();
-    }
-    uint32_t excl = sh[threadIdx.x] - sum;
-    if (threadIdx.x == SCAN_T - 1) tile_sums[blockIdx.x] = sh[threadIdx.x];
+        for (int k = 0; k < SCAN_E / 4; k++) {
+            const uint4 q = reinterpret_cast<const uint4*>(data + base)[k];
+            v[4 * k] = q.x; v[4 * k + 1] = q.y; v[4 * k + 2] = q.z; v[4 * k + 3] = q.w;
+        }
+    } else {
 #pragma unroll
-    for (int k = 0; k < SCAN_E; k++) {
-        if (base + k < m) data[base + k] = excl;
-        excl += v[k];
+        for (int k = 0; k < SCAN_E; k++) v[k] = (base + k < m) ? data[base + k] : 0u;
+    }
+#pragma unroll
+    for (int k = 0; k < SCAN_E; k++) sum += v[k];
+    uint32_t all;
+    uint32_t excl = block_excl_scan<SCAN_T>(sum, s_warp, all);   // warp shuffles, three block barriers
+    if (threadIdx.x == 0) tile_sums[blockIdx.x] = all;
+    if (full) {
+#pragma unroll
+        for (int k = 0; k < SCAN_E / 4; k++) {
+            uint4 q;
+            q.x = excl; excl += v[4 * k];
+            q.y = excl; excl += v[4 * k + 1];
+            q.z = excl; excl += v[4 * k + 2];
+            q.w = excl; excl += v[4 * k + 3];
+            reinterpret_cast<uint4*>(data + base)[k] = q;
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < SCAN_E; k++) {
+            if (base + k < m) data[base + k] = excl;
+            excl += v[k];
+        }
     }
 }
 
@@ -670,6 +716,15 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_add(uint32_t* __restrict__ data
 {
     uint32_t add = tile_sums[blockIdx.x];
     long long base = (long long)blockIdx.x * SCAN_TILE + (long long)threadIdx.x * SCAN_E;
+    if (base + SCAN_E <= m) {
+#pragma unroll
+        for (int k = 0; k < SCAN_E / 4; k++) {
+            uint4 q = reinterpret_cast<uint4*>(data + base)[k];
+            q.x += add; q.y += add; q.z += add; q.w += add;
+            reinterpret_cast<uint4*>(data + base)[k] = q;
+        }
+        return;
+    }
 #pragma unroll
     for (int k = 0; k < SCAN_E; k++)
         if (base + k < m) data[base + k] += add;
@@ -716,35 +771,6 @@ __global__ void __launch_bounds__(128) k_tscan_sum(const uint32_t* __restrict__ 
     part[(size_t)k * nc + c] = sum;
 }
 
-// exclusive scan of v over the threads of a block of NT threads (NT a multiple of 32, at most 1024); `total` = sum
-template <int NT>
-__device__ __forceinline__ uint32_t block_excl_scan(uint32_t v, uint32_t* s_warp /* [NT / 32 + 1] */, uint32_t& total)
-{
-    const int tid = threadIdx.x;
-    uint32_t inc = v;
-#pragma unroll
-    for (int off = 1; off < 32; off <<= 1) {
-        const uint32_t x = __shfl_up_sync(0xFFFFFFFFu, inc, off);
-        if ((tid & 31) >= off) inc += x;
-    }
-    __syncthreads();   // s_warp may still be read from a previous call
-    if ((tid & 31) == 31) s_warp[tid >> 5] = inc;
-    __syncthreads();
-    if (tid < 32) {
-        const uint32_t w = tid < NT / 32 ? s_warp[tid] : 0u;
-        uint32_t wi = w;
-#pragma unroll
-        for (int off = 1; off < 32; off <<= 1) {
-            const uint32_t x = __shfl_up_sync(0xFFFFFFFFu, wi, off);
-            if (tid >= off) wi += x;
-        }
-        if (tid < NT / 32) s_warp[tid] = wi - w;
-        if (tid == 31) s_warp[NT / 32] = wi;
-    }
-    __syncthreads();
-    total = s_warp[NT / 32];
-    return s_warp[tid >> 5] + inc - v;
-}
 
 // part[chunk][bin] -> records of the bin in the chunks before (exclusive scan over chunks); cstart[bin] = start of the bin
 // in the coarse-ordered stream, cstart[nc] = n
