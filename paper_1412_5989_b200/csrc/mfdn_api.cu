@@ -1,6 +1,7 @@
 // Host side of libmfdn_b200.so: context, A0 orbital tables, A1 CG-table build kernel,
 // A2 coupled-table upload + re-tiling kernels.  See include/mfdn_b200.h for the ABI.
 #include <algorithm>
+#include <array>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -652,6 +653,32 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
         }
         stmask.swap(packed);
     }
+    // The same look-up with the arithmetic done here: per tuple, indexed by [ima + imb][MT12 == 0], the channel set of all listed
+    // states with J12 >= |M12| and an admissible T12 (T12 = 0 only if MT12 = 0).  k_keys3s keeps this table in shared memory: S7 is
+    // then one 8-byte look-up per side without the J12-range arithmetic (22 -> 6 instructions per side).  Shared by content.
+    std::vector<unsigned long long> stm12;
+    std::vector<int32_t> stm12_off(nt);
+    {
+        std::map<std::array<int, 4>, int> seen;
+        for (int t = 0; t < nt; t++) {
+            const int4 d = tdesc[t];
+            const int jab = (d.x & 255) + ((d.x >> 8) & 255), J12min = d.y & 255, J12max = (d.y >> 8) & 255;
+            const std::array<int, 4> key{d.z, jab, J12min, J12max};
+            auto it = seen.find(key);
+            if (it == seen.end()) {
+                it = seen.emplace(key, (int)stm12.size()).first;
+                for (int i12 = 0; i12 <= jab; i12++) {
+                    const int lo = std::max(J12min, (std::abs(2 * i12 - jab) + 1) >> 1);
+                    for (int e = 0; e < 2; e++) {
+                        unsigned long long m = 0ull;
+                        if (lo <= J12max) m = (e ? stmask[d.z + (size_t)(lo - J12min) * 2] : 0ull) | stmask[d.z + (size_t)(lo - J12min) * 2 + 1];
+                        stm12.push_back(m);
+                    }
+                }
+            }
+            stm12_off[t] = it->second;
+        }
+    }
     auto range = [&](int4 d, int twoJ, int& lo, int& hi) {
         int jc = (d.x >> 16) & 255;
         lo = std::max(d.y & 255, std::abs(twoJ - jc) >> 1);
@@ -850,6 +877,7 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     std::vector<int4> tdesc_rt = tdesc;   // run-time copy: w = start of the tuple's sigma table (the row-map offset is upload-only)
     for (int t = 0; t < nt; t++) tdesc_rt[t].w = sigoff[t];
     size_t o_tid = res.add(tuple_id), o_desc_rt = res.add(tdesc_rt), o_sgrp = res.add(sgrp), o_sm = res.add(stmask);
+    size_t o_sm12 = res.add(stm12), o_sm12off = res.add(stm12_off);
     size_t o_gbase = res.add(gbase), o_rowbase = res.add(rowbase), o_colcum = res.add(colcum);
     size_t o_desc = tmp.add(tdesc), o_ab = res.add(ab);
     size_t o_tk = res.add(tk), o_jinfo = res.add(jinfo), o_sig = res.add(sig), o_sigoff = res.add(sigoff);
@@ -949,6 +977,9 @@ extern "C" int mfdn_coupled_upload_3b(mfdn_ctx* c, int32_t e3max, int32_t n_chan
     c->t.ab3 = ab_dense ? (const int2*)(dres + o_ab) : nullptr;
     c->t.slab3 = (const double*)dslab;
     c->t.stmask3 = (const unsigned long long*)(dres + o_sm);
+    c->t.stm12_3 = (const unsigned long long*)(dres + o_sm12);
+    c->t.stm12_off3 = (const int32_t*)(dres + o_sm12off);
+    c->t.stm12_len3 = (int)stm12.size();
     c->t.tk3 = q.tk;
     c->t.jinfo3 = (const int2*)(dres + o_jinfo);
     c->t.dtab3 = (const double*)ddtab;

@@ -119,6 +119,9 @@ struct Tables {
     const uint32_t* vw20;          // isospin-combined slabs, split word planes (see vw_stride)
     int vw_f32;                    // 1: the slabs hold fp32 values, one word each (MFDN_OPT_SLAB_FP32)
     const unsigned long long* stmask3;
+    const unsigned long long* stm12_3;   // S7 by direct look-up: [stm12_off3[tuple] + (ima + imb) * 2 + (MT12 == 0)] = channels (J, T) in which the
+    const int32_t* stm12_off3;           // tuple has a listed state with J12 >= |M12| and a T12 admissible for MT12 (built from stmask3 at upload)
+    int stm12_len3;
     const int4* tk3;               // [n_tup3] see above
     const int2* jinfo3;            // per (tuple, J): {offset of the J block in the tuple's coefficient table (doubles, even), rows nb(J)}
     const double* dtab3;           // per tuple and J block [sigma][row] = <ja ma jb mb|J12 M12> <J12 M12 jc mc|J M>, rows = J12 ascending

@@ -183,6 +183,15 @@ __device__ __forceinline__ bool mask3(const unsigned long long* stm, const Side3
     if (abs(B.twoMT) == 3) mm &= 0xAAAAAAAAAAAAAAAAull;        // T = 3/2 only
     return mm != 0;
 }
+// the same from the direct look-up table stm12 (Tables::stm12_3), zb / zk = the tuples' offsets in it
+__device__ __forceinline__ bool mask3s(const unsigned long long* stm12, const Side3& B, const Side3& K, int zb, int zk)
+{
+    const int eb = ((B.tz >> 2) ^ (B.tz >> 1)) & 1, ek = ((K.tz >> 2) ^ (K.tz >> 1)) & 1;   // MT12 == 0: the first two tz bits differ
+    unsigned long long mm = stm12[zb + (B.ima + B.imb) * 2 + eb] & stm12[zk + (K.ima + K.imb) * 2 + ek];
+    mm &= ~0ull << (2 * (abs(B.twoM) >> 1));                   // J >= |M|
+    if (abs(B.twoMT) == 3) mm &= 0xAAAAAAAAAAAAAAAAull;        // T = 3/2 only
+    return mm != 0;
+}
 __device__ __forceinline__ bool mask2(const Side2& B, int4 db, int4 dk)
 {
     unsigned long long mb = (unsigned long long)(uint32_t)db.z | ((unsigned long long)(uint32_t)db.w << 32);
@@ -549,8 +558,13 @@ __global__ void __launch_bounds__(KS_THREADS, 1) k_keys3s(Tables T, KeysSmem3 L,
     uint16_t* s_sig = reinterpret_cast<uint16_t*>(ks_smem + L.sig);
     uint8_t* s_tzbin = ks_smem + L.tzbin;
     const int tid = threadIdx.x, nt = T.n_tup3;
-    for (int k = tid; k < nt; k += KS_THREADS) { s_tdesc[k] = __ldg(T.tdesc3 + k); s_rowbase[k] = __ldg(T.rowbase3 + k); }
-    for (int k = tid; k < T.stmask_len3; k += KS_THREADS) s_stm[k] = __ldg(T.stmask3 + k);
+    for (int k = tid; k < nt; k += KS_THREADS) {
+        int4 d = __ldg(T.tdesc3 + k);
+        d.z = __ldg(T.stm12_off3 + k);   // this kernel's copy: offset in the direct S7 table instead of in stmask3
+        s_tdesc[k] = d;
+        s_rowbase[k] = __ldg(T.rowbase3 + k);
+    }
+    for (int k = tid; k < T.stm12_len3; k += KS_THREADS) s_stm[k] = __ldg(T.stm12_3 + k);
     for (int k = tid; k < T.n_orb * T.n_orb; k += KS_THREADS) s_ab[k] = __ldg(T.ab3 + k);
     for (int k = tid; k < T.n_sps; k += KS_THREADS) s_sps[k] = sps_pack_sorted(__ldg(T.sps_rec + k), k);
     for (int k = tid; k < T.ncls3 * nt; k += KS_THREADS) s_colcum[k] = __ldg(T.colcum3 + k);
@@ -585,7 +599,7 @@ __global__ void __launch_bounds__(KS_THREADS, 1) k_keys3s(Tables T, KeysSmem3 L,
                     const int sjk = (dk.x & 255) + ((dk.x >> 8) & 255) + ((dk.x >> 16) & 255);
                     key = s_rowbase[B.tup] + s_colcum[((db.x >> 26) & 31) * nt + K.tup] +
                           (uint32_t)(B.ima + B.imb + B.imc - ((sjb - min(sjb, sjk)) >> 1));
-                    mask = mask3<true>(s_stm, B, K, db, dk);
+                    mask = mask3s(s_stm, B, K, db.z, dk.z);
                     const int jb1 = ((db.x >> 8) & 255) + 1, jc1 = ((db.x >> 16) & 255) + 1;
                     const int je1 = ((dk.x >> 8) & 255) + 1, jf1 = ((dk.x >> 16) & 255) + 1;
                     const uint32_t sb = s_sig[db.w + (B.ima * jb1 + B.imb) * jc1 + B.imc];
@@ -2183,7 +2197,7 @@ int run(mfdn_ctx* c, int64_t n, const int32_t* d_req, double* d_out, uint8_t* d_
             auto up = [](uint32_t x) { return (x + 15u) & ~15u; };
             L.tdesc = 0;
             L.stm = up(L.tdesc + (uint32_t)nt * 16u);
-            L.ab = up(L.stm + (uint32_t)c->t.stmask_len3 * 8u);
+            L.ab = up(L.stm + (uint32_t)c->t.stm12_len3 * 8u);
             L.sps = up(L.ab + (uint32_t)(c->t.n_orb * c->t.n_orb) * 8u);
             L.rowbase = up(L.sps + (uint32_t)c->t.n_sps * 4u);
             L.ch = up(L.rowbase + (uint32_t)nt * 4u);
