@@ -61,3 +61,13 @@ def test_product_path_does_not_touch_oracle():
         if f.endswith((".py", ".c")):
             src = open(os.path.join(ROOT, "oracle", f)).read()
             assert "paper_1412_5989_b200.binding" not in src and "libmfdn" not in src and "csrc" not in src.replace("paper_1412_5989_b200/csrc", ""), f
+
+
+def test_static_scratch_size_matches_binding():
+    """include/mfdn_b200.h states the size of the static scratch array of mfdn_mscheme_static; the binding repeats it."""
+    from paper_1412_5989_b200 import binding
+    header = open(os.path.join(ROOT, "include", "mfdn_b200.h")).read()
+    m = re.search(r"#define\s+MFDN_STATIC_SCRATCH_BYTES\s+\((\d+)u\s*<<\s*(\d+)\)", header)
+    assert m, "MFDN_STATIC_SCRATCH_BYTES not found in the header"
+    assert int(m.group(1)) << int(m.group(2)) == binding.MFDN_STATIC_SCRATCH_BYTES
+    assert "mfdn_mscheme_static" in binding.SYMBOLS
