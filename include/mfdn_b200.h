@@ -201,7 +201,8 @@ int mfdn_mscheme_host(mfdn_ctx*, int body, int64_t n, const int32_t* h_req, doub
  *  - A batch that needs more scratch than the array holds is rejected with MFDN_ERR_OOM (mfdn_last_error names both
  *    sizes): the need is what mfdn_mscheme_2b/3b report for the same (n, flags) with d_work == NULL, about 45 bytes per
  *    3-body request on the group-sort path plus 4 bytes per sort bucket of the table (config 3: 6.4 MB + n * 45 B, i.e. up
- *    to ~5 * 10^5 requests per call; the paper's request buffers hold ~20 000).  2-body batches and 3-body
+ *    to ~5 * 10^5 requests per call; config 4, 7.7 M buckets = 30.7 MB: ~6 * 10^4; the paper's request buffers hold
+ *    ~20 000).  2-body batches and 3-body
  *    batches of up to 2^20 requests are evaluated thread per request unless a flag names the sort path, and need none.
  *  - MFDN_ERR_STATE while mfdn_profile is on (profiling creates events).
  *  - EVERY call in the process, from any context on the same device, uses the SAME array, and the array keeps the
