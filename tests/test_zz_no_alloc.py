@@ -59,7 +59,8 @@ def test_static_scratch_two_calls_in_a_row(torch, B):
         ctx.mscheme_static(d_reqs[1], outs[1], masks[1], flags)         # second call in a row on the same array
         ctx.mscheme_static(d_reqs[0], outs[0], masks[0], flags)         # and the first window again, on top of the second
         torch.cuda.synchronize()
-        assert torch.cuda.mem_get_info()[0] == free0, "device memory was allocated during mfdn_mscheme_static"
+        # the scratch of these calls would be >= 12 MB; 1 MiB of slack for anything the driver does on its own
+        assert torch.cuda.mem_get_info()[0] >= free0 - (1 << 20), "device memory was allocated during mfdn_mscheme_static"
         for k in range(2):
             got, gmask = outs[k].cpu().numpy(), masks[k].cpu().numpy()
             _compare(cfg, got, gmask, *ref[k])
